@@ -1,0 +1,470 @@
+"""Pins for the CPU oracle (oracle/clt_oracle.c): what the paper and the mathematics fix, none of it
+computed by the oracle itself or by the CUDA path.  CPU only.
+
+P1 closed form (stencils exact on polynomials)          PAPER.md L125 "4th order finite difference"
+P2 special case (vacuum field static state, K = 0)      eqs (1)-(6), L67-79
+P2b equilibrium invariance (U = U0 gives K = 0 exactly) eqs (11)-(14), L105-117
+P3 order of accuracy vs sympy-derived continuous operators and full RHS of eqs (1)-(6)/(11)-(14)
+P4 invariant (div_c B at round-off over RK4 steps)      eq (4)
+P5 invariant (rigid rotation: viscous operator = 0, centripetal acceleration exact)  eq (3)
+P6 reduction (U0 = 0: eqs (11)-(14) == a separately written numpy evaluation of eqs (1)-(4))
+P7 exact discrete Alfven response with the stencil's modified wavenumber
+P8 textbook RK4 order through oracle_rk4 and dt-halving on the MHD system   L125
+P10 SETDT closed form (Fig. 4), P11 diagnostics closed forms
+"""
+import numpy as np
+import pytest
+
+import oracle as orc
+from paper_1812_00525_b200 import inputs
+
+
+def make(nR=24, nphi=16, nZ=20, Rmin=2.0, Rmax=4.0, Zmin=-1.0, Zmax=1.0, **kw):
+    o = orc.Oracle(nR, nphi, nZ, Rmin, Rmax, Zmin, Zmax, **kw)
+    dR = (Rmax - Rmin) / (nR - 1)
+    dZ = (Zmax - Zmin) / (nZ - 1)
+    Lphi = kw.get("phi_extent", 0.0) or 2 * np.pi
+    R = Rmin + np.arange(nR) * dR
+    Z = Zmin + np.arange(nZ) * dZ
+    phi = np.arange(nphi) * (Lphi / nphi)
+    P, ZZ, RR = np.meshgrid(phi, Z, R, indexing="ij")      # [nphi][nZ][nR]
+    return o, RR, P, ZZ
+
+
+def interior(a):
+    return a[..., 2:-2, 2:-2]
+
+
+def deep(a):
+    return a[..., 4:-4, 4:-4]
+
+
+# ----------------------------------------------------------------------------------------------- P1
+@pytest.mark.parametrize("deg", range(0, 7))
+def test_P1_stencils_exact_on_polynomials(deg):
+    o, RR, P, ZZ = make(nR=20, nphi=12, nZ=18, Rmin=1.0, Rmax=2.0, Zmin=-0.5, Zmax=0.5, phi_extent=1.0)
+    # phi is periodic, so exactness in phi is checked on the middle planes only (j = 2..nphi-3)
+    for name, X, x0 in (("R", RR, 1.5), ("Z", ZZ, 0.1), ("P", P, 0.4)):
+        f = (X - x0) ** deg
+        d1 = o.scalar_op("d1" + name, f)
+        d2 = o.scalar_op("d2" + name, f)
+        e1 = deg * (X - x0) ** (deg - 1) if deg >= 1 else 0 * X
+        e2 = deg * (deg - 1) * (X - x0) ** (deg - 2) if deg >= 2 else 0 * X
+        sl = (slice(2, -2), slice(2, -2), slice(2, -2))
+        err1 = np.abs(d1 - e1)[sl].max()
+        err2 = np.abs(d2 - e2)[sl].max()
+        if deg <= 4:
+            assert err1 < 5e-13, (name, deg, err1)
+        else:
+            assert err1 > 1e-7, (name, deg, err1)          # a 4th-order stencil must miss degree 5
+        if deg <= 5:
+            assert err2 < 5e-10, (name, deg, err2)
+        else:
+            assert err2 > 1e-6, (name, deg, err2)
+
+
+def test_P1_weighted_radial_derivative():
+    o, RR, P, ZZ = make()
+    f = 1.0 + 0.3 * RR - 0.2 * RR ** 2 + 0.05 * RR ** 3            # R*f is degree 4: exact
+    got = o.scalar_op("d1R_Rf", f)
+    exp = 1.0 + 0.6 * RR - 0.6 * RR ** 2 + 0.2 * RR ** 3
+    assert np.abs(interior(got - exp)).max() < 1e-12
+
+
+# ----------------------------------------------------------------------------------------------- P2
+def test_P2_vacuum_field_static_state_has_zero_rhs():
+    o, RR, P, ZZ = make(eta=1e-3, nu=1e-3, D=1e-3, kappa=1e-3)
+    U = np.zeros((8,) + RR.shape)
+    U[0] = 1.3
+    U[1] = 0.07
+    U[6] = 2.5 / RR
+    U[7] = 0.4
+    K = o.rhs_of(U)
+    J = o.curl_J1(U)
+    assert np.abs(J).max() < 1e-12
+    assert np.abs(K).max() < 1e-13
+
+
+def test_P2b_state_equal_to_reference_state_has_exactly_zero_rhs():
+    prob = inputs.make_custom_problem(20, 8, 18, rotation=0.05)
+    cfg = prob.cfg
+    o = orc.Oracle(cfg.nR, cfg.nphi, cfg.nZ, cfg.Rmin, cfg.Rmax, cfg.Zmin, cfg.Zmax, eta=1e-3, nu=1e-3, D=1e-3,
+                   kappa=1e-3)
+    o.set_equilibrium(prob.U0)
+    U = np.repeat(prob.U0[:, None], cfg.nphi, axis=1)
+    assert np.all(o.rhs_of(U) == 0.0)
+
+
+# ----------------------------------------------------------------------------------------------- P3
+def _sympy_ops():
+    import sympy as sp
+    R, p, Z = sp.symbols("R phi Z", real=True)
+
+    def grad(f):
+        return [sp.diff(f, R), sp.diff(f, p) / R, sp.diff(f, Z)]
+
+    def div(a):
+        return sp.diff(R * a[0], R) / R + sp.diff(a[1], p) / R + sp.diff(a[2], Z)
+
+    def curl(a):
+        return [sp.diff(a[2], p) / R - sp.diff(a[1], Z),
+                sp.diff(a[0], Z) - sp.diff(a[2], R),
+                (sp.diff(R * a[1], R) - sp.diff(a[0], p)) / R]
+
+    def adv(a, b):          # (a.grad) b, cylindrical
+        return [sum(x * y for x, y in zip(a, grad(b[0]))) - a[1] * b[1] / R,
+                sum(x * y for x, y in zip(a, grad(b[1]))) + a[1] * b[0] / R,
+                sum(x * y for x, y in zip(a, grad(b[2])))]
+
+    def cross(a, b):
+        return [a[1] * b[2] - a[2] * b[1], a[2] * b[0] - a[0] * b[2], a[0] * b[1] - a[1] * b[0]]
+
+    def lap(f):
+        return div(grad(f))
+
+    def veclap(a):          # grad div - curl curl: independent of the oracle's component formula
+        gd = grad(div(a))
+        cc = curl(curl(a))
+        return [x - y for x, y in zip(gd, cc)]
+
+    return sp, (R, p, Z), dict(grad=grad, div=div, curl=curl, adv=adv, cross=cross, lap=lap, veclap=veclap)
+
+
+def _lamb(sp, syms, expr):
+    f = sp.lambdify(syms, expr, "numpy")
+    return lambda RR, P, ZZ: np.broadcast_to(np.asarray(f(RR, P, ZZ), dtype=float), RR.shape).copy()
+
+
+def _order(e_coarse, e_fine):
+    return np.log2(e_coarse / e_fine)
+
+
+def test_P3a_each_operator_converges_at_4th_order_to_the_continuous_operator():
+    sp, syms, op = _sympy_ops()
+    R, p, Z = syms
+    f = sp.sin(1.3 * R + 0.2) * sp.cos(2 * p + 0.3) * sp.exp(0.5 * Z) + R ** 2 * Z * sp.cos(p)
+    a = [sp.cos(0.9 * R) * sp.sin(p + 0.1) * (1 + 0.3 * Z), sp.sin(1.1 * R + Z) * sp.cos(2 * p) + 1 / R,
+         sp.exp(-0.4 * Z) * sp.sin(0.7 * R) * sp.sin(p - 0.2)]
+    b = [sp.sin(0.8 * R + 0.5 * Z) * sp.cos(p), sp.cos(1.2 * R) * sp.cos(p + 0.4) * Z, sp.sin(R * Z * 0.3) + sp.sin(2 * p)]
+    errs = {}
+    for n in (1, 2):
+        o, RR, P, ZZ = make(nR=20 * n + 1, nphi=16 * n, nZ=16 * n + 1)
+        ev = lambda e: _lamb(sp, syms, e)(RR, P, ZZ)
+        fa = ev(f)
+        aa = np.stack([ev(x) for x in a])
+        ba = np.stack([ev(x) for x in b])
+        cases = {
+            "laplacian": (o.scalar_op("laplacian", fa), ev(op["lap"](f))),
+            "divergence": (o.scalar_op("divergence", aa), ev(op["div"](a))),
+            "div_c": (o.scalar_op("div_c", aa), ev(op["div"](a))),
+            "grad": (o.vector_op("grad", fa), np.stack([ev(x) for x in op["grad"](f)])),
+            "curl_c": (o.vector_op("curl_c", aa), np.stack([ev(x) for x in op["curl"](a)])),
+            "vector_laplacian": (o.vector_op("vector_laplacian", aa), np.stack([ev(x) for x in op["veclap"](a)])),
+            "advect_vector": (o.vector_op("advect_vector", np.concatenate([aa, ba])),
+                              np.stack([ev(x) for x in op["adv"](a, b)])),
+        }
+        for k, (got, exp) in cases.items():
+            # compare on every other interior node of the fine grid = the coarse grid's nodes
+            errs.setdefault(k, []).append(np.abs(interior(got - exp)).max())
+    for k, (e1, e2) in errs.items():
+        assert 3.6 < _order(e1, e2) < 4.6, (k, e1, e2, _order(e1, e2))
+    # the paper's own example of section 8(c) P3: f = R^2 Z cos(phi)  =>  lap f = 3 Z cos(phi)
+    o, RR, P, ZZ = make(nR=41, nphi=32, nZ=33)
+    got = o.scalar_op("laplacian", RR ** 2 * ZZ * np.cos(P))
+    assert np.abs(interior(got - 3 * ZZ * np.cos(P))).max() < 2e-4
+
+
+def _manufactured(sp, syms, equilibrium_exact):
+    R, p, Z = syms
+    Om, c = sp.Rational(1, 5), sp.Rational(3, 2)
+    if equilibrium_exact:
+        # rigid rotor in a vacuum toroidal field: satisfies eqs (7)-(10) exactly
+        rho0 = sp.Integer(1)
+        v0 = [sp.Integer(0), Om * R, sp.Integer(0)]
+        p0 = sp.Rational(1, 2) + Om ** 2 * R ** 2 / 2
+        B0 = [sp.Integer(0), c / R, sp.Integer(0)]
+    else:
+        # arbitrary smooth axisymmetric reference state (does NOT satisfy (7)-(10))
+        rho0 = 1 + sp.Rational(1, 10) * sp.cos(R - 3) * sp.cos(Z)
+        v0 = [sp.Rational(1, 20) * sp.sin(Z) * R, Om * R * (1 + sp.Rational(1, 10) * Z), sp.Rational(1, 30) * sp.cos(R)]
+        p0 = sp.Rational(1, 2) - sp.Rational(1, 20) * ((R - 3) ** 2 + Z ** 2)
+        B0 = [sp.Rational(1, 5) * Z / R, c / R, -sp.Rational(1, 5) * (R - 3) / R]
+    rho1 = sp.Rational(1, 10) * sp.sin(1.1 * R + 0.3) * sp.cos(p + 0.2) * sp.cos(0.7 * Z)
+    p1 = sp.Rational(1, 20) * sp.cos(0.9 * R) * sp.sin(2 * p + 0.1) * sp.exp(0.3 * Z)
+    v1 = [sp.Rational(1, 10) * sp.sin(0.8 * R + 0.5 * Z) * sp.cos(p), sp.Rational(1, 10) * sp.cos(1.2 * R) * sp.cos(2 * p + 0.4) * (1 + Z / 2),
+          sp.Rational(1, 10) * sp.sin(R * Z * 0.3 + p)]
+    B1 = [sp.Rational(1, 10) * sp.cos(0.9 * R + 0.2) * sp.sin(p + 0.1) * (1 + 0.3 * Z),
+          sp.Rational(1, 10) * sp.sin(1.1 * R + Z) * sp.cos(2 * p),
+          sp.Rational(1, 10) * sp.exp(-0.4 * Z) * sp.sin(0.7 * R) * sp.sin(p - 0.2)]
+    return dict(rho0=rho0, p0=p0, v0=v0, B0=B0, rho1=rho1, p1=p1, v1=v1, B1=B1)
+
+
+def _continuous_rhs(sp, syms, op, m, par, subtracted):
+    """Continuous right-hand sides: eqs (1)-(6) on the total state, or eqs (11)-(14)."""
+    G, eta, nu, D, kap = par
+    rho = m["rho0"] + m["rho1"]
+    p = m["p0"] + m["p1"]
+    v = [a + b for a, b in zip(m["v0"], m["v1"])]
+    B = [a + b for a, b in zip(m["B0"], m["B1"])]
+    v0, v1, B0, B1 = m["v0"], m["v1"], m["B0"], m["B1"]
+    J = op["curl"](B)
+    J0 = op["curl"](B0)
+    J1 = [a - b for a, b in zip(J, J0)]
+    dot = lambda a, b: sum(x * y for x, y in zip(a, b))
+    if not subtracted:
+        E = [-x + eta * y for x, y in zip(op["cross"](v, B), J1)]                        # eq (5), d_i = 0
+        Krho = -op["div"]([rho * x for x in v]) + D * op["lap"](m["rho1"])             # eq (1)
+        Kp = -dot(v, op["grad"](p)) - G * p * op["div"](v) + kap * op["lap"](m["p1"])    # eq (2)
+        JxB = op["cross"](J, B)
+        gp = op["grad"](p)
+        vl = op["veclap"](v1)
+        Kv = [-a + (b - c) / rho + nu * d for a, b, c, d in zip(op["adv"](v, v), JxB, gp, vl)]   # eq (3)
+        KB = [-x for x in op["curl"](E)]                                                 # eq (4)
+    else:
+        E1 = [-x + y + eta * z for x, y, z in zip(op["cross"](v, B), op["cross"](v0, B0), J1)]
+        Krho = -op["div"]([rho * a + m["rho1"] * b for a, b in zip(v1, v0)]) + D * op["lap"](m["rho1"])   # eq (11)
+        Kp = (-dot(v1, op["grad"](p)) - dot(v0, op["grad"](m["p1"]))
+              - G * (p * op["div"](v1) + m["p1"] * op["div"](v0)) + kap * op["lap"](m["p1"]))              # eq (12)
+        t1, t2, t3 = op["adv"](v, v1), op["adv"](v1, v0), op["adv"](v0, v0)
+        f1, f2, gp1 = op["cross"](J1, B), op["cross"](J0, B1), op["grad"](m["p1"])
+        vl = op["veclap"](v1)
+        Kv = [-(a + b + m["rho1"] * c / rho) + (d + e - f) / rho + nu * g
+              for a, b, c, d, e, f, g in zip(t1, t2, t3, f1, f2, gp1, vl)]                                  # eq (13)
+        KB = [-x for x in op["curl"](E1)]                                                                  # eq (14)
+    return [Krho, Kp] + Kv + KB
+
+
+@pytest.mark.parametrize("equilibrium_exact", [True, False])
+def test_P3b_full_rhs_converges_at_4th_order_to_the_continuous_equations(equilibrium_exact):
+    sp, syms, op = _sympy_ops()
+    m = _manufactured(sp, syms, equilibrium_exact)
+    par = (5.0 / 3.0, 0.05, 0.04, 0.03, 0.02)
+    # with an exact equilibrium the ORIGINAL eqs (1)-(4) are the target; otherwise eqs (11)-(14)
+    target = _continuous_rhs(sp, syms, op, m, par, subtracted=not equilibrium_exact)
+    if equilibrium_exact:
+        # and the two continuous forms agree (checked numerically at a few points)
+        other = _continuous_rhs(sp, syms, op, m, par, subtracted=True)
+        pts = (np.array([2.3, 3.1]), np.array([0.4, 2.0]), np.array([-0.2, 0.5]))
+        for a, b in zip(target, other):
+            fa = sp.lambdify(syms, a, "numpy")(*pts)
+            fb = sp.lambdify(syms, b, "numpy")(*pts)
+            assert np.allclose(fa, fb, rtol=1e-11, atol=1e-13)
+    errs = []
+    for n in (2, 4):
+        o, RR, P, ZZ = make(nR=20 * n + 1, nphi=16 * n, nZ=16 * n + 1, gamma=par[0], eta=par[1], nu=par[2], D=par[3],
+                            kappa=par[4])
+        ev = lambda e: _lamb(sp, syms, e)(RR, P, ZZ)
+        U0 = np.stack([ev(m["rho0"]), ev(m["p0"])] + [ev(x) for x in m["v0"]] + [ev(x) for x in m["B0"]])
+        U1 = np.stack([ev(m["rho1"]), ev(m["p1"])] + [ev(x) for x in m["v1"]] + [ev(x) for x in m["B1"]])
+        o.set_equilibrium(U0[:, 0])
+        K = o.rhs_of(U0 + U1)
+        Kx = np.stack([ev(x) for x in target])
+        # rows next to the frozen layers see J1 = 0 on the boundary layers (reading R5) inside curl(eta J1):
+        # compare on the deep interior, where every stencil stays on interior nodes
+        errs.append([np.abs(deep(K[f] - Kx[f])).max() for f in range(8)])
+        scale = [np.abs(Kx[f]).max() for f in range(8)]
+    for f in range(8):
+        assert errs[1][f] < 2e-3 * scale[f], (f, errs[1][f], scale[f])
+        assert 3.5 < _order(errs[0][f], errs[1][f]) < 4.7, (f, errs[0][f], errs[1][f])
+
+
+# ----------------------------------------------------------------------------------------------- P4
+def test_P4_divB_stays_at_roundoff_over_rk4_steps():
+    prob = inputs.make_custom_problem(28, 12, 26)
+    cfg = prob.cfg
+    o = orc.Oracle(cfg.nR, cfg.nphi, cfg.nZ, cfg.Rmin, cfg.Rmax, cfg.Zmin, cfg.Zmax, eta=1e-3, nu=1e-3, D=1e-3,
+                   kappa=1e-3, dt=prob.dt)
+    o.set_equilibrium(prob.U0)
+    R, Z, phi = inputs.grid_axes(cfg)
+    P, ZZ, RR = np.meshgrid(phi, Z, R, indexing="ij")
+    env = inputs.envelope(cfg)[None]
+    A = 1e-3 * np.stack([env * np.sin(2 * RR + P) * np.cos(ZZ), env * np.cos(RR - 2 * P + ZZ), env * np.sin(3 * ZZ + P)])
+    U = prob.U.copy()
+    U[5:8] = np.repeat(prob.U0[5:8, None], cfg.nphi, axis=1) + o.vector_op("curl_c", A)
+    d0 = o.divB(U)
+    # the reference field itself is only divergence-free to truncation error: follow div_c(B) - div_c(B at t=0)
+    o.set_state(U)
+    scale = np.abs(U[5:8] - prob.U0[5:8, None]).max() / min(o.L and (cfg.Rmax - cfg.Rmin) / (cfg.nR - 1), 1.0)
+    for _ in range(4):
+        o.step(5)
+        d = o.divB(o.get_state())
+        assert np.abs(deep(d - d0)).max() < 1e-12 * max(scale, 1.0)
+    # and a field that is a pure discrete curl has div_c = 0 outright
+    U[5:8] = o.vector_op("curl_c", A)
+    assert np.abs(deep(o.divB(U))).max() < 1e-13 * np.abs(U[5:8]).max() / ((cfg.Rmax - cfg.Rmin) / (cfg.nR - 1))
+    # the state must really have moved
+    assert np.abs(o.get_state()[5:8] - prob.U[5:8]).max() > 1e-8
+
+
+# ----------------------------------------------------------------------------------------------- P5
+def test_P5_rigid_rotation():
+    o, RR, P, ZZ = make()
+    Om = 0.37
+    v = np.stack([0 * RR, Om * RR, 0 * RR])
+    L = o.vector_op("vector_laplacian", v)
+    assert np.abs(L).max() < 1e-12                     # the component-wise Laplacian would give Om/R in L_phi
+    adv = o.vector_op("advect_vector", np.concatenate([v, v]))
+    assert np.abs(interior(adv[0] + Om ** 2 * RR)).max() < 1e-13
+    assert np.abs(adv[1:]).max() < 1e-13
+
+
+# ----------------------------------------------------------------------------------------------- P6
+def _np_ops(nR, nphi, nZ, Rmin, Rmax, Zmin, Zmax):
+    dR, dZ, dP = (Rmax - Rmin) / (nR - 1), (Zmax - Zmin) / (nZ - 1), 2 * np.pi / nphi
+    Rv = (Rmin + np.arange(nR) * dR)[None, None, :]
+    ax = {"R": (2, dR), "Z": (1, dZ), "P": (0, dP)}
+
+    def d1(f, a):
+        axis, h = ax[a]
+        return (8 * (np.roll(f, -1, axis) - np.roll(f, 1, axis)) - (np.roll(f, -2, axis) - np.roll(f, 2, axis))) / (12 * h)
+
+    def d2(f, a):
+        axis, h = ax[a]
+        return (-np.roll(f, -2, axis) + 16 * np.roll(f, -1, axis) - 30 * f + 16 * np.roll(f, 1, axis) - np.roll(f, 2, axis)) / (12 * h * h)
+
+    return Rv, d1, d2
+
+
+def direct_eqs_1_to_4(U, grid, gamma, eta, nu, D, kappa):
+    """Eqs (1)-(6) of PAPER.md (L67-79) with rho0 = p0 = v0 = J0 = 0, written independently with numpy rolls."""
+    nR, nphi, nZ, Rmin, Rmax, Zmin, Zmax = grid
+    R, d1, d2 = _np_ops(*grid)
+    rho, p, vR, vP, vZ, BR, BP, BZ = U
+    mask = np.zeros_like(rho)
+    mask[:, 2:-2, 2:-2] = 1.0
+    JR = (d1(BZ, "P") / R - d1(BP, "Z")) * mask
+    JP = (d1(BR, "Z") - d1(BZ, "R")) * mask
+    JZ = (d1(R * BP, "R") / R - d1(BR, "P") / R) * mask
+    ER = -(vP * BZ - vZ * BP) + eta * JR
+    EP = -(vZ * BR - vR * BZ) + eta * JP
+    EZ = -(vR * BP - vP * BR) + eta * JZ
+    advs = lambda f: vR * d1(f, "R") + vP * d1(f, "P") / R + vZ * d1(f, "Z")
+    divv = d1(vR, "R") + vR / R + d1(vP, "P") / R + d1(vZ, "Z")
+    lap = lambda f: d2(f, "R") + d1(f, "R") / R + d2(f, "P") / R ** 2 + d2(f, "Z")
+    K = np.zeros_like(U)
+    K[0] = -advs(rho) - rho * divv + D * lap(rho)
+    K[1] = -advs(p) - gamma * p * divv + kappa * lap(p)
+    K[2] = -(advs(vR) - vP * vP / R) + (JP * BZ - JZ * BP - d1(p, "R")) / rho + nu * (lap(vR) - vR / R ** 2 - 2 * d1(vP, "P") / R ** 2)
+    K[3] = -(advs(vP) + vP * vR / R) + (JZ * BR - JR * BZ - d1(p, "P") / R) / rho + nu * (lap(vP) - vP / R ** 2 + 2 * d1(vR, "P") / R ** 2)
+    K[4] = -advs(vZ) + (JR * BP - JP * BR - d1(p, "Z")) / rho + nu * lap(vZ)
+    K[5] = -(d1(EZ, "P") / R - d1(EP, "Z"))
+    K[6] = -(d1(ER, "Z") - d1(EZ, "R"))
+    K[7] = -(d1(R * EP, "R") / R - d1(ER, "P") / R)
+    return K * mask
+
+
+def test_P6_zero_reference_state_reduces_to_eqs_1_to_4():
+    prob = inputs.make_custom_problem(26, 12, 22, amplitude_scale=300.0)     # 3 % perturbations: nonlinear terms matter
+    cfg = prob.cfg
+    par = dict(gamma=5.0 / 3.0, eta=2e-3, nu=3e-3, D=4e-3, kappa=5e-3)
+    o = orc.Oracle(cfg.nR, cfg.nphi, cfg.nZ, cfg.Rmin, cfg.Rmax, cfg.Zmin, cfg.Zmax, **par)
+    o.set_equilibrium(None)
+    K = o.rhs_of(prob.U)
+    Kd = direct_eqs_1_to_4(prob.U, (cfg.nR, cfg.nphi, cfg.nZ, cfg.Rmin, cfg.Rmax, cfg.Zmin, cfg.Zmax), **par)
+    for f in range(8):
+        s = np.abs(Kd[f]).max()
+        assert s > 1e-4
+        assert np.abs(K[f] - Kd[f]).max() < 2e-13 * max(s, 1.0), (f, np.abs(K[f] - Kd[f]).max(), s)
+    assert np.all(K[:, :, :2, :] == 0) and np.all(K[:, :, :, -2:] == 0)
+
+
+# ----------------------------------------------------------------------------------------------- P7
+@pytest.mark.parametrize("nmode", [1, 3])
+def test_P7_alfven_response_has_the_stencils_modified_wavenumber(nmode):
+    nphi, c, eps = 16, 2.0, 1e-3
+    o, RR, P, ZZ = make(nR=18, nphi=nphi, nZ=14, Rmin=99.0, Rmax=101.0, phi_extent=2 * np.pi / 100)
+    Lphi = 2 * np.pi / 100
+    h = Lphi / nphi
+    kphys = 2 * np.pi * nmode / Lphi
+    kstar = (8 * np.sin(kphys * h) - np.sin(2 * kphys * h)) / (6 * h)
+    U = np.zeros((8,) + RR.shape)
+    U[0], U[1], U[6] = 1.0, 0.3, c / RR
+    Ua = U.copy()
+    Ua[4] = eps * np.sin(kphys * P)
+    K = o.rhs_of(Ua)
+    exp = (c / RR) / RR * kstar * eps * np.cos(kphys * P)
+    assert np.abs(interior(K[7] - exp)).max() < 1e-10 * np.abs(exp).max()
+    Ub = U.copy()
+    Ub[7] = eps * np.sin(kphys * P)
+    K = o.rhs_of(Ub)
+    assert np.abs(interior(K[4] - exp)).max() < 1e-10 * np.abs(exp).max()       # rho = 1
+    # => omega^2 = kstar^2 B_phi^2 / (rho R^2): the discrete Alfven frequency of the near-slab limit
+
+
+# ----------------------------------------------------------------------------------------------- P8
+def test_P8_rk4_is_4th_order_on_linear_ode():
+    lam = np.array([-1.0, 0.5, -0.3])
+    u0 = np.array([1.0, 2.0, -1.5])
+    errs = []
+    for n in (8, 16, 32):
+        u = orc.rk4(u0, 1.0 / n, n, lambda u: lam * u)
+        errs.append(np.abs(u - u0 * np.exp(lam)).max())
+    assert 15.0 < errs[0] / errs[1] < 17.5 and 15.0 < errs[1] / errs[2] < 17.5
+    # one step reproduces the degree-4 Taylor polynomial of exp exactly
+    z = 0.3
+    u = orc.rk4(np.array([1.0]), z, 1, lambda u: u)
+    assert abs(u[0] - (1 + z + z ** 2 / 2 + z ** 3 / 6 + z ** 4 / 24)) < 1e-15
+
+
+def test_P8b_mhd_stepper_is_4th_order_in_dt():
+    prob = inputs.make_custom_problem(20, 8, 18, amplitude_scale=100.0)
+    cfg = prob.cfg
+    T = 16 * prob.dt
+    sols = []
+    for n in (16, 32, 64):
+        o = orc.Oracle(cfg.nR, cfg.nphi, cfg.nZ, cfg.Rmin, cfg.Rmax, cfg.Zmin, cfg.Zmax, eta=1e-3, nu=1e-3, D=1e-3,
+                       kappa=1e-3, dt=T / n)
+        o.set_equilibrium(prob.U0)
+        o.set_state(prob.U)
+        o.step(n)
+        assert o.step_count == n and abs(o.time - T) < 1e-14
+        sols.append(o.get_state())
+    e1 = np.abs(sols[0] - sols[1]).max()
+    e2 = np.abs(sols[1] - sols[2]).max()
+    assert 12.0 < e1 / e2 < 20.0, (e1, e2)
+    # frozen boundary layers
+    assert np.array_equal(sols[2][:, :, :2], prob.U[:, :, :2]) and np.array_equal(sols[2][..., -2:], prob.U[..., -2:])
+
+
+# ----------------------------------------------------------------------------------------------- P10, P11
+def test_P10_setdt_closed_form():
+    o, RR, P, ZZ = make(nR=24, nphi=16, nZ=20, gamma=5.0 / 3.0)
+    U = np.zeros((8,) + RR.shape)
+    U[0], U[1], U[2], U[3], U[4], U[6] = 2.0, 0.3, 0.1, -0.2, 0.05, 1.5
+    o.set_state(U)
+    c = np.sqrt(5.0 / 3.0 * 0.3 / 2.0 + 1.5 ** 2 / 2.0)
+    dR, dZ, dphi = 2.0 / 23, 2.0 / 19, 2 * np.pi / 16
+    Rmin_int = 2.0 + 2 * dR
+    exp = 0.4 * min(dR / (0.1 + c), dZ / (0.05 + c), Rmin_int * dphi / (0.2 + c))
+    assert abs(o.setdt(0.4) - exp) < 1e-14
+    prob = inputs.make_problem(1)
+    cfg = prob.cfg
+    o2 = orc.Oracle(cfg.nR, cfg.nphi, cfg.nZ, cfg.Rmin, cfg.Rmax, cfg.Zmin, cfg.Zmax, gamma=cfg.gamma)
+    o2.set_state(prob.U)
+    assert abs(o2.setdt(cfg.cfl) - prob.dt) < 1e-12 * prob.dt     # the input recipe's dt is Fig. 4's
+
+
+def test_P11_diagnostics_closed_forms():
+    o, RR, P, ZZ = make(nR=24, nphi=16, nZ=20)
+    dR, dZ, dphi = 2.0 / 23, 2.0 / 19, 2 * np.pi / 16
+    U = np.zeros((8,) + RR.shape)
+    U[0], U[2], U[3], U[4] = 2.0, 0.1, -0.2, 0.05
+    a, b = 0.3, -0.1
+    U[5] = 0.7 + a * np.cos(P) + b * np.sin(P) + 0.05 * np.cos(2 * P)
+    U[6] = 1.5
+    U0 = np.zeros((8, 20, 24))
+    U0[5], U0[6] = 0.7, 1.5
+    o.set_equilibrium(U0)
+    o.set_state(U)
+    d = o.diagnostics()
+    Ri = 2.0 + np.arange(2, 22) * dR
+    vol = Ri.sum() * (20 - 4) * 16 * dR * dZ * dphi
+    assert abs(d["kinetic"] - 0.5 * 2.0 * (0.01 + 0.04 + 0.0025) * vol) < 1e-13
+    area = Ri.sum() * (20 - 4) * dR * dZ
+    # sum_j over a full period: <(0.7 + a cos + b sin + .05 cos2)^2> = .49 + (a^2+b^2)/2 + .05^2/2
+    me = 0.5 * (0.49 + (a * a + b * b) / 2 + 0.05 ** 2 / 2 + 1.5 ** 2) * area * 2 * np.pi
+    assert abs(d["magnetic"] - me) < 1e-12
+    assert abs(d["magnetic_pert"] - 0.5 * ((a * a + b * b) / 2 + 0.05 ** 2 / 2) * area * 2 * np.pi) < 1e-13
+    assert abs(d["magnetic_n1"] - 0.25 * (a * a + b * b) * area * 2 * np.pi) < 1e-13
+    # div_c of B = (f(phi), const, 0) is f/R at every node
+    assert abs(d["max_divB"] - np.abs(deep(U[5] / RR)).max()) < 1e-12
