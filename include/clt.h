@@ -1,0 +1,162 @@
+/*
+ * clt.h -- C ABI of libclt: the B200-native (sm_100a, FP64) hot path of CLTx, arxiv 1812.00525.
+ *
+ * What the library computes (citations are PAPER.md line numbers / equation numbers):
+ *   the full resistive-MHD right-hand side in the equilibrium-subtracted form, eqs (11)-(14)
+ *   [L105-115], with J = curl B, eq (6) [L79], and E = -v x B + eta (J - J0), eq (5) [L77] with
+ *   d_i = 0, for the 8 fields rho, p, v_R, v_phi, v_Z, B_R, B_phi, B_Z [L139, L191-196] on a uniform
+ *   cylindrical (R, phi, Z) grid [L121-125] with 4th-order central finite differences in all three
+ *   directions [L125], advanced by the classical 4th-order Runge-Kutta scheme [L125, L139]
+ *   ("DERIVATIVES", "J, E", "RIGHT HANDS OF EQUATIONS", "STEP ON" modules of Fig. 2 [L139-141]),
+ *   with fixed values on two node layers per R/Z side [L123, L187-189] and phi periodic, plus the
+ *   DIAGN-type reductions (kinetic / magnetic energy [L430], max |div B|) and the SETDT CFL
+ *   time step of Fig. 4 [L180-215].  The exact discrete definitions are in DESIGN.md section 3.
+ *
+ * Conventions
+ *   - Every function returns CLT_OK (0) or a negative clt_status.  No exceptions, no aborts, nothing
+ *     is printed.  clt_strerror() gives a static string for a code.
+ *   - All floating-point data is IEEE binary64.  Array arguments may be HOST or DEVICE pointers; the
+ *     library finds out with cudaPointerGetAttributes.  The caller owns every buffer it passes; the
+ *     library copies in or out and keeps no pointer to it after the call returns, with one
+ *     exception: the workspace given to clt_create(), which the context sub-allocates and the
+ *     caller must keep alive (and not touch) until clt_destroy().
+ *   - User-visible array layout (dense, C order, R fastest -- the C image of CLTx's X(JX,JZ,JY,M)):
+ *        state / dUdt : double[8][nphi][nZ][nR]   fields rho, p, v_R, v_phi, v_Z, B_R, B_phi, B_Z
+ *        equilibrium  : double[8][nZ][nR]          axisymmetric
+ *        vector field : double[3][nphi][nZ][nR]    components R, phi, Z
+ *     Inside the workspace the library uses its own padded layout.
+ *   - One context = one CUDA stream (given at creation; NULL = the legacy default stream).  All work
+ *     is enqueued on that stream.  Calls are asynchronous with respect to the host except where
+ *     noted (a host destination pointer, or clt_diagnostics / clt_suggest_dt, which return scalars).
+ *     A context is not thread-safe.
+ *   - Call order: clt_create -> [clt_set_equilibrium] -> clt_set_state -> { clt_rhs | clt_step |
+ *     clt_curl_J1 | clt_diagnostics | clt_suggest_dt | clt_get_state | clt_set_dt }*  -> clt_destroy.
+ *     A call out of order returns CLT_ESTATE.
+ *   - There is no CPU fallback: without a usable CUDA device every compute entry point fails with
+ *     CLT_ECUDA.
+ */
+#ifndef CLT_H
+#define CLT_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    CLT_OK = 0,
+    CLT_EINVAL = -1,     /* bad argument, shape or parameter                         */
+    CLT_ENOMEM = -2,     /* workspace too small / misaligned                         */
+    CLT_ESTATE = -3,     /* call out of order (e.g. clt_step before clt_set_state)   */
+    CLT_ECUDA = -4,      /* a CUDA runtime error (sticky: see clt_last_cuda_error)   */
+    CLT_ENONFINITE = -5  /* clt_diagnostics found a non-finite sum                   */
+} clt_status;
+
+typedef struct clt_ctx clt_ctx;  /* opaque */
+
+/* Grid [L121-125].  Node counts include the two fixed layers per R/Z side, and the box edge is a
+ * node:  R_i = Rmin + i*(Rmax-Rmin)/(nR-1), i = 0..nR-1 (computed on the host in plain double
+ * arithmetic, no FMA), Z_k likewise; phi_j = j*dphi, dphi = L/nphi, L = phi_extent (0 means 2*pi),
+ * periodic.  Requirements: nR >= 9, nZ >= 9, nphi >= 5, Rmin > 0, Rmax > Rmin, Zmax > Zmin.     */
+typedef struct {
+    int32_t nR, nphi, nZ;
+    double Rmin, Rmax, Zmin, Zmax;
+    double phi_extent;
+} clt_grid;
+
+/* Physics and run parameters [L67-81]: ratio of specific heats Gamma, and the uniform dissipation
+ * coefficients eta (resistivity), nu (viscosity), D (density diffusion), kappa (heat conduction).
+ * dt > 0 is the fixed RK4 time step used by clt_step.  cfl is only used by clt_suggest_dt when its
+ * cfl argument is <= 0.  flags: reserved, must be 0.                                             */
+typedef struct {
+    double gamma, eta, nu, D, kappa;
+    double dt;
+    double cfl;
+    uint32_t flags;
+} clt_params;
+
+/* Diagnostics [L139, L149, L430]; sums run over interior nodes with weight R_i dR dphi dZ:
+ *   kinetic       = sum 1/2 rho |v|^2          magnetic      = sum 1/2 |B|^2
+ *   magnetic_pert = sum 1/2 |B - B0|^2         magnetic_n1   = energy of the n = 1 toroidal Fourier
+ *   harmonic of B - B0;  max_divB = max over the deep interior (i in [4,nR-5], k in [4,nZ-5]) of
+ *   |div_c B|, the conservative discrete divergence that the discrete curl annihilates.          */
+typedef struct {
+    double kinetic, magnetic, magnetic_pert, magnetic_n1, max_divB;
+    int64_t step;   /* RK4 steps taken since clt_set_state */
+    double time;    /* sum of the dt's of those steps      */
+} clt_diag;
+
+/* Device bytes clt_create() needs for this grid (35 padded fields + equilibrium tables + reduction
+ * scratch).  Returns 0 for an invalid grid.                                                      */
+size_t clt_workspace_bytes(const clt_grid *grid);
+
+/* Creates a context.  d_workspace: DEVICE memory, at least clt_workspace_bytes(grid) bytes, 256-byte
+ * aligned, owned by the caller (e.g. a torch tensor), zero-initialised or not.  cuda_stream: a
+ * cudaStream_t (NULL = default stream).  The equilibrium starts as all-zero.
+ * Errors: CLT_EINVAL (NULL pointers, bad grid, gamma/dt not finite, negative coefficients, flags),
+ * CLT_ENOMEM (bytes too small, pointer misaligned or not device memory), CLT_ECUDA.               */
+int clt_create(const clt_grid *grid, const clt_params *params, void *d_workspace, size_t bytes,
+               void *cuda_stream, clt_ctx **out);
+
+/* Releases the context (not the workspace).  Synchronises the stream.  NULL is allowed.           */
+int clt_destroy(clt_ctx *ctx);
+
+/* Sets the axisymmetric reference state U0[8][nZ][nR] of eqs (11)-(14) (host or device pointer;
+ * NULL = all zero, which makes the path evaluate eqs (1)-(4) directly).  Also computes J0 = curl B0
+ * and the other time-independent tables.  Must be called before clt_set_state (it invalidates the
+ * state: a later compute call returns CLT_ESTATE until clt_set_state is called again).            */
+int clt_set_equilibrium(clt_ctx *ctx, const double *U0);
+
+/* Sets the state U[8][nphi][nZ][nR] (host or device pointer), resets step/time to 0 and freezes the
+ * two boundary node layers per R/Z side at these values for all later steps [L123, L187-189].     */
+int clt_set_state(clt_ctx *ctx, const double *U);
+
+/* Copies the current state out (host or device pointer).  Synchronous if U is host memory.        */
+int clt_get_state(clt_ctx *ctx, double *U);
+
+/* dUdt[8][nphi][nZ][nR] = right-hand side of eqs (11)-(14) at the current state; exactly 0 on the
+ * boundary layers.  Does not change the state.  Synchronous if dUdt is host memory.               */
+int clt_rhs(clt_ctx *ctx, double *dUdt);
+
+/* J1[3][nphi][nZ][nR] = curl(B - B0) of the current state (eq (6)); 0 on the boundary layers.     */
+int clt_curl_J1(clt_ctx *ctx, double *J1);
+
+/* n >= 0 classical RK4 steps with the fixed time step params.dt (or the last clt_set_dt value).
+ * Asynchronous.                                                                                  */
+int clt_step(clt_ctx *ctx, int n);
+
+/* Changes the fixed time step (dt > 0, finite).                                                  */
+int clt_set_dt(clt_ctx *ctx, double dt);
+
+/* Reductions over the current state; synchronises the stream.  CLT_ENONFINITE if a sum is not
+ * finite (out is still filled).                                                                  */
+int clt_diagnostics(clt_ctx *ctx, clt_diag *out);
+
+/* SETDT of Fig. 4 [L180-215]: dt = min(100, min over interior nodes of min(dR/(|v_R|+c),
+ * dZ/(|v_Z|+c), R dphi/(|v_phi|+c)) * cfl), c = sqrt(|Gamma p/rho + |B|^2/rho|).  cfl <= 0 means
+ * params.cfl.  Synchronises the stream.  Does not change the context's dt.                        */
+int clt_suggest_dt(clt_ctx *ctx, double cfl, double *dt_out);
+
+/* Launch-shape knobs for measurement (all optional; 0 = library default): tile height in Z of the
+ * fused RHS kernel, number of phi chunks per tile, use of a CUDA graph for clt_step.              */
+int clt_set_tuning(clt_ctx *ctx, int tile_z, int phi_chunks, int use_graph);
+
+/* Number of kernels launched by this context so far (for bench.py's gpu_launches).               */
+int64_t clt_launch_count(const clt_ctx *ctx);
+
+/* The stream-ordered device time of the kernels is measured by the caller with CUDA events on the
+ * context's stream; the library offers the stream back for that.                                 */
+void *clt_stream(const clt_ctx *ctx);
+
+const char *clt_strerror(int code);
+/* Text of the last CUDA error seen by this context ("" if none).                                 */
+const char *clt_last_cuda_error(const clt_ctx *ctx);
+/* Library version string, e.g. "clt-b200 0.1 (sm_100a)".                                         */
+const char *clt_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CLT_H */

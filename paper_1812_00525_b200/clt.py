@@ -1,0 +1,214 @@
+"""Thin ctypes binding of libclt.so (include/clt.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of ``csrc/``; torch is used for device memory
+(the workspace tensor) and streams.  There is no CPU fallback: if ``libclt.so`` is missing or cannot
+be loaded, importing/using this module raises.  Never imports ``oracle``.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libclt.so")
+
+CLT_OK, CLT_EINVAL, CLT_ENOMEM, CLT_ESTATE, CLT_ECUDA, CLT_ENONFINITE = 0, -1, -2, -3, -4, -5
+
+
+class clt_grid(ctypes.Structure):
+    _fields_ = [("nR", ctypes.c_int32), ("nphi", ctypes.c_int32), ("nZ", ctypes.c_int32),
+                ("Rmin", ctypes.c_double), ("Rmax", ctypes.c_double), ("Zmin", ctypes.c_double),
+                ("Zmax", ctypes.c_double), ("phi_extent", ctypes.c_double)]
+
+
+class clt_params(ctypes.Structure):
+    _fields_ = [("gamma", ctypes.c_double), ("eta", ctypes.c_double), ("nu", ctypes.c_double),
+                ("D", ctypes.c_double), ("kappa", ctypes.c_double), ("dt", ctypes.c_double),
+                ("cfl", ctypes.c_double), ("flags", ctypes.c_uint32)]
+
+
+class clt_diag(ctypes.Structure):
+    _fields_ = [("kinetic", ctypes.c_double), ("magnetic", ctypes.c_double), ("magnetic_pert", ctypes.c_double),
+                ("magnetic_n1", ctypes.c_double), ("max_divB", ctypes.c_double), ("step", ctypes.c_int64),
+                ("time", ctypes.c_double)]
+
+
+# every symbol include/clt.h declares
+EXPORTS = ["clt_workspace_bytes", "clt_create", "clt_destroy", "clt_set_equilibrium", "clt_set_state", "clt_get_state",
+           "clt_rhs", "clt_curl_J1", "clt_step", "clt_set_dt", "clt_diagnostics", "clt_suggest_dt", "clt_set_tuning",
+           "clt_launch_count", "clt_stream", "clt_strerror", "clt_last_cuda_error", "clt_version"]
+
+_lib = None
+
+
+class CltError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"libclt error {code}: {msg}")
+        self.code = code
+
+
+def load():
+    """Loads libclt.so (loudly).  Building is a separate, explicit step: ``python -m paper_1812_00525_b200.build``."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} not found: build it with `python -m paper_1812_00525_b200.build` "
+                          "(there is no CPU fallback)")
+    L = ctypes.CDLL(LIB_PATH)
+    vp, i, d = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
+    L.clt_workspace_bytes.restype = ctypes.c_size_t
+    L.clt_workspace_bytes.argtypes = [ctypes.POINTER(clt_grid)]
+    L.clt_create.restype = i
+    L.clt_create.argtypes = [ctypes.POINTER(clt_grid), ctypes.POINTER(clt_params), vp, ctypes.c_size_t, vp,
+                             ctypes.POINTER(vp)]
+    for name in ("clt_destroy",):
+        getattr(L, name).restype = i
+        getattr(L, name).argtypes = [vp]
+    for name in ("clt_set_equilibrium", "clt_set_state", "clt_get_state", "clt_rhs", "clt_curl_J1"):
+        getattr(L, name).restype = i
+        getattr(L, name).argtypes = [vp, vp]
+    L.clt_step.restype = i
+    L.clt_step.argtypes = [vp, i]
+    L.clt_set_dt.restype = i
+    L.clt_set_dt.argtypes = [vp, d]
+    L.clt_diagnostics.restype = i
+    L.clt_diagnostics.argtypes = [vp, ctypes.POINTER(clt_diag)]
+    L.clt_suggest_dt.restype = i
+    L.clt_suggest_dt.argtypes = [vp, d, ctypes.POINTER(d)]
+    L.clt_set_tuning.restype = i
+    L.clt_set_tuning.argtypes = [vp, i, i, i]
+    L.clt_launch_count.restype = ctypes.c_int64
+    L.clt_launch_count.argtypes = [vp]
+    L.clt_stream.restype = vp
+    L.clt_stream.argtypes = [vp]
+    L.clt_strerror.restype = ctypes.c_char_p
+    L.clt_strerror.argtypes = [i]
+    L.clt_last_cuda_error.restype = ctypes.c_char_p
+    L.clt_last_cuda_error.argtypes = [vp]
+    L.clt_version.restype = ctypes.c_char_p
+    L.clt_version.argtypes = []
+    _lib = L
+    return L
+
+
+def _addr(a):
+    """Address of a buffer: torch tensor (host or device), numpy array, or None."""
+    if a is None:
+        return None
+    if isinstance(a, np.ndarray):
+        if a.dtype != np.float64 or not a.flags["C_CONTIGUOUS"]:
+            raise TypeError("numpy buffers must be C-contiguous float64")
+        return a.ctypes.data
+    import torch
+    if isinstance(a, torch.Tensor):
+        if a.dtype != torch.float64 or not a.is_contiguous():
+            raise TypeError("torch buffers must be contiguous float64")
+        return a.data_ptr()
+    raise TypeError(type(a))
+
+
+class Clt:
+    """One libclt context.  Method names and semantics are those of include/clt.h."""
+
+    def __init__(self, nR, nphi, nZ, Rmin, Rmax, Zmin, Zmax, phi_extent=0.0, gamma=5.0 / 3.0, eta=0.0, nu=0.0, D=0.0,
+                 kappa=0.0, dt=0.0, cfl=0.5, device="cuda:0", stream=None):
+        import torch
+        self.L = load()
+        if not torch.cuda.is_available():
+            raise RuntimeError("libclt needs a CUDA device (no CPU fallback)")
+        self.device = torch.device(device)
+        self.grid = clt_grid(nR, nphi, nZ, Rmin, Rmax, Zmin, Zmax, phi_extent)
+        self.params = clt_params(gamma, eta, nu, D, kappa, dt, cfl, 0)
+        self.shape = (8, nphi, nZ, nR)
+        nbytes = self.L.clt_workspace_bytes(ctypes.byref(self.grid))
+        if nbytes == 0:
+            raise CltError(CLT_EINVAL, "invalid grid")
+        self.workspace_bytes = nbytes
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)   # caching allocator: 512-B aligned
+            self.torch_stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            h = ctypes.c_void_p()
+            rc = self.L.clt_create(ctypes.byref(self.grid), ctypes.byref(self.params), self.workspace.data_ptr(), nbytes,
+                                   ctypes.c_void_p(self.torch_stream.cuda_stream), ctypes.byref(h))
+        self.h = h
+        if rc != 0:
+            self.h = None
+            raise CltError(rc, self.L.clt_strerror(rc).decode())
+
+    @classmethod
+    def from_config(cls, cfg, dt, **kw):
+        return cls(cfg.nR, cfg.nphi, cfg.nZ, cfg.Rmin, cfg.Rmax, cfg.Zmin, cfg.Zmax, cfg.phi_extent, cfg.gamma, cfg.eta,
+                   cfg.nu, cfg.D, cfg.kappa, dt, cfg.cfl, **kw)
+
+    def _ck(self, rc):
+        if rc != 0:
+            msg = self.L.clt_strerror(rc).decode()
+            if rc == CLT_ECUDA and self.h:
+                msg += " -- " + self.L.clt_last_cuda_error(self.h).decode()
+            raise CltError(rc, msg)
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.L.clt_destroy(self.h)
+            self.h = None
+            self.workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_equilibrium(self, U0):
+        self._ck(self.L.clt_set_equilibrium(self.h, _addr(U0)))
+
+    def set_state(self, U):
+        self._ck(self.L.clt_set_state(self.h, _addr(U)))
+
+    def get_state(self, out=None):
+        if out is None:
+            out = np.empty(self.shape)
+        self._ck(self.L.clt_get_state(self.h, _addr(out)))
+        return out
+
+    def rhs(self, out=None):
+        if out is None:
+            out = np.empty(self.shape)
+        self._ck(self.L.clt_rhs(self.h, _addr(out)))
+        return out
+
+    def curl_J1(self, out=None):
+        if out is None:
+            out = np.empty((3,) + self.shape[1:])
+        self._ck(self.L.clt_curl_J1(self.h, _addr(out)))
+        return out
+
+    def step(self, n=1):
+        self._ck(self.L.clt_step(self.h, int(n)))
+
+    def set_dt(self, dt):
+        self._ck(self.L.clt_set_dt(self.h, float(dt)))
+
+    def diagnostics(self):
+        d = clt_diag()
+        self._ck(self.L.clt_diagnostics(self.h, ctypes.byref(d)))
+        return {k: getattr(d, k) for k, _ in clt_diag._fields_}
+
+    def suggest_dt(self, cfl=0.0):
+        out = ctypes.c_double()
+        self._ck(self.L.clt_suggest_dt(self.h, float(cfl), ctypes.byref(out)))
+        return out.value
+
+    def set_tuning(self, tile_z=0, phi_chunks=0, use_graph=0):
+        self._ck(self.L.clt_set_tuning(self.h, int(tile_z), int(phi_chunks), int(use_graph)))
+
+    @property
+    def launch_count(self):
+        return int(self.L.clt_launch_count(self.h))
+
+
+def version():
+    return load().clt_version().decode()

@@ -1,0 +1,475 @@
+// clt_api.cu -- the C ABI of libclt (include/clt.h): context, workspace carving, stage scheduling.
+// Product code: no CPU fallback, shares nothing with oracle/.
+#include "clt.h"
+#include "clt_internal.h"
+
+#include <math.h>
+#include <new>
+#include <stdio.h>
+#include <string.h>
+#include <vector>
+
+using namespace clt;
+
+struct clt_ctx {
+    clt_grid grid;
+    clt_params par;
+    Layout L;
+    Phys ph;
+    cudaStream_t stream;
+    // workspace carving (device)
+    double *Un, *acc, *Ua, *Ub, *J1, *tab, *Rtab, *invRtab, *cs, *partial, *result;
+    int nblocks_diag;
+    bool has_state, has_v0;
+    int64_t step;
+    double time;
+    double dt;
+    int64_t launches;
+    int tile_z, phi_chunks, use_graph;
+    cudaGraphExec_t graph_exec;
+    double graph_dt;
+    int graph_tile_z, graph_chunks;
+    bool graph_v0;
+    char cuda_err[256];
+};
+
+namespace {
+
+constexpr size_t ALIGN = 128;   // every field and table base is 128-byte aligned
+inline size_t align_up(size_t n) { return (n + ALIGN - 1) / ALIGN * ALIGN; }
+
+bool grid_ok(const clt_grid *g)
+{
+    if (!g) return false;
+    if (g->nR < 9 || g->nZ < 9 || g->nphi < 5) return false;
+    if (g->nR > (1 << 20) || g->nZ > (1 << 20) || g->nphi > (1 << 20)) return false;
+    if (!(g->Rmin > 0.0) || !(g->Rmax > g->Rmin) || !(g->Zmax > g->Zmin)) return false;
+    if (!isfinite(g->Rmin) || !isfinite(g->Rmax) || !isfinite(g->Zmin) || !isfinite(g->Zmax)) return false;
+    if (!isfinite(g->phi_extent) || g->phi_extent < 0.0) return false;
+    return true;
+}
+
+Layout make_layout(const clt_grid *g)
+{
+    Layout L;
+    L.nR = g->nR; L.nphi = g->nphi; L.nZ = g->nZ;
+    L.pR = (LP + g->nR + 2 + 15) / 16 * 16;     // room for clamped halo reads two nodes past the edge
+    L.plane = (long long)L.nZ * L.pR;
+    L.field = (long long)L.nphi * L.plane;
+    return L;
+}
+
+struct Carve {
+    size_t field_b, table_b, rtab_b, cs_b, partial_b, result_b, total;
+    int nblocks;
+};
+Carve carve(const clt_grid *g)
+{
+    Layout L = make_layout(g);
+    Carve c;
+    c.field_b = align_up((size_t)L.field * sizeof(double));
+    c.table_b = align_up((size_t)L.plane * sizeof(double));
+    c.rtab_b = align_up((size_t)L.pR * sizeof(double));
+    c.cs_b = align_up((size_t)2 * g->nphi * sizeof(double));
+    c.nblocks = diag_blocks(L);
+    c.partial_b = align_up((size_t)c.nblocks * 6 * sizeof(double));
+    c.result_b = align_up(8 * sizeof(double));
+    c.total = 35 * c.field_b + T_COUNT * c.table_b + 2 * c.rtab_b + c.cs_b + c.partial_b + c.result_b;
+    return c;
+}
+
+int cuda_fail(clt_ctx *c, cudaError_t e, const char *where)
+{
+    if (c) snprintf(c->cuda_err, sizeof(c->cuda_err), "%s: %s", where, cudaGetErrorString(e));
+    return CLT_ECUDA;
+}
+#define CK(call)                                                      \
+    do {                                                              \
+        cudaError_t e_ = (call);                                      \
+        if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call);      \
+    } while (0)
+
+// dense user array [rows][nR]  <->  padded internal rows
+int copy_in(clt_ctx *ctx, double *dst_padded, const double *src, size_t rows)
+{
+    CK(cudaMemcpy2DAsync(dst_padded + LP, (size_t)ctx->L.pR * sizeof(double), src, (size_t)ctx->L.nR * sizeof(double),
+                         (size_t)ctx->L.nR * sizeof(double), rows, cudaMemcpyDefault, ctx->stream));
+    return CLT_OK;
+}
+int copy_out(clt_ctx *ctx, double *dst, const double *src_padded, size_t rows)
+{
+    CK(cudaMemcpy2DAsync(dst, (size_t)ctx->L.nR * sizeof(double), src_padded + LP, (size_t)ctx->L.pR * sizeof(double),
+                         (size_t)ctx->L.nR * sizeof(double), rows, cudaMemcpyDefault, ctx->stream));
+    cudaPointerAttributes at;
+    cudaError_t e = cudaPointerGetAttributes(&at, dst);
+    if (e != cudaSuccess) { cudaGetLastError(); at.type = cudaMemoryTypeUnregistered; }
+    if (at.type != cudaMemoryTypeDevice) CK(cudaStreamSynchronize(ctx->stream));   // host destination: synchronous
+    return CLT_OK;
+}
+
+void destroy_graph(clt_ctx *ctx)
+{
+    if (ctx->graph_exec) {
+        cudaGraphExecDestroy(ctx->graph_exec);
+        ctx->graph_exec = nullptr;
+    }
+}
+
+int effective_tile_z(const clt_ctx *ctx) { return ctx->tile_z ? ctx->tile_z : rhs_default_tile_z(); }
+int effective_chunks(const clt_ctx *ctx)
+{
+    int c = ctx->phi_chunks ? ctx->phi_chunks : 1;
+    if (c > ctx->L.nphi / 4) c = ctx->L.nphi / 4 > 0 ? ctx->L.nphi / 4 : 1;
+    return c;
+}
+
+int run_curl(clt_ctx *ctx, const double *U)
+{
+    CurlArgs a;
+    a.L = ctx->L; a.ph = ctx->ph;
+    a.B = U + 5 * ctx->L.field;
+    a.J1 = ctx->J1;
+    a.tab = ctx->tab;
+    a.R = ctx->Rtab + LP;
+    a.invR = ctx->invRtab + LP;
+    a.phi_chunks = effective_chunks(ctx);
+    CK(launch_curl(a, 0, ctx->stream));
+    ctx->launches++;
+    return CLT_OK;
+}
+
+int run_rhs(clt_ctx *ctx, int mode, const double *in, double *out, double a_next, double b_acc)
+{
+    RhsArgs a;
+    a.L = ctx->L; a.ph = ctx->ph;
+    a.in = in; a.J1 = ctx->J1; a.Un = ctx->Un; a.acc = ctx->acc; a.out = out;
+    a.tab = ctx->tab;
+    a.R = ctx->Rtab + LP;
+    a.invR = ctx->invRtab + LP;
+    a.a_next = a_next; a.b_acc = b_acc;
+    a.phi_chunks = effective_chunks(ctx);
+    a.prefetch = 1;
+    CK(launch_rhs(a, mode, ctx->has_v0, effective_tile_z(ctx), ctx->stream));
+    ctx->launches++;
+    return CLT_OK;
+}
+
+// a6: one classical RK4 step in accumulator form (O5):
+//   s1: Ua = Un + dt/2 K1, acc = Un + dt/6 K1      s2: Ub = Un + dt/2 K2, acc += dt/3 K2
+//   s3: Ua = Un + dt K3,   acc += dt/3 K3          s4: Un = acc + dt/6 K4
+int enqueue_step(clt_ctx *ctx)
+{
+    const double dt = ctx->dt;
+    int r;
+    if ((r = run_curl(ctx, ctx->Un))) return r;
+    if ((r = run_rhs(ctx, RHS_MODE_S1, ctx->Un, ctx->Ua, 0.5 * dt, dt / 6.0))) return r;
+    if ((r = run_curl(ctx, ctx->Ua))) return r;
+    if ((r = run_rhs(ctx, RHS_MODE_S2, ctx->Ua, ctx->Ub, 0.5 * dt, dt / 3.0))) return r;
+    if ((r = run_curl(ctx, ctx->Ub))) return r;
+    if ((r = run_rhs(ctx, RHS_MODE_S3, ctx->Ub, ctx->Ua, dt, dt / 3.0))) return r;
+    if ((r = run_curl(ctx, ctx->Ua))) return r;
+    if ((r = run_rhs(ctx, RHS_MODE_S4, ctx->Ua, ctx->Un, 0.0, dt / 6.0))) return r;
+    return CLT_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t clt_workspace_bytes(const clt_grid *grid)
+{
+    if (!grid_ok(grid)) return 0;
+    return carve(grid).total;
+}
+
+int clt_create(const clt_grid *grid, const clt_params *params, void *d_workspace, size_t bytes, void *cuda_stream,
+               clt_ctx **out)
+{
+    if (!out) return CLT_EINVAL;
+    *out = nullptr;
+    if (!grid_ok(grid) || !params || !d_workspace) return CLT_EINVAL;
+    if (!isfinite(params->gamma) || !isfinite(params->eta) || !isfinite(params->nu) || !isfinite(params->D)
+        || !isfinite(params->kappa) || !isfinite(params->dt) || !isfinite(params->cfl))
+        return CLT_EINVAL;
+    if (params->eta < 0 || params->nu < 0 || params->D < 0 || params->kappa < 0 || params->dt < 0 || params->flags != 0)
+        return CLT_EINVAL;
+    const Carve c = carve(grid);
+    if (bytes < c.total || ((uintptr_t)d_workspace % 256) != 0) return CLT_ENOMEM;
+    cudaPointerAttributes at;
+    cudaError_t e = cudaPointerGetAttributes(&at, d_workspace);
+    if (e != cudaSuccess) { cudaGetLastError(); return CLT_ECUDA; }
+    if (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeManaged) return CLT_ENOMEM;
+
+    clt_ctx *ctx = new (std::nothrow) clt_ctx();
+    if (!ctx) return CLT_ENOMEM;
+    memset(ctx, 0, sizeof(*ctx));
+    ctx->grid = *grid;
+    ctx->par = *params;
+    ctx->L = make_layout(grid);
+    ctx->stream = (cudaStream_t)cuda_stream;
+    ctx->dt = params->dt;
+    const double Lphi = grid->phi_extent == 0.0 ? 2.0 * M_PI : grid->phi_extent;
+    const double dR = (grid->Rmax - grid->Rmin) / (double)(grid->nR - 1);
+    const double dZ = (grid->Zmax - grid->Zmin) / (double)(grid->nZ - 1);
+    const double dphi = Lphi / (double)grid->nphi;
+    Phys &ph = ctx->ph;
+    ph.gamma = params->gamma; ph.eta = params->eta; ph.nu = params->nu; ph.D = params->D; ph.kappa = params->kappa;
+    ph.cR1 = 1.0 / (12.0 * dR); ph.cZ1 = 1.0 / (12.0 * dZ); ph.cP1 = 1.0 / (12.0 * dphi);
+    ph.cR2 = 1.0 / (12.0 * dR * dR); ph.cZ2 = 1.0 / (12.0 * dZ * dZ); ph.cP2 = 1.0 / (12.0 * dphi * dphi);
+    ph.dR = dR; ph.dZ = dZ; ph.dphi = dphi; ph.Lphi = Lphi;
+
+    char *p = (char *)d_workspace;
+    auto take = [&](size_t b) { double *r = (double *)p; p += b; return r; };
+    ctx->Un = take(8 * c.field_b); ctx->acc = take(8 * c.field_b);
+    ctx->Ua = take(8 * c.field_b); ctx->Ub = take(8 * c.field_b);
+    ctx->J1 = take(3 * c.field_b);
+    ctx->tab = take(T_COUNT * c.table_b);
+    ctx->Rtab = take(c.rtab_b); ctx->invRtab = take(c.rtab_b);
+    ctx->cs = take(c.cs_b);
+    ctx->partial = take(c.partial_b);
+    ctx->result = take(c.result_b);
+    ctx->nblocks_diag = c.nblocks;
+    // carve() aligns every field to 256 B but Layout::field is the unaligned stride: they must agree
+    if ((size_t)ctx->L.field * sizeof(double) != c.field_b || (size_t)ctx->L.plane * sizeof(double) != c.table_b) {
+        delete ctx;
+        return CLT_EINVAL;
+    }
+
+    int rc = CLT_OK;
+    do {
+        if ((e = cudaMemsetAsync(d_workspace, 0, c.total, ctx->stream)) != cudaSuccess) break;
+        // R_i = Rmin + i*dR in plain double arithmetic on the host (hazard H1); pad columns repeat the edge
+        std::vector<double> R(ctx->L.pR), iR(ctx->L.pR), cs(2 * (size_t)grid->nphi);
+        for (int col = 0; col < ctx->L.pR; ++col) {
+            int i = col - LP;
+            i = i < 0 ? 0 : (i > grid->nR - 1 ? grid->nR - 1 : i);
+            volatile double prod = (double)i * dR;      // no FMA contraction
+            R[col] = grid->Rmin + prod;
+            iR[col] = 1.0 / R[col];
+        }
+        for (int j = 0; j < grid->nphi; ++j) {
+            const double ang = 2.0 * M_PI * (double)j / (double)grid->nphi;
+            cs[j] = cos(ang);
+            cs[grid->nphi + j] = sin(ang);
+        }
+        if ((e = cudaMemcpyAsync(ctx->Rtab, R.data(), R.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream))) break;
+        if ((e = cudaMemcpyAsync(ctx->invRtab, iR.data(), iR.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream))) break;
+        if ((e = cudaMemcpyAsync(ctx->cs, cs.data(), cs.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream))) break;
+        if ((e = cudaStreamSynchronize(ctx->stream))) break;     // the host vectors go out of scope
+        if ((e = launch_tables(ctx->L, ctx->ph, ctx->tab, ctx->Rtab + LP, ctx->invRtab + LP, ctx->stream))) break;
+        ctx->launches++;
+    } while (0);
+    if (e != cudaSuccess) {
+        delete ctx;
+        cudaGetLastError();
+        return CLT_ECUDA;
+    }
+    *out = ctx;
+    return rc;
+}
+
+int clt_destroy(clt_ctx *ctx)
+{
+    if (!ctx) return CLT_OK;
+    cudaError_t e = cudaStreamSynchronize(ctx->stream);
+    destroy_graph(ctx);
+    delete ctx;
+    if (e != cudaSuccess) { cudaGetLastError(); return CLT_ECUDA; }
+    return CLT_OK;
+}
+
+int clt_set_equilibrium(clt_ctx *ctx, const double *U0)
+{
+    if (!ctx) return CLT_EINVAL;
+    ctx->has_state = false;
+    const size_t rows = (size_t)8 * ctx->L.nZ;
+    bool v0 = false;
+    if (U0) {
+        int r = copy_in(ctx, ctx->tab, U0, rows);          // tables 0..7 are U0 itself
+        if (r) return r;
+        // does the reference state move?  (selects the v0 = 0 specialisation of the kernels)
+        const size_t n = (size_t)3 * ctx->L.nZ * ctx->L.nR;
+        std::vector<double> h(n);
+        CK(cudaMemcpy2DAsync(h.data(), (size_t)ctx->L.nR * sizeof(double), ctx->tab + T_V0R * ctx->L.plane + LP,
+                             (size_t)ctx->L.pR * sizeof(double), (size_t)ctx->L.nR * sizeof(double), (size_t)3 * ctx->L.nZ,
+                             cudaMemcpyDeviceToHost, ctx->stream));
+        CK(cudaStreamSynchronize(ctx->stream));
+        for (size_t q = 0; q < n; ++q)
+            if (h[q] != 0.0) { v0 = true; break; }
+    } else {
+        CK(cudaMemsetAsync(ctx->tab, 0, (size_t)8 * ctx->L.plane * sizeof(double), ctx->stream));
+    }
+    ctx->has_v0 = v0;
+    CK(launch_tables(ctx->L, ctx->ph, ctx->tab, ctx->Rtab + LP, ctx->invRtab + LP, ctx->stream));
+    ctx->launches++;
+    return CLT_OK;
+}
+
+int clt_set_state(clt_ctx *ctx, const double *U)
+{
+    if (!ctx || !U) return CLT_EINVAL;
+    int r = copy_in(ctx, ctx->Un, U, (size_t)8 * ctx->L.nphi * ctx->L.nZ);
+    if (r) return r;
+    // a1: freeze the two boundary layers per R/Z side in every RK buffer
+    CK(launch_copy_boundary(ctx->L, 8, ctx->Un, ctx->acc, ctx->Ua, ctx->Ub, ctx->stream));
+    ctx->launches++;
+    cudaPointerAttributes at;
+    cudaError_t e = cudaPointerGetAttributes(&at, U);
+    if (e != cudaSuccess) { cudaGetLastError(); at.type = cudaMemoryTypeUnregistered; }
+    if (at.type != cudaMemoryTypeDevice) CK(cudaStreamSynchronize(ctx->stream));   // the caller may reuse host memory
+    ctx->has_state = true;
+    ctx->step = 0;
+    ctx->time = 0.0;
+    return CLT_OK;
+}
+
+int clt_get_state(clt_ctx *ctx, double *U)
+{
+    if (!ctx || !U) return CLT_EINVAL;
+    if (!ctx->has_state) return CLT_ESTATE;
+    return copy_out(ctx, U, ctx->Un, (size_t)8 * ctx->L.nphi * ctx->L.nZ);
+}
+
+int clt_rhs(clt_ctx *ctx, double *dUdt)
+{
+    if (!ctx || !dUdt) return CLT_EINVAL;
+    if (!ctx->has_state) return CLT_ESTATE;
+    int r;
+    if ((r = run_curl(ctx, ctx->Un))) return r;
+    CK(launch_zero_boundary(ctx->L, 8, ctx->Ub, ctx->stream));     // K = 0 on the boundary layers
+    ctx->launches++;
+    if ((r = run_rhs(ctx, RHS_MODE_K, ctx->Un, ctx->Ub, 0.0, 0.0))) return r;
+    if ((r = copy_out(ctx, dUdt, ctx->Ub, (size_t)8 * ctx->L.nphi * ctx->L.nZ))) return r;
+    CK(launch_copy_boundary(ctx->L, 8, ctx->Un, ctx->Ub, nullptr, nullptr, ctx->stream));   // restore the scratch buffer
+    ctx->launches++;
+    return CLT_OK;
+}
+
+int clt_curl_J1(clt_ctx *ctx, double *J1)
+{
+    if (!ctx || !J1) return CLT_EINVAL;
+    if (!ctx->has_state) return CLT_ESTATE;
+    int r;
+    if ((r = run_curl(ctx, ctx->Un))) return r;
+    return copy_out(ctx, J1, ctx->J1, (size_t)3 * ctx->L.nphi * ctx->L.nZ);
+}
+
+int clt_set_dt(clt_ctx *ctx, double dt)
+{
+    if (!ctx || !(dt > 0.0) || !isfinite(dt)) return CLT_EINVAL;
+    ctx->dt = dt;
+    return CLT_OK;
+}
+
+int clt_step(clt_ctx *ctx, int n)
+{
+    if (!ctx || n < 0) return CLT_EINVAL;
+    if (!ctx->has_state) return CLT_ESTATE;
+    if (!(ctx->dt > 0.0)) return CLT_EINVAL;
+    if (ctx->use_graph) {
+        const bool stale = !ctx->graph_exec || ctx->graph_dt != ctx->dt || ctx->graph_tile_z != effective_tile_z(ctx)
+                           || ctx->graph_chunks != effective_chunks(ctx) || ctx->graph_v0 != ctx->has_v0;
+        if (stale) {
+            destroy_graph(ctx);
+            cudaGraph_t g = nullptr;
+            CK(cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal));
+            const int64_t before = ctx->launches;
+            int r = enqueue_step(ctx);
+            ctx->launches = before;
+            cudaError_t e = cudaStreamEndCapture(ctx->stream, &g);
+            if (r) { if (g) cudaGraphDestroy(g); return r; }
+            if (e != cudaSuccess) return cuda_fail(ctx, e, "cudaStreamEndCapture");
+            e = cudaGraphInstantiate(&ctx->graph_exec, g, 0);
+            cudaGraphDestroy(g);
+            if (e != cudaSuccess) return cuda_fail(ctx, e, "cudaGraphInstantiate");
+            ctx->graph_dt = ctx->dt; ctx->graph_tile_z = effective_tile_z(ctx);
+            ctx->graph_chunks = effective_chunks(ctx); ctx->graph_v0 = ctx->has_v0;
+        }
+        for (int s = 0; s < n; ++s) {
+            CK(cudaGraphLaunch(ctx->graph_exec, ctx->stream));
+            ctx->launches += 8;
+        }
+    } else {
+        for (int s = 0; s < n; ++s) {
+            int r = enqueue_step(ctx);
+            if (r) return r;
+        }
+    }
+    ctx->step += n;
+    ctx->time += (double)n * ctx->dt;
+    return CLT_OK;
+}
+
+static int run_diag(clt_ctx *ctx, double cfl, double out6[6])
+{
+    DiagArgs a;
+    a.L = ctx->L; a.ph = ctx->ph;
+    a.U = ctx->Un; a.tab = ctx->tab;
+    a.R = ctx->Rtab + LP; a.invR = ctx->invRtab + LP;
+    a.cs = ctx->cs; a.partial = ctx->partial; a.cfl = cfl;
+    CK(launch_diag(a, ctx->nblocks_diag, ctx->result, ctx->stream));
+    ctx->launches += 2;
+    CK(cudaMemcpyAsync(out6, ctx->result, 6 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return CLT_OK;
+}
+
+int clt_diagnostics(clt_ctx *ctx, clt_diag *out)
+{
+    if (!ctx || !out) return CLT_EINVAL;
+    if (!ctx->has_state) return CLT_ESTATE;
+    double r6[6];
+    int r = run_diag(ctx, ctx->par.cfl > 0 ? ctx->par.cfl : 0.5, r6);
+    if (r) return r;
+    out->kinetic = r6[0]; out->magnetic = r6[1]; out->magnetic_pert = r6[2]; out->magnetic_n1 = r6[3];
+    out->max_divB = r6[4];
+    out->step = ctx->step;
+    out->time = ctx->time;
+    for (int q = 0; q < 5; ++q)
+        if (!isfinite(r6[q])) return CLT_ENONFINITE;
+    return CLT_OK;
+}
+
+int clt_suggest_dt(clt_ctx *ctx, double cfl, double *dt_out)
+{
+    if (!ctx || !dt_out) return CLT_EINVAL;
+    if (!ctx->has_state) return CLT_ESTATE;
+    if (!(cfl > 0.0)) cfl = ctx->par.cfl;
+    if (!(cfl > 0.0) || !isfinite(cfl)) return CLT_EINVAL;
+    double r6[6];
+    int r = run_diag(ctx, cfl, r6);
+    if (r) return r;
+    *dt_out = r6[5];
+    return CLT_OK;
+}
+
+int clt_set_tuning(clt_ctx *ctx, int tile_z, int phi_chunks, int use_graph)
+{
+    if (!ctx) return CLT_EINVAL;
+    if (tile_z != 0 && tile_z != 8 && tile_z != 12 && tile_z != 14 && tile_z != 16) return CLT_EINVAL;
+    if (phi_chunks < 0 || phi_chunks > 64) return CLT_EINVAL;
+    ctx->tile_z = tile_z;
+    ctx->phi_chunks = phi_chunks;
+    ctx->use_graph = use_graph ? 1 : 0;
+    return CLT_OK;
+}
+
+int64_t clt_launch_count(const clt_ctx *ctx) { return ctx ? ctx->launches : 0; }
+void *clt_stream(const clt_ctx *ctx) { return ctx ? (void *)ctx->stream : nullptr; }
+
+const char *clt_strerror(int code)
+{
+    switch (code) {
+    case CLT_OK: return "ok";
+    case CLT_EINVAL: return "invalid argument";
+    case CLT_ENOMEM: return "workspace too small, misaligned or not device memory";
+    case CLT_ESTATE: return "call out of order (set the state first)";
+    case CLT_ECUDA: return "CUDA error";
+    case CLT_ENONFINITE: return "non-finite diagnostic";
+    default: return "unknown error";
+    }
+}
+const char *clt_last_cuda_error(const clt_ctx *ctx) { return ctx ? ctx->cuda_err : ""; }
+const char *clt_version(void) { return "clt-b200 0.1 (sm_100a, fp64)"; }
+
+}  // extern "C"

@@ -1,0 +1,103 @@
+// clt_internal.h -- shared declarations of libclt's host side (clt_api.cu) and kernels (clt_kernels.cu).
+// Product code: shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+
+namespace clt {
+
+// ---------------------------------------------------------------------------------------------
+// Internal HBM layout.  A scalar field is [nphi][nZ][pR] doubles, R fastest.
+// Node i of a row sits at column LP + i with LP = 14, so that the first interior node (i = 2) of
+// every row is 128-byte aligned (pR is a multiple of 16 doubles and every field base is 256-byte
+// aligned).  The R/Z boundary layers are part of the array and are never written by the step
+// kernels; phi has no ghost planes (the plane index wraps).
+constexpr int LP = 14;
+
+struct Layout {
+    int nR, nphi, nZ;
+    int pR;             // row pitch in doubles
+    long long plane;    // nZ * pR
+    long long field;    // nphi * plane
+    __host__ __device__ long long at(int i, int k, int j) const {
+        return (long long)j * plane + (long long)k * pR + (LP + i);
+    }
+};
+
+// Indices of the axisymmetric tables ([nZ][pR] each, same row layout as a field plane).
+enum Table {
+    T_RHO0 = 0, T_P0, T_V0R, T_V0P, T_V0Z, T_B0R, T_B0P, T_B0Z,   // U0 (eqs 11-14)
+    T_J0R, T_J0P, T_J0Z,                                          // J0 = curl_c B0 (interior; 0 on boundary layers)
+    T_GR_RHO0, T_GZ_RHO0, T_GR_P0, T_GZ_P0,                       // d_R, d_Z of rho0, p0
+    T_E0R, T_E0P, T_E0Z,                                          // v0 x B0
+    T_GR_V0R, T_GZ_V0R, T_GR_V0P, T_GZ_V0P, T_GR_V0Z, T_GZ_V0Z,   // d_R, d_Z of v0
+    T_DIVV0,                                                      // div v0
+    T_A0R, T_A0P, T_A0Z,                                          // (v0.grad) v0
+    T_COUNT
+};
+
+struct Phys {
+    double gamma, eta, nu, D, kappa;
+    double cR1, cZ1, cP1;    // 1/(12 h)
+    double cR2, cZ2, cP2;    // 1/(12 h^2)
+    double dR, dZ, dphi, Lphi;
+};
+
+// Parameters of one fused RHS (+ RK4 stage combine) launch.
+struct RhsArgs {
+    Layout L;
+    Phys ph;
+    const double *in;     // stage state, 8 fields
+    const double *J1;     // 3 fields
+    const double *Un;     // U^n, 8 fields (modes 2, 3)
+    double *acc;          // RK4 accumulator, 8 fields (modes 1-4)
+    double *out;          // K (mode 0) | next stage state (modes 1-3) | U^{n+1} (mode 4), 8 fields
+    const double *tab;    // T_COUNT tables
+    const double *R;      // R_i, i = -LP .. : pointer already offset so that R[i] is node i; padded with valid numbers
+    const double *invR;   // 1/R_i, same indexing
+    double a_next;        // out = U^n + a_next * K   (modes 1-3)
+    double b_acc;         // acc += b_acc * K  /  out = acc + b_acc * K (mode 4)
+    int phi_chunks;       // number of chunks the phi range is split into (gridDim.z)
+    int prefetch;         // issue L2 prefetch hints
+};
+
+struct CurlArgs {
+    Layout L;
+    Phys ph;
+    const double *B;      // 3 fields (B_R, B_phi, B_Z of the stage state)
+    double *J1;           // 3 fields
+    const double *tab;
+    const double *R;
+    const double *invR;
+    int phi_chunks;
+};
+
+struct DiagArgs {
+    Layout L;
+    Phys ph;
+    const double *U;
+    const double *tab;
+    const double *R;
+    const double *invR;
+    const double *cs;     // cos/sin(2 pi j / nphi), [2][nphi]
+    double *partial;      // [nblocks][6]
+    double cfl;
+};
+
+enum { RHS_MODE_K = 0, RHS_MODE_S1 = 1, RHS_MODE_S2 = 2, RHS_MODE_S3 = 3, RHS_MODE_S4 = 4 };
+
+// kernel launchers (clt_kernels.cu); each returns the cudaGetLastError() of its launch
+cudaError_t launch_tables(const Layout &L, const Phys &ph, double *tab, const double *R, const double *invR,
+                          cudaStream_t s);
+cudaError_t launch_copy_boundary(const Layout &L, int nfields, const double *src, double *d0, double *d1, double *d2,
+                                 cudaStream_t s);
+cudaError_t launch_zero_boundary(const Layout &L, int nfields, double *dst, cudaStream_t s);
+cudaError_t launch_curl(const CurlArgs &a, int tile_z, cudaStream_t s);
+cudaError_t launch_rhs(const RhsArgs &a, int mode, bool has_v0, int tile_z, cudaStream_t s);
+cudaError_t launch_diag(const DiagArgs &a, int nblocks, double *result6, cudaStream_t s);
+int diag_blocks(const Layout &L);
+cudaError_t configure_kernels();
+int rhs_default_tile_z();
+
+}  // namespace clt

@@ -1,0 +1,743 @@
+// clt_kernels.cu -- sm_100a CUDA kernels of libclt (product code; shares nothing with oracle/).
+//
+// Hot path ("DERIVATIVES", "J, E", "RIGHT HANDS OF EQUATIONS", "STEP ON"):
+//   curl_kernel : J1 = curl_c(B - B0)                                   (eq 6)
+//   rhs_kernel  : E1, all derivatives, K of eqs (11)-(14) (L105-115) and the RK4 stage combine in
+//                 the epilogue, one read and one write of HBM per stage.
+// Both are 2.5-D sweeps: a CTA owns a TR x TZ tile of the (R, Z) plane and marches along phi;
+// in-plane neighbours come from a shared-memory tile with a radius-2 halo, phi neighbours from a
+// 5-deep register pipeline (rho1, p1, v1) and from shared-memory rings (E1, J x B force).
+// Everything differenced is a perturbation (U - U0): DESIGN.md section 3, hazard H2.
+#include "clt_internal.h"
+
+namespace clt {
+
+constexpr int TR = 32;        // tile width in R = one warp per tile row
+constexpr int SW = TR + 4;    // shared row width with the radius-2 halo
+
+__device__ __forceinline__ void prefetch_l2(const void *p)
+{
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+}
+
+// unscaled 4th-order central differences from five equally spaced samples:
+//   d1 * 1/(12h)   = first derivative,  d2 * 1/(12h^2) = second derivative
+__device__ __forceinline__ double fd1(double m2, double m1, double p1, double p2)
+{
+    return 8.0 * (p1 - m1) - (p2 - m2);
+}
+__device__ __forceinline__ double fd2(double m2, double m1, double c0, double p1, double p2)
+{
+    return (16.0 * (p1 + m1) - (p2 + m2)) - 30.0 * c0;
+}
+
+__device__ __forceinline__ int wrap_phi(int j, int n)
+{
+    return j < 0 ? j + n : (j >= n ? j - n : j);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Fused RHS + RK4 stage combine
+// ---------------------------------------------------------------------------------------------
+template <int TZ>
+struct RhsSmem {
+    static constexpr int HT = (TZ + 4) * SW;   // tile with halo
+    static constexpr int IT = TZ * TR;         // tile interior
+    double stage[2][5][HT];    // rho1, p1, v1_R, v1_phi, v1_Z of the centre plane (double-buffered)
+    double ering[5][3][HT];    // E1 of planes j-2 .. j+2 (halo part valid for the centre plane only)
+    double fring[3][3][IT];    // F = J1 x B + J0 x B1 of planes j .. j+2
+    double sR[SW];             // R_i of the tile columns i0-2 .. i0+33
+};
+
+template <int TZ, int MODE, bool V0>
+__global__ void __launch_bounds__(TR *TZ, 1) rhs_kernel(const __grid_constant__ RhsArgs a)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    RhsSmem<TZ> &S = *reinterpret_cast<RhsSmem<TZ> *>(smem_raw);
+    constexpr int IT = RhsSmem<TZ>::IT;
+    const Layout &L = a.L;
+    const Phys &ph = a.ph;
+
+    const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * TR + tx;
+    const int i0 = 2 + TR * blockIdx.x, k0 = 2 + TZ * blockIdx.y;
+    const int i = i0 + tx, k = k0 + ty;
+    const bool valid = (i <= L.nR - 3) && (k <= L.nZ - 3);
+    const int ic = min(i, L.nR - 1), kc = min(k, L.nZ - 1);
+    const int ja = (int)(((long long)L.nphi * blockIdx.z) / a.phi_chunks);
+    const int jb = (int)(((long long)L.nphi * (blockIdx.z + 1)) / a.phi_chunks);
+
+    const long long off2 = (long long)kc * L.pR + (LP + ic);     // offset inside a plane / a table
+    const int cs = (ty + 2) * SW + (tx + 2);                     // own slot in a halo tile
+    const int ci = ty * TR + tx;                                 // own slot in an interior tile
+
+    // halo nodes: 4 full rows (Z halo) then 4 columns (R halo); one node per thread, tid < NH
+    constexpr int NH = 4 * TR + 4 * TZ;
+    static_assert(NH <= TR * TZ, "tile too small for one halo node per thread");
+    int hx, hy;
+    if (tid < 4 * TR) {
+        const int r = tid / TR;
+        hx = tid % TR;
+        hy = (r < 2) ? r - 2 : TZ + (r - 2);
+    } else {
+        const int t = tid - 4 * TR, c = t & 3;
+        hy = t >> 2;
+        hx = (c < 2) ? c - 2 : TR + (c - 2);
+    }
+    const bool is_halo = tid < NH;
+    const int hi = min(i0 + hx, L.nR - 1), hk = min(k0 + hy, L.nZ - 1);
+    const long long hoff2 = (long long)hk * L.pR + (LP + hi);
+    const int hs = (hy + 2) * SW + (hx + 2);
+
+    if (tid < SW) S.sR[tid] = a.R[min(i0 - 2 + tid, L.nR - 1)];
+
+    const double *tab = a.tab;
+    const double eta = ph.eta;
+
+    // loads the 11 stage fields at one node of one plane, forms perturbations, E1 and (optionally) F
+    auto load_node = [&](long long o2, int jw, double q[5], double E[3], double F[3], bool wantF) {
+        const long long g = (long long)jw * L.plane + o2;
+        const double rho = __ldg(a.in + 0 * L.field + g), p = __ldg(a.in + 1 * L.field + g);
+        const double vR = __ldg(a.in + 2 * L.field + g), vP = __ldg(a.in + 3 * L.field + g),
+                     vZ = __ldg(a.in + 4 * L.field + g);
+        const double BR = __ldg(a.in + 5 * L.field + g), BP = __ldg(a.in + 6 * L.field + g),
+                     BZ = __ldg(a.in + 7 * L.field + g);
+        const double JR = __ldg(a.J1 + 0 * L.field + g), JP = __ldg(a.J1 + 1 * L.field + g),
+                     JZ = __ldg(a.J1 + 2 * L.field + g);
+        q[0] = rho - __ldg(tab + T_RHO0 * L.plane + o2);
+        q[1] = p - __ldg(tab + T_P0 * L.plane + o2);
+        if (V0) {
+            q[2] = vR - __ldg(tab + T_V0R * L.plane + o2);
+            q[3] = vP - __ldg(tab + T_V0P * L.plane + o2);
+            q[4] = vZ - __ldg(tab + T_V0Z * L.plane + o2);
+        } else {
+            q[2] = vR; q[3] = vP; q[4] = vZ;
+        }
+        // a4: E1 = -v x B + v0 x B0 + eta J1   (eq 5 with d_i = 0 minus E0, L77, L101)
+        E[0] = eta * JR - (vP * BZ - vZ * BP);
+        E[1] = eta * JP - (vZ * BR - vR * BZ);
+        E[2] = eta * JZ - (vR * BP - vP * BR);
+        if (V0) {
+            E[0] += __ldg(tab + T_E0R * L.plane + o2);
+            E[1] += __ldg(tab + T_E0P * L.plane + o2);
+            E[2] += __ldg(tab + T_E0Z * L.plane + o2);
+        }
+        if (wantF) {
+            const double B1R = BR - __ldg(tab + T_B0R * L.plane + o2), B1P = BP - __ldg(tab + T_B0P * L.plane + o2),
+                         B1Z = BZ - __ldg(tab + T_B0Z * L.plane + o2);
+            const double J0R = __ldg(tab + T_J0R * L.plane + o2), J0P = __ldg(tab + T_J0P * L.plane + o2),
+                         J0Z = __ldg(tab + T_J0Z * L.plane + o2);
+            // Lorentz force terms of eq (13): J1 x B + J0 x B1
+            F[0] = (JP * BZ - JZ * BP) + (J0P * B1Z - J0Z * B1P);
+            F[1] = (JZ * BR - JR * BZ) + (J0Z * B1R - J0R * B1Z);
+            F[2] = (JR * BP - JP * BR) + (J0R * B1P - J0P * B1R);
+        }
+    };
+
+    double q[5][5];      // phi pipeline: q[d][f], plane j-2+d, f = rho1, p1, v1R, v1P, v1Z
+    int se = 0, sf = 0;  // ring slots that receive plane j+2
+
+    auto lead = [&](int jl) {
+        double E[3], F[3];
+        load_node(off2, wrap_phi(jl, L.nphi), q[4], E, F, true);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            S.ering[se][c][cs] = E[c];
+            S.fring[sf][c][ci] = F[c];
+        }
+    };
+    auto advance = [&]() {
+#pragma unroll
+        for (int d = 0; d < 4; ++d)
+#pragma unroll
+            for (int f = 0; f < 5; ++f) q[d][f] = q[d + 1][f];
+        se = (se == 4) ? 0 : se + 1;
+        sf = (sf == 2) ? 0 : sf + 1;
+    };
+
+    // prologue: planes ja-2 .. ja+1
+#pragma unroll 1
+    for (int jl = ja - 2; jl <= ja + 1; ++jl) {
+        lead(jl);
+        advance();
+    }
+
+    const double iR = __ldg(a.invR + ic);
+    const double iR2 = iR * iR;
+
+#pragma unroll 1
+    for (int j = ja; j < jb; ++j) {
+        const int buf = j & 1;
+        const int jw = j;   // ja <= j < jb <= nphi: no wrap needed for the centre plane
+        // ---- phase A: stage plane j, bring in plane j+2 --------------------------------------
+        if (a.prefetch && (tx & 15) == 0) {
+            const long long g3 = (long long)wrap_phi(j + 3, L.nphi) * L.plane + off2;
+#pragma unroll
+            for (int m = 0; m < 8; ++m) prefetch_l2(a.in + m * L.field + g3);
+#pragma unroll
+            for (int m = 0; m < 3; ++m) prefetch_l2(a.J1 + m * L.field + g3);
+            if (MODE != RHS_MODE_K && j + 1 < jb) {
+                const long long g1 = (long long)(j + 1) * L.plane + off2;
+#pragma unroll
+                for (int m = 0; m < 8; ++m) {
+                    if (MODE == RHS_MODE_S2 || MODE == RHS_MODE_S3) prefetch_l2(a.Un + m * L.field + g1);
+                    if (MODE != RHS_MODE_S1) prefetch_l2(a.acc + m * L.field + g1);
+                }
+            }
+        }
+        lead(j + 2);
+#pragma unroll
+        for (int f = 0; f < 5; ++f) S.stage[buf][f][cs] = q[2][f];
+        const int sec = (se + 3 >= 5) ? se + 3 - 5 : se + 3;      // ring slot of the centre plane
+        if (is_halo) {
+            double hq[5], hE[3], hF[3];
+            load_node(hoff2, jw, hq, hE, hF, false);
+#pragma unroll
+            for (int f = 0; f < 5; ++f) S.stage[buf][f][hs] = hq[f];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) S.ering[sec][c][hs] = hE[c];
+        }
+        __syncthreads();
+
+        // ---- phase B: K at (i, k, j) -----------------------------------------------------------
+        const double rho1 = q[2][0], p1 = q[2][1], v1R = q[2][2], v1P = q[2][3], v1Z = q[2][4];
+        const double rho = rho1 + __ldg(tab + T_RHO0 * L.plane + off2);
+        const double p = p1 + __ldg(tab + T_P0 * L.plane + off2);
+        double vR = v1R, vP = v1P, vZ = v1Z;
+        if (V0) {
+            vR += __ldg(tab + T_V0R * L.plane + off2);
+            vP += __ldg(tab + T_V0P * L.plane + off2);
+            vZ += __ldg(tab + T_V0Z * L.plane + off2);
+        }
+        const double rinv = 1.0 / rho;
+
+        double A[5], lap[5];     // (v.grad) f and Laplacian f of the five staged fields
+        double divv1, gRp1, gPp1, gZp1, gPvR, gPvP;
+        // R direction (shared memory, stride 1)
+        {
+            const double vc = vR * ph.cR1, lc = iR * ph.cR1;
+#pragma unroll
+            for (int f = 0; f < 5; ++f) {
+                const double *s = &S.stage[buf][f][cs];
+                const double m2 = s[-2], m1 = s[-1], p1_ = s[1], p2 = s[2];
+                const double d1 = fd1(m2, m1, p1_, p2), d2 = fd2(m2, m1, q[2][f], p1_, p2);
+                A[f] = vc * d1;
+                lap[f] = d2 * ph.cR2 + lc * d1;
+                if (f == 1) gRp1 = d1 * ph.cR1;
+                if (f == 2) divv1 = d1 * ph.cR1 + v1R * iR;
+            }
+        }
+        // phi direction (register pipeline)
+        {
+            const double g1 = ph.cP1 * iR, vc = vP * g1, lc = ph.cP2 * iR2;
+#pragma unroll
+            for (int f = 0; f < 5; ++f) {
+                const double d1 = fd1(q[0][f], q[1][f], q[3][f], q[4][f]);
+                const double d2 = fd2(q[0][f], q[1][f], q[2][f], q[3][f], q[4][f]);
+                A[f] += vc * d1;
+                lap[f] += lc * d2;
+                if (f == 1) gPp1 = d1 * g1;
+                if (f == 2) gPvR = d1 * g1;
+                if (f == 3) { gPvP = d1 * g1; divv1 += gPvP; }
+            }
+        }
+        // Z direction (shared memory, stride SW)
+        {
+            const double vc = vZ * ph.cZ1;
+#pragma unroll
+            for (int f = 0; f < 5; ++f) {
+                const double *s = &S.stage[buf][f][cs];
+                const double m2 = s[-2 * SW], m1 = s[-SW], p1_ = s[SW], p2 = s[2 * SW];
+                const double d1 = fd1(m2, m1, p1_, p2), d2 = fd2(m2, m1, q[2][f], p1_, p2);
+                A[f] += vc * d1;
+                lap[f] += d2 * ph.cZ2;
+                if (f == 1) gZp1 = d1 * ph.cZ1;
+                if (f == 4) divv1 += d1 * ph.cZ1;
+            }
+        }
+
+        double K[8];
+        {
+            // eq (11), L105 and eq (12), with grad rho = grad rho1 + grad rho0 (tables)
+            double cr = A[0] + v1R * __ldg(tab + T_GR_RHO0 * L.plane + off2) + v1Z * __ldg(tab + T_GZ_RHO0 * L.plane + off2)
+                        + rho * divv1;
+            double cp = A[1] + v1R * __ldg(tab + T_GR_P0 * L.plane + off2) + v1Z * __ldg(tab + T_GZ_P0 * L.plane + off2);
+            double pd = p * divv1;
+            if (V0) {
+                const double dv0 = __ldg(tab + T_DIVV0 * L.plane + off2);
+                cr += rho1 * dv0;
+                pd += p1 * dv0;
+            }
+            K[0] = ph.D * lap[0] - cr;
+            K[1] = ph.kappa * lap[1] - cp - ph.gamma * pd;
+            // eq (13)
+            const int sfc = (sf + 1 >= 3) ? sf + 1 - 3 : sf + 1;  // ring slot of F at the centre plane
+            double aR = A[2] - vP * v1P * iR;
+            double aP = A[3] + vP * v1R * iR;
+            double aZ = A[4];
+            if (V0) {
+                const double v0R = vR - v1R, v0P = vP - v1P;
+                const double r1 = rho1 * rinv;
+                aR += v1R * __ldg(tab + T_GR_V0R * L.plane + off2) + v1Z * __ldg(tab + T_GZ_V0R * L.plane + off2)
+                      - v1P * v0P * iR + r1 * __ldg(tab + T_A0R * L.plane + off2);
+                aP += v1R * __ldg(tab + T_GR_V0P * L.plane + off2) + v1Z * __ldg(tab + T_GZ_V0P * L.plane + off2)
+                      + v1P * v0R * iR + r1 * __ldg(tab + T_A0P * L.plane + off2);
+                aZ += v1R * __ldg(tab + T_GR_V0Z * L.plane + off2) + v1Z * __ldg(tab + T_GZ_V0Z * L.plane + off2)
+                      + r1 * __ldg(tab + T_A0Z * L.plane + off2);
+            }
+            const double two_iR = 2.0 * iR;
+            K[2] = (S.fring[sfc][0][ci] - gRp1) * rinv - aR + ph.nu * (lap[2] - v1R * iR2 - two_iR * gPvP);
+            K[3] = (S.fring[sfc][1][ci] - gPp1) * rinv - aP + ph.nu * (lap[3] - v1P * iR2 + two_iR * gPvR);
+            K[4] = (S.fring[sfc][2][ci] - gZp1) * rinv - aZ + ph.nu * lap[4];
+            // eq (14): -curl_c(E1); the radial derivative differences R * E_phi
+            const double *eR = &S.ering[sec][0][cs], *eP = &S.ering[sec][1][cs], *eZ = &S.ering[sec][2][cs];
+            const int s0 = (se + 1 >= 5) ? se + 1 - 5 : se + 1;   // plane j-2
+            const int s1 = (se + 2 >= 5) ? se + 2 - 5 : se + 2;   // plane j-1
+            const int s3 = (se + 4 >= 5) ? se + 4 - 5 : se + 4;   // plane j+1
+            const int s4 = se;                                    // plane j+2
+            const double dP_EZ = fd1(S.ering[s0][2][cs], S.ering[s1][2][cs], S.ering[s3][2][cs], S.ering[s4][2][cs]);
+            const double dP_ER = fd1(S.ering[s0][0][cs], S.ering[s1][0][cs], S.ering[s3][0][cs], S.ering[s4][0][cs]);
+            const double dZ_EP = fd1(eP[-2 * SW], eP[-SW], eP[SW], eP[2 * SW]);
+            const double dZ_ER = fd1(eR[-2 * SW], eR[-SW], eR[SW], eR[2 * SW]);
+            const double dR_EZ = fd1(eZ[-2], eZ[-1], eZ[1], eZ[2]);
+            const double *r = &S.sR[tx + 2];
+            const double dR_REP = fd1(r[-2] * eP[-2], r[-1] * eP[-1], r[1] * eP[1], r[2] * eP[2]);
+            const double cPi = ph.cP1 * iR;
+            K[5] = dZ_EP * ph.cZ1 - dP_EZ * cPi;
+            K[6] = dR_EZ * ph.cR1 - dZ_ER * ph.cZ1;
+            K[7] = dP_ER * cPi - dR_REP * (ph.cR1 * iR);
+        }
+
+        // ---- a6: RK4 stage combine in the epilogue (L125, L139) --------------------------------
+        if (valid) {
+            const long long g = (long long)jw * L.plane + off2;
+#pragma unroll
+            for (int m = 0; m < 8; ++m) {
+                const long long gm = m * L.field + g;
+                if (MODE == RHS_MODE_K) {
+                    a.out[gm] = K[m];
+                } else if (MODE == RHS_MODE_S1) {
+                    const double un = __ldg(a.in + gm);
+                    a.out[gm] = fma(a.a_next, K[m], un);
+                    a.acc[gm] = fma(a.b_acc, K[m], un);
+                } else if (MODE == RHS_MODE_S4) {
+                    a.out[gm] = fma(a.b_acc, K[m], a.acc[gm]);
+                } else {
+                    const double un = __ldg(a.Un + gm);
+                    a.out[gm] = fma(a.a_next, K[m], un);
+                    a.acc[gm] = fma(a.b_acc, K[m], a.acc[gm]);
+                }
+            }
+        }
+        advance();
+    }
+}
+
+template <int TZ, int MODE, bool V0>
+static cudaError_t launch_rhs_t(const RhsArgs &a, cudaStream_t s)
+{
+    static bool configured = false;
+    auto kern = rhs_kernel<TZ, MODE, V0>;
+    const int smem = (int)sizeof(RhsSmem<TZ>);
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    dim3 block(TR, TZ, 1);
+    dim3 grid((a.L.nR - 4 + TR - 1) / TR, (a.L.nZ - 4 + TZ - 1) / TZ, a.phi_chunks);
+    kern<<<grid, block, smem, s>>>(a);
+    return cudaGetLastError();
+}
+
+template <int TZ>
+static cudaError_t launch_rhs_tz(const RhsArgs &a, int mode, bool v0, cudaStream_t s)
+{
+#define CLT_CASE(M)                                                      \
+    case M:                                                              \
+        return v0 ? launch_rhs_t<TZ, M, true>(a, s) : launch_rhs_t<TZ, M, false>(a, s);
+    switch (mode) {
+        CLT_CASE(RHS_MODE_K)
+        CLT_CASE(RHS_MODE_S1)
+        CLT_CASE(RHS_MODE_S2)
+        CLT_CASE(RHS_MODE_S3)
+        CLT_CASE(RHS_MODE_S4)
+    default:
+        return cudaErrorInvalidValue;
+    }
+#undef CLT_CASE
+}
+
+int rhs_default_tile_z() { return 14; }
+
+cudaError_t launch_rhs(const RhsArgs &a, int mode, bool has_v0, int tile_z, cudaStream_t s)
+{
+    switch (tile_z) {
+    case 8: return launch_rhs_tz<8>(a, mode, has_v0, s);
+    case 12: return launch_rhs_tz<12>(a, mode, has_v0, s);
+    case 14: return launch_rhs_tz<14>(a, mode, has_v0, s);
+    case 16: return launch_rhs_tz<16>(a, mode, has_v0, s);
+    default: return cudaErrorInvalidValue;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// curl_kernel: J1 = curl_c(B - B0) on interior nodes (eq 6).  Same sweep, 3 staged fields.
+// ---------------------------------------------------------------------------------------------
+template <int TZ>
+struct CurlSmem {
+    static constexpr int HT = (TZ + 4) * SW;
+    double stage[2][3][HT];    // B1_R, B1_phi, B1_Z of the centre plane
+    double sR[SW];
+};
+
+template <int TZ>
+__global__ void __launch_bounds__(TR *TZ, 2) curl_kernel(const __grid_constant__ CurlArgs a)
+{
+    __shared__ CurlSmem<TZ> S;
+    const Layout &L = a.L;
+    const Phys &ph = a.ph;
+    const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * TR + tx;
+    const int i0 = 2 + TR * blockIdx.x, k0 = 2 + TZ * blockIdx.y;
+    const int i = i0 + tx, k = k0 + ty;
+    const bool valid = (i <= L.nR - 3) && (k <= L.nZ - 3);
+    const int ic = min(i, L.nR - 1), kc = min(k, L.nZ - 1);
+    const int ja = (int)(((long long)L.nphi * blockIdx.z) / a.phi_chunks);
+    const int jb = (int)(((long long)L.nphi * (blockIdx.z + 1)) / a.phi_chunks);
+    const long long off2 = (long long)kc * L.pR + (LP + ic);
+    const int cs = (ty + 2) * SW + (tx + 2);
+
+    constexpr int NH = 4 * TR + 4 * TZ;
+    static_assert(NH <= TR * TZ, "tile too small for one halo node per thread");
+    int hx, hy;
+    if (tid < 4 * TR) {
+        const int r = tid / TR;
+        hx = tid % TR;
+        hy = (r < 2) ? r - 2 : TZ + (r - 2);
+    } else {
+        const int t = tid - 4 * TR, c = t & 3;
+        hy = t >> 2;
+        hx = (c < 2) ? c - 2 : TR + (c - 2);
+    }
+    const bool is_halo = tid < NH;
+    const int hi = min(i0 + hx, L.nR - 1), hk = min(k0 + hy, L.nZ - 1);
+    const long long hoff2 = (long long)hk * L.pR + (LP + hi);
+    const int hs = (hy + 2) * SW + (hx + 2);
+    if (tid < SW) S.sR[tid] = a.R[min(i0 - 2 + tid, L.nR - 1)];
+
+    const double *tab = a.tab;
+    const double b0R = __ldg(tab + T_B0R * L.plane + off2), b0P = __ldg(tab + T_B0P * L.plane + off2),
+                 b0Z = __ldg(tab + T_B0Z * L.plane + off2);
+    double h0R = 0.0, h0P = 0.0, h0Z = 0.0;
+    if (is_halo) {
+        h0R = __ldg(tab + T_B0R * L.plane + hoff2);
+        h0P = __ldg(tab + T_B0P * L.plane + hoff2);
+        h0Z = __ldg(tab + T_B0Z * L.plane + hoff2);
+    }
+    const double iR = __ldg(a.invR + ic);
+
+    double bR[5], bZ[5], bP[3];    // B1 of planes j-2..j+2 (R, Z) and j..j+2 (phi) at the own node
+    auto lead = [&](int jl) {
+        const long long g = (long long)wrap_phi(jl, L.nphi) * L.plane + off2;
+        bR[4] = __ldg(a.B + 0 * L.field + g) - b0R;    // equilibrium subtracted before differencing (H2)
+        bP[2] = __ldg(a.B + 1 * L.field + g) - b0P;
+        bZ[4] = __ldg(a.B + 2 * L.field + g) - b0Z;
+    };
+    auto advance = [&]() {
+#pragma unroll
+        for (int d = 0; d < 4; ++d) { bR[d] = bR[d + 1]; bZ[d] = bZ[d + 1]; }
+        bP[0] = bP[1]; bP[1] = bP[2];
+    };
+#pragma unroll 1
+    for (int jl = ja - 2; jl <= ja + 1; ++jl) { lead(jl); advance(); }
+
+#pragma unroll 1
+    for (int j = ja; j < jb; ++j) {
+        const int buf = j & 1;
+        lead(j + 2);
+        S.stage[buf][0][cs] = bR[2];
+        S.stage[buf][1][cs] = bP[0];
+        S.stage[buf][2][cs] = bZ[2];
+        if (is_halo) {
+            const long long g = (long long)j * L.plane + hoff2;
+            S.stage[buf][0][hs] = __ldg(a.B + 0 * L.field + g) - h0R;
+            S.stage[buf][1][hs] = __ldg(a.B + 1 * L.field + g) - h0P;
+            S.stage[buf][2][hs] = __ldg(a.B + 2 * L.field + g) - h0Z;
+        }
+        __syncthreads();
+        const double *sBR = &S.stage[buf][0][cs], *sBP = &S.stage[buf][1][cs], *sBZ = &S.stage[buf][2][cs];
+        const double cPi = ph.cP1 * iR;
+        const double dP_BZ = fd1(bZ[0], bZ[1], bZ[3], bZ[4]);
+        const double dP_BR = fd1(bR[0], bR[1], bR[3], bR[4]);
+        const double dZ_BP = fd1(sBP[-2 * SW], sBP[-SW], sBP[SW], sBP[2 * SW]);
+        const double dZ_BR = fd1(sBR[-2 * SW], sBR[-SW], sBR[SW], sBR[2 * SW]);
+        const double dR_BZ = fd1(sBZ[-2], sBZ[-1], sBZ[1], sBZ[2]);
+        const double *r = &S.sR[tx + 2];
+        const double dR_RBP = fd1(r[-2] * sBP[-2], r[-1] * sBP[-1], r[1] * sBP[1], r[2] * sBP[2]);
+        if (valid) {
+            const long long g = (long long)j * L.plane + off2;
+            a.J1[0 * L.field + g] = dP_BZ * cPi - dZ_BP * ph.cZ1;
+            a.J1[1 * L.field + g] = dZ_BR * ph.cZ1 - dR_BZ * ph.cR1;
+            a.J1[2 * L.field + g] = dR_RBP * (ph.cR1 * iR) - dP_BR * cPi;
+        }
+        advance();
+    }
+}
+
+cudaError_t launch_curl(const CurlArgs &a, int tile_z, cudaStream_t s)
+{
+    (void)tile_z;
+    constexpr int TZ = 8;
+    dim3 block(TR, TZ, 1);
+    dim3 grid((a.L.nR - 4 + TR - 1) / TR, (a.L.nZ - 4 + TZ - 1) / TZ, a.phi_chunks);
+    curl_kernel<TZ><<<grid, block, 0, s>>>(a);
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------
+// Axisymmetric tables (once per clt_set_equilibrium): J0 = curl_c B0 etc.
+// ---------------------------------------------------------------------------------------------
+__global__ void tables_kernel(Layout L, Phys ph, double *tab, const double *R, const double *invR)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, k = blockIdx.y * blockDim.y + threadIdx.y;
+    if (i >= L.nR || k >= L.nZ) return;
+    const long long o = (long long)k * L.pR + (LP + i);
+    auto T = [&](int t) -> double * { return tab + (long long)t * L.plane; };
+    const double v0R = T(T_V0R)[o], v0P = T(T_V0P)[o], v0Z = T(T_V0Z)[o];
+    const double B0R = T(T_B0R)[o], B0P = T(T_B0P)[o], B0Z = T(T_B0Z)[o];
+    // E0 = v0 x B0 at every node (E1 is needed on the boundary layers too)
+    T(T_E0R)[o] = v0P * B0Z - v0Z * B0P;
+    T(T_E0P)[o] = v0Z * B0R - v0R * B0Z;
+    T(T_E0Z)[o] = v0R * B0P - v0P * B0R;
+    const bool interior = i >= 2 && i <= L.nR - 3 && k >= 2 && k <= L.nZ - 3;
+    double out[T_COUNT];
+    for (int t = T_J0R; t < T_COUNT; ++t) out[t] = 0.0;
+    if (interior) {
+        const int pR = L.pR;
+        auto dR = [&](int t) { const double *f = T(t) + o; return fd1(f[-2], f[-1], f[1], f[2]) * ph.cR1; };
+        auto dZ = [&](int t) { const double *f = T(t) + o; return fd1(f[-2 * pR], f[-pR], f[pR], f[2 * pR]) * ph.cZ1; };
+        const double iR = invR[i];
+        const double *bp = T(T_B0P) + o;
+        const double dR_RB0P = fd1(R[i - 2] * bp[-2], R[i - 1] * bp[-1], R[i + 1] * bp[1], R[i + 2] * bp[2]) * ph.cR1;
+        out[T_J0R] = -dZ(T_B0P);
+        out[T_J0P] = dZ(T_B0R) - dR(T_B0Z);
+        out[T_J0Z] = dR_RB0P * iR;
+        out[T_GR_RHO0] = dR(T_RHO0); out[T_GZ_RHO0] = dZ(T_RHO0);
+        out[T_GR_P0] = dR(T_P0);     out[T_GZ_P0] = dZ(T_P0);
+        const double gRR = dR(T_V0R), gZR = dZ(T_V0R), gRP = dR(T_V0P), gZP = dZ(T_V0P), gRZ = dR(T_V0Z), gZZ = dZ(T_V0Z);
+        out[T_GR_V0R] = gRR; out[T_GZ_V0R] = gZR; out[T_GR_V0P] = gRP; out[T_GZ_V0P] = gZP;
+        out[T_GR_V0Z] = gRZ; out[T_GZ_V0Z] = gZZ;
+        out[T_DIVV0] = gRR + v0R * iR + gZZ;
+        out[T_A0R] = v0R * gRR + v0Z * gZR - v0P * v0P * iR;
+        out[T_A0P] = v0R * gRP + v0Z * gZP + v0P * v0R * iR;
+        out[T_A0Z] = v0R * gRZ + v0Z * gZZ;
+    }
+    for (int t = T_J0R; t < T_COUNT; ++t)
+        if (t < T_E0R || t > T_E0Z) T(t)[o] = out[t];
+}
+
+cudaError_t launch_tables(const Layout &L, const Phys &ph, double *tab, const double *R, const double *invR,
+                          cudaStream_t s)
+{
+    dim3 block(32, 8), grid((L.nR + 31) / 32, (L.nZ + 7) / 8);
+    tables_kernel<<<grid, block, 0, s>>>(L, ph, tab, R, invR);
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------
+// a1: boundary layers.  The two outer node layers in R and Z hold the values given to
+// clt_set_state in every RK buffer (L123, L187-189); the step kernels never write them.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ bool boundary_node(const Layout &L, long long n, int &i, int &k, long long &row)
+{
+    // enumerate boundary nodes of one plane: 4 full rows (k = 0,1,nZ-2,nZ-1) then 4 columns of the other rows
+    const long long per_plane = 4LL * L.nR + 4LL * (L.nZ - 4);
+    row = n / per_plane;               // (field, phi plane) index
+    const long long r = n % per_plane;
+    if (r < 4LL * L.nR) {
+        const int kk = (int)(r / L.nR);
+        k = kk < 2 ? kk : L.nZ - 4 + kk;
+        i = (int)(r % L.nR);
+    } else {
+        const long long t = r - 4LL * L.nR;
+        k = 2 + (int)(t >> 2);
+        const int c = (int)(t & 3);
+        i = c < 2 ? c : L.nR - 4 + c;
+    }
+    return true;
+}
+
+__global__ void copy_boundary_kernel(Layout L, long long total, const double *src, double *d0, double *d1, double *d2)
+{
+    for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < total;
+         n += (long long)gridDim.x * blockDim.x) {
+        int i, k;
+        long long row;
+        boundary_node(L, n, i, k, row);
+        const long long o = row * L.plane + (long long)k * L.pR + (LP + i);
+        const double v = src ? src[o] : 0.0;
+        if (d0) d0[o] = v;
+        if (d1) d1[o] = v;
+        if (d2) d2[o] = v;
+    }
+}
+
+cudaError_t launch_copy_boundary(const Layout &L, int nfields, const double *src, double *d0, double *d1, double *d2,
+                                 cudaStream_t s)
+{
+    const long long total = (long long)nfields * L.nphi * (4LL * L.nR + 4LL * (L.nZ - 4));
+    const int block = 256;
+    const int grid = (int)((total + block - 1) / block < 148 * 16 ? (total + block - 1) / block : 148 * 16);
+    copy_boundary_kernel<<<grid, block, 0, s>>>(L, total, src, d0, d1, d2);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_zero_boundary(const Layout &L, int nfields, double *dst, cudaStream_t s)
+{
+    return launch_copy_boundary(L, nfields, nullptr, dst, nullptr, nullptr, s);
+}
+
+// ---------------------------------------------------------------------------------------------
+// a7 diagnostics (L139, L149, L430) and the SETDT minimum (Fig. 4).
+// One thread per interior (i, k) column; warp-shuffle + shared-memory block reduction; the block
+// partials are combined in a fixed order by a second, single-block kernel (deterministic).
+// ---------------------------------------------------------------------------------------------
+constexpr int DG_BX = 32, DG_BY = 8, DG_N = 6;   // kinetic, magnetic, magnetic_pert, magnetic_n1, max divB, min dt
+
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ double warp_max(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+__device__ __forceinline__ double warp_min(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+
+__global__ void __launch_bounds__(DG_BX *DG_BY) diag_kernel(const __grid_constant__ DiagArgs a)
+{
+    const Layout &L = a.L;
+    const Phys &ph = a.ph;
+    const int i = 2 + blockIdx.x * DG_BX + threadIdx.x, k = 2 + blockIdx.y * DG_BY + threadIdx.y;
+    const bool valid = i <= L.nR - 3 && k <= L.nZ - 3;
+    const bool deep = i >= 4 && i <= L.nR - 5 && k >= 4 && k <= L.nZ - 5;
+    double ke = 0.0, me = 0.0, mep = 0.0, men1 = 0.0, mdiv = 0.0, mdt = 100.0;
+    if (valid) {
+        const long long o = (long long)k * L.pR + (LP + i);
+        const double Ri = a.R[i], iR = a.invR[i];
+        const double b0R = a.tab[T_B0R * L.plane + o], b0P = a.tab[T_B0P * L.plane + o], b0Z = a.tab[T_B0Z * L.plane + o];
+        double fa[3] = { 0, 0, 0 }, fb[3] = { 0, 0, 0 };
+        const double dRi = fabs(Ri - a.R[i - 1]);
+        for (int j = 0; j < L.nphi; ++j) {
+            const long long g = (long long)j * L.plane + o;
+            const double rho = a.U[g], p = a.U[L.field + g];
+            const double vR = a.U[2 * L.field + g], vP = a.U[3 * L.field + g], vZ = a.U[4 * L.field + g];
+            const double BR = a.U[5 * L.field + g], BP = a.U[6 * L.field + g], BZ = a.U[7 * L.field + g];
+            const double b2 = BR * BR + BP * BP + BZ * BZ;
+            ke += 0.5 * rho * (vR * vR + vP * vP + vZ * vZ);
+            me += 0.5 * b2;
+            const double b1[3] = { BR - b0R, BP - b0P, BZ - b0Z };
+            mep += 0.5 * (b1[0] * b1[0] + b1[1] * b1[1] + b1[2] * b1[2]);
+            const double c = a.cs[j], s = a.cs[L.nphi + j];
+#pragma unroll
+            for (int d = 0; d < 3; ++d) { fa[d] += b1[d] * c; fb[d] += b1[d] * s; }
+            // SETDT, Fig. 4
+            const double cf = sqrt(fabs(ph.gamma * p / rho + b2 / rho));
+            const double dtx = dRi / ((fabs(vR) + cf) / a.cfl);
+            const double dtz = ph.dZ / ((fabs(vZ) + cf) / a.cfl);
+            const double dty = fabs(Ri * ph.dphi) / ((fabs(vP) + cf) / a.cfl);
+            mdt = fmin(mdt, fmin(dty, fmin(dtx, dtz)));
+            if (deep) {
+                // div_c B = d_R(R B_R)/R + d_phi B_phi / R + d_Z B_Z
+                const double *br = a.U + 5 * L.field + g, *bz = a.U + 7 * L.field + g;
+                const double *bp = a.U + 6 * L.field + o;
+                const int n = L.nphi;
+                const double dRR = fd1(a.R[i - 2] * br[-2], a.R[i - 1] * br[-1], a.R[i + 1] * br[1], a.R[i + 2] * br[2]);
+                const double dP = fd1(bp[(long long)wrap_phi(j - 2, n) * L.plane], bp[(long long)wrap_phi(j - 1, n) * L.plane],
+                                      bp[(long long)wrap_phi(j + 1, n) * L.plane], bp[(long long)wrap_phi(j + 2, n) * L.plane]);
+                const double dZ = fd1(bz[-2 * L.pR], bz[-L.pR], bz[L.pR], bz[2 * L.pR]);
+                mdiv = fmax(mdiv, fabs(dRR * ph.cR1 * iR + dP * ph.cP1 * iR + dZ * ph.cZ1));
+            }
+        }
+        const double w = Ri * ph.dR * ph.dphi * ph.dZ;
+        ke *= w; me *= w; mep *= w;
+        const double sc = 2.0 / (double)L.nphi;
+        double e1 = 0.0;
+#pragma unroll
+        for (int d = 0; d < 3; ++d) { const double A = fa[d] * sc, B = fb[d] * sc; e1 += A * A + B * B; }
+        men1 = 0.25 * e1 * (Ri * ph.dR * ph.dZ * ph.Lphi);
+    }
+    __shared__ double red[DG_BY][DG_N];
+    ke = warp_sum(ke); me = warp_sum(me); mep = warp_sum(mep); men1 = warp_sum(men1);
+    mdiv = warp_max(mdiv); mdt = warp_min(mdt);
+    if (threadIdx.x == 0) {
+        double *r = red[threadIdx.y];
+        r[0] = ke; r[1] = me; r[2] = mep; r[3] = men1; r[4] = mdiv; r[5] = mdt;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0 && threadIdx.y == 0) {
+        double acc[DG_N] = { 0, 0, 0, 0, 0, 100.0 };
+        for (int w = 0; w < DG_BY; ++w) {
+            for (int q = 0; q < 4; ++q) acc[q] += red[w][q];
+            acc[4] = fmax(acc[4], red[w][4]);
+            acc[5] = fmin(acc[5], red[w][5]);
+        }
+        double *dst = a.partial + (long long)(blockIdx.y * gridDim.x + blockIdx.x) * DG_N;
+        for (int q = 0; q < DG_N; ++q) dst[q] = acc[q];
+    }
+}
+
+__global__ void __launch_bounds__(256) diag_final_kernel(const double *partial, int nblocks, double *result)
+{
+    __shared__ double red[8][DG_N];
+    double acc[DG_N] = { 0, 0, 0, 0, 0, 100.0 };
+    for (int b = threadIdx.x; b < nblocks; b += 256) {
+        const double *p = partial + (long long)b * DG_N;
+        for (int q = 0; q < 4; ++q) acc[q] += p[q];
+        acc[4] = fmax(acc[4], p[4]);
+        acc[5] = fmin(acc[5], p[5]);
+    }
+    for (int q = 0; q < 4; ++q) acc[q] = warp_sum(acc[q]);
+    acc[4] = warp_max(acc[4]);
+    acc[5] = warp_min(acc[5]);
+    const int w = threadIdx.x >> 5;
+    if ((threadIdx.x & 31) == 0)
+        for (int q = 0; q < DG_N; ++q) red[w][q] = acc[q];
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double out[DG_N] = { 0, 0, 0, 0, 0, 100.0 };
+        for (int ww = 0; ww < 8; ++ww) {
+            for (int q = 0; q < 4; ++q) out[q] += red[ww][q];
+            out[4] = fmax(out[4], red[ww][4]);
+            out[5] = fmin(out[5], red[ww][5]);
+        }
+        for (int q = 0; q < DG_N; ++q) result[q] = out[q];
+    }
+}
+
+int diag_blocks(const Layout &L)
+{
+    return ((L.nR - 4 + DG_BX - 1) / DG_BX) * ((L.nZ - 4 + DG_BY - 1) / DG_BY);
+}
+
+cudaError_t launch_diag(const DiagArgs &a, int nblocks, double *result6, cudaStream_t s)
+{
+    dim3 block(DG_BX, DG_BY), grid((a.L.nR - 4 + DG_BX - 1) / DG_BX, (a.L.nZ - 4 + DG_BY - 1) / DG_BY);
+    diag_kernel<<<grid, block, 0, s>>>(a);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    diag_final_kernel<<<1, 256, 0, s>>>(a.partial, nblocks, result6);
+    return cudaGetLastError();
+}
+
+cudaError_t configure_kernels() { return cudaSuccess; }
+
+}  // namespace clt

@@ -1,0 +1,45 @@
+"""Helpers shared by the GPU parity tests: build both sides from one seeded problem, error metric H4."""
+import numpy as np
+
+import oracle as orc
+from paper_1812_00525_b200 import inputs
+
+RHS_TOL = 1e-12      # BASELINE.json north_star: relative L-infinity per RHS call
+STEP_TOL = 1e-9      # ... and after 100 RK4 steps
+
+
+def make_oracle(prob, **over):
+    c = prob.cfg
+    par = dict(gamma=c.gamma, eta=c.eta, nu=c.nu, D=c.D, kappa=c.kappa, dt=prob.dt)
+    par.update(over)
+    o = orc.Oracle(c.nR, c.nphi, c.nZ, c.Rmin, c.Rmax, c.Zmin, c.Zmax, c.phi_extent, **par)
+    o.set_equilibrium(prob.U0)
+    o.set_state(prob.U)
+    return o
+
+
+def make_gpu(prob, set_eq=True, **over):
+    from paper_1812_00525_b200 import clt
+    c = prob.cfg
+    par = dict(gamma=c.gamma, eta=c.eta, nu=c.nu, D=c.D, kappa=c.kappa, dt=prob.dt, cfl=c.cfl)
+    par.update(over)
+    g = clt.Clt(c.nR, c.nphi, c.nZ, c.Rmin, c.Rmax, c.Zmin, c.Zmax, c.phi_extent, **par)
+    if set_eq:
+        g.set_equilibrium(np.ascontiguousarray(prob.U0))
+    g.set_state(np.ascontiguousarray(prob.U))
+    return g
+
+
+def rel_linf(got, exp):
+    """Per leading-index field: max|g - c| / max(max|c|, tiny) over all nodes (boundary layers must agree too)."""
+    out = []
+    for f in range(exp.shape[0]):
+        s = max(np.abs(exp[f]).max(), 1e-300)
+        out.append(float(np.abs(got[f] - exp[f]).max() / s))
+    return out
+
+
+def assert_close(got, exp, tol, what):
+    errs = rel_linf(got, exp)
+    assert max(errs) <= tol, f"{what}: rel Linf per field {errs} > {tol}"
+    return errs

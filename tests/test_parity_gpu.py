@@ -1,0 +1,142 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same seeded
+inputs.  Tolerances are BASELINE.json's: rel. L-infinity 1e-12 per RHS call, 1e-9 after 100 RK4 steps."""
+import numpy as np
+import pytest
+
+from paper_1812_00525_b200 import inputs
+from parity_util import RHS_TOL, STEP_TOL, assert_close, make_gpu, make_oracle, rel_linf
+
+pytestmark = pytest.mark.gpu
+
+
+def _problems():
+    return {
+        "config1": lambda: inputs.make_problem(1),
+        # ragged tails in both tile directions, odd sizes, several tiles: 32-wide x 14-high tiles
+        "ragged-77x9x53": lambda: inputs.make_custom_problem(77, 9, 53, index=11),
+        "min-9x5x9": lambda: inputs.make_custom_problem(9, 5, 9, index=12),
+        "rotating-v0": lambda: inputs.make_custom_problem(45, 8, 37, index=13, rotation=0.05),
+        "big-amplitude": lambda: inputs.make_custom_problem(40, 12, 40, index=14, amplitude_scale=200.0),
+    }
+
+
+@pytest.mark.parametrize("name", list(_problems()))
+def test_curl_J1_matches_oracle(name):
+    prob = _problems()[name]()
+    o, g = make_oracle(prob), make_gpu(prob)
+    J_o = o.curl_J1(prob.U)
+    J_g = g.curl_J1()
+    assert_close(J_g, J_o, RHS_TOL, f"curl_J1 {name}")
+    assert np.all(J_g[:, :, :2] == 0) and np.all(J_g[..., -2:] == 0)
+
+
+@pytest.mark.parametrize("name", list(_problems()))
+@pytest.mark.parametrize("tile_z", [0, 8, 12, 16])
+def test_rhs_matches_oracle(name, tile_z):
+    prob = _problems()[name]()
+    o, g = make_oracle(prob), make_gpu(prob)
+    g.set_tuning(tile_z=tile_z)
+    K_o = o.rhs()
+    K_g = g.rhs()
+    assert_close(K_g, K_o, RHS_TOL, f"rhs {name} tile_z={tile_z}")
+    assert np.all(K_g[:, :, :2] == 0) and np.all(K_g[:, :, -2:] == 0) and np.all(K_g[..., :2] == 0) and np.all(K_g[..., -2:] == 0)
+    # the state is untouched by clt_rhs, scratch buffers restored: a second call gives the same bits
+    assert np.array_equal(g.get_state(), prob.U)
+    assert np.array_equal(g.rhs(), K_g)
+
+
+def test_rhs_with_zero_equilibrium_matches_oracle():
+    prob = inputs.make_custom_problem(40, 8, 36, index=15, amplitude_scale=100.0)
+    o = make_oracle(prob)
+    o.set_equilibrium(None)
+    g = make_gpu(prob, set_eq=False)
+    assert_close(g.rhs(), o.rhs(), RHS_TOL, "rhs, U0 = 0")
+
+
+def test_rhs_with_large_dissipation_matches_oracle():
+    prob = inputs.make_custom_problem(40, 8, 36, index=16, amplitude_scale=50.0)
+    over = dict(eta=3e-3, nu=2e-3, D=1e-3, kappa=4e-3)
+    o, g = make_oracle(prob, **over), make_gpu(prob, **over)
+    assert_close(g.rhs(), o.rhs(), RHS_TOL, "rhs, large dissipation")
+
+
+@pytest.mark.parametrize("name,steps", [("config1", 10), ("ragged-77x9x53", 100), ("rotating-v0", 100), ("min-9x5x9", 20)])
+def test_steps_match_oracle(name, steps):
+    prob = _problems()[name]()
+    o, g = make_oracle(prob), make_gpu(prob)
+    o.step(steps)
+    g.step(steps)
+    U_o, U_g = o.get_state(), g.get_state()
+    assert_close(U_g, U_o, STEP_TOL, f"{steps} RK4 steps {name}")
+    # the perturbation (what actually evolves) must agree too, relative to its own size
+    ref = np.repeat(prob.U0[:, None], prob.cfg.nphi, axis=1)
+    assert_close(U_g - ref + 1e-300, U_o - ref + 1e-300, 1e-7, f"{steps} RK4 steps {name}, perturbation")
+    # frozen boundary layers
+    assert np.array_equal(U_g[:, :, :2], prob.U[:, :, :2]) and np.array_equal(U_g[..., -2:], prob.U[..., -2:])
+    d = g.diagnostics()
+    assert d["step"] == steps and abs(d["time"] - steps * prob.dt) < 1e-12
+    assert np.abs(U_g - prob.U).max() > 1e-7          # the state really moved
+
+
+def test_config2_100_steps_match_oracle():
+    prob = inputs.make_problem(2)
+    o, g = make_oracle(prob), make_gpu(prob)
+    o.step(prob.cfg.steps)
+    g.step(prob.cfg.steps)
+    assert_close(g.get_state(), o.get_state(), STEP_TOL, "config 2, 100 RK4 steps")
+
+
+@pytest.mark.parametrize("chunks,graph", [(2, 0), (4, 0), (1, 1), (2, 1)])
+def test_phi_chunks_and_graph_give_identical_bits(chunks, graph):
+    prob = inputs.make_problem(1)
+    g0 = make_gpu(prob)
+    g0.step(3)
+    ref = g0.get_state()
+    g1 = make_gpu(prob)
+    g1.set_tuning(phi_chunks=chunks, use_graph=graph)
+    g1.step(2)
+    g1.step(1)
+    assert np.array_equal(g1.get_state(), ref)
+
+
+def test_diagnostics_and_suggest_dt_match_oracle():
+    prob = inputs.make_custom_problem(45, 16, 37, index=17, amplitude_scale=30.0)
+    o, g = make_oracle(prob), make_gpu(prob)
+    o.step(3)
+    g.step(3)
+    do, dg = o.diagnostics(), g.diagnostics()
+    for k in ("kinetic", "magnetic", "magnetic_pert", "magnetic_n1"):
+        assert abs(dg[k] - do[k]) <= 1e-12 * abs(do[k]), (k, dg[k], do[k])
+    assert abs(dg["max_divB"] - do["max_divB"]) <= 1e-10 * abs(do["max_divB"]) + 1e-15, (dg["max_divB"], do["max_divB"])
+    assert abs(g.suggest_dt(0.5) - o.setdt(0.5)) <= 1e-13 * o.setdt(0.5)
+    assert abs(g.suggest_dt(0.0) - o.setdt(prob.cfg.cfl)) <= 1e-13 * o.setdt(prob.cfg.cfl)
+
+
+def test_device_pointers_and_call_order():
+    import torch
+    from paper_1812_00525_b200 import clt
+    prob = inputs.make_problem(1)
+    c = prob.cfg
+    g = clt.Clt.from_config(c, prob.dt)
+    with pytest.raises(clt.CltError) as e:
+        g.step(1)
+    assert e.value.code == clt.CLT_ESTATE
+    with pytest.raises(clt.CltError):
+        g.rhs()
+    U0d = torch.from_numpy(prob.U0).cuda()
+    Ud = torch.from_numpy(prob.U).cuda()
+    g.set_equilibrium(U0d)
+    g.set_state(Ud)
+    out = torch.empty_like(Ud)
+    g.get_state(out)
+    torch.cuda.synchronize()
+    assert torch.equal(out, Ud)
+    Kd = torch.empty_like(Ud)
+    g.rhs(Kd)
+    torch.cuda.synchronize()
+    g2 = make_gpu(prob)
+    assert np.array_equal(Kd.cpu().numpy(), g2.rhs())
+    g.set_equilibrium(U0d)                       # invalidates the state
+    with pytest.raises(clt.CltError):
+        g.step(1)
+    assert g.launch_count > 0
