@@ -1,0 +1,290 @@
+#!/usr/bin/env python
+"""bench.py -- measures BASELINE.json's metric: FP64 grid-point RK4 updates/s of the fused CLTx hot path
+(curl J1 + fused RHS/RK4 kernels) on config 4 (512 x 64 x 512), and the achieved fraction of the HBM roofline.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 4]
+
+One "step" = one classical RK4 step = 4 x (curl_J1 + fused RHS) over the whole grid = all rows of SURVEY 8(a).
+Multi-GPU: the path does not shard in this round (north_star: one GPU, no halo exchange) -- "replicas only":
+N ranks run N independent replicas, value = sum of the replicas' updates / max-over-ranks time.
+--impl reference times the CPU oracle (oracle/) on a bounded sample of the same workload, rank 0 only.
+Prints ONE JSON line.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "FP64 grid-point RK4 updates/sec"
+UNIT = "updates/s"
+BYTES_PER_UPDATE = 164 * 8          # 164 doubles per grid point per RK4 step
+RHS_DOUBLES = {1: 27, 2: 43, 3: 43, 4: 27}   # per point per launch of the fused RHS+RK4 kernel
+CURL_DOUBLES = 6
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p)).get("hbm_gbs"), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+                for n, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                continue
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_rate(grid, steps, warmup=0):
+    """Times the CPU oracle as it stands on a bounded sample (same recipe, smaller grid). Returns dict."""
+    import oracle as orc
+    from paper_1812_00525_b200 import inputs
+    nR, nphi, nZ = grid
+    prob = inputs.make_custom_problem(nR, nphi, nZ, index=4)
+    c = prob.cfg
+    o = orc.Oracle(c.nR, c.nphi, c.nZ, c.Rmin, c.Rmax, c.Zmin, c.Zmax, c.phi_extent, gamma=c.gamma, eta=c.eta, nu=c.nu,
+                   D=c.D, kappa=c.kappa, dt=prob.dt)
+    o.set_equilibrium(prob.U0)
+    o.set_state(prob.U)
+    if warmup:
+        o.step(warmup)
+    t0 = time.perf_counter()
+    o.step(steps)
+    dt = time.perf_counter() - t0
+    cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    return {"value": c.interior * steps / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{steps} RK4 step(s) of the config-4 recipe on a {nR}x{nphi}x{nZ} grid ({c.interior} interior nodes), "
+                      f"oracle/clt_oracle.c as it stands (gcc -O2, OpenMP over nodes)", "seconds": dt, "ms_per_step": 1e3 * dt / steps}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cores = os.cpu_count() or 1
+    # bounded sample: about (K+W) steps within ~2-3 minutes at ~0.05 M updates/s/core
+    budget_updates = 0.05e6 * cores * 150.0 / max(1, args.steps + args.warmup)
+    grid = (128, 16, 128) if budget_updates < 2.0e6 else (256, 32, 256)
+    if budget_updates < 0.25e6:
+        grid = (64, 16, 64)
+    r = oracle_rate(grid, args.steps, args.warmup)
+    line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "config 4 recipe (512x64x512 box, seeded perturbations), bounded sample: " + r["sample"]},
+            "cpu_baseline": {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_1812_00525_b200 import build as clt_build
+    from paper_1812_00525_b200 import clt, inputs
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        clt_build.build()
+    if world > 1:
+        dist.barrier()
+
+    prob = inputs.make_problem(args.config)
+    cfg = prob.cfg
+    g = clt.Clt.from_config(cfg, prob.dt, device=f"cuda:{local}")
+    if args.tile_z or args.phi_chunks or args.graph:
+        g.set_tuning(args.tile_z, args.phi_chunks, args.graph)
+    hU0 = torch.from_numpy(prob.U0).pin_memory()
+    hU = torch.from_numpy(prob.U).pin_memory()
+    hOut = torch.empty_like(hU).pin_memory()
+    g.set_equilibrium(hU0)
+    g.set_state(hU)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    # ---- device-resident throughput -------------------------------------------------------------
+    g.step(args.warmup)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    g.set_profiling(not args.graph)
+    launches0 = g.launch_count
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(g.torch_stream)
+    g.step(args.steps)
+    e1.record(g.torch_stream)
+    barrier()
+    ms = e0.elapsed_time(e1)
+    launches = g.launch_count - launches0
+    prof = g.get_profile()
+    g.set_profiling(False)
+    clocks = sampler.stop()
+    if world > 1:
+        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    d = g.diagnostics()
+    finite = all(np.isfinite(d[k]) for k in ("kinetic", "magnetic", "max_divB"))
+
+    # ---- end to end through the C ABI with host buffers -----------------------------------------
+    e2e_steps = max(1, min(args.e2e_steps, args.steps))
+    g.set_state(hU); g.step(1); g.get_state(hOut)        # warm-up of the copy path
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        g.set_state(hU)          # H2D of the step's input from pinned host memory
+        g.step(1)
+        g.get_state(hOut)        # D2H of the result (synchronous: host destination)
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    state_bytes = int(np.prod(cfg.shape)) * 8
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    ms_step = ms / args.steps
+    value = world * cfg.interior * args.steps / (ms * 1e-3)
+    peak, peak_src = measured_peaks()
+    # dominant kernel: the fused RHS + RK4 stage-combine kernel (its four stage variants pooled)
+    n_rhs = sum(prof["n_rhs"][1:5])
+    ms_rhs = sum(prof["ms_rhs"][1:5])
+    roof = None
+    if n_rhs:
+        bytes_per_launch = sum(RHS_DOUBLES[s] * prof["n_rhs"][s] for s in (1, 2, 3, 4)) * 8.0 * cfg.interior / n_rhs
+        dur = ms_rhs / n_rhs * 1e-3
+        ach = bytes_per_launch / dur / 1e9
+        per_stage = {f"stage{s}": {"ms": prof["ms_rhs"][s] / prof["n_rhs"][s],
+                                   "GBps": RHS_DOUBLES[s] * 8.0 * cfg.interior / (prof["ms_rhs"][s] / prof["n_rhs"][s] * 1e-3) / 1e9}
+                     for s in (1, 2, 3, 4) if prof["n_rhs"][s]}
+        curl = None
+        if prof["n_curl"]:
+            cms = prof["ms_curl"] / prof["n_curl"]
+            curl = {"ms": cms, "GBps": CURL_DOUBLES * 8.0 * cfg.interior / (cms * 1e-3) / 1e9}
+        roof = {"bound": "hbm", "kernel": "rhs_kernel (fused RHS + RK4 stage combine, 4 stage variants pooled)",
+                "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": args.traffic,
+                "peak_source": peak_src + ", burst figure", "avg_launch_ms": ms_rhs / n_rhs,
+                "algorithmic_bytes_per_launch": bytes_per_launch, "share_of_step": ms_rhs / (ms_rhs + prof["ms_curl"]),
+                "per_stage": per_stage, "curl_kernel": curl,
+                "whole_step": {"GBps": BYTES_PER_UPDATE * cfg.interior / (ms_step * 1e-3) / 1e9,
+                               "frac": BYTES_PER_UPDATE * cfg.interior / (ms_step * 1e-3) / 1e9 / peak}}
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        cores = os.cpu_count() or 1
+        grid = (256, 32, 256) if cores >= 16 else (128, 16, 128)
+        cpu = oracle_rate(grid, 2 if cores >= 16 else 6)
+        cpu = {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample")}
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": f"config {cfg.index}: {cfg.nR}x{cfg.nphi}x{cfg.nZ} (R x phi x Z), {cfg.interior} interior nodes, "
+                                   f"seeded reference state + perturbations (BASELINE.json configs[{cfg.index - 1}])",
+                       "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "l2": f"working set {g.workspace_bytes / 1e9:.2f} GB per replica, far larger than the 126 MB L2 (no flush needed)",
+                       "dt": prob.dt, "tile_z": args.tile_z, "phi_chunks": args.phi_chunks, "graph": args.graph,
+                       "state_finite_after_run": bool(finite)},
+            "clocks": clocks,
+            "e2e": {"value": world * cfg.interior * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": state_bytes,
+                    "d2h_bytes_per_step": state_bytes, "steps": e2e_steps,
+                    "how": "clt_set_state(pinned host) + clt_step(1) + clt_get_state(pinned host) per step, wall clock"},
+            "gpu_launches": launches,
+            "roofline": roof, "cpu_baseline": cpu,
+            "achieved_GBps_whole_step": BYTES_PER_UPDATE * cfg.interior / (ms_step * 1e-3) / 1e9}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--tile-z", dest="tile_z", type=int, default=0)
+    ap.add_argument("--phi-chunks", dest="phi_chunks", type=int, default=0)
+    ap.add_argument("--graph", type=int, default=0)
+    ap.add_argument("--e2e-steps", dest="e2e_steps", type=int, default=3)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--traffic", type=float, default=None,
+                    help="dram bytes per launch of the dominant kernel from an ncu --set full capture (profiles/)")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

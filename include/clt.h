@@ -143,6 +143,19 @@ int clt_suggest_dt(clt_ctx *ctx, double cfl, double *dt_out);
  * fused RHS kernel, number of phi chunks per tile, use of a CUDA graph for clt_step.              */
 int clt_set_tuning(clt_ctx *ctx, int tile_z, int phi_chunks, int use_graph);
 
+/* Per-kernel device timing for the roofline report.  With profiling enabled (and use_graph = 0)
+ * every hot-path launch of clt_step / clt_rhs is bracketed by CUDA events on the context's stream;
+ * clt_get_profile() synchronises, sums the elapsed times per kernel kind since profiling was
+ * (re-)enabled, and resets the record.  rhs index = RK4 stage 1..4, 0 = clt_rhs' K-only variant.
+ * At most 8192 launches are recorded; later ones are counted in `dropped`.                       */
+typedef struct {
+    double ms_curl;  int64_t n_curl;
+    double ms_rhs[5]; int64_t n_rhs[5];
+    int64_t dropped;
+} clt_profile;
+int clt_set_profiling(clt_ctx *ctx, int enable);
+int clt_get_profile(clt_ctx *ctx, clt_profile *out);
+
 /* Number of kernels launched by this context so far (for bench.py's gpu_launches).               */
 int64_t clt_launch_count(const clt_ctx *ctx);
 

@@ -35,10 +35,15 @@ class clt_diag(ctypes.Structure):
                 ("time", ctypes.c_double)]
 
 
+class clt_profile(ctypes.Structure):
+    _fields_ = [("ms_curl", ctypes.c_double), ("n_curl", ctypes.c_int64), ("ms_rhs", ctypes.c_double * 5),
+                ("n_rhs", ctypes.c_int64 * 5), ("dropped", ctypes.c_int64)]
+
+
 # every symbol include/clt.h declares
 EXPORTS = ["clt_workspace_bytes", "clt_create", "clt_destroy", "clt_set_equilibrium", "clt_set_state", "clt_get_state",
            "clt_rhs", "clt_curl_J1", "clt_step", "clt_set_dt", "clt_diagnostics", "clt_suggest_dt", "clt_set_tuning",
-           "clt_launch_count", "clt_stream", "clt_strerror", "clt_last_cuda_error", "clt_version"]
+           "clt_set_profiling", "clt_get_profile", "clt_launch_count", "clt_stream", "clt_strerror", "clt_last_cuda_error", "clt_version"]
 
 _lib = None
 
@@ -80,6 +85,10 @@ def load():
     L.clt_suggest_dt.argtypes = [vp, d, ctypes.POINTER(d)]
     L.clt_set_tuning.restype = i
     L.clt_set_tuning.argtypes = [vp, i, i, i]
+    L.clt_set_profiling.restype = i
+    L.clt_set_profiling.argtypes = [vp, i]
+    L.clt_get_profile.restype = i
+    L.clt_get_profile.argtypes = [vp, ctypes.POINTER(clt_profile)]
     L.clt_launch_count.restype = ctypes.c_int64
     L.clt_launch_count.argtypes = [vp]
     L.clt_stream.restype = vp
@@ -204,6 +213,15 @@ class Clt:
 
     def set_tuning(self, tile_z=0, phi_chunks=0, use_graph=0):
         self._ck(self.L.clt_set_tuning(self.h, int(tile_z), int(phi_chunks), int(use_graph)))
+
+    def set_profiling(self, enable=True):
+        self._ck(self.L.clt_set_profiling(self.h, int(bool(enable))))
+
+    def get_profile(self):
+        p = clt_profile()
+        self._ck(self.L.clt_get_profile(self.h, ctypes.byref(p)))
+        return {"ms_curl": p.ms_curl, "n_curl": p.n_curl, "ms_rhs": list(p.ms_rhs), "n_rhs": list(p.n_rhs),
+                "dropped": p.dropped}
 
     @property
     def launch_count(self):

@@ -31,6 +31,12 @@ struct clt_ctx {
     int graph_tile_z, graph_chunks;
     bool graph_v0;
     char cuda_err[256];
+    // per-kernel event timing (clt_set_profiling)
+    bool profiling;
+    std::vector<cudaEvent_t> *ev;      // pairs: start, stop
+    std::vector<int> *ev_kind;         // 0..4 rhs mode, 5 curl
+    size_t ev_used;
+    int64_t ev_dropped;
 };
 
 namespace {
@@ -107,6 +113,17 @@ int copy_out(clt_ctx *ctx, double *dst, const double *src_padded, size_t rows)
     return CLT_OK;
 }
 
+void free_profile(clt_ctx *ctx)
+{
+    if (ctx->ev) {
+        for (cudaEvent_t e : *ctx->ev) cudaEventDestroy(e);
+        delete ctx->ev;
+        ctx->ev = nullptr;
+    }
+    delete ctx->ev_kind;
+    ctx->ev_kind = nullptr;
+}
+
 void destroy_graph(clt_ctx *ctx)
 {
     if (ctx->graph_exec) {
@@ -123,6 +140,29 @@ int effective_chunks(const clt_ctx *ctx)
     return c;
 }
 
+constexpr size_t MAX_PROFILED = 8192;
+
+// returns the index of the event pair to use for this launch, or -1
+long prof_begin(clt_ctx *ctx, int kind)
+{
+    if (!ctx->profiling || ctx->use_graph) return -1;
+    if (ctx->ev_used >= MAX_PROFILED) { ctx->ev_dropped++; return -1; }
+    if (ctx->ev->size() < 2 * (ctx->ev_used + 1)) {
+        cudaEvent_t a, b;
+        if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) { cudaGetLastError(); return -1; }
+        ctx->ev->push_back(a); ctx->ev->push_back(b);
+        ctx->ev_kind->push_back(kind);
+    }
+    const long n = (long)ctx->ev_used++;
+    (*ctx->ev_kind)[n] = kind;
+    cudaEventRecord((*ctx->ev)[2 * n], ctx->stream);
+    return n;
+}
+void prof_end(clt_ctx *ctx, long n)
+{
+    if (n >= 0) cudaEventRecord((*ctx->ev)[2 * n + 1], ctx->stream);
+}
+
 int run_curl(clt_ctx *ctx, const double *U)
 {
     CurlArgs a;
@@ -133,7 +173,9 @@ int run_curl(clt_ctx *ctx, const double *U)
     a.R = ctx->Rtab + LP;
     a.invR = ctx->invRtab + LP;
     a.phi_chunks = effective_chunks(ctx);
+    const long pe = prof_begin(ctx, 5);
     CK(launch_curl(a, 0, ctx->stream));
+    prof_end(ctx, pe);
     ctx->launches++;
     return CLT_OK;
 }
@@ -149,7 +191,9 @@ int run_rhs(clt_ctx *ctx, int mode, const double *in, double *out, double a_next
     a.a_next = a_next; a.b_acc = b_acc;
     a.phi_chunks = effective_chunks(ctx);
     a.prefetch = 1;
+    const long pe = prof_begin(ctx, mode);
     CK(launch_rhs(a, mode, ctx->has_v0, effective_tile_z(ctx), ctx->stream));
+    prof_end(ctx, pe);
     ctx->launches++;
     return CLT_OK;
 }
@@ -203,6 +247,8 @@ int clt_create(const clt_grid *grid, const clt_params *params, void *d_workspace
     clt_ctx *ctx = new (std::nothrow) clt_ctx();
     if (!ctx) return CLT_ENOMEM;
     memset(ctx, 0, sizeof(*ctx));
+    ctx->ev = new std::vector<cudaEvent_t>();
+    ctx->ev_kind = new std::vector<int>();
     ctx->grid = *grid;
     ctx->par = *params;
     ctx->L = make_layout(grid);
@@ -231,6 +277,7 @@ int clt_create(const clt_grid *grid, const clt_params *params, void *d_workspace
     ctx->nblocks_diag = c.nblocks;
     // carve() aligns every field to 256 B but Layout::field is the unaligned stride: they must agree
     if ((size_t)ctx->L.field * sizeof(double) != c.field_b || (size_t)ctx->L.plane * sizeof(double) != c.table_b) {
+        free_profile(ctx);
         delete ctx;
         return CLT_EINVAL;
     }
@@ -260,6 +307,7 @@ int clt_create(const clt_grid *grid, const clt_params *params, void *d_workspace
         ctx->launches++;
     } while (0);
     if (e != cudaSuccess) {
+        free_profile(ctx);
         delete ctx;
         cudaGetLastError();
         return CLT_ECUDA;
@@ -273,6 +321,7 @@ int clt_destroy(clt_ctx *ctx)
     if (!ctx) return CLT_OK;
     cudaError_t e = cudaStreamSynchronize(ctx->stream);
     destroy_graph(ctx);
+    free_profile(ctx);
     delete ctx;
     if (e != cudaSuccess) { cudaGetLastError(); return CLT_ECUDA; }
     return CLT_OK;
@@ -372,11 +421,19 @@ int clt_step(clt_ctx *ctx, int n)
         if (stale) {
             destroy_graph(ctx);
             cudaGraph_t g = nullptr;
-            CK(cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal));
+            // capture on a private stream (the legacy default stream cannot be captured); the instantiated
+            // graph is launched on the context's stream
+            cudaStream_t cap = nullptr, user = ctx->stream;
+            CK(cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
+            cudaError_t e = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal);
+            if (e != cudaSuccess) { cudaStreamDestroy(cap); return cuda_fail(ctx, e, "cudaStreamBeginCapture"); }
             const int64_t before = ctx->launches;
+            ctx->stream = cap;
             int r = enqueue_step(ctx);
+            ctx->stream = user;
             ctx->launches = before;
-            cudaError_t e = cudaStreamEndCapture(ctx->stream, &g);
+            e = cudaStreamEndCapture(cap, &g);
+            cudaStreamDestroy(cap);
             if (r) { if (g) cudaGraphDestroy(g); return r; }
             if (e != cudaSuccess) return cuda_fail(ctx, e, "cudaStreamEndCapture");
             e = cudaGraphInstantiate(&ctx->graph_exec, g, 0);
@@ -451,6 +508,34 @@ int clt_set_tuning(clt_ctx *ctx, int tile_z, int phi_chunks, int use_graph)
     ctx->tile_z = tile_z;
     ctx->phi_chunks = phi_chunks;
     ctx->use_graph = use_graph ? 1 : 0;
+    return CLT_OK;
+}
+
+int clt_set_profiling(clt_ctx *ctx, int enable)
+{
+    if (!ctx) return CLT_EINVAL;
+    CK(cudaStreamSynchronize(ctx->stream));
+    ctx->profiling = enable != 0;
+    ctx->ev_used = 0;
+    ctx->ev_dropped = 0;
+    return CLT_OK;
+}
+
+int clt_get_profile(clt_ctx *ctx, clt_profile *out)
+{
+    if (!ctx || !out) return CLT_EINVAL;
+    CK(cudaStreamSynchronize(ctx->stream));
+    memset(out, 0, sizeof(*out));
+    for (size_t n = 0; n < ctx->ev_used; ++n) {
+        float ms = 0.f;
+        CK(cudaEventElapsedTime(&ms, (*ctx->ev)[2 * n], (*ctx->ev)[2 * n + 1]));
+        const int kind = (*ctx->ev_kind)[n];
+        if (kind == 5) { out->ms_curl += ms; out->n_curl++; }
+        else { out->ms_rhs[kind] += ms; out->n_rhs[kind]++; }
+    }
+    out->dropped = ctx->ev_dropped;
+    ctx->ev_used = 0;
+    ctx->ev_dropped = 0;
     return CLT_OK;
 }
 
