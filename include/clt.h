@@ -143,6 +143,12 @@ int clt_suggest_dt(clt_ctx *ctx, double cfl, double *dt_out);
  * fused RHS kernel, number of phi chunks per tile, use of a CUDA graph for clt_step.              */
 int clt_set_tuning(clt_ctx *ctx, int tile_z, int phi_chunks, int use_graph);
 
+/* Selects the implementation of the fused RHS kernel: 0 (default) = shared-memory tiles fed by TMA
+ * (cp.async.bulk.tensor + mbarrier), 1 = the same arithmetic fed by plain global loads (kept for A/B
+ * measurements; also used for tile heights the TMA variant has no shared memory for).  Results of the
+ * two are bit-identical.                                                                          */
+int clt_set_kernel_variant(clt_ctx *ctx, int variant);
+
 /* Per-kernel device timing for the roofline report.  With profiling enabled (and use_graph = 0)
  * every hot-path launch of clt_step / clt_rhs is bracketed by CUDA events on the context's stream;
  * clt_get_profile() synchronises, sums the elapsed times per kernel kind since profiling was

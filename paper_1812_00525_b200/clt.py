@@ -43,7 +43,7 @@ class clt_profile(ctypes.Structure):
 # every symbol include/clt.h declares
 EXPORTS = ["clt_workspace_bytes", "clt_create", "clt_destroy", "clt_set_equilibrium", "clt_set_state", "clt_get_state",
            "clt_rhs", "clt_curl_J1", "clt_step", "clt_set_dt", "clt_diagnostics", "clt_suggest_dt", "clt_set_tuning",
-           "clt_set_profiling", "clt_get_profile", "clt_launch_count", "clt_stream", "clt_strerror", "clt_last_cuda_error", "clt_version"]
+           "clt_set_kernel_variant", "clt_set_profiling", "clt_get_profile", "clt_launch_count", "clt_stream", "clt_strerror", "clt_last_cuda_error", "clt_version"]
 
 _lib = None
 
@@ -85,6 +85,8 @@ def load():
     L.clt_suggest_dt.argtypes = [vp, d, ctypes.POINTER(d)]
     L.clt_set_tuning.restype = i
     L.clt_set_tuning.argtypes = [vp, i, i, i]
+    L.clt_set_kernel_variant.restype = i
+    L.clt_set_kernel_variant.argtypes = [vp, i]
     L.clt_set_profiling.restype = i
     L.clt_set_profiling.argtypes = [vp, i]
     L.clt_get_profile.restype = i
@@ -213,6 +215,9 @@ class Clt:
 
     def set_tuning(self, tile_z=0, phi_chunks=0, use_graph=0):
         self._ck(self.L.clt_set_tuning(self.h, int(tile_z), int(phi_chunks), int(use_graph)))
+
+    def set_kernel_variant(self, variant=0):
+        self._ck(self.L.clt_set_kernel_variant(self.h, int(variant)))
 
     def set_profiling(self, enable=True):
         self._ck(self.L.clt_set_profiling(self.h, int(bool(enable))))

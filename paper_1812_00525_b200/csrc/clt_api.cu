@@ -3,6 +3,8 @@
 #include "clt.h"
 #include "clt_internal.h"
 
+#include <cuda.h>
+
 #include <math.h>
 #include <new>
 #include <stdio.h>
@@ -26,6 +28,7 @@ struct clt_ctx {
     double dt;
     int64_t launches;
     int tile_z, phi_chunks, use_graph;
+    int variant;      // 0 = TMA-fed fused RHS kernel (default), 1 = plain-load variant
     cudaGraphExec_t graph_exec;
     double graph_dt;
     int graph_tile_z, graph_chunks;
@@ -133,6 +136,40 @@ void destroy_graph(clt_ctx *ctx)
 }
 
 int effective_tile_z(const clt_ctx *ctx) { return ctx->tile_z ? ctx->tile_z : rhs_default_tile_z(); }
+
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link-time dependency on libcuda)
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_tiled()
+{
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess
+            && q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+        else
+            cudaGetLastError();
+    }
+    return fn;
+}
+
+// 4-D map (R column, Z row, phi plane, field) over nfields consecutive padded fields; box = tile with halo
+bool make_map(const clt_ctx *ctx, const double *base, int nfields, int tile_z, CUtensorMap *out)
+{
+    EncodeTiledFn enc = encode_tiled();
+    if (!enc) return false;
+    const Layout &L = ctx->L;
+    const cuuint64_t dims[4] = { (cuuint64_t)L.pR, (cuuint64_t)L.nZ, (cuuint64_t)L.nphi, (cuuint64_t)nfields };
+    const cuuint64_t strides[3] = { (cuuint64_t)L.pR * 8, (cuuint64_t)L.plane * 8, (cuuint64_t)L.field * 8 };
+    const cuuint32_t box[4] = { 32 + 4, (cuuint32_t)tile_z + 4, 1, 1 };
+    const cuuint32_t estr[4] = { 1, 1, 1, 1 };
+    return enc(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, (void *)base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE)
+           == CUDA_SUCCESS;
+}
 int effective_chunks(const clt_ctx *ctx)
 {
     int c = ctx->phi_chunks ? ctx->phi_chunks : 1;
@@ -191,8 +228,18 @@ int run_rhs(clt_ctx *ctx, int mode, const double *in, double *out, double a_next
     a.a_next = a_next; a.b_acc = b_acc;
     a.phi_chunks = effective_chunks(ctx);
     a.prefetch = 1;
+    const int tz = effective_tile_z(ctx);
+    const bool tma = ctx->variant == 0 && rhs_tma_supports(tz);
+    alignas(64) CUtensorMap tmU, tmJ;
+    if (tma && (!make_map(ctx, in, 8, tz, &tmU) || !make_map(ctx, ctx->J1, 3, tz, &tmJ))) {
+        snprintf(ctx->cuda_err, sizeof(ctx->cuda_err), "cuTensorMapEncodeTiled failed");
+        return CLT_ECUDA;
+    }
     const long pe = prof_begin(ctx, mode);
-    CK(launch_rhs(a, mode, ctx->has_v0, effective_tile_z(ctx), ctx->stream));
+    if (tma)
+        CK(launch_rhs_tma(a, &tmU, &tmJ, mode, ctx->has_v0, tz, ctx->stream));
+    else
+        CK(launch_rhs(a, mode, ctx->has_v0, tz, ctx->stream));
     prof_end(ctx, pe);
     ctx->launches++;
     return CLT_OK;
@@ -503,7 +550,8 @@ int clt_suggest_dt(clt_ctx *ctx, double cfl, double *dt_out)
 int clt_set_tuning(clt_ctx *ctx, int tile_z, int phi_chunks, int use_graph)
 {
     if (!ctx) return CLT_EINVAL;
-    if (tile_z != 0 && tile_z != 8 && tile_z != 12 && tile_z != 14 && tile_z != 16) return CLT_EINVAL;
+    if (tile_z != 0 && tile_z != 7 && tile_z != 8 && tile_z != 12 && tile_z != 13 && tile_z != 14 && tile_z != 16)
+        return CLT_EINVAL;
     if (phi_chunks < 0 || phi_chunks > 64) return CLT_EINVAL;
     ctx->tile_z = tile_z;
     ctx->phi_chunks = phi_chunks;
@@ -536,6 +584,14 @@ int clt_get_profile(clt_ctx *ctx, clt_profile *out)
     out->dropped = ctx->ev_dropped;
     ctx->ev_used = 0;
     ctx->ev_dropped = 0;
+    return CLT_OK;
+}
+
+int clt_set_kernel_variant(clt_ctx *ctx, int variant)
+{
+    if (!ctx || variant < 0 || variant > 1) return CLT_EINVAL;
+    ctx->variant = variant;
+    destroy_graph(ctx);
     return CLT_OK;
 }
 

@@ -95,6 +95,11 @@ cudaError_t launch_copy_boundary(const Layout &L, int nfields, const double *src
 cudaError_t launch_zero_boundary(const Layout &L, int nfields, double *dst, cudaStream_t s);
 cudaError_t launch_curl(const CurlArgs &a, int tile_z, cudaStream_t s);
 cudaError_t launch_rhs(const RhsArgs &a, int mode, bool has_v0, int tile_z, cudaStream_t s);
+// TMA variant: tmU / tmJ point to CUtensorMap objects over the stage state (4-D: pR, nZ, nphi, 8) and J1 (.., 3)
+// with box (TR+4, tile_z+4, 1, 1)
+cudaError_t launch_rhs_tma(const RhsArgs &a, const void *tmU, const void *tmJ, int mode, bool has_v0, int tile_z,
+                           cudaStream_t s);
+bool rhs_tma_supports(int tile_z);
 cudaError_t launch_diag(const DiagArgs &a, int nblocks, double *result6, cudaStream_t s);
 int diag_blocks(const Layout &L);
 cudaError_t configure_kernels();

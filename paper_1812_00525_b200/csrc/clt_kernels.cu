@@ -9,6 +9,7 @@
 // 5-deep register pipeline (rho1, p1, v1) and from shared-memory rings (E1, J x B force).
 // Everything differenced is a perturbation (U - U0): DESIGN.md section 3, hazard H2.
 #include "clt_internal.h"
+#include <cuda.h>
 
 namespace clt {
 
@@ -37,6 +38,127 @@ __device__ __forceinline__ int wrap_phi(int j, int n)
 }
 
 // ---------------------------------------------------------------------------------------------
+// a3-a5 at one node: K of eqs (11)-(14) from
+//   stg  [5][HT]    centre-plane tile (with halo) of rho1, p1, v1_R, v1_phi, v1_Z
+//   er   [5][3][HT] ring of E1 tiles, slot se = plane j+2 (so j-2 -> se+1, j-1 -> se+2, j -> se+3, j+1 -> se+4)
+//   fr   [3][IT]    F = J1 x B + J0 x B1 at the centre plane (tile interior)
+//   q    [5][5]     phi pipeline of the five fluid perturbations at this node, planes j-2..j+2
+// ---------------------------------------------------------------------------------------------
+template <bool V0>
+__device__ __forceinline__ void rhs_point(const double *stg, const double *er, const double *fr, const double *sR, int HT,
+                                          int IT, int cs, int ci, int tx, int se, const double (&q)[5][5],
+                                          const double *tab, long long off2, long long plane, const Phys &ph, double iR,
+                                          double iR2, double (&K)[8])
+{
+    const double rho1 = q[2][0], p1 = q[2][1], v1R = q[2][2], v1P = q[2][3], v1Z = q[2][4];
+    const double rho = rho1 + __ldg(tab + T_RHO0 * plane + off2);
+    const double p = p1 + __ldg(tab + T_P0 * plane + off2);
+    double vR = v1R, vP = v1P, vZ = v1Z;
+    if (V0) {
+        vR += __ldg(tab + T_V0R * plane + off2);
+        vP += __ldg(tab + T_V0P * plane + off2);
+        vZ += __ldg(tab + T_V0Z * plane + off2);
+    }
+    const double rinv = 1.0 / rho;
+
+    double A[5], lap[5];     // (v.grad) f and Laplacian f of the five staged fields
+    double divv1, gRp1, gPp1, gZp1, gPvR, gPvP;
+    // R direction (shared memory, stride 1)
+    {
+        const double vc = vR * ph.cR1, lc = iR * ph.cR1;
+#pragma unroll
+        for (int f = 0; f < 5; ++f) {
+            const double *s = stg + f * HT + cs;
+            const double m2 = s[-2], m1 = s[-1], p1_ = s[1], p2 = s[2];
+            const double d1 = fd1(m2, m1, p1_, p2), d2 = fd2(m2, m1, q[2][f], p1_, p2);
+            A[f] = vc * d1;
+            lap[f] = d2 * ph.cR2 + lc * d1;
+            if (f == 1) gRp1 = d1 * ph.cR1;
+            if (f == 2) divv1 = d1 * ph.cR1 + v1R * iR;
+        }
+    }
+    // phi direction (register pipeline)
+    {
+        const double g1 = ph.cP1 * iR, vc = vP * g1, lc = ph.cP2 * iR2;
+#pragma unroll
+        for (int f = 0; f < 5; ++f) {
+            const double d1 = fd1(q[0][f], q[1][f], q[3][f], q[4][f]);
+            const double d2 = fd2(q[0][f], q[1][f], q[2][f], q[3][f], q[4][f]);
+            A[f] += vc * d1;
+            lap[f] += lc * d2;
+            if (f == 1) gPp1 = d1 * g1;
+            if (f == 2) gPvR = d1 * g1;
+            if (f == 3) { gPvP = d1 * g1; divv1 += gPvP; }
+        }
+    }
+    // Z direction (shared memory, stride SW)
+    {
+        const double vc = vZ * ph.cZ1;
+#pragma unroll
+        for (int f = 0; f < 5; ++f) {
+            const double *s = stg + f * HT + cs;
+            const double m2 = s[-2 * SW], m1 = s[-SW], p1_ = s[SW], p2 = s[2 * SW];
+            const double d1 = fd1(m2, m1, p1_, p2), d2 = fd2(m2, m1, q[2][f], p1_, p2);
+            A[f] += vc * d1;
+            lap[f] += d2 * ph.cZ2;
+            if (f == 1) gZp1 = d1 * ph.cZ1;
+            if (f == 4) divv1 += d1 * ph.cZ1;
+        }
+    }
+
+    // eq (11), L105 and eq (12), with grad rho = grad rho1 + grad rho0 (tables)
+    double cr = A[0] + v1R * __ldg(tab + T_GR_RHO0 * plane + off2) + v1Z * __ldg(tab + T_GZ_RHO0 * plane + off2)
+                + rho * divv1;
+    double cp = A[1] + v1R * __ldg(tab + T_GR_P0 * plane + off2) + v1Z * __ldg(tab + T_GZ_P0 * plane + off2);
+    double pd = p * divv1;
+    if (V0) {
+        const double dv0 = __ldg(tab + T_DIVV0 * plane + off2);
+        cr += rho1 * dv0;
+        pd += p1 * dv0;
+    }
+    K[0] = ph.D * lap[0] - cr;
+    K[1] = ph.kappa * lap[1] - cp - ph.gamma * pd;
+    // eq (13)
+    double aR = A[2] - vP * v1P * iR;
+    double aP = A[3] + vP * v1R * iR;
+    double aZ = A[4];
+    if (V0) {
+        const double v0R = vR - v1R, v0P = vP - v1P;
+        const double r1 = rho1 * rinv;
+        aR += v1R * __ldg(tab + T_GR_V0R * plane + off2) + v1Z * __ldg(tab + T_GZ_V0R * plane + off2)
+              - v1P * v0P * iR + r1 * __ldg(tab + T_A0R * plane + off2);
+        aP += v1R * __ldg(tab + T_GR_V0P * plane + off2) + v1Z * __ldg(tab + T_GZ_V0P * plane + off2)
+              + v1P * v0R * iR + r1 * __ldg(tab + T_A0P * plane + off2);
+        aZ += v1R * __ldg(tab + T_GR_V0Z * plane + off2) + v1Z * __ldg(tab + T_GZ_V0Z * plane + off2)
+              + r1 * __ldg(tab + T_A0Z * plane + off2);
+    }
+    const double two_iR = 2.0 * iR;
+    K[2] = (fr[0 * IT + ci] - gRp1) * rinv - aR + ph.nu * (lap[2] - v1R * iR2 - two_iR * gPvP);
+    K[3] = (fr[1 * IT + ci] - gPp1) * rinv - aP + ph.nu * (lap[3] - v1P * iR2 + two_iR * gPvR);
+    K[4] = (fr[2 * IT + ci] - gZp1) * rinv - aZ + ph.nu * lap[4];
+    // eq (14): -curl_c(E1); the radial derivative differences R * E_phi
+    const int s0 = (se + 1 >= 5) ? se + 1 - 5 : se + 1;   // plane j-2
+    const int s1 = (se + 2 >= 5) ? se + 2 - 5 : se + 2;   // plane j-1
+    const int sc = (se + 3 >= 5) ? se + 3 - 5 : se + 3;   // plane j
+    const int s3 = (se + 4 >= 5) ? se + 4 - 5 : se + 4;   // plane j+1
+    const int s4 = se;                                    // plane j+2
+    const double *eR = er + (sc * 3 + 0) * HT + cs, *eP = er + (sc * 3 + 1) * HT + cs, *eZ = er + (sc * 3 + 2) * HT + cs;
+    const double dP_EZ = fd1(er[(s0 * 3 + 2) * HT + cs], er[(s1 * 3 + 2) * HT + cs], er[(s3 * 3 + 2) * HT + cs],
+                             er[(s4 * 3 + 2) * HT + cs]);
+    const double dP_ER = fd1(er[(s0 * 3 + 0) * HT + cs], er[(s1 * 3 + 0) * HT + cs], er[(s3 * 3 + 0) * HT + cs],
+                             er[(s4 * 3 + 0) * HT + cs]);
+    const double dZ_EP = fd1(eP[-2 * SW], eP[-SW], eP[SW], eP[2 * SW]);
+    const double dZ_ER = fd1(eR[-2 * SW], eR[-SW], eR[SW], eR[2 * SW]);
+    const double dR_EZ = fd1(eZ[-2], eZ[-1], eZ[1], eZ[2]);
+    const double *r = sR + tx + 2;
+    const double dR_REP = fd1(r[-2] * eP[-2], r[-1] * eP[-1], r[1] * eP[1], r[2] * eP[2]);
+    const double cPi = ph.cP1 * iR;
+    K[5] = dZ_EP * ph.cZ1 - dP_EZ * cPi;
+    K[6] = dR_EZ * ph.cR1 - dZ_ER * ph.cZ1;
+    K[7] = dP_ER * cPi - dR_REP * (ph.cR1 * iR);
+}
+
+// ---------------------------------------------------------------------------------------------
 // Fused RHS + RK4 stage combine
 // ---------------------------------------------------------------------------------------------
 template <int TZ>
@@ -50,7 +172,7 @@ struct RhsSmem {
 };
 
 template <int TZ, int MODE, bool V0>
-__global__ void __launch_bounds__(TR *TZ, 1) rhs_kernel(const __grid_constant__ RhsArgs a)
+__global__ void __launch_bounds__(TR *TZ, (TZ <= 8 ? 2 : 1)) rhs_kernel(const __grid_constant__ RhsArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     RhsSmem<TZ> &S = *reinterpret_cast<RhsSmem<TZ> *>(smem_raw);
@@ -199,112 +321,11 @@ __global__ void __launch_bounds__(TR *TZ, 1) rhs_kernel(const __grid_constant__ 
         __syncthreads();
 
         // ---- phase B: K at (i, k, j) -----------------------------------------------------------
-        const double rho1 = q[2][0], p1 = q[2][1], v1R = q[2][2], v1P = q[2][3], v1Z = q[2][4];
-        const double rho = rho1 + __ldg(tab + T_RHO0 * L.plane + off2);
-        const double p = p1 + __ldg(tab + T_P0 * L.plane + off2);
-        double vR = v1R, vP = v1P, vZ = v1Z;
-        if (V0) {
-            vR += __ldg(tab + T_V0R * L.plane + off2);
-            vP += __ldg(tab + T_V0P * L.plane + off2);
-            vZ += __ldg(tab + T_V0Z * L.plane + off2);
-        }
-        const double rinv = 1.0 / rho;
-
-        double A[5], lap[5];     // (v.grad) f and Laplacian f of the five staged fields
-        double divv1, gRp1, gPp1, gZp1, gPvR, gPvP;
-        // R direction (shared memory, stride 1)
-        {
-            const double vc = vR * ph.cR1, lc = iR * ph.cR1;
-#pragma unroll
-            for (int f = 0; f < 5; ++f) {
-                const double *s = &S.stage[buf][f][cs];
-                const double m2 = s[-2], m1 = s[-1], p1_ = s[1], p2 = s[2];
-                const double d1 = fd1(m2, m1, p1_, p2), d2 = fd2(m2, m1, q[2][f], p1_, p2);
-                A[f] = vc * d1;
-                lap[f] = d2 * ph.cR2 + lc * d1;
-                if (f == 1) gRp1 = d1 * ph.cR1;
-                if (f == 2) divv1 = d1 * ph.cR1 + v1R * iR;
-            }
-        }
-        // phi direction (register pipeline)
-        {
-            const double g1 = ph.cP1 * iR, vc = vP * g1, lc = ph.cP2 * iR2;
-#pragma unroll
-            for (int f = 0; f < 5; ++f) {
-                const double d1 = fd1(q[0][f], q[1][f], q[3][f], q[4][f]);
-                const double d2 = fd2(q[0][f], q[1][f], q[2][f], q[3][f], q[4][f]);
-                A[f] += vc * d1;
-                lap[f] += lc * d2;
-                if (f == 1) gPp1 = d1 * g1;
-                if (f == 2) gPvR = d1 * g1;
-                if (f == 3) { gPvP = d1 * g1; divv1 += gPvP; }
-            }
-        }
-        // Z direction (shared memory, stride SW)
-        {
-            const double vc = vZ * ph.cZ1;
-#pragma unroll
-            for (int f = 0; f < 5; ++f) {
-                const double *s = &S.stage[buf][f][cs];
-                const double m2 = s[-2 * SW], m1 = s[-SW], p1_ = s[SW], p2 = s[2 * SW];
-                const double d1 = fd1(m2, m1, p1_, p2), d2 = fd2(m2, m1, q[2][f], p1_, p2);
-                A[f] += vc * d1;
-                lap[f] += d2 * ph.cZ2;
-                if (f == 1) gZp1 = d1 * ph.cZ1;
-                if (f == 4) divv1 += d1 * ph.cZ1;
-            }
-        }
-
         double K[8];
         {
-            // eq (11), L105 and eq (12), with grad rho = grad rho1 + grad rho0 (tables)
-            double cr = A[0] + v1R * __ldg(tab + T_GR_RHO0 * L.plane + off2) + v1Z * __ldg(tab + T_GZ_RHO0 * L.plane + off2)
-                        + rho * divv1;
-            double cp = A[1] + v1R * __ldg(tab + T_GR_P0 * L.plane + off2) + v1Z * __ldg(tab + T_GZ_P0 * L.plane + off2);
-            double pd = p * divv1;
-            if (V0) {
-                const double dv0 = __ldg(tab + T_DIVV0 * L.plane + off2);
-                cr += rho1 * dv0;
-                pd += p1 * dv0;
-            }
-            K[0] = ph.D * lap[0] - cr;
-            K[1] = ph.kappa * lap[1] - cp - ph.gamma * pd;
-            // eq (13)
             const int sfc = (sf + 1 >= 3) ? sf + 1 - 3 : sf + 1;  // ring slot of F at the centre plane
-            double aR = A[2] - vP * v1P * iR;
-            double aP = A[3] + vP * v1R * iR;
-            double aZ = A[4];
-            if (V0) {
-                const double v0R = vR - v1R, v0P = vP - v1P;
-                const double r1 = rho1 * rinv;
-                aR += v1R * __ldg(tab + T_GR_V0R * L.plane + off2) + v1Z * __ldg(tab + T_GZ_V0R * L.plane + off2)
-                      - v1P * v0P * iR + r1 * __ldg(tab + T_A0R * L.plane + off2);
-                aP += v1R * __ldg(tab + T_GR_V0P * L.plane + off2) + v1Z * __ldg(tab + T_GZ_V0P * L.plane + off2)
-                      + v1P * v0R * iR + r1 * __ldg(tab + T_A0P * L.plane + off2);
-                aZ += v1R * __ldg(tab + T_GR_V0Z * L.plane + off2) + v1Z * __ldg(tab + T_GZ_V0Z * L.plane + off2)
-                      + r1 * __ldg(tab + T_A0Z * L.plane + off2);
-            }
-            const double two_iR = 2.0 * iR;
-            K[2] = (S.fring[sfc][0][ci] - gRp1) * rinv - aR + ph.nu * (lap[2] - v1R * iR2 - two_iR * gPvP);
-            K[3] = (S.fring[sfc][1][ci] - gPp1) * rinv - aP + ph.nu * (lap[3] - v1P * iR2 + two_iR * gPvR);
-            K[4] = (S.fring[sfc][2][ci] - gZp1) * rinv - aZ + ph.nu * lap[4];
-            // eq (14): -curl_c(E1); the radial derivative differences R * E_phi
-            const double *eR = &S.ering[sec][0][cs], *eP = &S.ering[sec][1][cs], *eZ = &S.ering[sec][2][cs];
-            const int s0 = (se + 1 >= 5) ? se + 1 - 5 : se + 1;   // plane j-2
-            const int s1 = (se + 2 >= 5) ? se + 2 - 5 : se + 2;   // plane j-1
-            const int s3 = (se + 4 >= 5) ? se + 4 - 5 : se + 4;   // plane j+1
-            const int s4 = se;                                    // plane j+2
-            const double dP_EZ = fd1(S.ering[s0][2][cs], S.ering[s1][2][cs], S.ering[s3][2][cs], S.ering[s4][2][cs]);
-            const double dP_ER = fd1(S.ering[s0][0][cs], S.ering[s1][0][cs], S.ering[s3][0][cs], S.ering[s4][0][cs]);
-            const double dZ_EP = fd1(eP[-2 * SW], eP[-SW], eP[SW], eP[2 * SW]);
-            const double dZ_ER = fd1(eR[-2 * SW], eR[-SW], eR[SW], eR[2 * SW]);
-            const double dR_EZ = fd1(eZ[-2], eZ[-1], eZ[1], eZ[2]);
-            const double *r = &S.sR[tx + 2];
-            const double dR_REP = fd1(r[-2] * eP[-2], r[-1] * eP[-1], r[1] * eP[1], r[2] * eP[2]);
-            const double cPi = ph.cP1 * iR;
-            K[5] = dZ_EP * ph.cZ1 - dP_EZ * cPi;
-            K[6] = dR_EZ * ph.cR1 - dZ_ER * ph.cZ1;
-            K[7] = dP_ER * cPi - dR_REP * (ph.cR1 * iR);
+            rhs_point<V0>(&S.stage[buf][0][0], &S.ering[0][0][0], &S.fring[sfc][0][0], S.sR, RhsSmem<TZ>::HT, IT, cs, ci, tx,
+                          se, q, tab, off2, L.plane, ph, iR, iR2, K);
         }
 
         // ---- a6: RK4 stage combine in the epilogue (L125, L139) --------------------------------
@@ -367,15 +388,317 @@ static cudaError_t launch_rhs_tz(const RhsArgs &a, int mode, bool v0, cudaStream
 #undef CLT_CASE
 }
 
-int rhs_default_tile_z() { return 14; }
+int rhs_default_tile_z() { return 12; }
 
 cudaError_t launch_rhs(const RhsArgs &a, int mode, bool has_v0, int tile_z, cudaStream_t s)
 {
     switch (tile_z) {
+    case 7: return launch_rhs_tz<7>(a, mode, has_v0, s);
+    case 13: return launch_rhs_tz<13>(a, mode, has_v0, s);
     case 8: return launch_rhs_tz<8>(a, mode, has_v0, s);
     case 12: return launch_rhs_tz<12>(a, mode, has_v0, s);
     case 14: return launch_rhs_tz<14>(a, mode, has_v0, s);
     case 16: return launch_rhs_tz<16>(a, mode, has_v0, s);
+    default: return cudaErrorInvalidValue;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// TMA variant of the fused RHS kernel (the default).  Same arithmetic (rhs_point), but the 11 stage
+// fields of plane j+3 arrive as halo'd (TR+4) x (TZ+4) boxes through cp.async.bulk.tensor into one
+// shared "raw" buffer while plane j is being computed, completing on an mbarrier: the long-latency
+// HBM/L2 reads never sit in front of the FP64 work and cost no registers.  Every plane is read from
+// L2 exactly once per CTA (interior + halo in one box); its halo values wait in small thread-private
+// rings until the plane becomes the centre plane.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra.uni WAIT_DONE;\n"
+        "bra.uni WAIT_LOOP;\n"
+        "WAIT_DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, int c0, int c1, int c2, int c3,
+                                            unsigned long long *bar)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];" ::"r"(
+            smem_u32(dst)),
+        "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar))
+        : "memory");
+}
+
+template <int TZ>
+struct RhsTmaSmem {
+    static constexpr int HT = (TZ + 4) * SW;
+    static constexpr int IT = TZ * TR;
+    static constexpr int NH = 4 * TR + 4 * TZ;
+    static constexpr int HTP = (HT + 15) / 16 * 16;   // every TMA destination 128-byte aligned
+    alignas(128) double raw[11][HTP];  // TMA destination: U (8) and J1 (3) of one plane, tile with halo
+    double stage[2][5][HT];            // rho1, p1, v1 of the centre plane (double-buffered)
+    double ering[5][3][HT];            // E1 of planes j-2 .. j+2, tile with halo
+    double fring[3][3][IT];            // F of planes j .. j+2
+    double hring[3][5][NH];            // rho1, p1, v1 at the halo nodes of planes j .. j+2 (thread-private)
+    double sR[SW];
+    alignas(8) unsigned long long bar;
+};
+
+template <int TZ, int MODE, bool V0>
+__global__ void __launch_bounds__(TR *TZ, 1)
+rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmJ)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    using SM = RhsTmaSmem<TZ>;
+    SM &S = *reinterpret_cast<SM *>(smem_raw);
+    constexpr int HT = SM::HT, IT = SM::IT, NH = SM::NH;
+    static_assert(NH <= TR * TZ, "tile too small for one halo node per thread");
+    const Layout &L = a.L;
+    const Phys &ph = a.ph;
+
+    const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * TR + tx;
+    const int i0 = 2 + TR * blockIdx.x, k0 = 2 + TZ * blockIdx.y;
+    const int i = i0 + tx, k = k0 + ty;
+    const bool valid = (i <= L.nR - 3) && (k <= L.nZ - 3);
+    const int ic = min(i, L.nR - 1), kc = min(k, L.nZ - 1);
+    const int ja = (int)(((long long)L.nphi * blockIdx.z) / a.phi_chunks);
+    const int jb = (int)(((long long)L.nphi * (blockIdx.z + 1)) / a.phi_chunks);
+    const long long off2 = (long long)kc * L.pR + (LP + ic);
+    const int cs = (ty + 2) * SW + (tx + 2);
+    const int ci = ty * TR + tx;
+
+    int hx, hy;
+    if (tid < 4 * TR) {
+        const int r = tid / TR;
+        hx = tid % TR;
+        hy = (r < 2) ? r - 2 : TZ + (r - 2);
+    } else {
+        const int t = tid - 4 * TR, c = t & 3;
+        hy = t >> 2;
+        hx = (c < 2) ? c - 2 : TR + (c - 2);
+    }
+    const bool is_halo = tid < NH;
+    const int hi = min(i0 + hx, L.nR - 1), hk = min(k0 + hy, L.nZ - 1);
+    const long long hoff2 = (long long)hk * L.pR + (LP + hi);
+    const int hs = (hy + 2) * SW + (hx + 2);
+
+    if (tid < SW) S.sR[tid] = a.R[min(i0 - 2 + tid, L.nR - 1)];
+    if (tid == 0) {
+        mbar_init(&S.bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmU) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmJ) : "memory");
+    }
+    __syncthreads();
+
+    const double *tab = a.tab;
+    const double eta = ph.eta;
+    unsigned parity = 0;
+
+    // one elected thread: fetch the 11 fields of plane jl (tile with halo) into S.raw
+    auto issue = [&](int jl) {
+        const int jw = wrap_phi(jl, L.nphi);
+        mbar_expect_tx(&S.bar, (unsigned)(11 * HT * sizeof(double)));
+#pragma unroll
+        for (int m = 0; m < 8; ++m) tma_load_4d(&S.raw[m][0], &tmU, LP + i0 - 2, k0 - 2, jw, m, &S.bar);
+#pragma unroll
+        for (int m = 0; m < 3; ++m) tma_load_4d(&S.raw[8 + m][0], &tmJ, LP + i0 - 2, k0 - 2, jw, m, &S.bar);
+    };
+
+    // forms perturbations, E1 and (optionally) F from the raw tile at slot s; o2 = table offset of the node
+    auto node = [&](int s, long long o2, double q[5], double E[3], double F[3], bool wantF) {
+        const double rho = S.raw[0][s], p = S.raw[1][s];
+        const double vR = S.raw[2][s], vP = S.raw[3][s], vZ = S.raw[4][s];
+        const double BR = S.raw[5][s], BP = S.raw[6][s], BZ = S.raw[7][s];
+        const double JR = S.raw[8][s], JP = S.raw[9][s], JZ = S.raw[10][s];
+        q[0] = rho - __ldg(tab + T_RHO0 * L.plane + o2);
+        q[1] = p - __ldg(tab + T_P0 * L.plane + o2);
+        if (V0) {
+            q[2] = vR - __ldg(tab + T_V0R * L.plane + o2);
+            q[3] = vP - __ldg(tab + T_V0P * L.plane + o2);
+            q[4] = vZ - __ldg(tab + T_V0Z * L.plane + o2);
+        } else {
+            q[2] = vR; q[3] = vP; q[4] = vZ;
+        }
+        // a4: E1 = -v x B + v0 x B0 + eta J1   (eq 5 with d_i = 0 minus E0, L77, L101)
+        E[0] = eta * JR - (vP * BZ - vZ * BP);
+        E[1] = eta * JP - (vZ * BR - vR * BZ);
+        E[2] = eta * JZ - (vR * BP - vP * BR);
+        if (V0) {
+            E[0] += __ldg(tab + T_E0R * L.plane + o2);
+            E[1] += __ldg(tab + T_E0P * L.plane + o2);
+            E[2] += __ldg(tab + T_E0Z * L.plane + o2);
+        }
+        if (wantF) {
+            const double B1R = BR - __ldg(tab + T_B0R * L.plane + o2), B1P = BP - __ldg(tab + T_B0P * L.plane + o2),
+                         B1Z = BZ - __ldg(tab + T_B0Z * L.plane + o2);
+            const double J0R = __ldg(tab + T_J0R * L.plane + o2), J0P = __ldg(tab + T_J0P * L.plane + o2),
+                         J0Z = __ldg(tab + T_J0Z * L.plane + o2);
+            F[0] = (JP * BZ - JZ * BP) + (J0P * B1Z - J0Z * B1P);
+            F[1] = (JZ * BR - JR * BZ) + (J0Z * B1R - J0R * B1Z);
+            F[2] = (JR * BP - JP * BR) + (J0R * B1P - J0P * B1R);
+        }
+    };
+
+    double q[5][5];
+    int se = 0, sf = 0;
+
+    // consume the raw tile (the plane that becomes plane j+2)
+    auto lead = [&]() {
+        mbar_wait(&S.bar, parity);
+        parity ^= 1u;
+        double E[3], F[3];
+        node(cs, off2, q[4], E, F, true);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            S.ering[se][c][cs] = E[c];
+            S.fring[sf][c][ci] = F[c];
+        }
+        if (is_halo) {
+            double hq[5], hE[3], hF[3];
+            node(hs, hoff2, hq, hE, hF, false);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) S.ering[se][c][hs] = hE[c];
+#pragma unroll
+            for (int f = 0; f < 5; ++f) S.hring[sf][f][tid] = hq[f];
+        }
+    };
+    auto advance = [&]() {
+#pragma unroll
+        for (int d = 0; d < 4; ++d)
+#pragma unroll
+            for (int f = 0; f < 5; ++f) q[d][f] = q[d + 1][f];
+        se = (se == 4) ? 0 : se + 1;
+        sf = (sf == 2) ? 0 : sf + 1;
+    };
+
+    // prologue: planes ja-2 .. ja+1
+    if (tid == 0) issue(ja - 2);
+#pragma unroll 1
+    for (int jl = ja - 2; jl <= ja + 1; ++jl) {
+        lead();
+        __syncthreads();                 // every thread has read the raw tile
+        if (tid == 0) issue(jl + 1);
+        advance();
+    }
+
+    const double iR = __ldg(a.invR + ic);
+    const double iR2 = iR * iR;
+
+#pragma unroll 1
+    for (int j = ja; j < jb; ++j) {
+        const int buf = j & 1;
+        // ---- phase A: consume plane j+2, stage plane j ----------------------------------------
+        if (a.prefetch && MODE != RHS_MODE_K && (tx & 15) == 0 && j + 1 < jb) {
+            const long long g1 = (long long)(j + 1) * L.plane + off2;
+#pragma unroll
+            for (int m = 0; m < 8; ++m) {
+                if (MODE == RHS_MODE_S2 || MODE == RHS_MODE_S3) prefetch_l2(a.Un + m * L.field + g1);
+                if (MODE != RHS_MODE_S1) prefetch_l2(a.acc + m * L.field + g1);
+            }
+        }
+        lead();
+        const int sfc = (sf + 1 >= 3) ? sf + 1 - 3 : sf + 1;      // slot of the centre plane in the 3-rings
+#pragma unroll
+        for (int f = 0; f < 5; ++f) S.stage[buf][f][cs] = q[2][f];
+        if (is_halo) {
+#pragma unroll
+            for (int f = 0; f < 5; ++f) S.stage[buf][f][hs] = S.hring[sfc][f][tid];
+        }
+        __syncthreads();
+        if (tid == 0 && j + 3 <= jb + 1) issue(j + 3);           // overlaps the whole of phase B
+
+        // ---- phase B: K at (i, k, j) -----------------------------------------------------------
+        double K[8];
+        rhs_point<V0>(&S.stage[buf][0][0], &S.ering[0][0][0], &S.fring[sfc][0][0], S.sR, HT, IT, cs, ci, tx, se, q, tab,
+                      off2, L.plane, ph, iR, iR2, K);
+
+        // ---- a6: RK4 stage combine in the epilogue (L125, L139) --------------------------------
+        if (valid) {
+            const long long g = (long long)j * L.plane + off2;
+#pragma unroll
+            for (int m = 0; m < 8; ++m) {
+                const long long gm = m * L.field + g;
+                if (MODE == RHS_MODE_K) {
+                    a.out[gm] = K[m];
+                } else if (MODE == RHS_MODE_S1) {
+                    const double un = __ldg(a.in + gm);
+                    a.out[gm] = fma(a.a_next, K[m], un);
+                    a.acc[gm] = fma(a.b_acc, K[m], un);
+                } else if (MODE == RHS_MODE_S4) {
+                    a.out[gm] = fma(a.b_acc, K[m], a.acc[gm]);
+                } else {
+                    const double un = __ldg(a.Un + gm);
+                    a.out[gm] = fma(a.a_next, K[m], un);
+                    a.acc[gm] = fma(a.b_acc, K[m], a.acc[gm]);
+                }
+            }
+        }
+        advance();
+    }
+}
+
+template <int TZ, int MODE, bool V0>
+static cudaError_t launch_rhs_tma_t(const RhsArgs &a, const CUtensorMap &tmU, const CUtensorMap &tmJ, cudaStream_t s)
+{
+    static bool configured = false;
+    auto kern = rhs_tma_kernel<TZ, MODE, V0>;
+    const int smem = (int)sizeof(RhsTmaSmem<TZ>);
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    dim3 block(TR, TZ, 1);
+    dim3 grid((a.L.nR - 4 + TR - 1) / TR, (a.L.nZ - 4 + TZ - 1) / TZ, a.phi_chunks);
+    kern<<<grid, block, smem, s>>>(a, tmU, tmJ);
+    return cudaGetLastError();
+}
+
+template <int TZ>
+static cudaError_t launch_rhs_tma_tz(const RhsArgs &a, const CUtensorMap &tmU, const CUtensorMap &tmJ, int mode, bool v0,
+                                     cudaStream_t s)
+{
+#define CLT_CASE(M)                                                                                        \
+    case M:                                                                                                \
+        return v0 ? launch_rhs_tma_t<TZ, M, true>(a, tmU, tmJ, s) : launch_rhs_tma_t<TZ, M, false>(a, tmU, tmJ, s);
+    switch (mode) {
+        CLT_CASE(RHS_MODE_K)
+        CLT_CASE(RHS_MODE_S1)
+        CLT_CASE(RHS_MODE_S2)
+        CLT_CASE(RHS_MODE_S3)
+        CLT_CASE(RHS_MODE_S4)
+    default:
+        return cudaErrorInvalidValue;
+    }
+#undef CLT_CASE
+}
+
+bool rhs_tma_supports(int tile_z) { return tile_z == 8 || tile_z == 12 || tile_z == 13; }
+
+cudaError_t launch_rhs_tma(const RhsArgs &a, const void *tmU, const void *tmJ, int mode, bool has_v0, int tile_z,
+                           cudaStream_t s)
+{
+    const CUtensorMap &mU = *reinterpret_cast<const CUtensorMap *>(tmU);
+    const CUtensorMap &mJ = *reinterpret_cast<const CUtensorMap *>(tmJ);
+    switch (tile_z) {
+    case 8: return launch_rhs_tma_tz<8>(a, mU, mJ, mode, has_v0, s);
+    case 12: return launch_rhs_tma_tz<12>(a, mU, mJ, mode, has_v0, s);
+    case 13: return launch_rhs_tma_tz<13>(a, mU, mJ, mode, has_v0, s);
     default: return cudaErrorInvalidValue;
     }
 }

@@ -30,15 +30,20 @@ def test_curl_J1_matches_oracle(name):
     assert np.all(J_g[:, :, :2] == 0) and np.all(J_g[..., -2:] == 0)
 
 
+# (kernel variant, tile height): 0 = TMA-fed kernel (default), 1 = plain-load kernel
+VARIANTS = [(0, 0), (0, 8), (0, 13), (1, 7), (1, 12), (1, 14), (1, 16)]
+
+
 @pytest.mark.parametrize("name", list(_problems()))
-@pytest.mark.parametrize("tile_z", [0, 8, 12, 16])
-def test_rhs_matches_oracle(name, tile_z):
+@pytest.mark.parametrize("variant,tile_z", VARIANTS)
+def test_rhs_matches_oracle(name, variant, tile_z):
     prob = _problems()[name]()
     o, g = make_oracle(prob), make_gpu(prob)
+    g.set_kernel_variant(variant)
     g.set_tuning(tile_z=tile_z)
     K_o = o.rhs()
     K_g = g.rhs()
-    assert_close(K_g, K_o, RHS_TOL, f"rhs {name} tile_z={tile_z}")
+    assert_close(K_g, K_o, RHS_TOL, f"rhs {name} variant={variant} tile_z={tile_z}")
     assert np.all(K_g[:, :, :2] == 0) and np.all(K_g[:, :, -2:] == 0) and np.all(K_g[..., :2] == 0) and np.all(K_g[..., -2:] == 0)
     # the state is untouched by clt_rhs, scratch buffers restored: a second call gives the same bits
     assert np.array_equal(g.get_state(), prob.U)
@@ -86,14 +91,16 @@ def test_config2_100_steps_match_oracle():
     assert_close(g.get_state(), o.get_state(), STEP_TOL, "config 2, 100 RK4 steps")
 
 
-@pytest.mark.parametrize("chunks,graph", [(2, 0), (4, 0), (1, 1), (2, 1)])
-def test_phi_chunks_and_graph_give_identical_bits(chunks, graph):
+@pytest.mark.parametrize("chunks,graph,variant,tile_z", [(2, 0, 0, 0), (4, 0, 0, 8), (1, 1, 0, 0), (2, 1, 0, 13), (1, 0, 1, 14),
+                                                         (3, 1, 1, 12)])
+def test_launch_shapes_variants_and_graph_give_identical_bits(chunks, graph, variant, tile_z):
     prob = inputs.make_problem(1)
     g0 = make_gpu(prob)
     g0.step(3)
     ref = g0.get_state()
     g1 = make_gpu(prob)
-    g1.set_tuning(phi_chunks=chunks, use_graph=graph)
+    g1.set_kernel_variant(variant)
+    g1.set_tuning(tile_z=tile_z, phi_chunks=chunks, use_graph=graph)
     g1.step(2)
     g1.step(1)
     assert np.array_equal(g1.get_state(), ref)
