@@ -550,7 +550,7 @@ int clt_suggest_dt(clt_ctx *ctx, double cfl, double *dt_out)
 int clt_set_tuning(clt_ctx *ctx, int tile_z, int phi_chunks, int use_graph)
 {
     if (!ctx) return CLT_EINVAL;
-    if (tile_z != 0 && tile_z != 7 && tile_z != 8 && tile_z != 12 && tile_z != 13 && tile_z != 14 && tile_z != 16)
+    if (tile_z != 0 && tile_z != 7 && tile_z != 8 && tile_z != 10 && tile_z != 12 && tile_z != 13 && tile_z != 14 && tile_z != 16)
         return CLT_EINVAL;
     if (phi_chunks < 0 || phi_chunks > 64) return CLT_EINVAL;
     ctx->tile_z = tile_z;

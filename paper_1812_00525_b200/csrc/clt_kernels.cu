@@ -44,15 +44,32 @@ __device__ __forceinline__ int wrap_phi(int j, int n)
 //   fr   [3][IT]    F = J1 x B + J0 x B1 at the centre plane (tile interior)
 //   q    [5][5]     phi pipeline of the five fluid perturbations at this node, planes j-2..j+2
 // ---------------------------------------------------------------------------------------------
+// axisymmetric table values of one node that the centre-plane arithmetic needs (phi-invariant, so a
+// thread can keep them in registers for the whole sweep)
+struct CentreTab {
+    double rho0, p0, gRrho0, gZrho0, gRp0, gZp0;
+};
+__device__ __forceinline__ CentreTab load_centre_tab(const double *tab, long long plane, long long off2)
+{
+    CentreTab t;
+    t.rho0 = __ldg(tab + T_RHO0 * plane + off2);
+    t.p0 = __ldg(tab + T_P0 * plane + off2);
+    t.gRrho0 = __ldg(tab + T_GR_RHO0 * plane + off2);
+    t.gZrho0 = __ldg(tab + T_GZ_RHO0 * plane + off2);
+    t.gRp0 = __ldg(tab + T_GR_P0 * plane + off2);
+    t.gZp0 = __ldg(tab + T_GZ_P0 * plane + off2);
+    return t;
+}
+
 template <bool V0>
 __device__ __forceinline__ void rhs_point(const double *stg, const double *er, const double *fr, const double *sR, int HT,
                                           int IT, int cs, int ci, int tx, int se, const double (&q)[5][5],
-                                          const double *tab, long long off2, long long plane, const Phys &ph, double iR,
-                                          double iR2, double (&K)[8])
+                                          const CentreTab &ct, const double *tab, long long off2, long long plane,
+                                          const Phys &ph, double iR, double iR2, double (&K)[8])
 {
     const double rho1 = q[2][0], p1 = q[2][1], v1R = q[2][2], v1P = q[2][3], v1Z = q[2][4];
-    const double rho = rho1 + __ldg(tab + T_RHO0 * plane + off2);
-    const double p = p1 + __ldg(tab + T_P0 * plane + off2);
+    const double rho = rho1 + ct.rho0;
+    const double p = p1 + ct.p0;
     double vR = v1R, vP = v1P, vZ = v1Z;
     if (V0) {
         vR += __ldg(tab + T_V0R * plane + off2);
@@ -107,9 +124,8 @@ __device__ __forceinline__ void rhs_point(const double *stg, const double *er, c
     }
 
     // eq (11), L105 and eq (12), with grad rho = grad rho1 + grad rho0 (tables)
-    double cr = A[0] + v1R * __ldg(tab + T_GR_RHO0 * plane + off2) + v1Z * __ldg(tab + T_GZ_RHO0 * plane + off2)
-                + rho * divv1;
-    double cp = A[1] + v1R * __ldg(tab + T_GR_P0 * plane + off2) + v1Z * __ldg(tab + T_GZ_P0 * plane + off2);
+    double cr = A[0] + v1R * ct.gRrho0 + v1Z * ct.gZrho0 + rho * divv1;
+    double cp = A[1] + v1R * ct.gRp0 + v1Z * ct.gZp0;
     double pd = p * divv1;
     if (V0) {
         const double dv0 = __ldg(tab + T_DIVV0 * plane + off2);
@@ -324,8 +340,9 @@ __global__ void __launch_bounds__(TR *TZ, (TZ <= 8 ? 2 : 1)) rhs_kernel(const __
         double K[8];
         {
             const int sfc = (sf + 1 >= 3) ? sf + 1 - 3 : sf + 1;  // ring slot of F at the centre plane
+            const CentreTab ct = load_centre_tab(tab, L.plane, off2);
             rhs_point<V0>(&S.stage[buf][0][0], &S.ering[0][0][0], &S.fring[sfc][0][0], S.sR, RhsSmem<TZ>::HT, IT, cs, ci, tx,
-                          se, q, tab, off2, L.plane, ph, iR, iR2, K);
+                          se, q, ct, tab, off2, L.plane, ph, iR, iR2, K);
         }
 
         // ---- a6: RK4 stage combine in the epilogue (L125, L139) --------------------------------
@@ -396,6 +413,7 @@ cudaError_t launch_rhs(const RhsArgs &a, int mode, bool has_v0, int tile_z, cuda
     case 7: return launch_rhs_tz<7>(a, mode, has_v0, s);
     case 13: return launch_rhs_tz<13>(a, mode, has_v0, s);
     case 8: return launch_rhs_tz<8>(a, mode, has_v0, s);
+    case 10: return launch_rhs_tz<10>(a, mode, has_v0, s);
     case 12: return launch_rhs_tz<12>(a, mode, has_v0, s);
     case 14: return launch_rhs_tz<14>(a, mode, has_v0, s);
     case 16: return launch_rhs_tz<16>(a, mode, has_v0, s);
@@ -411,6 +429,15 @@ cudaError_t launch_rhs(const RhsArgs &a, int mode, bool has_v0, int tile_z, cuda
 // L2 exactly once per CTA (interior + halo in one box); its halo values wait in small thread-private
 // rings until the plane becomes the centre plane.
 // ---------------------------------------------------------------------------------------------
+// streaming 8-byte load that does not allocate in L1 (the epilogue operands are touched exactly once);
+// volatile so that it is issued where it is written: ahead of the FP64 work that hides its latency
+__device__ __forceinline__ double ld_stream(const double *p)
+{
+    double v;
+    asm volatile("ld.global.L1::no_allocate.f64 %0, [%1];" : "=d"(v) : "l"(p) : "memory");
+    return v;
+}
+
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
 
 __device__ __forceinline__ void mbar_init(unsigned long long *bar, unsigned count)
@@ -519,14 +546,22 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
         for (int m = 0; m < 3; ++m) tma_load_4d(&S.raw[8 + m][0], &tmJ, LP + i0 - 2, k0 - 2, jw, m, &S.bar);
     };
 
+    // phi-invariant table values of the own node and of the halo node, kept in registers for the whole sweep
+    const CentreTab ct = load_centre_tab(tab, L.plane, off2);
+    const double b0R = __ldg(tab + T_B0R * L.plane + off2), b0P = __ldg(tab + T_B0P * L.plane + off2),
+                 b0Z = __ldg(tab + T_B0Z * L.plane + off2);
+    const double j0R = __ldg(tab + T_J0R * L.plane + off2), j0P = __ldg(tab + T_J0P * L.plane + off2),
+                 j0Z = __ldg(tab + T_J0Z * L.plane + off2);
+    const double h_rho0 = __ldg(tab + T_RHO0 * L.plane + hoff2), h_p0 = __ldg(tab + T_P0 * L.plane + hoff2);
+
     // forms perturbations, E1 and (optionally) F from the raw tile at slot s; o2 = table offset of the node
-    auto node = [&](int s, long long o2, double q[5], double E[3], double F[3], bool wantF) {
+    auto node = [&](int s, long long o2, double rho0, double p0, double q[5], double E[3], double F[3], bool wantF) {
         const double rho = S.raw[0][s], p = S.raw[1][s];
         const double vR = S.raw[2][s], vP = S.raw[3][s], vZ = S.raw[4][s];
         const double BR = S.raw[5][s], BP = S.raw[6][s], BZ = S.raw[7][s];
         const double JR = S.raw[8][s], JP = S.raw[9][s], JZ = S.raw[10][s];
-        q[0] = rho - __ldg(tab + T_RHO0 * L.plane + o2);
-        q[1] = p - __ldg(tab + T_P0 * L.plane + o2);
+        q[0] = rho - rho0;
+        q[1] = p - p0;
         if (V0) {
             q[2] = vR - __ldg(tab + T_V0R * L.plane + o2);
             q[3] = vP - __ldg(tab + T_V0P * L.plane + o2);
@@ -544,13 +579,10 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
             E[2] += __ldg(tab + T_E0Z * L.plane + o2);
         }
         if (wantF) {
-            const double B1R = BR - __ldg(tab + T_B0R * L.plane + o2), B1P = BP - __ldg(tab + T_B0P * L.plane + o2),
-                         B1Z = BZ - __ldg(tab + T_B0Z * L.plane + o2);
-            const double J0R = __ldg(tab + T_J0R * L.plane + o2), J0P = __ldg(tab + T_J0P * L.plane + o2),
-                         J0Z = __ldg(tab + T_J0Z * L.plane + o2);
-            F[0] = (JP * BZ - JZ * BP) + (J0P * B1Z - J0Z * B1P);
-            F[1] = (JZ * BR - JR * BZ) + (J0Z * B1R - J0R * B1Z);
-            F[2] = (JR * BP - JP * BR) + (J0R * B1P - J0P * B1R);
+            const double B1R = BR - b0R, B1P = BP - b0P, B1Z = BZ - b0Z;
+            F[0] = (JP * BZ - JZ * BP) + (j0P * B1Z - j0Z * B1P);
+            F[1] = (JZ * BR - JR * BZ) + (j0Z * B1R - j0R * B1Z);
+            F[2] = (JR * BP - JP * BR) + (j0R * B1P - j0P * B1R);
         }
     };
 
@@ -562,7 +594,7 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
         mbar_wait(&S.bar, parity);
         parity ^= 1u;
         double E[3], F[3];
-        node(cs, off2, q[4], E, F, true);
+        node(cs, off2, ct.rho0, ct.p0, q[4], E, F, true);
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
             S.ering[se][c][cs] = E[c];
@@ -570,7 +602,7 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
         }
         if (is_halo) {
             double hq[5], hE[3], hF[3];
-            node(hs, hoff2, hq, hE, hF, false);
+            node(hs, hoff2, h_rho0, h_p0, hq, hE, hF, false);
 #pragma unroll
             for (int c = 0; c < 3; ++c) S.ering[se][c][hs] = hE[c];
 #pragma unroll
@@ -622,29 +654,37 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
         __syncthreads();
         if (tid == 0 && j + 3 <= jb + 1) issue(j + 3);           // overlaps the whole of phase B
 
+        // ---- a6 inputs: U^n / acc of this node, requested now so that they arrive during phase B ---
+        const long long g = (long long)j * L.plane + off2;
+        double un[8], ac[8];
+#pragma unroll
+        for (int m = 0; m < 8; ++m) {
+            const long long gm = m * L.field + g;
+            if (MODE == RHS_MODE_S1) un[m] = ld_stream(a.in + gm);
+            if (MODE == RHS_MODE_S2 || MODE == RHS_MODE_S3) un[m] = ld_stream(a.Un + gm);
+            if (MODE == RHS_MODE_S2 || MODE == RHS_MODE_S3 || MODE == RHS_MODE_S4) ac[m] = ld_stream(a.acc + gm);
+        }
+
         // ---- phase B: K at (i, k, j) -----------------------------------------------------------
         double K[8];
-        rhs_point<V0>(&S.stage[buf][0][0], &S.ering[0][0][0], &S.fring[sfc][0][0], S.sR, HT, IT, cs, ci, tx, se, q, tab,
+        rhs_point<V0>(&S.stage[buf][0][0], &S.ering[0][0][0], &S.fring[sfc][0][0], S.sR, HT, IT, cs, ci, tx, se, q, ct, tab,
                       off2, L.plane, ph, iR, iR2, K);
 
         // ---- a6: RK4 stage combine in the epilogue (L125, L139) --------------------------------
         if (valid) {
-            const long long g = (long long)j * L.plane + off2;
 #pragma unroll
             for (int m = 0; m < 8; ++m) {
                 const long long gm = m * L.field + g;
                 if (MODE == RHS_MODE_K) {
                     a.out[gm] = K[m];
                 } else if (MODE == RHS_MODE_S1) {
-                    const double un = __ldg(a.in + gm);
-                    a.out[gm] = fma(a.a_next, K[m], un);
-                    a.acc[gm] = fma(a.b_acc, K[m], un);
+                    a.out[gm] = fma(a.a_next, K[m], un[m]);
+                    a.acc[gm] = fma(a.b_acc, K[m], un[m]);
                 } else if (MODE == RHS_MODE_S4) {
-                    a.out[gm] = fma(a.b_acc, K[m], a.acc[gm]);
+                    a.out[gm] = fma(a.b_acc, K[m], ac[m]);
                 } else {
-                    const double un = __ldg(a.Un + gm);
-                    a.out[gm] = fma(a.a_next, K[m], un);
-                    a.acc[gm] = fma(a.b_acc, K[m], a.acc[gm]);
+                    a.out[gm] = fma(a.a_next, K[m], un[m]);
+                    a.acc[gm] = fma(a.b_acc, K[m], ac[m]);
                 }
             }
         }
@@ -688,7 +728,7 @@ static cudaError_t launch_rhs_tma_tz(const RhsArgs &a, const CUtensorMap &tmU, c
 #undef CLT_CASE
 }
 
-bool rhs_tma_supports(int tile_z) { return tile_z == 8 || tile_z == 12 || tile_z == 13; }
+bool rhs_tma_supports(int tile_z) { return tile_z == 8 || tile_z == 10 || tile_z == 12 || tile_z == 13; }
 
 cudaError_t launch_rhs_tma(const RhsArgs &a, const void *tmU, const void *tmJ, int mode, bool has_v0, int tile_z,
                            cudaStream_t s)
@@ -697,6 +737,7 @@ cudaError_t launch_rhs_tma(const RhsArgs &a, const void *tmU, const void *tmJ, i
     const CUtensorMap &mJ = *reinterpret_cast<const CUtensorMap *>(tmJ);
     switch (tile_z) {
     case 8: return launch_rhs_tma_tz<8>(a, mU, mJ, mode, has_v0, s);
+    case 10: return launch_rhs_tma_tz<10>(a, mU, mJ, mode, has_v0, s);
     case 12: return launch_rhs_tma_tz<12>(a, mU, mJ, mode, has_v0, s);
     case 13: return launch_rhs_tma_tz<13>(a, mU, mJ, mode, has_v0, s);
     default: return cudaErrorInvalidValue;
