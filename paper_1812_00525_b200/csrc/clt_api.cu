@@ -210,8 +210,17 @@ int run_curl(clt_ctx *ctx, const double *U)
     a.R = ctx->Rtab + LP;
     a.invR = ctx->invRtab + LP;
     a.phi_chunks = effective_chunks(ctx);
+    alignas(64) CUtensorMap tmB;
+    const bool tma = ctx->variant == 0;
+    if (tma && !make_map(ctx, a.B, 3, curl_tma_tile_z(), &tmB)) {
+        snprintf(ctx->cuda_err, sizeof(ctx->cuda_err), "cuTensorMapEncodeTiled failed");
+        return CLT_ECUDA;
+    }
     const long pe = prof_begin(ctx, 5);
-    CK(launch_curl(a, 0, ctx->stream));
+    if (tma)
+        CK(launch_curl_tma(a, &tmB, ctx->stream));
+    else
+        CK(launch_curl(a, 0, ctx->stream));
     prof_end(ctx, pe);
     ctx->launches++;
     return CLT_OK;

@@ -100,6 +100,10 @@ cudaError_t launch_rhs(const RhsArgs &a, int mode, bool has_v0, int tile_z, cuda
 cudaError_t launch_rhs_tma(const RhsArgs &a, const void *tmU, const void *tmJ, int mode, bool has_v0, int tile_z,
                            cudaStream_t s);
 bool rhs_tma_supports(int tile_z);
+// TMA variant of the curl kernel: tmB is a CUtensorMap over B_R, B_phi, B_Z of the stage state with box
+// (TR+4, curl_tma_tile_z()+4, 1, 1)
+cudaError_t launch_curl_tma(const CurlArgs &a, const void *tmB, cudaStream_t s);
+int curl_tma_tile_z();
 cudaError_t launch_diag(const DiagArgs &a, int nblocks, double *result6, cudaStream_t s);
 int diag_blocks(const Layout &L);
 cudaError_t configure_kernels();

@@ -858,6 +858,135 @@ cudaError_t launch_curl(const CurlArgs &a, int tile_z, cudaStream_t s)
 }
 
 // ---------------------------------------------------------------------------------------------
+// TMA variant of the curl kernel (the default): an NS-deep shared-memory ring of raw B tiles (with
+// halo) filled by cp.async.bulk.tensor three planes ahead; threads read their stencil neighbours
+// straight from the ring and subtract the (phi-invariant) B0 values they keep in registers, so the
+// equilibrium is still removed before differencing (H2).  No staging, one __syncthreads per plane
+// (only to hand the consumed ring slot back to the producer thread).
+// ---------------------------------------------------------------------------------------------
+template <int TZ, int NS>
+struct CurlTmaSmem {
+    static constexpr int HT = (TZ + 4) * SW;
+    static constexpr int HTP = (HT + 15) / 16 * 16;
+    alignas(128) double raw[NS][3][HTP];
+    alignas(8) unsigned long long full[NS];
+};
+
+template <int TZ, int NS>
+__global__ void __launch_bounds__(TR *TZ, 1) curl_tma_kernel(const __grid_constant__ CurlArgs a, const __grid_constant__ CUtensorMap tmB)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    using SM = CurlTmaSmem<TZ, NS>;
+    SM &S = *reinterpret_cast<SM *>(smem_raw);
+    const Layout &L = a.L;
+    const Phys &ph = a.ph;
+    const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * TR + tx;
+    const int i0 = 2 + TR * blockIdx.x, k0 = 2 + TZ * blockIdx.y;
+    const int i = i0 + tx, k = k0 + ty;
+    const bool valid = (i <= L.nR - 3) && (k <= L.nZ - 3);
+    const int ic = min(i, L.nR - 3), kc = min(k, L.nZ - 3);     // clamped to an interior node: +-2 stays in range
+    const int ja = (int)(((long long)L.nphi * blockIdx.z) / a.phi_chunks);
+    const int jb = (int)(((long long)L.nphi * (blockIdx.z + 1)) / a.phi_chunks);
+    const long long off2 = (long long)kc * L.pR + (LP + ic);
+    const int cs = (ty + 2) * SW + (tx + 2);
+    const int total = jb - ja + 4;                               // planes ja-2 .. jb+1
+
+    if (tid == 0) {
+        for (int n = 0; n < NS; ++n) mbar_init(&S.full[n], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmB) : "memory");
+    }
+    __syncthreads();
+    auto issue = [&](int n) {      // plane number n counts from ja-2
+        const int jw = wrap_phi(ja - 2 + n, L.nphi);
+        const int st = n % NS;
+        mbar_expect_tx(&S.full[st], (unsigned)(3 * SM::HT * sizeof(double)));
+#pragma unroll
+        for (int m = 0; m < 3; ++m) tma_load_4d(&S.raw[st][m][0], &tmB, LP + i0 - 2, k0 - 2, jw, m, &S.full[st]);
+    };
+    if (tid == 0)
+        for (int n = 0; n < NS && n < total; ++n) issue(n);
+
+    // phi-invariant operands in registers: B0 at the own node and at the 8 in-plane neighbours, R_i
+    const double *tab = a.tab;
+    const double *t0R = tab + T_B0R * L.plane + off2, *t0P = tab + T_B0P * L.plane + off2, *t0Z = tab + T_B0Z * L.plane + off2;
+    const double o0R = __ldg(t0R), o0Z = __ldg(t0Z);
+    double z0P[4], z0R[4], r0Z[4], r0P[4], rr[4];
+#pragma unroll
+    for (int d = 0; d < 4; ++d) {
+        const int o = (d < 2) ? d - 2 : d - 1;          // -2, -1, +1, +2
+        z0P[d] = __ldg(t0P + (long long)o * L.pR);
+        z0R[d] = __ldg(t0R + (long long)o * L.pR);
+        r0Z[d] = __ldg(t0Z + o);
+        r0P[d] = __ldg(t0P + o);
+        rr[d] = __ldg(a.R + ic + o);
+    }
+    const double iR = __ldg(a.invR + ic);
+    const double cPi = ph.cP1 * iR;
+
+    double bR[5], bZ[5];           // B1_R, B1_Z of planes j-2 .. j+2 at the own node
+    auto lead = [&](int n) {
+        const int st = n % NS;
+        mbar_wait(&S.full[st], (unsigned)((n / NS) & 1));
+        bR[4] = S.raw[st][0][cs] - o0R;
+        bZ[4] = S.raw[st][2][cs] - o0Z;
+    };
+    auto advance = [&]() {
+#pragma unroll
+        for (int d = 0; d < 4; ++d) { bR[d] = bR[d + 1]; bZ[d] = bZ[d + 1]; }
+    };
+#pragma unroll 1
+    for (int n = 0; n < 4; ++n) { lead(n); advance(); }
+    __syncthreads();                                   // planes 0 and 1 are never centre planes: recycle their slots
+    if (tid == 0) {
+        if (NS < total) issue(NS);
+        if (NS + 1 < total) issue(NS + 1);
+    }
+
+#pragma unroll 1
+    for (int j = ja; j < jb; ++j) {
+        const int nc = j - ja + 2;                     // plane number of the centre plane
+        lead(nc + 2);
+        const int st = nc % NS;
+        const double *sR_ = &S.raw[st][0][cs], *sP_ = &S.raw[st][1][cs], *sZ_ = &S.raw[st][2][cs];
+        const double dP_BZ = fd1(bZ[0], bZ[1], bZ[3], bZ[4]);
+        const double dP_BR = fd1(bR[0], bR[1], bR[3], bR[4]);
+        const double dZ_BP = fd1(sP_[-2 * SW] - z0P[0], sP_[-SW] - z0P[1], sP_[SW] - z0P[2], sP_[2 * SW] - z0P[3]);
+        const double dZ_BR = fd1(sR_[-2 * SW] - z0R[0], sR_[-SW] - z0R[1], sR_[SW] - z0R[2], sR_[2 * SW] - z0R[3]);
+        const double dR_BZ = fd1(sZ_[-2] - r0Z[0], sZ_[-1] - r0Z[1], sZ_[1] - r0Z[2], sZ_[2] - r0Z[3]);
+        const double dR_RBP = fd1(rr[0] * (sP_[-2] - r0P[0]), rr[1] * (sP_[-1] - r0P[1]), rr[2] * (sP_[1] - r0P[2]),
+                                  rr[3] * (sP_[2] - r0P[3]));
+        if (valid) {
+            const long long g = (long long)j * L.plane + off2;
+            a.J1[0 * L.field + g] = dP_BZ * cPi - dZ_BP * ph.cZ1;
+            a.J1[1 * L.field + g] = dZ_BR * ph.cZ1 - dR_BZ * ph.cR1;
+            a.J1[2 * L.field + g] = dR_RBP * (ph.cR1 * iR) - dP_BR * cPi;
+        }
+        advance();
+        __syncthreads();                               // the centre plane's slot is free again
+        if (tid == 0 && nc + NS < total) issue(nc + NS);
+    }
+}
+
+cudaError_t launch_curl_tma(const CurlArgs &a, const void *tmB, cudaStream_t s)
+{
+    constexpr int TZ = 14, NS = 8;
+    static bool configured = false;
+    auto kern = curl_tma_kernel<TZ, NS>;
+    const int smem = (int)sizeof(CurlTmaSmem<TZ, NS>);
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    dim3 block(TR, TZ, 1);
+    dim3 grid((a.L.nR - 4 + TR - 1) / TR, (a.L.nZ - 4 + TZ - 1) / TZ, a.phi_chunks);
+    kern<<<grid, block, smem, s>>>(a, *reinterpret_cast<const CUtensorMap *>(tmB));
+    return cudaGetLastError();
+}
+int curl_tma_tile_z() { return 14; }
+
+// ---------------------------------------------------------------------------------------------
 // Axisymmetric tables (once per clt_set_equilibrium): J0 = curl_c B0 etc.
 // ---------------------------------------------------------------------------------------------
 __global__ void tables_kernel(Layout L, Phys ph, double *tab, const double *R, const double *invR)
