@@ -41,6 +41,20 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def profiled_traffic(kernel="rhs_tma"):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed ncu --set full
+    summary (profiles/traffic.csv names the source file); None if there is no capture."""
+    p = os.path.join(ROOT, "profiles", "traffic.csv")
+    try:
+        for line in open(p).read().splitlines()[1:]:
+            k, v, _src = line.split(",", 2)
+            if k == kernel:
+                return float(v)
+    except Exception:
+        pass
+    return None
+
+
 class ClockSampler:
     """Samples nvidia-smi clocks / throttle reasons while the timed region runs."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -133,7 +147,7 @@ def run_ours(args):
     import torch
     import torch.distributed as dist
     from paper_1812_00525_b200 import build as clt_build
-    from paper_1812_00525_b200 import clt, inputs
+    from paper_1812_00525_b200 import clt, inputs, replicas
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -160,10 +174,7 @@ def run_ours(args):
     g.set_state(hU)
 
     def barrier():
-        torch.cuda.synchronize()
-        if world > 1:
-            dist.barrier()
-            torch.cuda.synchronize()
+        replicas.barrier(f"cuda:{local}")
 
     # ---- device-resident throughput -------------------------------------------------------------
     g.step(args.warmup)
@@ -183,10 +194,8 @@ def run_ours(args):
     prof = g.get_profile()
     g.set_profiling(False)
     clocks = sampler.stop()
-    if world > 1:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    total_updates, secs, value = replicas.aggregate(cfg.interior * args.steps, ms * 1e-3, device=f"cuda:{local}")
+    ms = secs * 1e3
     d = g.diagnostics()
     finite = all(np.isfinite(d[k]) for k in ("kinetic", "magnetic", "max_divB"))
 
@@ -201,10 +210,7 @@ def run_ours(args):
         g.get_state(hOut)        # D2H of the result (synchronous: host destination)
     barrier()
     e2e_s = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    _, e2e_s, e2e_value = replicas.aggregate(cfg.interior * e2e_steps, e2e_s, device=f"cuda:{local}")
     state_bytes = int(np.prod(cfg.shape)) * 8
 
     if rank != 0:
@@ -213,7 +219,6 @@ def run_ours(args):
         return
 
     ms_step = ms / args.steps
-    value = world * cfg.interior * args.steps / (ms * 1e-3)
     peak, peak_src = measured_peaks()
     # dominant kernel: the fused RHS + RK4 stage-combine kernel (its four stage variants pooled)
     n_rhs = sum(prof["n_rhs"][1:5])
@@ -230,8 +235,9 @@ def run_ours(args):
         if prof["n_curl"]:
             cms = prof["ms_curl"] / prof["n_curl"]
             curl = {"ms": cms, "GBps": CURL_DOUBLES * 8.0 * cfg.interior / (cms * 1e-3) / 1e9}
-        roof = {"bound": "hbm", "kernel": "rhs_kernel (fused RHS + RK4 stage combine, 4 stage variants pooled)",
-                "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": args.traffic,
+        roof = {"bound": "hbm", "kernel": "rhs_tma_kernel (fused RHS + RK4 stage combine, its 4 stage variants pooled)",
+                "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                "traffic": args.traffic if args.traffic is not None else (profiled_traffic() if cfg.index == 4 else None),
                 "peak_source": peak_src + ", burst figure", "avg_launch_ms": ms_rhs / n_rhs,
                 "algorithmic_bytes_per_launch": bytes_per_launch, "share_of_step": ms_rhs / (ms_rhs + prof["ms_curl"]),
                 "per_stage": per_stage, "curl_kernel": curl,
@@ -253,7 +259,7 @@ def run_ours(args):
                        "dt": prob.dt, "tile_z": args.tile_z, "phi_chunks": args.phi_chunks, "graph": args.graph,
                        "state_finite_after_run": bool(finite)},
             "clocks": clocks,
-            "e2e": {"value": world * cfg.interior * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": state_bytes,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": state_bytes,
                     "d2h_bytes_per_step": state_bytes, "steps": e2e_steps,
                     "how": "clt_set_state(pinned host) + clt_step(1) + clt_get_state(pinned host) per step, wall clock"},
             "gpu_launches": launches,

@@ -468,3 +468,47 @@ def test_P11_diagnostics_closed_forms():
     assert abs(d["magnetic_n1"] - 0.25 * (a * a + b * b) * area * 2 * np.pi) < 1e-13
     # div_c of B = (f(phi), const, 0) is f/R at every node
     assert abs(d["max_divB"] - np.abs(deep(U[5] / RR)).max()) < 1e-12
+
+
+# ----------------------------------------------------------------------------------------------- tolerance derivation
+def test_rounding_noise_floor_of_the_oracle_itself(tmp_path):
+    """Not a pin but the measurement behind reading R10: the SAME oracle source compiled with FMA contraction (a pure
+    change of rounding) moves the tiny v_phi of a config-5-like run by far more than 1e-12 of itself after 60 steps,
+    while every field measured as a physical quantity (rho, p, vector v, vector B) stays below 1e-9."""
+    import ctypes
+    import os
+    import subprocess
+    from parity_util import rel_linf, rel_linf_physical
+    src = os.path.join(os.path.dirname(orc.__file__), "clt_oracle.c")
+    so = str(tmp_path / "liboracle_fma.so")
+    r = subprocess.run(["gcc", "-O2", "-ffp-contract=fast", "-march=native", "-fopenmp", "-shared", "-fPIC", "-std=c11", "-o", so,
+                        src, "-lm"], capture_output=True)
+    if r.returncode != 0 or "fma" not in open("/proc/cpuinfo").read():
+        pytest.skip("no FMA-capable host compiler/CPU")
+    cfg = inputs.Config(5, "tearing-small", 64, 12, 64, 60, kind="tearing")
+    U0 = inputs.reference_state(cfg)
+    U = inputs.initial_state(cfg, U0)
+    dt = inputs.cfl_time_step(cfg, U)
+    outs = []
+    for lib in (None, so):
+        o = orc.Oracle(cfg.nR, cfg.nphi, cfg.nZ, cfg.Rmin, cfg.Rmax, cfg.Zmin, cfg.Zmax, gamma=cfg.gamma, eta=cfg.eta,
+                       nu=cfg.nu, D=cfg.D, kappa=cfg.kappa, dt=dt)
+        if lib is not None:           # same prototypes, other rounding: rebind this instance to the FMA build
+            L2 = ctypes.CDLL(lib)
+            for name in ("oracle_create", "oracle_destroy", "oracle_set_equilibrium", "oracle_set_state", "oracle_get_state",
+                         "oracle_step"):
+                getattr(L2, name).argtypes = getattr(o.L, name).argtypes
+                getattr(L2, name).restype = getattr(o.L, name).restype
+            o.close()
+            o.L = L2
+            o.h = L2.oracle_create(cfg.nR, cfg.nphi, cfg.nZ, cfg.Rmin, cfg.Rmax, cfg.Zmin, cfg.Zmax, 0.0, cfg.gamma, cfg.eta,
+                                   cfg.nu, cfg.D, cfg.kappa, dt)
+        o.set_equilibrium(U0)
+        o.set_state(U)
+        o.step(cfg.steps)
+        outs.append(o.get_state())
+    per_component = rel_linf(outs[1], outs[0])
+    physical = rel_linf_physical(outs[1], outs[0])
+    assert max(physical) < 1e-9, physical
+    assert per_component[3] > 1e-12, per_component      # v_phi: rounding alone already costs this much
+    assert max(per_component[f] for f in (0, 1, 5, 6, 7)) < 1e-13
