@@ -40,7 +40,9 @@ __device__ __forceinline__ int wrap_phi(int j, int n)
 // ---------------------------------------------------------------------------------------------
 // a3-a5 at one node: K of eqs (11)-(14) from
 //   stg  [5][HT]    centre-plane tile (with halo) of rho1, p1, v1_R, v1_phi, v1_Z
-//   er   [5][3][HT] ring of E1 tiles, slot se = plane j+2 (so j-2 -> se+1, j-1 -> se+2, j -> se+3, j+1 -> se+4)
+//   eRr, eZr        E1_R / E1_Z tiles (with halo) of a 5-slot ring, slot s at eRr + s*estride; slot se = plane j+2
+//                   (so j-2 -> se+1, j-1 -> se+2, j -> se+3, j+1 -> se+4, all mod 5)
+//   ePc  [HT]       E1_phi tile (with halo) of the centre plane
 //   fr   [3][IT]    F = J1 x B + J0 x B1 at the centre plane (tile interior)
 //   q    [5][5]     phi pipeline of the five fluid perturbations at this node, planes j-2..j+2
 // ---------------------------------------------------------------------------------------------
@@ -62,8 +64,9 @@ __device__ __forceinline__ CentreTab load_centre_tab(const double *tab, long lon
 }
 
 template <bool V0>
-__device__ __forceinline__ void rhs_point(const double *stg, const double *er, const double *fr, const double *sR, int HT,
-                                          int IT, int cs, int ci, int tx, int se, const double (&q)[5][5],
+__device__ __forceinline__ void rhs_point(const double *stg, const double *eRr, const double *eZr, int estride,
+                                          const double *ePc, const double *fr, const double *sR, int HT, int IT, int cs,
+                                          int ci, int tx, int se, const double (&q)[5][5],
                                           const CentreTab &ct, const double *tab, long long off2, long long plane,
                                           const Phys &ph, double iR, double iR2, double (&K)[8])
 {
@@ -158,11 +161,9 @@ __device__ __forceinline__ void rhs_point(const double *stg, const double *er, c
     const int sc = (se + 3 >= 5) ? se + 3 - 5 : se + 3;   // plane j
     const int s3 = (se + 4 >= 5) ? se + 4 - 5 : se + 4;   // plane j+1
     const int s4 = se;                                    // plane j+2
-    const double *eR = er + (sc * 3 + 0) * HT + cs, *eP = er + (sc * 3 + 1) * HT + cs, *eZ = er + (sc * 3 + 2) * HT + cs;
-    const double dP_EZ = fd1(er[(s0 * 3 + 2) * HT + cs], er[(s1 * 3 + 2) * HT + cs], er[(s3 * 3 + 2) * HT + cs],
-                             er[(s4 * 3 + 2) * HT + cs]);
-    const double dP_ER = fd1(er[(s0 * 3 + 0) * HT + cs], er[(s1 * 3 + 0) * HT + cs], er[(s3 * 3 + 0) * HT + cs],
-                             er[(s4 * 3 + 0) * HT + cs]);
+    const double *eR = eRr + sc * estride + cs, *eP = ePc + cs, *eZ = eZr + sc * estride + cs;
+    const double dP_EZ = fd1(eZr[s0 * estride + cs], eZr[s1 * estride + cs], eZr[s3 * estride + cs], eZr[s4 * estride + cs]);
+    const double dP_ER = fd1(eRr[s0 * estride + cs], eRr[s1 * estride + cs], eRr[s3 * estride + cs], eRr[s4 * estride + cs]);
     const double dZ_EP = fd1(eP[-2 * SW], eP[-SW], eP[SW], eP[2 * SW]);
     const double dZ_ER = fd1(eR[-2 * SW], eR[-SW], eR[SW], eR[2 * SW]);
     const double dR_EZ = fd1(eZ[-2], eZ[-1], eZ[1], eZ[2]);
@@ -341,8 +342,9 @@ __global__ void __launch_bounds__(TR *TZ, (TZ <= 8 ? 2 : 1)) rhs_kernel(const __
         {
             const int sfc = (sf + 1 >= 3) ? sf + 1 - 3 : sf + 1;  // ring slot of F at the centre plane
             const CentreTab ct = load_centre_tab(tab, L.plane, off2);
-            rhs_point<V0>(&S.stage[buf][0][0], &S.ering[0][0][0], &S.fring[sfc][0][0], S.sR, RhsSmem<TZ>::HT, IT, cs, ci, tx,
-                          se, q, ct, tab, off2, L.plane, ph, iR, iR2, K);
+            rhs_point<V0>(&S.stage[buf][0][0], &S.ering[0][0][0], &S.ering[0][2][0], 3 * RhsSmem<TZ>::HT, &S.ering[sec][1][0],
+                          &S.fring[sfc][0][0], S.sR, RhsSmem<TZ>::HT, IT, cs, ci, tx, se, q, ct, tab, off2, L.plane, ph, iR,
+                          iR2, K);
         }
 
         // ---- a6: RK4 stage combine in the epilogue (L125, L139) --------------------------------
@@ -405,7 +407,7 @@ static cudaError_t launch_rhs_tz(const RhsArgs &a, int mode, bool v0, cudaStream
 #undef CLT_CASE
 }
 
-int rhs_default_tile_z() { return 12; }
+int rhs_default_tile_z() { return 8; }
 
 cudaError_t launch_rhs(const RhsArgs &a, int mode, bool has_v0, int tile_z, cudaStream_t s)
 {
@@ -470,27 +472,28 @@ __device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, i
         : "memory");
 }
 
-template <int TZ>
+template <int TZ, int NRAW>
 struct RhsTmaSmem {
     static constexpr int HT = (TZ + 4) * SW;
     static constexpr int IT = TZ * TR;
     static constexpr int NH = 4 * TR + 4 * TZ;
     static constexpr int HTP = (HT + 15) / 16 * 16;   // every TMA destination 128-byte aligned
-    alignas(128) double raw[11][HTP];  // TMA destination: U (8) and J1 (3) of one plane, tile with halo
+    alignas(128) double raw[NRAW][11][HTP];  // TMA destinations: U (8) and J1 (3) of one plane, tile with halo
     double stage[2][5][HT];            // rho1, p1, v1 of the centre plane (double-buffered)
-    double ering[5][3][HT];            // E1 of planes j-2 .. j+2, tile with halo
+    double erz[5][2][HT];              // E1_R, E1_Z of planes j-2 .. j+2, tile with halo
+    double ep[4][HT];                  // E1_phi of planes j-1 .. j+2, tile with halo
     double fring[3][3][IT];            // F of planes j .. j+2
     double hring[3][5][NH];            // rho1, p1, v1 at the halo nodes of planes j .. j+2 (thread-private)
     double sR[SW];
-    alignas(8) unsigned long long bar;
+    alignas(8) unsigned long long bar[NRAW];
 };
 
-template <int TZ, int MODE, bool V0>
+template <int TZ, int NRAW, int MODE, bool V0>
 __global__ void __launch_bounds__(TR *TZ, 1)
 rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmJ)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    using SM = RhsTmaSmem<TZ>;
+    using SM = RhsTmaSmem<TZ, NRAW>;
     SM &S = *reinterpret_cast<SM *>(smem_raw);
     constexpr int HT = SM::HT, IT = SM::IT, NH = SM::NH;
     static_assert(NH <= TR * TZ, "tile too small for one halo node per thread");
@@ -525,7 +528,7 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
 
     if (tid < SW) S.sR[tid] = a.R[min(i0 - 2 + tid, L.nR - 1)];
     if (tid == 0) {
-        mbar_init(&S.bar, 1);
+        for (int b = 0; b < NRAW; ++b) mbar_init(&S.bar[b], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmU) : "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmJ) : "memory");
@@ -534,16 +537,18 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
 
     const double *tab = a.tab;
     const double eta = ph.eta;
-    unsigned parity = 0;
+    // planes are numbered n = 0, 1, .. from ja-2; plane n uses raw buffer n % NRAW, its (n / NRAW)-th use
+    int nlead = 0;     // number of the plane the next lead() consumes
 
-    // one elected thread: fetch the 11 fields of plane jl (tile with halo) into S.raw
-    auto issue = [&](int jl) {
-        const int jw = wrap_phi(jl, L.nphi);
-        mbar_expect_tx(&S.bar, (unsigned)(11 * HT * sizeof(double)));
+    // one elected thread: fetch the 11 fields of plane number n (tile with halo) into its raw buffer
+    auto issue = [&](int n) {
+        const int jw = wrap_phi(ja - 2 + n, L.nphi);
+        const int b = n % NRAW;
+        mbar_expect_tx(&S.bar[b], (unsigned)(11 * HT * sizeof(double)));
 #pragma unroll
-        for (int m = 0; m < 8; ++m) tma_load_4d(&S.raw[m][0], &tmU, LP + i0 - 2, k0 - 2, jw, m, &S.bar);
+        for (int m = 0; m < 8; ++m) tma_load_4d(&S.raw[b][m][0], &tmU, LP + i0 - 2, k0 - 2, jw, m, &S.bar[b]);
 #pragma unroll
-        for (int m = 0; m < 3; ++m) tma_load_4d(&S.raw[8 + m][0], &tmJ, LP + i0 - 2, k0 - 2, jw, m, &S.bar);
+        for (int m = 0; m < 3; ++m) tma_load_4d(&S.raw[b][8 + m][0], &tmJ, LP + i0 - 2, k0 - 2, jw, m, &S.bar[b]);
     };
 
     // phi-invariant table values of the own node and of the halo node, kept in registers for the whole sweep
@@ -555,11 +560,12 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
     const double h_rho0 = __ldg(tab + T_RHO0 * L.plane + hoff2), h_p0 = __ldg(tab + T_P0 * L.plane + hoff2);
 
     // forms perturbations, E1 and (optionally) F from the raw tile at slot s; o2 = table offset of the node
-    auto node = [&](int s, long long o2, double rho0, double p0, double q[5], double E[3], double F[3], bool wantF) {
-        const double rho = S.raw[0][s], p = S.raw[1][s];
-        const double vR = S.raw[2][s], vP = S.raw[3][s], vZ = S.raw[4][s];
-        const double BR = S.raw[5][s], BP = S.raw[6][s], BZ = S.raw[7][s];
-        const double JR = S.raw[8][s], JP = S.raw[9][s], JZ = S.raw[10][s];
+    auto node = [&](const double (*raw)[SM::HTP], int s, long long o2, double rho0, double p0, double q[5], double E[3],
+                    double F[3], bool wantF) {
+        const double rho = raw[0][s], p = raw[1][s];
+        const double vR = raw[2][s], vP = raw[3][s], vZ = raw[4][s];
+        const double BR = raw[5][s], BP = raw[6][s], BZ = raw[7][s];
+        const double JR = raw[8][s], JP = raw[9][s], JZ = raw[10][s];
         q[0] = rho - rho0;
         q[1] = p - p0;
         if (V0) {
@@ -587,24 +593,27 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
     };
 
     double q[5][5];
-    int se = 0, sf = 0;
+    int se = 0, sf = 0, sp = 0;     // ring slots (5-, 3-, 4-rings) that receive the plane being consumed (plane j+2)
 
-    // consume the raw tile (the plane that becomes plane j+2)
+    // consume the raw tile of plane number nlead (the plane that becomes plane j+2)
     auto lead = [&]() {
-        mbar_wait(&S.bar, parity);
-        parity ^= 1u;
+        const int b = nlead % NRAW;
+        mbar_wait(&S.bar[b], (unsigned)((nlead / NRAW) & 1));
+        ++nlead;
+        const double (*raw)[SM::HTP] = S.raw[b];
         double E[3], F[3];
-        node(cs, off2, ct.rho0, ct.p0, q[4], E, F, true);
+        node(raw, cs, off2, ct.rho0, ct.p0, q[4], E, F, true);
+        S.erz[se][0][cs] = E[0];
+        S.ep[sp][cs] = E[1];
+        S.erz[se][1][cs] = E[2];
 #pragma unroll
-        for (int c = 0; c < 3; ++c) {
-            S.ering[se][c][cs] = E[c];
-            S.fring[sf][c][ci] = F[c];
-        }
+        for (int c = 0; c < 3; ++c) S.fring[sf][c][ci] = F[c];
         if (is_halo) {
             double hq[5], hE[3], hF[3];
-            node(hs, hoff2, h_rho0, h_p0, hq, hE, hF, false);
-#pragma unroll
-            for (int c = 0; c < 3; ++c) S.ering[se][c][hs] = hE[c];
+            node(raw, hs, hoff2, h_rho0, h_p0, hq, hE, hF, false);
+            S.erz[se][0][hs] = hE[0];
+            S.ep[sp][hs] = hE[1];
+            S.erz[se][1][hs] = hE[2];
 #pragma unroll
             for (int f = 0; f < 5; ++f) S.hring[sf][f][tid] = hq[f];
         }
@@ -616,15 +625,18 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
             for (int f = 0; f < 5; ++f) q[d][f] = q[d + 1][f];
         se = (se == 4) ? 0 : se + 1;
         sf = (sf == 2) ? 0 : sf + 1;
+        sp = (sp + 1) & 3;
     };
 
-    // prologue: planes ja-2 .. ja+1
-    if (tid == 0) issue(ja - 2);
+    // prologue: planes number 0 .. 3 (ja-2 .. ja+1); NRAW planes are kept in flight
+    const int total = jb - ja + 4;
+    if (tid == 0)
+        for (int n = 0; n < NRAW && n < total; ++n) issue(n);
 #pragma unroll 1
-    for (int jl = ja - 2; jl <= ja + 1; ++jl) {
+    for (int n = 0; n < 4; ++n) {
         lead();
         __syncthreads();                 // every thread has read the raw tile
-        if (tid == 0) issue(jl + 1);
+        if (tid == 0 && n + NRAW < total) issue(n + NRAW);
         advance();
     }
 
@@ -645,6 +657,7 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
         }
         lead();
         const int sfc = (sf + 1 >= 3) ? sf + 1 - 3 : sf + 1;      // slot of the centre plane in the 3-rings
+        const int spc = (sp + 2) & 3;                             // ... in the 4-ring of E_phi
 #pragma unroll
         for (int f = 0; f < 5; ++f) S.stage[buf][f][cs] = q[2][f];
         if (is_halo) {
@@ -652,7 +665,10 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
             for (int f = 0; f < 5; ++f) S.stage[buf][f][hs] = S.hring[sfc][f][tid];
         }
         __syncthreads();
-        if (tid == 0 && j + 3 <= jb + 1) issue(j + 3);           // overlaps the whole of phase B
+        {   // the raw buffer just consumed (plane number j-ja+4) is free: refill it NRAW planes ahead
+            const int n = j - ja + 4 + NRAW;
+            if (tid == 0 && n < total) issue(n);                  // overlaps phase B (and NRAW-1 more iterations)
+        }
 
         // ---- a6 inputs: U^n / acc of this node, requested now so that they arrive during phase B ---
         const long long g = (long long)j * L.plane + off2;
@@ -667,8 +683,8 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
 
         // ---- phase B: K at (i, k, j) -----------------------------------------------------------
         double K[8];
-        rhs_point<V0>(&S.stage[buf][0][0], &S.ering[0][0][0], &S.fring[sfc][0][0], S.sR, HT, IT, cs, ci, tx, se, q, ct, tab,
-                      off2, L.plane, ph, iR, iR2, K);
+        rhs_point<V0>(&S.stage[buf][0][0], &S.erz[0][0][0], &S.erz[0][1][0], 2 * HT, &S.ep[spc][0], &S.fring[sfc][0][0], S.sR,
+                      HT, IT, cs, ci, tx, se, q, ct, tab, off2, L.plane, ph, iR, iR2, K);
 
         // ---- a6: RK4 stage combine in the epilogue (L125, L139) --------------------------------
         if (valid) {
@@ -692,12 +708,13 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
     }
 }
 
-template <int TZ, int MODE, bool V0>
+template <int TZ, int NRAW, int MODE, bool V0>
 static cudaError_t launch_rhs_tma_t(const RhsArgs &a, const CUtensorMap &tmU, const CUtensorMap &tmJ, cudaStream_t s)
 {
     static bool configured = false;
-    auto kern = rhs_tma_kernel<TZ, MODE, V0>;
-    const int smem = (int)sizeof(RhsTmaSmem<TZ>);
+    auto kern = rhs_tma_kernel<TZ, NRAW, MODE, V0>;
+    const int smem = (int)sizeof(RhsTmaSmem<TZ, NRAW>);
+    static_assert(sizeof(RhsTmaSmem<TZ, NRAW>) <= 232448, "shared memory of the TMA RHS kernel exceeds 227 KB");
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
@@ -709,13 +726,13 @@ static cudaError_t launch_rhs_tma_t(const RhsArgs &a, const CUtensorMap &tmU, co
     return cudaGetLastError();
 }
 
-template <int TZ>
+template <int TZ, int NRAW>
 static cudaError_t launch_rhs_tma_tz(const RhsArgs &a, const CUtensorMap &tmU, const CUtensorMap &tmJ, int mode, bool v0,
                                      cudaStream_t s)
 {
 #define CLT_CASE(M)                                                                                        \
     case M:                                                                                                \
-        return v0 ? launch_rhs_tma_t<TZ, M, true>(a, tmU, tmJ, s) : launch_rhs_tma_t<TZ, M, false>(a, tmU, tmJ, s);
+        return v0 ? launch_rhs_tma_t<TZ, NRAW, M, true>(a, tmU, tmJ, s) : launch_rhs_tma_t<TZ, NRAW, M, false>(a, tmU, tmJ, s);
     switch (mode) {
         CLT_CASE(RHS_MODE_K)
         CLT_CASE(RHS_MODE_S1)
@@ -736,10 +753,11 @@ cudaError_t launch_rhs_tma(const RhsArgs &a, const void *tmU, const void *tmJ, i
     const CUtensorMap &mU = *reinterpret_cast<const CUtensorMap *>(tmU);
     const CUtensorMap &mJ = *reinterpret_cast<const CUtensorMap *>(tmJ);
     switch (tile_z) {
-    case 8: return launch_rhs_tma_tz<8>(a, mU, mJ, mode, has_v0, s);
-    case 10: return launch_rhs_tma_tz<10>(a, mU, mJ, mode, has_v0, s);
-    case 12: return launch_rhs_tma_tz<12>(a, mU, mJ, mode, has_v0, s);
-    case 13: return launch_rhs_tma_tz<13>(a, mU, mJ, mode, has_v0, s);
+    // two raw buffers (TMA two planes ahead) where shared memory allows, one otherwise
+    case 8: return launch_rhs_tma_tz<8, 2>(a, mU, mJ, mode, has_v0, s);
+    case 10: return launch_rhs_tma_tz<10, 2>(a, mU, mJ, mode, has_v0, s);
+    case 12: return launch_rhs_tma_tz<12, 1>(a, mU, mJ, mode, has_v0, s);
+    case 13: return launch_rhs_tma_tz<13, 1>(a, mU, mJ, mode, has_v0, s);
     default: return cudaErrorInvalidValue;
     }
 }
