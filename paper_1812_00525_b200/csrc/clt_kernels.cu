@@ -63,12 +63,15 @@ __device__ __forceinline__ CentreTab load_centre_tab(const double *tab, long lon
     return t;
 }
 
-template <bool V0>
+// `sync` is called once, after everything that needs no other thread's shared-memory data (centre values, the
+// phi direction from the register pipeline, the phi differences of E1 at the own node) and before the first read
+// of a neighbour's staged value: the caller puts the wait half of its split barrier there.
+template <bool V0, class Sync>
 __device__ __forceinline__ void rhs_point(const double *stg, const double *eRr, const double *eZr, int estride,
                                           const double *ePc, const double *fr, const double *sR, int HT, int IT, int cs,
                                           int ci, int tx, int se, const double (&q)[5][5],
                                           const CentreTab &ct, const double *tab, long long off2, long long plane,
-                                          const Phys &ph, double iR, double iR2, double (&K)[8])
+                                          const Phys &ph, double iR, double iR2, double (&K)[8], Sync &&sync)
 {
     const double rho1 = q[2][0], p1 = q[2][1], v1R = q[2][2], v1P = q[2][3], v1Z = q[2][4];
     const double rho = rho1 + ct.rho0;
@@ -83,6 +86,32 @@ __device__ __forceinline__ void rhs_point(const double *stg, const double *eRr, 
 
     double A[5], lap[5];     // (v.grad) f and Laplacian f of the five staged fields
     double divv1, gRp1, gPp1, gZp1, gPvR, gPvP;
+    // phi direction (register pipeline)
+    {
+        const double g1 = ph.cP1 * iR, vc = vP * g1, lc = ph.cP2 * iR2;
+#pragma unroll
+        for (int f = 0; f < 5; ++f) {
+            const double d1 = fd1(q[0][f], q[1][f], q[3][f], q[4][f]);
+            const double d2 = fd2(q[0][f], q[1][f], q[2][f], q[3][f], q[4][f]);
+            A[f] = vc * d1;
+            lap[f] = lc * d2;
+            if (f == 1) gPp1 = d1 * g1;
+            if (f == 2) gPvR = d1 * g1;
+            if (f == 3) { gPvP = d1 * g1; divv1 = gPvP + v1R * iR; }
+        }
+    }
+    // phi differences of E1_Z, E1_R at the own node (slots written by this very thread)
+    const int s0 = (se + 1 >= 5) ? se + 1 - 5 : se + 1;   // plane j-2
+    const int s1 = (se + 2 >= 5) ? se + 2 - 5 : se + 2;   // plane j-1
+    const int sc = (se + 3 >= 5) ? se + 3 - 5 : se + 3;   // plane j
+    const int s3 = (se + 4 >= 5) ? se + 4 - 5 : se + 4;   // plane j+1
+    const int s4 = se;                                    // plane j+2
+    const double dP_EZ = fd1(eZr[s0 * estride + cs], eZr[s1 * estride + cs], eZr[s3 * estride + cs], eZr[s4 * estride + cs]);
+    const double dP_ER = fd1(eRr[s0 * estride + cs], eRr[s1 * estride + cs], eRr[s3 * estride + cs], eRr[s4 * estride + cs]);
+    const double fR = fr[0 * IT + ci], fP = fr[1 * IT + ci], fZ = fr[2 * IT + ci];
+
+    sync();
+
     // R direction (shared memory, stride 1)
     {
         const double vc = vR * ph.cR1, lc = iR * ph.cR1;
@@ -91,24 +120,10 @@ __device__ __forceinline__ void rhs_point(const double *stg, const double *eRr, 
             const double *s = stg + f * HT + cs;
             const double m2 = s[-2], m1 = s[-1], p1_ = s[1], p2 = s[2];
             const double d1 = fd1(m2, m1, p1_, p2), d2 = fd2(m2, m1, q[2][f], p1_, p2);
-            A[f] = vc * d1;
-            lap[f] = d2 * ph.cR2 + lc * d1;
-            if (f == 1) gRp1 = d1 * ph.cR1;
-            if (f == 2) divv1 = d1 * ph.cR1 + v1R * iR;
-        }
-    }
-    // phi direction (register pipeline)
-    {
-        const double g1 = ph.cP1 * iR, vc = vP * g1, lc = ph.cP2 * iR2;
-#pragma unroll
-        for (int f = 0; f < 5; ++f) {
-            const double d1 = fd1(q[0][f], q[1][f], q[3][f], q[4][f]);
-            const double d2 = fd2(q[0][f], q[1][f], q[2][f], q[3][f], q[4][f]);
             A[f] += vc * d1;
-            lap[f] += lc * d2;
-            if (f == 1) gPp1 = d1 * g1;
-            if (f == 2) gPvR = d1 * g1;
-            if (f == 3) { gPvP = d1 * g1; divv1 += gPvP; }
+            lap[f] += d2 * ph.cR2 + lc * d1;
+            if (f == 1) gRp1 = d1 * ph.cR1;
+            if (f == 2) divv1 += d1 * ph.cR1;
         }
     }
     // Z direction (shared memory, stride SW)
@@ -152,18 +167,11 @@ __device__ __forceinline__ void rhs_point(const double *stg, const double *eRr, 
               + r1 * __ldg(tab + T_A0Z * plane + off2);
     }
     const double two_iR = 2.0 * iR;
-    K[2] = (fr[0 * IT + ci] - gRp1) * rinv - aR + ph.nu * (lap[2] - v1R * iR2 - two_iR * gPvP);
-    K[3] = (fr[1 * IT + ci] - gPp1) * rinv - aP + ph.nu * (lap[3] - v1P * iR2 + two_iR * gPvR);
-    K[4] = (fr[2 * IT + ci] - gZp1) * rinv - aZ + ph.nu * lap[4];
+    K[2] = (fR - gRp1) * rinv - aR + ph.nu * (lap[2] - v1R * iR2 - two_iR * gPvP);
+    K[3] = (fP - gPp1) * rinv - aP + ph.nu * (lap[3] - v1P * iR2 + two_iR * gPvR);
+    K[4] = (fZ - gZp1) * rinv - aZ + ph.nu * lap[4];
     // eq (14): -curl_c(E1); the radial derivative differences R * E_phi
-    const int s0 = (se + 1 >= 5) ? se + 1 - 5 : se + 1;   // plane j-2
-    const int s1 = (se + 2 >= 5) ? se + 2 - 5 : se + 2;   // plane j-1
-    const int sc = (se + 3 >= 5) ? se + 3 - 5 : se + 3;   // plane j
-    const int s3 = (se + 4 >= 5) ? se + 4 - 5 : se + 4;   // plane j+1
-    const int s4 = se;                                    // plane j+2
     const double *eR = eRr + sc * estride + cs, *eP = ePc + cs, *eZ = eZr + sc * estride + cs;
-    const double dP_EZ = fd1(eZr[s0 * estride + cs], eZr[s1 * estride + cs], eZr[s3 * estride + cs], eZr[s4 * estride + cs]);
-    const double dP_ER = fd1(eRr[s0 * estride + cs], eRr[s1 * estride + cs], eRr[s3 * estride + cs], eRr[s4 * estride + cs]);
     const double dZ_EP = fd1(eP[-2 * SW], eP[-SW], eP[SW], eP[2 * SW]);
     const double dZ_ER = fd1(eR[-2 * SW], eR[-SW], eR[SW], eR[2 * SW]);
     const double dR_EZ = fd1(eZ[-2], eZ[-1], eZ[1], eZ[2]);
@@ -344,7 +352,7 @@ __global__ void __launch_bounds__(TR *TZ, (TZ <= 8 ? 2 : 1)) rhs_kernel(const __
             const CentreTab ct = load_centre_tab(tab, L.plane, off2);
             rhs_point<V0>(&S.stage[buf][0][0], &S.ering[0][0][0], &S.ering[0][2][0], 3 * RhsSmem<TZ>::HT, &S.ering[sec][1][0],
                           &S.fring[sfc][0][0], S.sR, RhsSmem<TZ>::HT, IT, cs, ci, tx, se, q, ct, tab, off2, L.plane, ph, iR,
-                          iR2, K);
+                          iR2, K, [] {});
         }
 
         // ---- a6: RK4 stage combine in the epilogue (L125, L139) --------------------------------
@@ -450,6 +458,10 @@ __device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, unsigned
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void mbar_arrive(unsigned long long *bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
 __device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity)
 {
     asm volatile(
@@ -485,7 +497,8 @@ struct RhsTmaSmem {
     double fring[3][3][IT];            // F of planes j .. j+2
     double hring[3][5][NH];            // rho1, p1, v1 at the halo nodes of planes j .. j+2 (thread-private)
     double sR[SW];
-    alignas(8) unsigned long long bar[NRAW];
+    alignas(8) unsigned long long bar[NRAW];   // TMA completion, one per raw buffer
+    alignas(8) unsigned long long ready;       // split CTA barrier: "this plane is staged" (count = all threads)
 };
 
 template <int TZ, int NRAW, int MODE, bool V0>
@@ -529,6 +542,7 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
     if (tid < SW) S.sR[tid] = a.R[min(i0 - 2 + tid, L.nR - 1)];
     if (tid == 0) {
         for (int b = 0; b < NRAW; ++b) mbar_init(&S.bar[b], 1);
+        mbar_init(&S.ready, TR * TZ);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmU) : "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmJ) : "memory");
@@ -639,6 +653,7 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
         if (tid == 0 && n + NRAW < total) issue(n + NRAW);
         advance();
     }
+    unsigned ready_parity = 0;
 
     const double iR = __ldg(a.invR + ic);
     const double iR2 = iR * iR;
@@ -664,10 +679,22 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
 #pragma unroll
             for (int f = 0; f < 5; ++f) S.stage[buf][f][hs] = S.hring[sfc][f][tid];
         }
-        __syncthreads();
-        {   // the raw buffer just consumed (plane number j-ja+4) is free: refill it NRAW planes ahead
+        // split barrier: announce "my part of plane j is staged", keep working on what needs nobody else's data
+        // (epilogue operand loads, the phi direction), and only then wait for the other warps.  Measured: a gain
+        // for the stage variants that are not yet HBM-bound (1, 4, K-only), a small loss for stages 2 and 3,
+        // which keep the plain barrier (and the TMA refill) right here.
+        constexpr bool SPLIT = (MODE != RHS_MODE_S2 && MODE != RHS_MODE_S3);
+        auto refill = [&]() {
+            // every thread has consumed the raw buffer of plane number j-ja+4: refill it NRAW planes ahead
+            // (overlaps the rest of phase B and NRAW-1 more iterations)
             const int n = j - ja + 4 + NRAW;
-            if (tid == 0 && n < total) issue(n);                  // overlaps phase B (and NRAW-1 more iterations)
+            if (tid == 0 && n < total) issue(n);
+        };
+        if (SPLIT) {
+            mbar_arrive(&S.ready);
+        } else {
+            __syncthreads();
+            refill();
         }
 
         // ---- a6 inputs: U^n / acc of this node, requested now so that they arrive during phase B ---
@@ -684,7 +711,13 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
         // ---- phase B: K at (i, k, j) -----------------------------------------------------------
         double K[8];
         rhs_point<V0>(&S.stage[buf][0][0], &S.erz[0][0][0], &S.erz[0][1][0], 2 * HT, &S.ep[spc][0], &S.fring[sfc][0][0], S.sR,
-                      HT, IT, cs, ci, tx, se, q, ct, tab, off2, L.plane, ph, iR, iR2, K);
+                      HT, IT, cs, ci, tx, se, q, ct, tab, off2, L.plane, ph, iR, iR2, K, [&] {
+                          if (SPLIT) {
+                              mbar_wait(&S.ready, ready_parity);
+                              refill();
+                          }
+                      });
+        ready_parity ^= 1u;
 
         // ---- a6: RK4 stage combine in the epilogue (L125, L139) --------------------------------
         if (valid) {
