@@ -254,19 +254,19 @@ int run_rhs(clt_ctx *ctx, int mode, const double *in, double *out, double a_next
     return CLT_OK;
 }
 
-// a6: one classical RK4 step in accumulator form (O5):
-//   s1: Ua = Un + dt/2 K1, acc = Un + dt/6 K1      s2: Ub = Un + dt/2 K2, acc += dt/3 K2
-//   s3: Ua = Un + dt K3,   acc += dt/3 K3          s4: Un = acc + dt/6 K4
+// a6: one classical RK4 step in the reduced-traffic accumulator form (clt_kernels.cu):
+//   s1: Ua = Un + dt/2 K1                          s2: Ub = Un + dt/2 K2, acc = Un + (Ua - Un)/3 + dt/3 K2
+//   s3: Ua = Un + dt K3                            s4: Un = acc + (Ua - Un)/3 + dt/6 K4
 int enqueue_step(clt_ctx *ctx)
 {
     const double dt = ctx->dt;
     int r;
     if ((r = run_curl(ctx, ctx->Un))) return r;
-    if ((r = run_rhs(ctx, RHS_MODE_S1, ctx->Un, ctx->Ua, 0.5 * dt, dt / 6.0))) return r;
+    if ((r = run_rhs(ctx, RHS_MODE_S1, ctx->Un, ctx->Ua, 0.5 * dt, 0.0))) return r;
     if ((r = run_curl(ctx, ctx->Ua))) return r;
     if ((r = run_rhs(ctx, RHS_MODE_S2, ctx->Ua, ctx->Ub, 0.5 * dt, dt / 3.0))) return r;
     if ((r = run_curl(ctx, ctx->Ub))) return r;
-    if ((r = run_rhs(ctx, RHS_MODE_S3, ctx->Ub, ctx->Ua, dt, dt / 3.0))) return r;
+    if ((r = run_rhs(ctx, RHS_MODE_S3, ctx->Ub, ctx->Ua, dt, 0.0))) return r;
     if ((r = run_curl(ctx, ctx->Ua))) return r;
     if ((r = run_rhs(ctx, RHS_MODE_S4, ctx->Ua, ctx->Un, 0.0, dt / 6.0))) return r;
     return CLT_OK;

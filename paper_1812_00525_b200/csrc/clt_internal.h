@@ -50,14 +50,14 @@ struct RhsArgs {
     Phys ph;
     const double *in;     // stage state, 8 fields
     const double *J1;     // 3 fields
-    const double *Un;     // U^n, 8 fields (modes 2, 3)
-    double *acc;          // RK4 accumulator, 8 fields (modes 1-4)
+    const double *Un;     // U^n, 8 fields (modes 2, 3, 4; mode 4 updates it in place through `out`)
+    double *acc;          // RK4 accumulator, 8 fields (written by mode 2, read by mode 4)
     double *out;          // K (mode 0) | next stage state (modes 1-3) | U^{n+1} (mode 4), 8 fields
     const double *tab;    // T_COUNT tables
     const double *R;      // R_i, i = -LP .. : pointer already offset so that R[i] is node i; padded with valid numbers
     const double *invR;   // 1/R_i, same indexing
     double a_next;        // out = U^n + a_next * K   (modes 1-3)
-    double b_acc;         // acc += b_acc * K  /  out = acc + b_acc * K (mode 4)
+    double b_acc;         // weight of K in the accumulator (mode 2) / in U^{n+1} (mode 4)
     int phi_chunks;       // number of chunks the phi range is split into (gridDim.z)
     int prefetch;         // issue L2 prefetch hints
 };

@@ -13,6 +13,15 @@
 
 namespace clt {
 
+// bit m set: the rhs_tma_kernel instantiation of mode m (0 = K only, 1..4 = RK4 stage) uses the split CTA barrier
+#ifndef CLT_SPLIT_MASK
+#define CLT_SPLIT_MASK 0x1F
+#endif
+// number of TMA raw buffers (planes in flight) of the default 32 x 8 tile
+#ifndef CLT_NRAW8
+#define CLT_NRAW8 2
+#endif
+
 constexpr int TR = 32;        // tile width in R = one warp per tile row
 constexpr int SW = TR + 4;    // shared row width with the radius-2 halo
 
@@ -39,11 +48,11 @@ __device__ __forceinline__ int wrap_phi(int j, int n)
 
 // ---------------------------------------------------------------------------------------------
 // a3-a5 at one node: K of eqs (11)-(14) from
-//   stg  [5][HT]    centre-plane tile (with halo) of rho1, p1, v1_R, v1_phi, v1_Z
-//   eRr, eZr        E1_R / E1_Z tiles (with halo) of a 5-slot ring, slot s at eRr + s*estride; slot se = plane j+2
-//                   (so j-2 -> se+1, j-1 -> se+2, j -> se+3, j+1 -> se+4, all mod 5)
-//   ePc  [HT]       E1_phi tile (with halo) of the centre plane
-//   fr   [3][IT]    F = J1 x B + J0 x B1 at the centre plane (tile interior)
+//   stg  [5][HT]    centre-plane tile (with halo) of rho1, p1, v1_R, v1_phi, v1_Z; field f at stg + f*HT
+//   eRc, ePc, eZc   E1_R / E1_phi / E1_Z tiles (with halo) of the centre plane
+//   dP_EZ, dP_ER    unscaled phi differences (fd1) of E1_Z, E1_R at the own node
+//   F    [3]        J1 x B + J0 x B1 at the own node of the centre plane
+//   rr   [4]        R_{i-2}, R_{i-1}, R_{i+1}, R_{i+2}
 //   q    [5][5]     phi pipeline of the five fluid perturbations at this node, planes j-2..j+2
 // ---------------------------------------------------------------------------------------------
 // axisymmetric table values of one node that the centre-plane arithmetic needs (phi-invariant, so a
@@ -67,11 +76,10 @@ __device__ __forceinline__ CentreTab load_centre_tab(const double *tab, long lon
 // phi direction from the register pipeline, the phi differences of E1 at the own node) and before the first read
 // of a neighbour's staged value: the caller puts the wait half of its split barrier there.
 template <bool V0, class Sync>
-__device__ __forceinline__ void rhs_point(const double *stg, const double *eRr, const double *eZr, int estride,
-                                          const double *ePc, const double *fr, const double *sR, int HT, int IT, int cs,
-                                          int ci, int tx, int se, const double (&q)[5][5],
-                                          const CentreTab &ct, const double *tab, long long off2, long long plane,
-                                          const Phys &ph, double iR, double iR2, double (&K)[8], Sync &&sync)
+__device__ __forceinline__ void rhs_point(const double *stg, int HT, const double *eRc, const double *ePc, const double *eZc,
+                                          double dP_EZ, double dP_ER, const double (&F)[3], const double (&rr)[4], int cs,
+                                          const double (&q)[5][5], const CentreTab &ct, const double *tab, long long off2,
+                                          long long plane, const Phys &ph, double iR, double iR2, double (&K)[8], Sync &&sync)
 {
     const double rho1 = q[2][0], p1 = q[2][1], v1R = q[2][2], v1P = q[2][3], v1Z = q[2][4];
     const double rho = rho1 + ct.rho0;
@@ -100,15 +108,7 @@ __device__ __forceinline__ void rhs_point(const double *stg, const double *eRr, 
             if (f == 3) { gPvP = d1 * g1; divv1 = gPvP + v1R * iR; }
         }
     }
-    // phi differences of E1_Z, E1_R at the own node (slots written by this very thread)
-    const int s0 = (se + 1 >= 5) ? se + 1 - 5 : se + 1;   // plane j-2
-    const int s1 = (se + 2 >= 5) ? se + 2 - 5 : se + 2;   // plane j-1
-    const int sc = (se + 3 >= 5) ? se + 3 - 5 : se + 3;   // plane j
-    const int s3 = (se + 4 >= 5) ? se + 4 - 5 : se + 4;   // plane j+1
-    const int s4 = se;                                    // plane j+2
-    const double dP_EZ = fd1(eZr[s0 * estride + cs], eZr[s1 * estride + cs], eZr[s3 * estride + cs], eZr[s4 * estride + cs]);
-    const double dP_ER = fd1(eRr[s0 * estride + cs], eRr[s1 * estride + cs], eRr[s3 * estride + cs], eRr[s4 * estride + cs]);
-    const double fR = fr[0 * IT + ci], fP = fr[1 * IT + ci], fZ = fr[2 * IT + ci];
+    const double fR = F[0], fP = F[1], fZ = F[2];
 
     sync();
 
@@ -171,16 +171,64 @@ __device__ __forceinline__ void rhs_point(const double *stg, const double *eRr, 
     K[3] = (fP - gPp1) * rinv - aP + ph.nu * (lap[3] - v1P * iR2 + two_iR * gPvR);
     K[4] = (fZ - gZp1) * rinv - aZ + ph.nu * lap[4];
     // eq (14): -curl_c(E1); the radial derivative differences R * E_phi
-    const double *eR = eRr + sc * estride + cs, *eP = ePc + cs, *eZ = eZr + sc * estride + cs;
+    const double *eR = eRc + cs, *eP = ePc + cs, *eZ = eZc + cs;
     const double dZ_EP = fd1(eP[-2 * SW], eP[-SW], eP[SW], eP[2 * SW]);
     const double dZ_ER = fd1(eR[-2 * SW], eR[-SW], eR[SW], eR[2 * SW]);
     const double dR_EZ = fd1(eZ[-2], eZ[-1], eZ[1], eZ[2]);
-    const double *r = sR + tx + 2;
-    const double dR_REP = fd1(r[-2] * eP[-2], r[-1] * eP[-1], r[1] * eP[1], r[2] * eP[2]);
+    const double dR_REP = fd1(rr[0] * eP[-2], rr[1] * eP[-1], rr[2] * eP[1], rr[3] * eP[2]);
     const double cPi = ph.cP1 * iR;
     K[5] = dZ_EP * ph.cZ1 - dP_EZ * cPi;
     K[6] = dR_EZ * ph.cR1 - dZ_ER * ph.cZ1;
     K[7] = dP_ER * cPi - dR_REP * (ph.cR1 * iR);
+}
+
+// ---------------------------------------------------------------------------------------------
+// a6: RK4 stage combine (L125, L139) in a reduced-traffic accumulator form.
+// Classical RK4, U^{n+1} = U^n + dt/6 (K1 + 2 K2 + 2 K3 + K4); the partial sums are rebuilt from stage
+// states that are read anyway instead of being written and re-read through a separate array:
+//   S1: U_a = U^n + dt/2 K1                                        (no accumulator write)
+//   S2: U_b = U^n + dt/2 K2,  acc = U^n + (U_a - U^n)/3 + dt/3 K2   ((U_a - U^n)/3 = dt/6 K1)
+//   S3: U_a = U^n + dt K3                                          (no accumulator traffic)
+//   S4: U^{n+1} = acc + (U_a - U^n)/3 + dt/6 K4                     ((U_a - U^n)/3 = dt/3 K3)
+// Identical to the textbook scheme up to rounding order.  Per node and step this moves 19 + 35 + 27 + 35
+// doubles through the fused kernel instead of 27 + 43 + 43 + 27.
+// ---------------------------------------------------------------------------------------------
+struct EpiOperands {
+    double un[8];   // U^n at the node
+    double us[8];   // stage state at the node (S2: U_a of stage 1, S4: U_a of stage 3)
+    double ac[8];   // accumulator (S4)
+};
+template <int MODE, class Load>
+__device__ __forceinline__ void epilogue_load(const RhsArgs &a, long long g, long long field, EpiOperands &e, Load &&ld)
+{
+#pragma unroll
+    for (int m = 0; m < 8; ++m) {
+        const long long gm = m * field + g;
+        if (MODE == RHS_MODE_S1) e.un[m] = ld(a.in + gm);
+        if (MODE == RHS_MODE_S2 || MODE == RHS_MODE_S3 || MODE == RHS_MODE_S4) e.un[m] = ld(a.Un + gm);
+        if (MODE == RHS_MODE_S2 || MODE == RHS_MODE_S4) e.us[m] = ld(a.in + gm);
+        if (MODE == RHS_MODE_S4) e.ac[m] = ld(a.acc + gm);
+    }
+}
+template <int MODE>
+__device__ __forceinline__ void epilogue_store(const RhsArgs &a, long long g, long long field, const EpiOperands &e,
+                                               const double (&K)[8])
+{
+    constexpr double third = 1.0 / 3.0;
+#pragma unroll
+    for (int m = 0; m < 8; ++m) {
+        const long long gm = m * field + g;
+        if (MODE == RHS_MODE_K) {
+            a.out[gm] = K[m];
+        } else if (MODE == RHS_MODE_S1 || MODE == RHS_MODE_S3) {
+            a.out[gm] = fma(a.a_next, K[m], e.un[m]);
+        } else if (MODE == RHS_MODE_S2) {
+            a.out[gm] = fma(a.a_next, K[m], e.un[m]);
+            a.acc[gm] = fma(a.b_acc, K[m], fma(e.us[m] - e.un[m], third, e.un[m]));
+        } else {
+            a.out[gm] = fma(a.b_acc, K[m], fma(e.us[m] - e.un[m], third, e.ac[m]));
+        }
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -199,9 +247,8 @@ struct RhsSmem {
 template <int TZ, int MODE, bool V0>
 __global__ void __launch_bounds__(TR *TZ, (TZ <= 8 ? 2 : 1)) rhs_kernel(const __grid_constant__ RhsArgs a)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     RhsSmem<TZ> &S = *reinterpret_cast<RhsSmem<TZ> *>(smem_raw);
-    constexpr int IT = RhsSmem<TZ>::IT;
     const Layout &L = a.L;
     const Phys &ph = a.ph;
 
@@ -326,8 +373,8 @@ __global__ void __launch_bounds__(TR *TZ, (TZ <= 8 ? 2 : 1)) rhs_kernel(const __
                 const long long g1 = (long long)(j + 1) * L.plane + off2;
 #pragma unroll
                 for (int m = 0; m < 8; ++m) {
-                    if (MODE == RHS_MODE_S2 || MODE == RHS_MODE_S3) prefetch_l2(a.Un + m * L.field + g1);
-                    if (MODE != RHS_MODE_S1) prefetch_l2(a.acc + m * L.field + g1);
+                    if (MODE != RHS_MODE_S1) prefetch_l2(a.Un + m * L.field + g1);
+                    if (MODE == RHS_MODE_S4) prefetch_l2(a.acc + m * L.field + g1);
                 }
             }
         }
@@ -350,31 +397,24 @@ __global__ void __launch_bounds__(TR *TZ, (TZ <= 8 ? 2 : 1)) rhs_kernel(const __
         {
             const int sfc = (sf + 1 >= 3) ? sf + 1 - 3 : sf + 1;  // ring slot of F at the centre plane
             const CentreTab ct = load_centre_tab(tab, L.plane, off2);
-            rhs_point<V0>(&S.stage[buf][0][0], &S.ering[0][0][0], &S.ering[0][2][0], 3 * RhsSmem<TZ>::HT, &S.ering[sec][1][0],
-                          &S.fring[sfc][0][0], S.sR, RhsSmem<TZ>::HT, IT, cs, ci, tx, se, q, ct, tab, off2, L.plane, ph, iR,
-                          iR2, K, [] {});
+            // phi differences of E1_Z, E1_R at the own node (ring slots written by this very thread):
+            // slot se = plane j+2, so j-2 -> se+1, j-1 -> se+2, j+1 -> se+4 (mod 5)
+            const int s0 = (se + 1 >= 5) ? se + 1 - 5 : se + 1, s1 = (se + 2 >= 5) ? se + 2 - 5 : se + 2;
+            const int s3 = (se + 4 >= 5) ? se + 4 - 5 : se + 4;
+            const double dP_EZ = fd1(S.ering[s0][2][cs], S.ering[s1][2][cs], S.ering[s3][2][cs], S.ering[se][2][cs]);
+            const double dP_ER = fd1(S.ering[s0][0][cs], S.ering[s1][0][cs], S.ering[s3][0][cs], S.ering[se][0][cs]);
+            const double F[3] = { S.fring[sfc][0][ci], S.fring[sfc][1][ci], S.fring[sfc][2][ci] };
+            const double rr[4] = { S.sR[tx], S.sR[tx + 1], S.sR[tx + 3], S.sR[tx + 4] };
+            rhs_point<V0>(&S.stage[buf][0][0], RhsSmem<TZ>::HT, &S.ering[sec][0][0], &S.ering[sec][1][0], &S.ering[sec][2][0],
+                          dP_EZ, dP_ER, F, rr, cs, q, ct, tab, off2, L.plane, ph, iR, iR2, K, [] {});
         }
 
         // ---- a6: RK4 stage combine in the epilogue (L125, L139) --------------------------------
         if (valid) {
             const long long g = (long long)jw * L.plane + off2;
-#pragma unroll
-            for (int m = 0; m < 8; ++m) {
-                const long long gm = m * L.field + g;
-                if (MODE == RHS_MODE_K) {
-                    a.out[gm] = K[m];
-                } else if (MODE == RHS_MODE_S1) {
-                    const double un = __ldg(a.in + gm);
-                    a.out[gm] = fma(a.a_next, K[m], un);
-                    a.acc[gm] = fma(a.b_acc, K[m], un);
-                } else if (MODE == RHS_MODE_S4) {
-                    a.out[gm] = fma(a.b_acc, K[m], a.acc[gm]);
-                } else {
-                    const double un = __ldg(a.Un + gm);
-                    a.out[gm] = fma(a.a_next, K[m], un);
-                    a.acc[gm] = fma(a.b_acc, K[m], a.acc[gm]);
-                }
-            }
+            EpiOperands eo;
+            epilogue_load<MODE>(a, g, L.field, eo, [](const double *p) { return __ldg(p); });
+            epilogue_store<MODE>(a, g, L.field, eo, K);
         }
         advance();
     }
@@ -436,8 +476,10 @@ cudaError_t launch_rhs(const RhsArgs &a, int mode, bool has_v0, int tile_z, cuda
 // fields of plane j+3 arrive as halo'd (TR+4) x (TZ+4) boxes through cp.async.bulk.tensor into one
 // shared "raw" buffer while plane j is being computed, completing on an mbarrier: the long-latency
 // HBM/L2 reads never sit in front of the FP64 work and cost no registers.  Every plane is read from
-// L2 exactly once per CTA (interior + halo in one box); its halo values wait in small thread-private
-// rings until the plane becomes the centre plane.
+// L2 exactly once per CTA (interior + halo in one box) and converted once, on arrival, into the
+// perturbations and E1 that the stencils need (4-slot shared rings, tile with halo); everything that only
+// the own node needs along phi (fluid pipeline, E1_R/E1_Z pipeline, the Lorentz term F, R neighbours)
+// lives in registers: shared-memory bandwidth is the second roof of this kernel.
 // ---------------------------------------------------------------------------------------------
 // streaming 8-byte load that does not allocate in L1 (the epilogue operands are touched exactly once);
 // volatile so that it is issued where it is written: ahead of the FP64 work that hides its latency
@@ -487,16 +529,14 @@ __device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, i
 template <int TZ, int NRAW>
 struct RhsTmaSmem {
     static constexpr int HT = (TZ + 4) * SW;
-    static constexpr int IT = TZ * TR;
     static constexpr int NH = 4 * TR + 4 * TZ;
     static constexpr int HTP = (HT + 15) / 16 * 16;   // every TMA destination 128-byte aligned
     alignas(128) double raw[NRAW][11][HTP];  // TMA destinations: U (8) and J1 (3) of one plane, tile with halo
-    double stage[2][5][HT];            // rho1, p1, v1 of the centre plane (double-buffered)
-    double erz[5][2][HT];              // E1_R, E1_Z of planes j-2 .. j+2, tile with halo
-    double ep[4][HT];                  // E1_phi of planes j-1 .. j+2, tile with halo
-    double fring[3][3][IT];            // F of planes j .. j+2
-    double hring[3][5][NH];            // rho1, p1, v1 at the halo nodes of planes j .. j+2 (thread-private)
-    double sR[SW];
+    // 4-slot rings, tile with halo, written once when a plane arrives (as plane j+2) and read by the in-plane
+    // stencils when it is the centre plane (two iterations later).  Four slots, not three: the slot that receives
+    // plane j+2 held plane j-2, whose last readers are separated from this write by the barrier of iteration j-1.
+    double sring[4][5][HT];            // rho1, p1, v1
+    double ering[4][3][HT];            // E1
     alignas(8) unsigned long long bar[NRAW];   // TMA completion, one per raw buffer
     alignas(8) unsigned long long ready;       // split CTA barrier: "this plane is staged" (count = all threads)
 };
@@ -508,7 +548,7 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
     extern __shared__ __align__(128) unsigned char smem_raw[];
     using SM = RhsTmaSmem<TZ, NRAW>;
     SM &S = *reinterpret_cast<SM *>(smem_raw);
-    constexpr int HT = SM::HT, IT = SM::IT, NH = SM::NH;
+    constexpr int HT = SM::HT, NH = SM::NH;
     static_assert(NH <= TR * TZ, "tile too small for one halo node per thread");
     const Layout &L = a.L;
     const Phys &ph = a.ph;
@@ -522,7 +562,6 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
     const int jb = (int)(((long long)L.nphi * (blockIdx.z + 1)) / a.phi_chunks);
     const long long off2 = (long long)kc * L.pR + (LP + ic);
     const int cs = (ty + 2) * SW + (tx + 2);
-    const int ci = ty * TR + tx;
 
     int hx, hy;
     if (tid < 4 * TR) {
@@ -539,7 +578,6 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
     const long long hoff2 = (long long)hk * L.pR + (LP + hi);
     const int hs = (hy + 2) * SW + (hx + 2);
 
-    if (tid < SW) S.sR[tid] = a.R[min(i0 - 2 + tid, L.nR - 1)];
     if (tid == 0) {
         for (int b = 0; b < NRAW; ++b) mbar_init(&S.bar[b], 1);
         mbar_init(&S.ready, TR * TZ);
@@ -565,13 +603,15 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
         for (int m = 0; m < 3; ++m) tma_load_4d(&S.raw[b][8 + m][0], &tmJ, LP + i0 - 2, k0 - 2, jw, m, &S.bar[b]);
     };
 
-    // phi-invariant table values of the own node and of the halo node, kept in registers for the whole sweep
+    // phi-invariant values of the own node and of the halo node, kept in registers for the whole sweep
     const CentreTab ct = load_centre_tab(tab, L.plane, off2);
     const double b0R = __ldg(tab + T_B0R * L.plane + off2), b0P = __ldg(tab + T_B0P * L.plane + off2),
                  b0Z = __ldg(tab + T_B0Z * L.plane + off2);
     const double j0R = __ldg(tab + T_J0R * L.plane + off2), j0P = __ldg(tab + T_J0P * L.plane + off2),
                  j0Z = __ldg(tab + T_J0Z * L.plane + off2);
     const double h_rho0 = __ldg(tab + T_RHO0 * L.plane + hoff2), h_p0 = __ldg(tab + T_P0 * L.plane + hoff2);
+    const double rr[4] = { __ldg(a.R + min(i - 2, L.nR - 1)), __ldg(a.R + min(i - 1, L.nR - 1)), __ldg(a.R + min(i + 1, L.nR - 1)),
+                           __ldg(a.R + min(i + 2, L.nR - 1)) };
 
     // forms perturbations, E1 and (optionally) F from the raw tile at slot s; o2 = table offset of the node
     auto node = [&](const double (*raw)[SM::HTP], int s, long long o2, double rho0, double p0, double q[5], double E[3],
@@ -606,8 +646,11 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
         }
     };
 
-    double q[5][5];
-    int se = 0, sf = 0, sp = 0;     // ring slots (5-, 3-, 4-rings) that receive the plane being consumed (plane j+2)
+    // thread-private phi pipelines at the own node
+    double q[5][5];        // rho1, p1, v1 of planes j-2 .. j+2
+    double eR[5], eZ[5];   // E1_R, E1_Z of planes j-2 .. j+2
+    double Fp[3][3];       // F = J1 x B + J0 x B1 of planes j .. j+2
+    int sl = 0;            // ring slot that receives the plane being consumed (plane j+2)
 
     // consume the raw tile of plane number nlead (the plane that becomes plane j+2)
     auto lead = [&]() {
@@ -615,31 +658,34 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
         mbar_wait(&S.bar[b], (unsigned)((nlead / NRAW) & 1));
         ++nlead;
         const double (*raw)[SM::HTP] = S.raw[b];
-        double E[3], F[3];
-        node(raw, cs, off2, ct.rho0, ct.p0, q[4], E, F, true);
-        S.erz[se][0][cs] = E[0];
-        S.ep[sp][cs] = E[1];
-        S.erz[se][1][cs] = E[2];
+        double E[3];
+        node(raw, cs, off2, ct.rho0, ct.p0, q[4], E, Fp[2], true);
+        eR[4] = E[0];
+        eZ[4] = E[2];
 #pragma unroll
-        for (int c = 0; c < 3; ++c) S.fring[sf][c][ci] = F[c];
+        for (int c = 0; c < 3; ++c) S.ering[sl][c][cs] = E[c];
+#pragma unroll
+        for (int f = 0; f < 5; ++f) S.sring[sl][f][cs] = q[4][f];
         if (is_halo) {
             double hq[5], hE[3], hF[3];
             node(raw, hs, hoff2, h_rho0, h_p0, hq, hE, hF, false);
-            S.erz[se][0][hs] = hE[0];
-            S.ep[sp][hs] = hE[1];
-            S.erz[se][1][hs] = hE[2];
 #pragma unroll
-            for (int f = 0; f < 5; ++f) S.hring[sf][f][tid] = hq[f];
+            for (int c = 0; c < 3; ++c) S.ering[sl][c][hs] = hE[c];
+#pragma unroll
+            for (int f = 0; f < 5; ++f) S.sring[sl][f][hs] = hq[f];
         }
     };
     auto advance = [&]() {
 #pragma unroll
-        for (int d = 0; d < 4; ++d)
+        for (int d = 0; d < 4; ++d) {
 #pragma unroll
             for (int f = 0; f < 5; ++f) q[d][f] = q[d + 1][f];
-        se = (se == 4) ? 0 : se + 1;
-        sf = (sf == 2) ? 0 : sf + 1;
-        sp = (sp + 1) & 3;
+            eR[d] = eR[d + 1];
+            eZ[d] = eZ[d + 1];
+        }
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { Fp[0][c] = Fp[1][c]; Fp[1][c] = Fp[2][c]; }
+        sl = (sl + 1) & 3;
     };
 
     // prologue: planes number 0 .. 3 (ja-2 .. ja+1); NRAW planes are kept in flight
@@ -660,30 +706,21 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
 
 #pragma unroll 1
     for (int j = ja; j < jb; ++j) {
-        const int buf = j & 1;
-        // ---- phase A: consume plane j+2, stage plane j ----------------------------------------
+        // ---- phase A: consume plane j+2 --------------------------------------------------------
         if (a.prefetch && MODE != RHS_MODE_K && (tx & 15) == 0 && j + 1 < jb) {
             const long long g1 = (long long)(j + 1) * L.plane + off2;
 #pragma unroll
             for (int m = 0; m < 8; ++m) {
-                if (MODE == RHS_MODE_S2 || MODE == RHS_MODE_S3) prefetch_l2(a.Un + m * L.field + g1);
-                if (MODE != RHS_MODE_S1) prefetch_l2(a.acc + m * L.field + g1);
+                if (MODE != RHS_MODE_S1) prefetch_l2(a.Un + m * L.field + g1);
+                if (MODE == RHS_MODE_S4) prefetch_l2(a.acc + m * L.field + g1);
             }
         }
         lead();
-        const int sfc = (sf + 1 >= 3) ? sf + 1 - 3 : sf + 1;      // slot of the centre plane in the 3-rings
-        const int spc = (sp + 2) & 3;                             // ... in the 4-ring of E_phi
-#pragma unroll
-        for (int f = 0; f < 5; ++f) S.stage[buf][f][cs] = q[2][f];
-        if (is_halo) {
-#pragma unroll
-            for (int f = 0; f < 5; ++f) S.stage[buf][f][hs] = S.hring[sfc][f][tid];
-        }
-        // split barrier: announce "my part of plane j is staged", keep working on what needs nobody else's data
-        // (epilogue operand loads, the phi direction), and only then wait for the other warps.  Measured: a gain
-        // for the stage variants that are not yet HBM-bound (1, 4, K-only), a small loss for stages 2 and 3,
-        // which keep the plain barrier (and the TMA refill) right here.
-        constexpr bool SPLIT = (MODE != RHS_MODE_S2 && MODE != RHS_MODE_S3);
+        const int sc = (sl + 2) & 3;                              // ring slot of the centre plane
+        // split barrier: announce "my part of plane j+2 is in the rings", keep working on what needs nobody else's
+        // data (epilogue operand loads, the phi direction), and only then wait for the other warps.  Which stage
+        // variants use it is a measured choice (CLT_SPLIT_MASK); the others keep the plain barrier right here.
+        constexpr bool SPLIT = ((CLT_SPLIT_MASK >> MODE) & 1) != 0;
         auto refill = [&]() {
             // every thread has consumed the raw buffer of plane number j-ja+4: refill it NRAW planes ahead
             // (overlaps the rest of phase B and NRAW-1 more iterations)
@@ -697,21 +734,17 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
             refill();
         }
 
-        // ---- a6 inputs: U^n / acc of this node, requested now so that they arrive during phase B ---
+        // ---- a6 inputs: U^n / stage state / acc of this node, requested now so that they arrive during phase B ---
         const long long g = (long long)j * L.plane + off2;
-        double un[8], ac[8];
-#pragma unroll
-        for (int m = 0; m < 8; ++m) {
-            const long long gm = m * L.field + g;
-            if (MODE == RHS_MODE_S1) un[m] = ld_stream(a.in + gm);
-            if (MODE == RHS_MODE_S2 || MODE == RHS_MODE_S3) un[m] = ld_stream(a.Un + gm);
-            if (MODE == RHS_MODE_S2 || MODE == RHS_MODE_S3 || MODE == RHS_MODE_S4) ac[m] = ld_stream(a.acc + gm);
-        }
+        EpiOperands eo;
+        epilogue_load<MODE>(a, g, L.field, eo, [](const double *p) { return ld_stream(p); });
 
         // ---- phase B: K at (i, k, j) -----------------------------------------------------------
         double K[8];
-        rhs_point<V0>(&S.stage[buf][0][0], &S.erz[0][0][0], &S.erz[0][1][0], 2 * HT, &S.ep[spc][0], &S.fring[sfc][0][0], S.sR,
-                      HT, IT, cs, ci, tx, se, q, ct, tab, off2, L.plane, ph, iR, iR2, K, [&] {
+        const double dP_EZ = fd1(eZ[0], eZ[1], eZ[3], eZ[4]);
+        const double dP_ER = fd1(eR[0], eR[1], eR[3], eR[4]);
+        rhs_point<V0>(&S.sring[sc][0][0], HT, &S.ering[sc][0][0], &S.ering[sc][1][0], &S.ering[sc][2][0], dP_EZ, dP_ER, Fp[0], rr,
+                      cs, q, ct, tab, off2, L.plane, ph, iR, iR2, K, [&] {
                           if (SPLIT) {
                               mbar_wait(&S.ready, ready_parity);
                               refill();
@@ -720,23 +753,7 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
         ready_parity ^= 1u;
 
         // ---- a6: RK4 stage combine in the epilogue (L125, L139) --------------------------------
-        if (valid) {
-#pragma unroll
-            for (int m = 0; m < 8; ++m) {
-                const long long gm = m * L.field + g;
-                if (MODE == RHS_MODE_K) {
-                    a.out[gm] = K[m];
-                } else if (MODE == RHS_MODE_S1) {
-                    a.out[gm] = fma(a.a_next, K[m], un[m]);
-                    a.acc[gm] = fma(a.b_acc, K[m], un[m]);
-                } else if (MODE == RHS_MODE_S4) {
-                    a.out[gm] = fma(a.b_acc, K[m], ac[m]);
-                } else {
-                    a.out[gm] = fma(a.a_next, K[m], un[m]);
-                    a.acc[gm] = fma(a.b_acc, K[m], ac[m]);
-                }
-            }
-        }
+        if (valid) epilogue_store<MODE>(a, g, L.field, eo, K);
         advance();
     }
 }
@@ -787,7 +804,7 @@ cudaError_t launch_rhs_tma(const RhsArgs &a, const void *tmU, const void *tmJ, i
     const CUtensorMap &mJ = *reinterpret_cast<const CUtensorMap *>(tmJ);
     switch (tile_z) {
     // two raw buffers (TMA two planes ahead) where shared memory allows, one otherwise
-    case 8: return launch_rhs_tma_tz<8, 2>(a, mU, mJ, mode, has_v0, s);
+    case 8: return launch_rhs_tma_tz<8, CLT_NRAW8>(a, mU, mJ, mode, has_v0, s);
     case 10: return launch_rhs_tma_tz<10, 2>(a, mU, mJ, mode, has_v0, s);
     case 12: return launch_rhs_tma_tz<12, 1>(a, mU, mJ, mode, has_v0, s);
     case 13: return launch_rhs_tma_tz<13, 1>(a, mU, mJ, mode, has_v0, s);
