@@ -58,6 +58,8 @@ def lib():
             L.oracle_get_time.argtypes = [ctypes.c_void_p]
             L.oracle_curl_J1.argtypes = [ctypes.c_void_p, _dp, _dp]
             L.oracle_E1.argtypes = [ctypes.c_void_p, _dp, _dp]
+            L.oracle_hall_G.argtypes = [ctypes.c_void_p, _dp, _dp]
+            L.oracle_set_hall.argtypes = [ctypes.c_void_p, ctypes.c_double]
             L.oracle_rhs_of.argtypes = [ctypes.c_void_p, _dp, _dp]
             L.oracle_rhs.argtypes = [ctypes.c_void_p, _dp]
             L.oracle_step.argtypes = [ctypes.c_void_p, ctypes.c_int]
@@ -89,7 +91,7 @@ class Oracle:
     """
 
     def __init__(self, nR, nphi, nZ, Rmin, Rmax, Zmin, Zmax, phi_extent=0.0, gamma=5.0 / 3.0, eta=0.0, nu=0.0,
-                 D=0.0, kappa=0.0, dt=0.0):
+                 D=0.0, kappa=0.0, dt=0.0, d_i=0.0):
         self.L = lib()
         self.nR, self.nphi, self.nZ = int(nR), int(nphi), int(nZ)
         self.h = self.L.oracle_create(self.nR, self.nphi, self.nZ, Rmin, Rmax, Zmin, Zmax, phi_extent, gamma, eta,
@@ -98,6 +100,8 @@ class Oracle:
             raise ValueError("oracle_create rejected the grid")
         self.shape = (self.nphi, self.nZ, self.nR)
         self.L.oracle_set_equilibrium(self.h, None)
+        if d_i:
+            self.L.oracle_set_hall(self.h, float(d_i))
 
     def close(self):
         if getattr(self, "h", None):
@@ -152,6 +156,14 @@ class Oracle:
         out = np.empty((3,) + self.shape)
         self.L.oracle_E1(self.h, _ptr(self._chk(U, 8)), _ptr(out))
         return out
+
+    def hall_G(self, U):
+        out = np.empty((3,) + self.shape)
+        self.L.oracle_hall_G(self.h, _ptr(self._chk(U, 8)), _ptr(out))
+        return out
+
+    def set_hall(self, d_i):
+        self.L.oracle_set_hall(self.h, float(d_i))
 
     def rhs_of(self, U):
         K = np.empty((8,) + self.shape)

@@ -3,7 +3,8 @@
  *
  * Plain, slow, obviously-correct CPU evaluation (FP64) of the hot path of CLTx
  * (arxiv 1812.00525): the resistive-MHD right-hand side in the equilibrium-subtracted
- * form, eqs (11)-(14) [PAPER.md L105-115] with Ohm/Ampere, eqs (5)-(6) [L77-79] (d_i = 0),
+ * form, eqs (11)-(14) [PAPER.md L105-115] with Ohm/Ampere, eqs (5)-(6) [L77-79] (Hall term of eq (5)
+ * optional: d_i = 0 unless oracle_set_hall() is called),
  * on a uniform cylindrical (R, phi, Z) grid with 4th-order central differences [L125],
  * advanced by the classical 4th-order Runge-Kutta scheme [L125, L139], plus the
  * kinetic/magnetic-energy and div B diagnostics [L139, L149, L430] and the SETDT CFL
@@ -23,7 +24,9 @@
  * a sympy-derived analytic RHS of eqs (1)-(6); P4 div_c B stays at round-off over steps;
  * P5 rigid rotation annihilated by the viscous operator; P6 U0 = 0 reduces to a separately
  * written numpy evaluation of eqs (1)-(4); P7 Alfven modified-wavenumber identity; P8 RK4 order
- * on du/dt = lambda u through oracle_rk4 and on the MHD system by dt-halving.
+ * on du/dt = lambda u through oracle_rk4 and on the MHD system by dt-halving.  P12 Hall term of eq (5):
+ * exact discrete whistler-type response with the squared modified wavenumber, d_i = 0 reduction, and the
+ * sympy convergence pin P3b run with d_i != 0.
  * Parity unpinned: none of the exported functions (each is covered by at least one pin); the
  * absolute value of a generic RHS has no paper-printed number to compare with (PAPER.md prints
  * no worked example), so the pins above are mathematical ones.
@@ -44,6 +47,7 @@ typedef struct oracle {
     double Rmin, Rmax, Zmin, Zmax, Lphi;
     double dR, dZ, dphi;
     double gamma, eta, nu, D, kappa, dt;
+    double d_i;         /* ion inertial length of the Hall term in eq (5); 0 = resistive MHD */
     double *R;          /* R_i = Rmin + i*dR  (reading R1; hazard H1)           */
     double *Z;          /* Z_k = Zmin + k*dZ                                     */
     size_t N;           /* nodes per field                                       */
@@ -57,6 +61,7 @@ typedef struct oracle {
     double *U1;         /* 8N  perturbation U - U0                               */
     double *J1;         /* 3N                                                    */
     double *E1;         /* 3N                                                    */
+    double *G;          /* 3N  Hall field (J1 x B + J0 x B1 - grad p1)/rho - rho1 (v0.grad)v0/rho on interior nodes */
     double *K1, *K2, *K3, *K4, *Us;   /* 8N each, RK4 work                      */
     int64_t step;
     double time;
@@ -240,6 +245,7 @@ oracle *oracle_create(int nR, int nphi, int nZ, double Rmin, double Rmax, double
     size_t N = o->N;
     o->U0 = zalloc(8 * N); o->J0 = zalloc(3 * N); o->divv0 = zalloc(N); o->v0gv0 = zalloc(3 * N);
     o->U = zalloc(8 * N); o->U1 = zalloc(8 * N); o->J1 = zalloc(3 * N); o->E1 = zalloc(3 * N);
+    o->G = zalloc(3 * N);
     o->K1 = zalloc(8 * N); o->K2 = zalloc(8 * N); o->K3 = zalloc(8 * N); o->K4 = zalloc(8 * N);
     o->Us = zalloc(8 * N);
     return o;
@@ -249,12 +255,14 @@ void oracle_destroy(oracle *o)
 {
     if (!o) return;
     free(o->R); free(o->Z); free(o->U0); free(o->J0); free(o->divv0); free(o->v0gv0);
-    free(o->U); free(o->U1); free(o->J1); free(o->E1);
+    free(o->U); free(o->U1); free(o->J1); free(o->E1); free(o->G);
     free(o->K1); free(o->K2); free(o->K3); free(o->K4); free(o->Us);
     free(o);
 }
 
 void oracle_set_dt(oracle *o, double dt) { o->dt = dt; }
+/* switches the Hall term of eq (5) [L77] on (d_i != 0) or off (d_i = 0, the default) */
+void oracle_set_hall(oracle *o, double d_i) { o->d_i = d_i; }
 
 /* O3: equilibrium U0(R,Z), axisymmetric, [8][nZ][nR]; NULL = all zero.  J0 = curl_c(B0) on
  * interior nodes, once (reading R5: 0 on the boundary layers).                              */
@@ -317,8 +325,33 @@ static void compute_U1_J1_E1(oracle *o, const double *U)
                 curl_c(o, B1, i, k, j, c);
                 o->J1[n] = c[0]; o->J1[N + n] = c[1]; o->J1[2 * N + n] = c[2];
             }
-    /* a4: E1 = -v x B + v0 x B0 + eta J1 at every node (eq 5 with d_i = 0, minus E0 = -v0 x B0,
-     * eq 10; readings G5, G6).  On the boundary layers J1 = 0.                                */
+    /* Hall field of eq (5) [L77] in the equilibrium-subtracted form (reading R11):
+     *   E - E0 with E0 = -v0 x B0 + (d_i/rho0)(J0 x B0 - grad p0) [curl-free by eq (10)] and eq (9) used exactly
+     *   as eq (13) uses it gives  d_i * G,
+     *   G = (J1 x B + J0 x B1 - grad p1)/rho - (rho1/rho) (v0.grad)v0      -- the force bracket of eq (13).
+     * On interior nodes; G = 0 on the boundary layers (like J1, reading R5).                    */
+    memset(o->G, 0, 3 * N * sizeof(double));
+    if (o->d_i != 0.0) {
+#pragma omp parallel for collapse(2) schedule(static)
+        for (int j = 0; j < o->nphi; ++j)
+            for (int k = 2; k <= o->nZ - 3; ++k)
+                for (int i = 2; i <= o->nR - 3; ++i) {
+                    size_t n = idx(o, i, k, j);
+                    double BB[3]  = { U[5 * N + n], U[6 * N + n], U[7 * N + n] };
+                    double BB1[3] = { B1[n], B1[N + n], B1[2 * N + n] };
+                    double JJ1[3] = { o->J1[n], o->J1[N + n], o->J1[2 * N + n] };
+                    double JJ0[3] = { o->J0[n], o->J0[N + n], o->J0[2 * N + n] };
+                    double J1xB[3], J0xB1[3], gp1[3];
+                    cross(JJ1, BB, J1xB);
+                    cross(JJ0, BB1, J0xB1);
+                    grad(o, o->U1 + N, i, k, j, gp1);
+                    for (int c = 0; c < 3; ++c)
+                        o->G[(size_t)c * N + n] = (J1xB[c] + J0xB1[c] - gp1[c]) / U[n]
+                                                  - o->U1[n] * o->v0gv0[(size_t)c * N + n] / U[n];
+                }
+    }
+    /* a4: E1 = -v x B + v0 x B0 + eta J1 + d_i G at every node (eq 5 minus E0, eq 10; readings G5, R11).
+     * On the boundary layers J1 = 0 and G = 0.                                                  */
 #pragma omp parallel for schedule(static)
     for (size_t n = 0; n < N; ++n) {
         double v[3] = { U[2 * N + n], U[3 * N + n], U[4 * N + n] };
@@ -328,8 +361,11 @@ static void compute_U1_J1_E1(oracle *o, const double *U)
         double vxB[3], v0xB0[3];
         cross(v, B, vxB);
         cross(v0, B0, v0xB0);
-        for (int c = 0; c < 3; ++c)
-            o->E1[(size_t)c * N + n] = -vxB[c] + v0xB0[c] + o->eta * o->J1[(size_t)c * N + n];
+        for (int c = 0; c < 3; ++c) {
+            double e = -vxB[c] + v0xB0[c] + o->eta * o->J1[(size_t)c * N + n];
+            if (o->d_i != 0.0) e += o->d_i * o->G[(size_t)c * N + n];
+            o->E1[(size_t)c * N + n] = e;
+        }
     }
 }
 
@@ -342,6 +378,11 @@ void oracle_E1(oracle *o, const double *U, double *E1_out)
 {
     compute_U1_J1_E1(o, U);
     memcpy(E1_out, o->E1, 3 * o->N * sizeof(double));
+}
+void oracle_hall_G(oracle *o, const double *U, double *G_out)
+{
+    compute_U1_J1_E1(o, U);
+    memcpy(G_out, o->G, 3 * o->N * sizeof(double));
 }
 
 /* a3-a5: K = dU/dt from eqs (11)-(14) on interior nodes, K = 0 on the boundary layers.

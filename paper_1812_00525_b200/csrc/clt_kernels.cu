@@ -17,6 +17,16 @@ namespace clt {
 #ifndef CLT_SPLIT_MASK
 #define CLT_SPLIT_MASK 0x1F
 #endif
+// launch shape of curl_tma_kernel: tile height, ring depth (planes), CTAs per SM
+#ifndef CLT_CURL_TZ
+#define CLT_CURL_TZ 10
+#define CLT_CURL_NS 6
+#define CLT_CURL_MINB 2
+#endif
+// how many planes ahead of their use the epilogue operands (U^n, acc) are prefetched into L2
+#ifndef CLT_PF_DIST
+#define CLT_PF_DIST 1
+#endif
 // number of TMA raw buffers (planes in flight) of the default 32 x 8 tile
 #ifndef CLT_NRAW8
 #define CLT_NRAW8 2
@@ -707,8 +717,8 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
 #pragma unroll 1
     for (int j = ja; j < jb; ++j) {
         // ---- phase A: consume plane j+2 --------------------------------------------------------
-        if (a.prefetch && MODE != RHS_MODE_K && (tx & 15) == 0 && j + 1 < jb) {
-            const long long g1 = (long long)(j + 1) * L.plane + off2;
+        if (a.prefetch && MODE != RHS_MODE_K && (tx & 15) == 0 && j + CLT_PF_DIST < jb) {
+            const long long g1 = (long long)(j + CLT_PF_DIST) * L.plane + off2;
 #pragma unroll
             for (int m = 0; m < 8; ++m) {
                 if (MODE != RHS_MODE_S1) prefetch_l2(a.Un + m * L.field + g1);
@@ -941,7 +951,7 @@ struct CurlTmaSmem {
 };
 
 template <int TZ, int NS>
-__global__ void __launch_bounds__(TR *TZ, 1) curl_tma_kernel(const __grid_constant__ CurlArgs a, const __grid_constant__ CUtensorMap tmB)
+__global__ void __launch_bounds__(TR *TZ, CLT_CURL_MINB) curl_tma_kernel(const __grid_constant__ CurlArgs a, const __grid_constant__ CUtensorMap tmB)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     using SM = CurlTmaSmem<TZ, NS>;
@@ -1038,7 +1048,7 @@ __global__ void __launch_bounds__(TR *TZ, 1) curl_tma_kernel(const __grid_consta
 
 cudaError_t launch_curl_tma(const CurlArgs &a, const void *tmB, cudaStream_t s)
 {
-    constexpr int TZ = 14, NS = 8;
+    constexpr int TZ = CLT_CURL_TZ, NS = CLT_CURL_NS;
     static bool configured = false;
     auto kern = curl_tma_kernel<TZ, NS>;
     const int smem = (int)sizeof(CurlTmaSmem<TZ, NS>);
@@ -1052,7 +1062,7 @@ cudaError_t launch_curl_tma(const CurlArgs &a, const void *tmB, cudaStream_t s)
     kern<<<grid, block, smem, s>>>(a, *reinterpret_cast<const CUtensorMap *>(tmB));
     return cudaGetLastError();
 }
-int curl_tma_tile_z() { return 14; }
+int curl_tma_tile_z() { return CLT_CURL_TZ; }
 
 // ---------------------------------------------------------------------------------------------
 // Axisymmetric tables (once per clt_set_equilibrium): J0 = curl_c B0 etc.
