@@ -11,6 +11,8 @@ P6 reduction (U0 = 0: eqs (11)-(14) == a separately written numpy evaluation of 
 P7 exact discrete Alfven response with the stencil's modified wavenumber
 P8 textbook RK4 order through oracle_rk4 and dt-halving on the MHD system   L125
 P10 SETDT closed form (Fig. 4), P11 diagnostics closed forms
+P12 Hall term of eq (5): exact whistler-type response with k*^2, momentum bracket identity, d_i = 0 reduction
+    (and P3b runs with d_i != 0 against the sympy-derived continuous eq (5))
 """
 import numpy as np
 import pytest
@@ -199,7 +201,7 @@ def _manufactured(sp, syms, equilibrium_exact):
     return dict(rho0=rho0, p0=p0, v0=v0, B0=B0, rho1=rho1, p1=p1, v1=v1, B1=B1)
 
 
-def _continuous_rhs(sp, syms, op, m, par, subtracted):
+def _continuous_rhs(sp, syms, op, m, par, subtracted, d_i=0):
     """Continuous right-hand sides: eqs (1)-(6) on the total state, or eqs (11)-(14)."""
     G, eta, nu, D, kap = par
     rho = m["rho0"] + m["rho1"]
@@ -212,7 +214,8 @@ def _continuous_rhs(sp, syms, op, m, par, subtracted):
     J1 = [a - b for a, b in zip(J, J0)]
     dot = lambda a, b: sum(x * y for x, y in zip(a, b))
     if not subtracted:
-        E = [-x + eta * y for x, y in zip(op["cross"](v, B), J1)]                        # eq (5), d_i = 0
+        hall = [(a - b) / rho for a, b in zip(op["cross"](J, B), op["grad"](p))]            # (J x B - grad p)/rho
+        E = [-x + eta * y + d_i * h for x, y, h in zip(op["cross"](v, B), J1, hall)]      # eq (5)
         Krho = -op["div"]([rho * x for x in v]) + D * op["lap"](m["rho1"])             # eq (1)
         Kp = -dot(v, op["grad"](p)) - G * p * op["div"](v) + kap * op["lap"](m["p1"])    # eq (2)
         JxB = op["cross"](J, B)
@@ -222,6 +225,12 @@ def _continuous_rhs(sp, syms, op, m, par, subtracted):
         KB = [-x for x in op["curl"](E)]                                                 # eq (4)
     else:
         E1 = [-x + y + eta * z for x, y, z in zip(op["cross"](v, B), op["cross"](v0, B0), J1)]
+        if d_i:
+            # reading R11: E - E0 with eq (9) used as in eq (13): d_i * (force bracket of eq (13))
+            a0 = op["adv"](v0, v0)
+            Gh = [(a + b - c) / rho - m["rho1"] * d / rho
+                  for a, b, c, d in zip(op["cross"](J1, B), op["cross"](J0, B1), op["grad"](m["p1"]), a0)]
+            E1 = [e + d_i * g for e, g in zip(E1, Gh)]
         Krho = -op["div"]([rho * a + m["rho1"] * b for a, b in zip(v1, v0)]) + D * op["lap"](m["rho1"])   # eq (11)
         Kp = (-dot(v1, op["grad"](p)) - dot(v0, op["grad"](m["p1"]))
               - G * (p * op["div"](v1) + m["p1"] * op["div"](v0)) + kap * op["lap"](m["p1"]))              # eq (12)
@@ -234,16 +243,16 @@ def _continuous_rhs(sp, syms, op, m, par, subtracted):
     return [Krho, Kp] + Kv + KB
 
 
-@pytest.mark.parametrize("equilibrium_exact", [True, False])
-def test_P3b_full_rhs_converges_at_4th_order_to_the_continuous_equations(equilibrium_exact):
+@pytest.mark.parametrize("equilibrium_exact,d_i", [(True, 0), (False, 0), (True, 0.07), (False, 0.07)])
+def test_P3b_full_rhs_converges_at_4th_order_to_the_continuous_equations(equilibrium_exact, d_i):
     sp, syms, op = _sympy_ops()
     m = _manufactured(sp, syms, equilibrium_exact)
     par = (5.0 / 3.0, 0.05, 0.04, 0.03, 0.02)
     # with an exact equilibrium the ORIGINAL eqs (1)-(4) are the target; otherwise eqs (11)-(14)
-    target = _continuous_rhs(sp, syms, op, m, par, subtracted=not equilibrium_exact)
+    target = _continuous_rhs(sp, syms, op, m, par, subtracted=not equilibrium_exact, d_i=d_i)
     if equilibrium_exact:
         # and the two continuous forms agree (checked numerically at a few points)
-        other = _continuous_rhs(sp, syms, op, m, par, subtracted=True)
+        other = _continuous_rhs(sp, syms, op, m, par, subtracted=True, d_i=d_i)
         pts = (np.array([2.3, 3.1]), np.array([0.4, 2.0]), np.array([-0.2, 0.5]))
         for a, b in zip(target, other):
             fa = sp.lambdify(syms, a, "numpy")(*pts)
@@ -252,7 +261,7 @@ def test_P3b_full_rhs_converges_at_4th_order_to_the_continuous_equations(equilib
     errs = []
     for n in (2, 4):
         o, RR, P, ZZ = make(nR=20 * n + 1, nphi=16 * n, nZ=16 * n + 1, gamma=par[0], eta=par[1], nu=par[2], D=par[3],
-                            kappa=par[4])
+                            kappa=par[4], d_i=d_i)
         ev = lambda e: _lamb(sp, syms, e)(RR, P, ZZ)
         U0 = np.stack([ev(m["rho0"]), ev(m["p0"])] + [ev(x) for x in m["v0"]] + [ev(x) for x in m["B0"]])
         U1 = np.stack([ev(m["rho1"]), ev(m["p1"])] + [ev(x) for x in m["v1"]] + [ev(x) for x in m["B1"]])
@@ -262,10 +271,19 @@ def test_P3b_full_rhs_converges_at_4th_order_to_the_continuous_equations(equilib
         # rows next to the frozen layers see J1 = 0 on the boundary layers (reading R5) inside curl(eta J1):
         # compare on the deep interior, where every stencil stays on interior nodes
         errs.append([np.abs(deep(K[f] - Kx[f])).max() for f in range(8)])
+        if d_i:
+            assert np.abs(deep(K[5:] - o_noh(o, U0, U1)[5:])).max() > 1e-3      # the Hall term really contributes
         scale = [np.abs(Kx[f]).max() for f in range(8)]
     for f in range(8):
         assert errs[1][f] < 2e-3 * scale[f], (f, errs[1][f], scale[f])
         assert 3.5 < _order(errs[0][f], errs[1][f]) < 4.7, (f, errs[0][f], errs[1][f])
+
+
+def o_noh(o, U0, U1):
+    """RHS of the same oracle context with the Hall term switched off (and back on)."""
+    o.set_hall(0.0)
+    K = o.rhs_of(U0 + U1)
+    return K
 
 
 # ----------------------------------------------------------------------------------------------- P4
@@ -389,6 +407,36 @@ def test_P7_alfven_response_has_the_stencils_modified_wavenumber(nmode):
     K = o.rhs_of(Ub)
     assert np.abs(interior(K[4] - exp)).max() < 1e-10 * np.abs(exp).max()       # rho = 1
     # => omega^2 = kstar^2 B_phi^2 / (rho R^2): the discrete Alfven frequency of the near-slab limit
+
+
+# ----------------------------------------------------------------------------------------------- P12
+@pytest.mark.parametrize("nmode", [1, 2])
+def test_P12_hall_term_whistler_response_and_reductions(nmode):
+    """Hall term of eq (5) [L77].  Near-slab B = (0, c/R, eps sin(k phi)), rho = 1, p uniform, v = 0, U0 = 0:
+    J_R = eps k* cos(k phi)/R, G_Z = (J x B)_Z / rho = J_R B_phi, E_Z = d_i G_Z, so
+    K_{B_R} = -d_phi(E_Z)/R = d_i c k*^2 eps sin(k phi) / R^3 exactly, k* the stencil's modified wavenumber
+    (the whistler's k^2 dependence); its sign fixes the sign of the Hall term."""
+    nphi, c, eps, d_i = 16, 2.0, 1e-3, 0.3
+    Lphi = 2 * np.pi / 100
+    o, RR, P, ZZ = make(nR=18, nphi=nphi, nZ=18, Rmin=99.0, Rmax=101.0, phi_extent=Lphi, d_i=d_i)
+    h = Lphi / nphi
+    kphys = 2 * np.pi * nmode / Lphi
+    kstar = (8 * np.sin(kphys * h) - np.sin(2 * kphys * h)) / (6 * h)
+    U = np.zeros((8,) + RR.shape)
+    U[0], U[1], U[6] = 1.0, 0.3, c / RR
+    U[7] = eps * np.sin(kphys * P)
+    K = o.rhs_of(U)
+    exp = d_i * c * kstar ** 2 * eps * np.sin(kphys * P) / RR ** 3
+    assert np.abs(deep(K[5] - exp)).max() < 1e-10 * np.abs(exp).max()
+    # with v = 0 and v0 = 0 the momentum equation (13) is exactly the Hall field G (nu = 0 here)
+    G = o.hall_G(U)
+    assert np.abs(interior(G - K[2:5])).max() <= 1e-15 * np.abs(G).max()
+    assert np.all(G[:, :, :2] == 0) and np.all(G[..., -2:] == 0)
+    # d_i = 0 is bit-identical to resistive MHD, and G is then not formed at all
+    o.set_hall(0.0)
+    o2, *_ = make(nR=18, nphi=nphi, nZ=18, Rmin=99.0, Rmax=101.0, phi_extent=Lphi)
+    assert np.array_equal(o.rhs_of(U), o2.rhs_of(U))
+    assert np.all(o.hall_G(U) == 0)
 
 
 # ----------------------------------------------------------------------------------------------- P8
