@@ -69,12 +69,17 @@ typedef struct {
 /* Physics and run parameters [L67-81]: ratio of specific heats Gamma, and the uniform dissipation
  * coefficients eta (resistivity), nu (viscosity), D (density diffusion), kappa (heat conduction).
  * dt > 0 is the fixed RK4 time step used by clt_step.  cfl is only used by clt_suggest_dt when its
- * cfl argument is <= 0.  flags: reserved, must be 0.                                             */
+ * cfl argument is <= 0.  flags: reserved, must be 0.  d_i >= 0 is the ion inertial length of the Hall
+ * term (d_i/rho)(J x B - grad p) of eq (5) [L77]; 0 (the measured configs) = resistive MHD.  With
+ * d_i > 0 the curl pass also forms G = (J1 x B + J0 x B1 - grad p1)/rho - (rho1/rho)(v0.grad)v0 on
+ * interior nodes and E1 gains d_i G (reading R11); this needs the default kernel variant and
+ * tile height (clt_rhs / clt_step return CLT_EINVAL otherwise).                                   */
 typedef struct {
     double gamma, eta, nu, D, kappa;
     double dt;
     double cfl;
     uint32_t flags;
+    double d_i;
 } clt_params;
 
 /* Diagnostics [L139, L149, L430]; sums run over interior nodes with weight R_i dR dphi dZ:
@@ -88,7 +93,7 @@ typedef struct {
     double time;    /* sum of the dt's of those steps      */
 } clt_diag;
 
-/* Device bytes clt_create() needs for this grid (35 padded fields + equilibrium tables + reduction
+/* Device bytes clt_create() needs for this grid (38 padded fields + equilibrium tables + reduction
  * scratch).  Returns 0 for an invalid grid.                                                      */
 size_t clt_workspace_bytes(const clt_grid *grid);
 
@@ -122,6 +127,11 @@ int clt_rhs(clt_ctx *ctx, double *dUdt);
 
 /* J1[3][nphi][nZ][nR] = curl(B - B0) of the current state (eq (6)); 0 on the boundary layers.     */
 int clt_curl_J1(clt_ctx *ctx, double *J1);
+
+/* G[3][nphi][nZ][nR] = Hall field (J1 x B + J0 x B1 - grad p1)/rho - (rho1/rho)(v0.grad)v0 of the current
+ * state (eq (5) [L77], reading R11); 0 on the boundary layers.  CLT_EINVAL if params.d_i = 0
+ * or with the plain-load kernel variant.                                                         */
+int clt_hall_G(clt_ctx *ctx, double *G);
 
 /* n >= 0 classical RK4 steps with the fixed time step params.dt (or the last clt_set_dt value).
  * Asynchronous.                                                                                  */

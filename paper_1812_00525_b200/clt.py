@@ -26,7 +26,7 @@ class clt_grid(ctypes.Structure):
 class clt_params(ctypes.Structure):
     _fields_ = [("gamma", ctypes.c_double), ("eta", ctypes.c_double), ("nu", ctypes.c_double),
                 ("D", ctypes.c_double), ("kappa", ctypes.c_double), ("dt", ctypes.c_double),
-                ("cfl", ctypes.c_double), ("flags", ctypes.c_uint32)]
+                ("cfl", ctypes.c_double), ("flags", ctypes.c_uint32), ("d_i", ctypes.c_double)]
 
 
 class clt_diag(ctypes.Structure):
@@ -42,7 +42,7 @@ class clt_profile(ctypes.Structure):
 
 # every symbol include/clt.h declares
 EXPORTS = ["clt_workspace_bytes", "clt_create", "clt_destroy", "clt_set_equilibrium", "clt_set_state", "clt_get_state",
-           "clt_rhs", "clt_curl_J1", "clt_step", "clt_set_dt", "clt_diagnostics", "clt_suggest_dt", "clt_set_tuning",
+           "clt_rhs", "clt_curl_J1", "clt_hall_G", "clt_step", "clt_set_dt", "clt_diagnostics", "clt_suggest_dt", "clt_set_tuning",
            "clt_set_kernel_variant", "clt_set_profiling", "clt_get_profile", "clt_launch_count", "clt_stream", "clt_strerror", "clt_last_cuda_error", "clt_version"]
 
 _lib = None
@@ -72,7 +72,7 @@ def load():
     for name in ("clt_destroy",):
         getattr(L, name).restype = i
         getattr(L, name).argtypes = [vp]
-    for name in ("clt_set_equilibrium", "clt_set_state", "clt_get_state", "clt_rhs", "clt_curl_J1"):
+    for name in ("clt_set_equilibrium", "clt_set_state", "clt_get_state", "clt_rhs", "clt_curl_J1", "clt_hall_G"):
         getattr(L, name).restype = i
         getattr(L, name).argtypes = [vp, vp]
     L.clt_step.restype = i
@@ -125,14 +125,14 @@ class Clt:
     """One libclt context.  Method names and semantics are those of include/clt.h."""
 
     def __init__(self, nR, nphi, nZ, Rmin, Rmax, Zmin, Zmax, phi_extent=0.0, gamma=5.0 / 3.0, eta=0.0, nu=0.0, D=0.0,
-                 kappa=0.0, dt=0.0, cfl=0.5, device="cuda:0", stream=None):
+                 kappa=0.0, dt=0.0, cfl=0.5, d_i=0.0, device="cuda:0", stream=None):
         import torch
         self.L = load()
         if not torch.cuda.is_available():
             raise RuntimeError("libclt needs a CUDA device (no CPU fallback)")
         self.device = torch.device(device)
         self.grid = clt_grid(nR, nphi, nZ, Rmin, Rmax, Zmin, Zmax, phi_extent)
-        self.params = clt_params(gamma, eta, nu, D, kappa, dt, cfl, 0)
+        self.params = clt_params(gamma, eta, nu, D, kappa, dt, cfl, 0, d_i)
         self.shape = (8, nphi, nZ, nR)
         nbytes = self.L.clt_workspace_bytes(ctypes.byref(self.grid))
         if nbytes == 0:
@@ -195,6 +195,12 @@ class Clt:
         if out is None:
             out = np.empty((3,) + self.shape[1:])
         self._ck(self.L.clt_curl_J1(self.h, _addr(out)))
+        return out
+
+    def hall_G(self, out=None):
+        if out is None:
+            out = np.empty((3,) + self.shape[1:])
+        self._ck(self.L.clt_hall_G(self.h, _addr(out)))
         return out
 
     def step(self, n=1):

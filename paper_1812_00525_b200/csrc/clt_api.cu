@@ -20,9 +20,9 @@ struct clt_ctx {
     Phys ph;
     cudaStream_t stream;
     // workspace carving (device)
-    double *Un, *acc, *Ua, *Ub, *J1, *tab, *Rtab, *invRtab, *cs, *partial, *result;
+    double *Un, *acc, *Ua, *Ub, *J1, *G, *tab, *Rtab, *invRtab, *cs, *partial, *result;
     int nblocks_diag;
-    bool has_state, has_v0;
+    bool has_state, has_v0, hall;
     int64_t step;
     double time;
     double dt;
@@ -83,7 +83,7 @@ Carve carve(const clt_grid *g)
     c.nblocks = diag_blocks(L);
     c.partial_b = align_up((size_t)c.nblocks * 6 * sizeof(double));
     c.result_b = align_up(8 * sizeof(double));
-    c.total = 35 * c.field_b + T_COUNT * c.table_b + 2 * c.rtab_b + c.cs_b + c.partial_b + c.result_b;
+    c.total = 38 * c.field_b + T_COUNT * c.table_b + 2 * c.rtab_b + c.cs_b + c.partial_b + c.result_b;
     return c;
 }
 
@@ -206,19 +206,20 @@ int run_curl(clt_ctx *ctx, const double *U)
     a.L = ctx->L; a.ph = ctx->ph;
     a.B = U + 5 * ctx->L.field;
     a.J1 = ctx->J1;
+    a.G = ctx->G;
     a.tab = ctx->tab;
     a.R = ctx->Rtab + LP;
     a.invR = ctx->invRtab + LP;
     a.phi_chunks = effective_chunks(ctx);
-    alignas(64) CUtensorMap tmB;
+    alignas(64) CUtensorMap tmU;
     const bool tma = ctx->variant == 0;
-    if (tma && !make_map(ctx, a.B, 3, curl_tma_tile_z(), &tmB)) {
+    if (tma && !make_map(ctx, U, 8, curl_tma_tile_z(), &tmU)) {
         snprintf(ctx->cuda_err, sizeof(ctx->cuda_err), "cuTensorMapEncodeTiled failed");
         return CLT_ECUDA;
     }
     const long pe = prof_begin(ctx, 5);
     if (tma)
-        CK(launch_curl_tma(a, &tmB, ctx->stream));
+        CK(launch_curl_tma(a, &tmU, ctx->hall, ctx->stream));
     else
         CK(launch_curl(a, 0, ctx->stream));
     prof_end(ctx, pe);
@@ -238,15 +239,19 @@ int run_rhs(clt_ctx *ctx, int mode, const double *in, double *out, double a_next
     a.phi_chunks = effective_chunks(ctx);
     a.prefetch = 1;
     const int tz = effective_tile_z(ctx);
-    const bool tma = ctx->variant == 0 && rhs_tma_supports(tz);
+    const bool tma = ctx->variant == 0 && rhs_tma_supports(tz, ctx->hall);
+    if (ctx->hall && !tma) {
+        snprintf(ctx->cuda_err, sizeof(ctx->cuda_err), "the Hall term needs the default kernel variant and tile height");
+        return CLT_EINVAL;
+    }
     alignas(64) CUtensorMap tmU, tmJ;
-    if (tma && (!make_map(ctx, in, 8, tz, &tmU) || !make_map(ctx, ctx->J1, 3, tz, &tmJ))) {
+    if (tma && (!make_map(ctx, in, 8, tz, &tmU) || !make_map(ctx, ctx->J1, ctx->hall ? 6 : 3, tz, &tmJ))) {
         snprintf(ctx->cuda_err, sizeof(ctx->cuda_err), "cuTensorMapEncodeTiled failed");
         return CLT_ECUDA;
     }
     const long pe = prof_begin(ctx, mode);
     if (tma)
-        CK(launch_rhs_tma(a, &tmU, &tmJ, mode, ctx->has_v0, tz, ctx->stream));
+        CK(launch_rhs_tma(a, &tmU, &tmJ, mode, ctx->has_v0, ctx->hall, tz, ctx->stream));
     else
         CK(launch_rhs(a, mode, ctx->has_v0, tz, ctx->stream));
     prof_end(ctx, pe);
@@ -293,6 +298,7 @@ int clt_create(const clt_grid *grid, const clt_params *params, void *d_workspace
         return CLT_EINVAL;
     if (params->eta < 0 || params->nu < 0 || params->D < 0 || params->kappa < 0 || params->dt < 0 || params->flags != 0)
         return CLT_EINVAL;
+    if (!isfinite(params->d_i) || params->d_i < 0) return CLT_EINVAL;
     const Carve c = carve(grid);
     if (bytes < c.total || ((uintptr_t)d_workspace % 256) != 0) return CLT_ENOMEM;
     cudaPointerAttributes at;
@@ -315,6 +321,8 @@ int clt_create(const clt_grid *grid, const clt_params *params, void *d_workspace
     const double dZ = (grid->Zmax - grid->Zmin) / (double)(grid->nZ - 1);
     const double dphi = Lphi / (double)grid->nphi;
     Phys &ph = ctx->ph;
+    ph.d_i = params->d_i;
+    ctx->hall = params->d_i != 0.0;
     ph.gamma = params->gamma; ph.eta = params->eta; ph.nu = params->nu; ph.D = params->D; ph.kappa = params->kappa;
     ph.cR1 = 1.0 / (12.0 * dR); ph.cZ1 = 1.0 / (12.0 * dZ); ph.cP1 = 1.0 / (12.0 * dphi);
     ph.cR2 = 1.0 / (12.0 * dR * dR); ph.cZ2 = 1.0 / (12.0 * dZ * dZ); ph.cP2 = 1.0 / (12.0 * dphi * dphi);
@@ -325,6 +333,7 @@ int clt_create(const clt_grid *grid, const clt_params *params, void *d_workspace
     ctx->Un = take(8 * c.field_b); ctx->acc = take(8 * c.field_b);
     ctx->Ua = take(8 * c.field_b); ctx->Ub = take(8 * c.field_b);
     ctx->J1 = take(3 * c.field_b);
+    ctx->G = take(3 * c.field_b);      // right behind J1: one tensor map covers both (Hall variant)
     ctx->tab = take(T_COUNT * c.table_b);
     ctx->Rtab = take(c.rtab_b); ctx->invRtab = take(c.rtab_b);
     ctx->cs = take(c.cs_b);
@@ -457,6 +466,16 @@ int clt_curl_J1(clt_ctx *ctx, double *J1)
     int r;
     if ((r = run_curl(ctx, ctx->Un))) return r;
     return copy_out(ctx, J1, ctx->J1, (size_t)3 * ctx->L.nphi * ctx->L.nZ);
+}
+
+int clt_hall_G(clt_ctx *ctx, double *G)
+{
+    if (!ctx || !G) return CLT_EINVAL;
+    if (!ctx->has_state) return CLT_ESTATE;
+    if (!ctx->hall) return CLT_EINVAL;
+    int r;
+    if ((r = run_curl(ctx, ctx->Un))) return r;
+    return copy_out(ctx, G, ctx->G, (size_t)3 * ctx->L.nphi * ctx->L.nZ);
 }
 
 int clt_set_dt(clt_ctx *ctx, double dt)

@@ -39,6 +39,7 @@ enum Table {
 
 struct Phys {
     double gamma, eta, nu, D, kappa;
+    double d_i;              // ion inertial length of the Hall term of eq (5); 0 = resistive MHD
     double cR1, cZ1, cP1;    // 1/(12 h)
     double cR2, cZ2, cP2;    // 1/(12 h^2)
     double dR, dZ, dphi, Lphi;
@@ -49,7 +50,7 @@ struct RhsArgs {
     Layout L;
     Phys ph;
     const double *in;     // stage state, 8 fields
-    const double *J1;     // 3 fields
+    const double *J1;     // 3 fields (the Hall variant reads 3 more right behind them: G)
     const double *Un;     // U^n, 8 fields (modes 2, 3, 4; mode 4 updates it in place through `out`)
     double *acc;          // RK4 accumulator, 8 fields (written by mode 2, read by mode 4)
     double *out;          // K (mode 0) | next stage state (modes 1-3) | U^{n+1} (mode 4), 8 fields
@@ -67,6 +68,7 @@ struct CurlArgs {
     Phys ph;
     const double *B;      // 3 fields (B_R, B_phi, B_Z of the stage state)
     double *J1;           // 3 fields
+    double *G;            // 3 fields: Hall field (written by the Hall variant only)
     const double *tab;
     const double *R;
     const double *invR;
@@ -97,12 +99,13 @@ cudaError_t launch_curl(const CurlArgs &a, int tile_z, cudaStream_t s);
 cudaError_t launch_rhs(const RhsArgs &a, int mode, bool has_v0, int tile_z, cudaStream_t s);
 // TMA variant: tmU / tmJ point to CUtensorMap objects over the stage state (4-D: pR, nZ, nphi, 8) and J1 (.., 3)
 // with box (TR+4, tile_z+4, 1, 1)
-cudaError_t launch_rhs_tma(const RhsArgs &a, const void *tmU, const void *tmJ, int mode, bool has_v0, int tile_z,
+// hall: tmJ maps 6 fields (J1 then G) and the kernel adds d_i * G to E1 (default tile height only)
+cudaError_t launch_rhs_tma(const RhsArgs &a, const void *tmU, const void *tmJ, int mode, bool has_v0, bool hall, int tile_z,
                            cudaStream_t s);
-bool rhs_tma_supports(int tile_z);
-// TMA variant of the curl kernel: tmB is a CUtensorMap over B_R, B_phi, B_Z of the stage state with box
-// (TR+4, curl_tma_tile_z()+4, 1, 1)
-cudaError_t launch_curl_tma(const CurlArgs &a, const void *tmB, cudaStream_t s);
+bool rhs_tma_supports(int tile_z, bool hall);
+// TMA variant of the curl kernel: tmU is a CUtensorMap over the 8 fields of the stage state with box
+// (TR+4, curl_tma_tile_z()+4, 1, 1); hall = also write the Hall field G
+cudaError_t launch_curl_tma(const CurlArgs &a, const void *tmU, bool hall, cudaStream_t s);
 int curl_tma_tile_z();
 cudaError_t launch_diag(const DiagArgs &a, int nblocks, double *result6, cudaStream_t s);
 int diag_blocks(const Layout &L);

@@ -536,12 +536,12 @@ __device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, i
         : "memory");
 }
 
-template <int TZ, int NRAW>
+template <int TZ, int NRAW, int NF>
 struct RhsTmaSmem {
     static constexpr int HT = (TZ + 4) * SW;
     static constexpr int NH = 4 * TR + 4 * TZ;
     static constexpr int HTP = (HT + 15) / 16 * 16;   // every TMA destination 128-byte aligned
-    alignas(128) double raw[NRAW][11][HTP];  // TMA destinations: U (8) and J1 (3) of one plane, tile with halo
+    alignas(128) double raw[NRAW][NF][HTP];  // TMA destinations: U (8), J1 (3) [and G (3), Hall] of one plane, tile with halo
     // 4-slot rings, tile with halo, written once when a plane arrives (as plane j+2) and read by the in-plane
     // stencils when it is the centre plane (two iterations later).  Four slots, not three: the slot that receives
     // plane j+2 held plane j-2, whose last readers are separated from this write by the barrier of iteration j-1.
@@ -551,12 +551,13 @@ struct RhsTmaSmem {
     alignas(8) unsigned long long ready;       // split CTA barrier: "this plane is staged" (count = all threads)
 };
 
-template <int TZ, int NRAW, int MODE, bool V0>
+template <int TZ, int NRAW, int MODE, bool V0, bool HALL>
 __global__ void __launch_bounds__(TR *TZ, 1)
 rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmJ)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    using SM = RhsTmaSmem<TZ, NRAW>;
+    constexpr int NF = HALL ? 14 : 11;
+    using SM = RhsTmaSmem<TZ, NRAW, NF>;
     SM &S = *reinterpret_cast<SM *>(smem_raw);
     constexpr int HT = SM::HT, NH = SM::NH;
     static_assert(NH <= TR * TZ, "tile too small for one halo node per thread");
@@ -606,11 +607,11 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
     auto issue = [&](int n) {
         const int jw = wrap_phi(ja - 2 + n, L.nphi);
         const int b = n % NRAW;
-        mbar_expect_tx(&S.bar[b], (unsigned)(11 * HT * sizeof(double)));
+        mbar_expect_tx(&S.bar[b], (unsigned)(NF * HT * sizeof(double)));
 #pragma unroll
         for (int m = 0; m < 8; ++m) tma_load_4d(&S.raw[b][m][0], &tmU, LP + i0 - 2, k0 - 2, jw, m, &S.bar[b]);
 #pragma unroll
-        for (int m = 0; m < 3; ++m) tma_load_4d(&S.raw[b][8 + m][0], &tmJ, LP + i0 - 2, k0 - 2, jw, m, &S.bar[b]);
+        for (int m = 0; m < NF - 8; ++m) tma_load_4d(&S.raw[b][8 + m][0], &tmJ, LP + i0 - 2, k0 - 2, jw, m, &S.bar[b]);
     };
 
     // phi-invariant values of the own node and of the halo node, kept in registers for the whole sweep
@@ -647,6 +648,11 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
             E[0] += __ldg(tab + T_E0R * L.plane + o2);
             E[1] += __ldg(tab + T_E0P * L.plane + o2);
             E[2] += __ldg(tab + T_E0Z * L.plane + o2);
+        }
+        if (HALL) {      // Hall term of eq (5): + d_i G (reading R11); G = 0 on the boundary layers
+            E[0] = fma(ph.d_i, raw[NF - 3][s], E[0]);
+            E[1] = fma(ph.d_i, raw[NF - 2][s], E[1]);
+            E[2] = fma(ph.d_i, raw[NF - 1][s], E[2]);
         }
         if (wantF) {
             const double B1R = BR - b0R, B1P = BP - b0P, B1Z = BZ - b0Z;
@@ -768,13 +774,14 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
     }
 }
 
-template <int TZ, int NRAW, int MODE, bool V0>
+template <int TZ, int NRAW, int MODE, bool V0, bool HALL>
 static cudaError_t launch_rhs_tma_t(const RhsArgs &a, const CUtensorMap &tmU, const CUtensorMap &tmJ, cudaStream_t s)
 {
     static bool configured = false;
-    auto kern = rhs_tma_kernel<TZ, NRAW, MODE, V0>;
-    const int smem = (int)sizeof(RhsTmaSmem<TZ, NRAW>);
-    static_assert(sizeof(RhsTmaSmem<TZ, NRAW>) <= 232448, "shared memory of the TMA RHS kernel exceeds 227 KB");
+    auto kern = rhs_tma_kernel<TZ, NRAW, MODE, V0, HALL>;
+    using SM = RhsTmaSmem<TZ, NRAW, HALL ? 14 : 11>;
+    const int smem = (int)sizeof(SM);
+    static_assert(sizeof(SM) <= 232448, "shared memory of the TMA RHS kernel exceeds 227 KB");
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
@@ -786,13 +793,14 @@ static cudaError_t launch_rhs_tma_t(const RhsArgs &a, const CUtensorMap &tmU, co
     return cudaGetLastError();
 }
 
-template <int TZ, int NRAW>
+template <int TZ, int NRAW, bool HALL>
 static cudaError_t launch_rhs_tma_tz(const RhsArgs &a, const CUtensorMap &tmU, const CUtensorMap &tmJ, int mode, bool v0,
                                      cudaStream_t s)
 {
-#define CLT_CASE(M)                                                                                        \
-    case M:                                                                                                \
-        return v0 ? launch_rhs_tma_t<TZ, NRAW, M, true>(a, tmU, tmJ, s) : launch_rhs_tma_t<TZ, NRAW, M, false>(a, tmU, tmJ, s);
+#define CLT_CASE(M)                                                                           \
+    case M:                                                                                   \
+        return v0 ? launch_rhs_tma_t<TZ, NRAW, M, true, HALL>(a, tmU, tmJ, s)                 \
+                  : launch_rhs_tma_t<TZ, NRAW, M, false, HALL>(a, tmU, tmJ, s);
     switch (mode) {
         CLT_CASE(RHS_MODE_K)
         CLT_CASE(RHS_MODE_S1)
@@ -805,19 +813,24 @@ static cudaError_t launch_rhs_tma_tz(const RhsArgs &a, const CUtensorMap &tmU, c
 #undef CLT_CASE
 }
 
-bool rhs_tma_supports(int tile_z) { return tile_z == 8 || tile_z == 10 || tile_z == 12 || tile_z == 13; }
+bool rhs_tma_supports(int tile_z, bool hall)
+{
+    if (hall) return tile_z == 8;
+    return tile_z == 8 || tile_z == 10 || tile_z == 12 || tile_z == 13;
+}
 
-cudaError_t launch_rhs_tma(const RhsArgs &a, const void *tmU, const void *tmJ, int mode, bool has_v0, int tile_z,
+cudaError_t launch_rhs_tma(const RhsArgs &a, const void *tmU, const void *tmJ, int mode, bool has_v0, bool hall, int tile_z,
                            cudaStream_t s)
 {
     const CUtensorMap &mU = *reinterpret_cast<const CUtensorMap *>(tmU);
     const CUtensorMap &mJ = *reinterpret_cast<const CUtensorMap *>(tmJ);
+    if (hall) return tile_z == 8 ? launch_rhs_tma_tz<8, 2, true>(a, mU, mJ, mode, has_v0, s) : cudaErrorInvalidValue;
     switch (tile_z) {
     // two raw buffers (TMA two planes ahead) where shared memory allows, one otherwise
-    case 8: return launch_rhs_tma_tz<8, CLT_NRAW8>(a, mU, mJ, mode, has_v0, s);
-    case 10: return launch_rhs_tma_tz<10, 2>(a, mU, mJ, mode, has_v0, s);
-    case 12: return launch_rhs_tma_tz<12, 1>(a, mU, mJ, mode, has_v0, s);
-    case 13: return launch_rhs_tma_tz<13, 1>(a, mU, mJ, mode, has_v0, s);
+    case 8: return launch_rhs_tma_tz<8, CLT_NRAW8, false>(a, mU, mJ, mode, has_v0, s);
+    case 10: return launch_rhs_tma_tz<10, 2, false>(a, mU, mJ, mode, has_v0, s);
+    case 12: return launch_rhs_tma_tz<12, 1, false>(a, mU, mJ, mode, has_v0, s);
+    case 13: return launch_rhs_tma_tz<13, 1, false>(a, mU, mJ, mode, has_v0, s);
     default: return cudaErrorInvalidValue;
     }
 }
@@ -942,19 +955,24 @@ cudaError_t launch_curl(const CurlArgs &a, int tile_z, cudaStream_t s)
 // equilibrium is still removed before differencing (H2).  No staging, one __syncthreads per plane
 // (only to hand the consumed ring slot back to the producer thread).
 // ---------------------------------------------------------------------------------------------
-template <int TZ, int NS>
+template <int TZ, int NS, int NF>
 struct CurlTmaSmem {
     static constexpr int HT = (TZ + 4) * SW;
     static constexpr int HTP = (HT + 15) / 16 * 16;
-    alignas(128) double raw[NS][3][HTP];
+    alignas(128) double raw[NS][NF][HTP];      // B_R, B_phi, B_Z (and rho, p for the Hall variant)
     alignas(8) unsigned long long full[NS];
 };
 
-template <int TZ, int NS>
-__global__ void __launch_bounds__(TR *TZ, CLT_CURL_MINB) curl_tma_kernel(const __grid_constant__ CurlArgs a, const __grid_constant__ CUtensorMap tmB)
+// HALL = true additionally forms the Hall field of eq (5) [L77] in its equilibrium-subtracted form (DESIGN.md
+// reading R11),  G = (J1 x B + J0 x B1 - grad p1)/rho - (rho1/rho)(v0.grad)v0,  on interior nodes: the same sweep
+// with rho and p staged next to B (p1 = p - p0 is formed before differencing, H2).  tmU maps the whole stage state.
+template <int TZ, int NS, bool HALL>
+__global__ void __launch_bounds__(TR *TZ, HALL ? 1 : CLT_CURL_MINB)
+curl_tma_kernel(const __grid_constant__ CurlArgs a, const __grid_constant__ CUtensorMap tmU)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    using SM = CurlTmaSmem<TZ, NS>;
+    constexpr int NF = HALL ? 5 : 3;
+    using SM = CurlTmaSmem<TZ, NS, NF>;
     SM &S = *reinterpret_cast<SM *>(smem_raw);
     const Layout &L = a.L;
     const Phys &ph = a.ph;
@@ -972,15 +990,19 @@ __global__ void __launch_bounds__(TR *TZ, CLT_CURL_MINB) curl_tma_kernel(const _
     if (tid == 0) {
         for (int n = 0; n < NS; ++n) mbar_init(&S.full[n], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmB) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmU) : "memory");
     }
     __syncthreads();
     auto issue = [&](int n) {      // plane number n counts from ja-2
         const int jw = wrap_phi(ja - 2 + n, L.nphi);
         const int st = n % NS;
-        mbar_expect_tx(&S.full[st], (unsigned)(3 * SM::HT * sizeof(double)));
+        mbar_expect_tx(&S.full[st], (unsigned)(NF * SM::HT * sizeof(double)));
 #pragma unroll
-        for (int m = 0; m < 3; ++m) tma_load_4d(&S.raw[st][m][0], &tmB, LP + i0 - 2, k0 - 2, jw, m, &S.full[st]);
+        for (int m = 0; m < 3; ++m) tma_load_4d(&S.raw[st][m][0], &tmU, LP + i0 - 2, k0 - 2, jw, 5 + m, &S.full[st]);
+        if (HALL) {
+            tma_load_4d(&S.raw[st][3][0], &tmU, LP + i0 - 2, k0 - 2, jw, 0, &S.full[st]);
+            tma_load_4d(&S.raw[st][4][0], &tmU, LP + i0 - 2, k0 - 2, jw, 1, &S.full[st]);
+        }
     };
     if (tid == 0)
         for (int n = 0; n < NS && n < total; ++n) issue(n);
@@ -990,6 +1012,7 @@ __global__ void __launch_bounds__(TR *TZ, CLT_CURL_MINB) curl_tma_kernel(const _
     const double *t0R = tab + T_B0R * L.plane + off2, *t0P = tab + T_B0P * L.plane + off2, *t0Z = tab + T_B0Z * L.plane + off2;
     const double o0R = __ldg(t0R), o0Z = __ldg(t0Z);
     double z0P[4], z0R[4], r0Z[4], r0P[4], rr[4];
+    double zp0[4], rp0[4];          // p0 at the in-plane neighbours (Hall)
 #pragma unroll
     for (int d = 0; d < 4; ++d) {
         const int o = (d < 2) ? d - 2 : d - 1;          // -2, -1, +1, +2
@@ -998,20 +1021,37 @@ __global__ void __launch_bounds__(TR *TZ, CLT_CURL_MINB) curl_tma_kernel(const _
         r0Z[d] = __ldg(t0Z + o);
         r0P[d] = __ldg(t0P + o);
         rr[d] = __ldg(a.R + ic + o);
+        if (HALL) {
+            zp0[d] = __ldg(tab + T_P0 * L.plane + off2 + (long long)o * L.pR);
+            rp0[d] = __ldg(tab + T_P0 * L.plane + off2 + o);
+        }
+    }
+    double o0P = 0.0, rho0 = 0.0, j0R = 0.0, j0P = 0.0, j0Z = 0.0, a0R = 0.0, a0P = 0.0, a0Z = 0.0;
+    if (HALL) {
+        o0P = __ldg(t0P);
+        rho0 = __ldg(tab + T_RHO0 * L.plane + off2);
+        j0R = __ldg(tab + T_J0R * L.plane + off2); j0P = __ldg(tab + T_J0P * L.plane + off2); j0Z = __ldg(tab + T_J0Z * L.plane + off2);
+        a0R = __ldg(tab + T_A0R * L.plane + off2); a0P = __ldg(tab + T_A0P * L.plane + off2); a0Z = __ldg(tab + T_A0Z * L.plane + off2);
     }
     const double iR = __ldg(a.invR + ic);
     const double cPi = ph.cP1 * iR;
 
     double bR[5], bZ[5];           // B1_R, B1_Z of planes j-2 .. j+2 at the own node
+    double pP[5];                  // p of planes j-2 .. j+2 at the own node (Hall; d_phi p1 = d_phi p)
     auto lead = [&](int n) {
         const int st = n % NS;
         mbar_wait(&S.full[st], (unsigned)((n / NS) & 1));
         bR[4] = S.raw[st][0][cs] - o0R;
         bZ[4] = S.raw[st][2][cs] - o0Z;
+        if (HALL) pP[4] = S.raw[st][NF - 1][cs];
     };
     auto advance = [&]() {
 #pragma unroll
-        for (int d = 0; d < 4; ++d) { bR[d] = bR[d + 1]; bZ[d] = bZ[d + 1]; }
+        for (int d = 0; d < 4; ++d) {
+            bR[d] = bR[d + 1];
+            bZ[d] = bZ[d + 1];
+            if (HALL) pP[d] = pP[d + 1];
+        }
     };
 #pragma unroll 1
     for (int n = 0; n < 4; ++n) { lead(n); advance(); }
@@ -1034,11 +1074,33 @@ __global__ void __launch_bounds__(TR *TZ, CLT_CURL_MINB) curl_tma_kernel(const _
         const double dR_BZ = fd1(sZ_[-2] - r0Z[0], sZ_[-1] - r0Z[1], sZ_[1] - r0Z[2], sZ_[2] - r0Z[3]);
         const double dR_RBP = fd1(rr[0] * (sP_[-2] - r0P[0]), rr[1] * (sP_[-1] - r0P[1]), rr[2] * (sP_[1] - r0P[2]),
                                   rr[3] * (sP_[2] - r0P[3]));
+        const double JR = dP_BZ * cPi - dZ_BP * ph.cZ1;
+        const double JP = dZ_BR * ph.cZ1 - dR_BZ * ph.cR1;
+        const double JZ = dR_RBP * (ph.cR1 * iR) - dP_BR * cPi;
+        double GR = 0.0, GP = 0.0, GZ = 0.0;
+        if (HALL) {
+            const double *sp_ = &S.raw[st][NF - 1][cs];
+            const double rho = S.raw[st][NF - 2][cs];
+            const double BR = sR_[0], BP = sP_[0], BZ = sZ_[0];
+            const double B1R = bR[2], B1P = BP - o0P, B1Z = bZ[2];
+            const double gR = fd1(sp_[-2] - rp0[0], sp_[-1] - rp0[1], sp_[1] - rp0[2], sp_[2] - rp0[3]) * ph.cR1;
+            const double gZ = fd1(sp_[-2 * SW] - zp0[0], sp_[-SW] - zp0[1], sp_[SW] - zp0[2], sp_[2 * SW] - zp0[3]) * ph.cZ1;
+            const double gP = fd1(pP[0], pP[1], pP[3], pP[4]) * cPi;
+            const double rinv = 1.0 / rho, r1 = (rho - rho0) * rinv;
+            GR = ((JP * BZ - JZ * BP) + (j0P * B1Z - j0Z * B1P) - gR) * rinv - r1 * a0R;
+            GP = ((JZ * BR - JR * BZ) + (j0Z * B1R - j0R * B1Z) - gP) * rinv - r1 * a0P;
+            GZ = ((JR * BP - JP * BR) + (j0R * B1P - j0P * B1R) - gZ) * rinv - r1 * a0Z;
+        }
         if (valid) {
             const long long g = (long long)j * L.plane + off2;
-            a.J1[0 * L.field + g] = dP_BZ * cPi - dZ_BP * ph.cZ1;
-            a.J1[1 * L.field + g] = dZ_BR * ph.cZ1 - dR_BZ * ph.cR1;
-            a.J1[2 * L.field + g] = dR_RBP * (ph.cR1 * iR) - dP_BR * cPi;
+            a.J1[0 * L.field + g] = JR;
+            a.J1[1 * L.field + g] = JP;
+            a.J1[2 * L.field + g] = JZ;
+            if (HALL) {
+                a.G[0 * L.field + g] = GR;
+                a.G[1 * L.field + g] = GP;
+                a.G[2 * L.field + g] = GZ;
+            }
         }
         advance();
         __syncthreads();                               // the centre plane's slot is free again
@@ -1046,12 +1108,13 @@ __global__ void __launch_bounds__(TR *TZ, CLT_CURL_MINB) curl_tma_kernel(const _
     }
 }
 
-cudaError_t launch_curl_tma(const CurlArgs &a, const void *tmB, cudaStream_t s)
+template <bool HALL>
+static cudaError_t launch_curl_tma_t(const CurlArgs &a, const void *tmU, cudaStream_t s)
 {
     constexpr int TZ = CLT_CURL_TZ, NS = CLT_CURL_NS;
     static bool configured = false;
-    auto kern = curl_tma_kernel<TZ, NS>;
-    const int smem = (int)sizeof(CurlTmaSmem<TZ, NS>);
+    auto kern = curl_tma_kernel<TZ, NS, HALL>;
+    const int smem = (int)sizeof(CurlTmaSmem<TZ, NS, HALL ? 5 : 3>);
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
@@ -1059,8 +1122,13 @@ cudaError_t launch_curl_tma(const CurlArgs &a, const void *tmB, cudaStream_t s)
     }
     dim3 block(TR, TZ, 1);
     dim3 grid((a.L.nR - 4 + TR - 1) / TR, (a.L.nZ - 4 + TZ - 1) / TZ, a.phi_chunks);
-    kern<<<grid, block, smem, s>>>(a, *reinterpret_cast<const CUtensorMap *>(tmB));
+    kern<<<grid, block, smem, s>>>(a, *reinterpret_cast<const CUtensorMap *>(tmU));
     return cudaGetLastError();
+}
+
+cudaError_t launch_curl_tma(const CurlArgs &a, const void *tmU, bool hall, cudaStream_t s)
+{
+    return hall ? launch_curl_tma_t<true>(a, tmU, s) : launch_curl_tma_t<false>(a, tmU, s);
 }
 int curl_tma_tile_z() { return CLT_CURL_TZ; }
 

@@ -225,3 +225,50 @@ def test_config4_rhs_and_2_steps_match_oracle_in_the_bench_launch_configuration(
     assert d["step"] == 50 and all(np.isfinite(d[k]) for k in ("kinetic", "magnetic", "magnetic_pert", "magnetic_n1", "max_divB"))
     assert abs(d["max_divB"] - d2["max_divB"]) <= 1e-6 * d2["max_divB"] + 1e-12
     assert abs(d["magnetic"] - d2["magnetic"]) <= 1e-6 * d2["magnetic"]
+
+
+# ------------------------------------------------------------------------------ NEXT-3: Hall term of eq (5)
+HALL_CASES = ["config1", "ragged-77x9x53", "rotating-v0", "min-9x5x9", "big-amplitude"]
+
+
+@pytest.mark.parametrize("name", HALL_CASES)
+def test_hall_field_and_rhs_match_oracle(name):
+    prob = _problems()[name]()
+    over = dict(d_i=0.05, eta=1e-4)
+    o, g = make_oracle(prob, **over), make_gpu(prob, **over)
+    G_o, G_g = o.hall_G(prob.U), g.hall_G()
+    assert_close(G_g, G_o, RHS_TOL, f"Hall field G {name}")
+    assert np.all(G_g[:, :, :2] == 0) and np.all(G_g[:, :, -2:] == 0) and np.all(G_g[..., :2] == 0) and np.all(G_g[..., -2:] == 0)
+    assert_close(g.curl_J1(), o.curl_J1(prob.U), RHS_TOL, f"curl_J1 (Hall variant of the kernel) {name}")
+    K_o, K_g = o.rhs(), g.rhs()
+    assert_close(K_g, K_o, RHS_TOL, f"rhs with Hall term {name}")
+    # the Hall term really acts: the same state without it has a different dB/dt
+    K_0 = make_oracle(prob, eta=1e-4).rhs()
+    assert np.abs(K_o[5:] - K_0[5:]).max() > 1e-3 * np.abs(K_0[5:]).max()
+
+
+@pytest.mark.parametrize("name,steps", [("config1", 20), ("rotating-v0", 50), ("ragged-77x9x53", 30)])
+def test_hall_steps_match_oracle(name, steps):
+    prob = _problems()[name]()
+    over = dict(d_i=0.03, dt=0.2 * prob.dt)       # whistler CFL: d_i k^2 B dt stays well below the RK4 limit
+    o, g = make_oracle(prob, **over), make_gpu(prob, **over)
+    o.step(steps)
+    g.step(steps)
+    assert_close(g.get_state(), o.get_state(), STEP_TOL, f"{steps} RK4 steps with Hall term {name}")
+    assert np.isfinite(g.diagnostics()["magnetic"])
+
+
+def test_hall_needs_the_default_kernel_variant():
+    from paper_1812_00525_b200 import clt
+    prob = inputs.make_problem(1)
+    g = make_gpu(prob, d_i=0.05)
+    g.set_kernel_variant(1)
+    with pytest.raises(clt.CltError):
+        g.rhs()
+    g.set_kernel_variant(0)
+    g.set_tuning(tile_z=12)
+    with pytest.raises(clt.CltError):
+        g.step(1)
+    g0 = make_gpu(prob)
+    with pytest.raises(clt.CltError):
+        g0.hall_G()
