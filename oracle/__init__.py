@@ -60,6 +60,7 @@ def lib():
             L.oracle_E1.argtypes = [ctypes.c_void_p, _dp, _dp]
             L.oracle_hall_G.argtypes = [ctypes.c_void_p, _dp, _dp]
             L.oracle_set_hall.argtypes = [ctypes.c_void_p, ctypes.c_double]
+            L.oracle_set_phi_scheme.argtypes = [ctypes.c_void_p, ctypes.c_int]
             L.oracle_rhs_of.argtypes = [ctypes.c_void_p, _dp, _dp]
             L.oracle_rhs.argtypes = [ctypes.c_void_p, _dp]
             L.oracle_step.argtypes = [ctypes.c_void_p, ctypes.c_int]
@@ -91,7 +92,7 @@ class Oracle:
     """
 
     def __init__(self, nR, nphi, nZ, Rmin, Rmax, Zmin, Zmax, phi_extent=0.0, gamma=5.0 / 3.0, eta=0.0, nu=0.0,
-                 D=0.0, kappa=0.0, dt=0.0, d_i=0.0):
+                 D=0.0, kappa=0.0, dt=0.0, d_i=0.0, phi_scheme=0):
         self.L = lib()
         self.nR, self.nphi, self.nZ = int(nR), int(nphi), int(nZ)
         self.h = self.L.oracle_create(self.nR, self.nphi, self.nZ, Rmin, Rmax, Zmin, Zmax, phi_extent, gamma, eta,
@@ -102,6 +103,8 @@ class Oracle:
         self.L.oracle_set_equilibrium(self.h, None)
         if d_i:
             self.L.oracle_set_hall(self.h, float(d_i))
+        if phi_scheme:
+            self.L.oracle_set_phi_scheme(self.h, int(phi_scheme))
 
     def close(self):
         if getattr(self, "h", None):
@@ -164,6 +167,10 @@ class Oracle:
 
     def set_hall(self, d_i):
         self.L.oracle_set_hall(self.h, float(d_i))
+
+    def set_phi_scheme(self, scheme):
+        """0 = 4th-order finite differences in phi, 1 = pseudo-spectral."""
+        self.L.oracle_set_phi_scheme(self.h, int(scheme))
 
     def rhs_of(self, U):
         K = np.empty((8,) + self.shape)

@@ -26,7 +26,8 @@
  * written numpy evaluation of eqs (1)-(4); P7 Alfven modified-wavenumber identity; P8 RK4 order
  * on du/dt = lambda u through oracle_rk4 and on the MHD system by dt-halving.  P12 Hall term of eq (5):
  * exact discrete whistler-type response with the squared modified wavenumber, d_i = 0 reduction, and the
- * sympy convergence pin P3b run with d_i != 0.
+ * sympy convergence pin P3b run with d_i != 0.  P13 pseudo-spectral phi scheme: against numpy.fft, exact on
+ * resolved Fourier modes, the Alfven identity with the exact wavenumber, P3b with the spectral scheme.
  * Parity unpinned: none of the exported functions (each is covered by at least one pin); the
  * absolute value of a generic RHS has no paper-printed number to compare with (PAPER.md prints
  * no worked example), so the pins above are mathematical ones.
@@ -47,6 +48,8 @@ typedef struct oracle {
     double Rmin, Rmax, Zmin, Zmax, Lphi;
     double dR, dZ, dphi;
     double gamma, eta, nu, D, kappa, dt;
+    int phi_scheme;     /* 0 = 4th-order central differences in phi, 1 = pseudo-spectral (L125) */
+    double *c1, *c2;    /* pseudo-spectral derivative weights, see oracle_set_phi_scheme         */
     double d_i;         /* ion inertial length of the Hall term in eq (5); 0 = resistive MHD */
     double *R;          /* R_i = Rmin + i*dR  (reading R1; hazard H1)           */
     double *Z;          /* Z_k = Zmin + k*dZ                                     */
@@ -103,6 +106,11 @@ static inline double d1Z(const oracle *o, const double *f, int i, int k, int j)
 }
 static inline double d1P(const oracle *o, const double *f, int i, int k, int j)
 {
+    if (o->phi_scheme == 1) {       /* pseudo-spectral: sum_m c1[m] f_{j+m}, see oracle_set_phi_scheme */
+        double s = 0.0;
+        for (int m = 0; m < o->nphi; ++m) s += o->c1[m] * f[idx(o, i, k, wrapphi(o, j + m))];
+        return s;
+    }
     return (8.0 * (f[idx(o, i, k, wrapphi(o, j + 1))] - f[idx(o, i, k, wrapphi(o, j - 1))])
             - (f[idx(o, i, k, wrapphi(o, j + 2))] - f[idx(o, i, k, wrapphi(o, j - 2))]))
            / (12.0 * o->dphi);
@@ -127,6 +135,11 @@ static inline double d2Z(const oracle *o, const double *f, int i, int k, int j)
 }
 static inline double d2P(const oracle *o, const double *f, int i, int k, int j)
 {
+    if (o->phi_scheme == 1) {
+        double s = 0.0;
+        for (int m = 0; m < o->nphi; ++m) s += o->c2[m] * f[idx(o, i, k, wrapphi(o, j + m))];
+        return s;
+    }
     return (-f[idx(o, i, k, wrapphi(o, j + 2))] + 16.0 * f[idx(o, i, k, wrapphi(o, j + 1))]
             - 30.0 * f[idx(o, i, k, j)]
             + 16.0 * f[idx(o, i, k, wrapphi(o, j - 1))] - f[idx(o, i, k, wrapphi(o, j - 2))])
@@ -255,12 +268,44 @@ void oracle_destroy(oracle *o)
 {
     if (!o) return;
     free(o->R); free(o->Z); free(o->U0); free(o->J0); free(o->divv0); free(o->v0gv0);
-    free(o->U); free(o->U1); free(o->J1); free(o->E1); free(o->G);
+    free(o->U); free(o->U1); free(o->J1); free(o->E1); free(o->G); free(o->c1); free(o->c2);
     free(o->K1); free(o->K2); free(o->K3); free(o->K4); free(o->Us);
     free(o);
 }
 
 void oracle_set_dt(oracle *o, double dt) { o->dt = dt; }
+
+/* phi scheme [L125: "in the phi direction, either 4th order finite difference or pseudo-spectrum method can be
+ * used"].  scheme 1 = pseudo-spectral (reading R12): the periodic samples f_j, j = 0..N-1 on length L are
+ * expanded in the discrete Fourier modes e^{i kappa q phi}, kappa = 2 pi / L, q = -Q..Q, Q = floor((N-1)/2)
+ * [plus the Nyquist mode q = N/2 when N is even], each mode is differentiated exactly and the series is
+ * evaluated back on the nodes.  The Nyquist mode (-1)^j has no defined phase: its first derivative is
+ * taken as 0, its second derivative as -(kappa N/2)^2 times itself (the usual convention).  Written in
+ * physical space that is the circulant sum  d f_j = sum_m c[m] f_{j+m}  with
+ *   c1[m] = (1/N) sum_q (i kappa q) e^{-2 pi i q m/N}       = (2 kappa/N) sum_{q=1..Q} q sin(2 pi q m/N)
+ *   c2[m] = (1/N) sum_q -(kappa q)^2 e^{-2 pi i q m/N}      = -(kappa^2/N)[2 sum_{q=1..Q} q^2 cos(2 pi q m/N)
+ *                                                              + (N even) (N/2)^2 cos(pi m)]
+ * summed here exactly as written (long double).                                                   */
+void oracle_set_phi_scheme(oracle *o, int scheme)
+{
+    int N = o->nphi;
+    o->phi_scheme = scheme ? 1 : 0;
+    if (!o->phi_scheme) return;
+    if (!o->c1) { o->c1 = zalloc((size_t)N); o->c2 = zalloc((size_t)N); }
+    long double kappa = 2.0L * 3.141592653589793238462643383279502884L / (long double)o->Lphi;
+    int Q = (N - 1) / 2;
+    for (int m = 0; m < N; ++m) {
+        long double s1 = 0.0L, s2 = 0.0L;
+        for (int q = 1; q <= Q; ++q) {
+            long double th = 2.0L * 3.141592653589793238462643383279502884L * (long double)q * (long double)m / (long double)N;
+            s1 += (long double)q * sinl(th);
+            s2 += 2.0L * (long double)q * (long double)q * cosl(th);
+        }
+        if (N % 2 == 0) s2 += (long double)(N / 2) * (long double)(N / 2) * ((m % 2) ? -1.0L : 1.0L);
+        o->c1[m] = (double)(2.0L * kappa / (long double)N * s1);
+        o->c2[m] = (double)(-kappa * kappa / (long double)N * s2);
+    }
+}
 /* switches the Hall term of eq (5) [L77] on (d_i != 0) or off (d_i = 0, the default) */
 void oracle_set_hall(oracle *o, double d_i) { o->d_i = d_i; }
 

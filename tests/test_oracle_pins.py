@@ -13,6 +13,8 @@ P8 textbook RK4 order through oracle_rk4 and dt-halving on the MHD system   L125
 P10 SETDT closed form (Fig. 4), P11 diagnostics closed forms
 P12 Hall term of eq (5): exact whistler-type response with k*^2, momentum bracket identity, d_i = 0 reduction
     (and P3b runs with d_i != 0 against the sympy-derived continuous eq (5))
+P13 pseudo-spectral phi scheme (L125): against numpy.fft, exact on every resolved mode, Alfven response with the
+    physical wavenumber; P3b also runs with the spectral scheme
 """
 import numpy as np
 import pytest
@@ -243,8 +245,9 @@ def _continuous_rhs(sp, syms, op, m, par, subtracted, d_i=0):
     return [Krho, Kp] + Kv + KB
 
 
-@pytest.mark.parametrize("equilibrium_exact,d_i", [(True, 0), (False, 0), (True, 0.07), (False, 0.07)])
-def test_P3b_full_rhs_converges_at_4th_order_to_the_continuous_equations(equilibrium_exact, d_i):
+@pytest.mark.parametrize("equilibrium_exact,d_i,phi_scheme", [(True, 0, 0), (False, 0, 0), (True, 0.07, 0), (False, 0.07, 0),
+                                                              (True, 0, 1), (False, 0.07, 1)])
+def test_P3b_full_rhs_converges_at_4th_order_to_the_continuous_equations(equilibrium_exact, d_i, phi_scheme):
     sp, syms, op = _sympy_ops()
     m = _manufactured(sp, syms, equilibrium_exact)
     par = (5.0 / 3.0, 0.05, 0.04, 0.03, 0.02)
@@ -261,7 +264,7 @@ def test_P3b_full_rhs_converges_at_4th_order_to_the_continuous_equations(equilib
     errs = []
     for n in (2, 4):
         o, RR, P, ZZ = make(nR=20 * n + 1, nphi=16 * n, nZ=16 * n + 1, gamma=par[0], eta=par[1], nu=par[2], D=par[3],
-                            kappa=par[4], d_i=d_i)
+                            kappa=par[4], d_i=d_i, phi_scheme=phi_scheme)
         ev = lambda e: _lamb(sp, syms, e)(RR, P, ZZ)
         U0 = np.stack([ev(m["rho0"]), ev(m["p0"])] + [ev(x) for x in m["v0"]] + [ev(x) for x in m["B0"]])
         U1 = np.stack([ev(m["rho1"]), ev(m["p1"])] + [ev(x) for x in m["v1"]] + [ev(x) for x in m["B1"]])
@@ -437,6 +440,62 @@ def test_P12_hall_term_whistler_response_and_reductions(nmode):
     o2, *_ = make(nR=18, nphi=nphi, nZ=18, Rmin=99.0, Rmax=101.0, phi_extent=Lphi)
     assert np.array_equal(o.rhs_of(U), o2.rhs_of(U))
     assert np.all(o.hall_G(U) == 0)
+
+
+# ----------------------------------------------------------------------------------------------- P13
+def _fft_derivs(f, L):
+    """Reference pseudo-spectral derivatives along axis 0 by numpy.fft (library routine, reading R12's convention)."""
+    N = f.shape[0]
+    q = np.fft.fftfreq(N, d=1.0 / N)                 # integer mode numbers
+    kap = 2 * np.pi / L
+    F = np.fft.fft(f, axis=0)
+    k1 = 1j * kap * q
+    if N % 2 == 0:
+        k1[N // 2] = 0.0                             # Nyquist mode: first derivative taken as 0
+    shp = (N,) + (1,) * (f.ndim - 1)
+    d1 = np.fft.ifft(k1.reshape(shp) * F, axis=0).real
+    d2 = np.fft.ifft((-(kap * q) ** 2).reshape(shp) * F, axis=0).real
+    return d1, d2
+
+
+@pytest.mark.parametrize("nphi,extent", [(16, 0.0), (9, 0.0), (12, 2 * np.pi / 100), (5, 0.0)])
+def test_P13_pseudo_spectral_phi_derivatives(nphi, extent):
+    L = extent or 2 * np.pi
+    o, RR, P, ZZ = make(nR=10, nphi=nphi, nZ=9, phi_extent=extent, phi_scheme=1)
+    rng = np.random.default_rng(5)
+    f = rng.standard_normal(RR.shape)
+    e1, e2 = _fft_derivs(f, L)
+    g1, g2 = o.scalar_op("d1P", f), o.scalar_op("d2P", f)
+    assert np.abs(interior(g1 - e1)).max() < 1e-12 * np.abs(e1).max()
+    assert np.abs(interior(g2 - e2)).max() < 1e-12 * np.abs(e2).max()
+    # exact on every resolved mode (the FD stencil is not: its error for the highest mode is O(1))
+    kap = 2 * np.pi / L
+    for n in range(0, (nphi - 1) // 2 + 1):
+        f = np.cos(n * kap * P + 0.3) * (1 + 0.1 * RR)
+        assert np.abs(interior(o.scalar_op("d1P", f) + n * kap * np.sin(n * kap * P + 0.3) * (1 + 0.1 * RR))).max() < 1e-11 * max(n * kap, 1)
+        assert np.abs(interior(o.scalar_op("d2P", f) + (n * kap) ** 2 * f)).max() < 1e-10 * max((n * kap) ** 2, 1)
+    # the R and Z stencils are untouched by the phi scheme
+    o0, *_ = make(nR=10, nphi=nphi, nZ=9, phi_extent=extent)
+    assert np.array_equal(o.scalar_op("d1R", f), o0.scalar_op("d1R", f))
+    assert np.array_equal(o.scalar_op("d2Z", f), o0.scalar_op("d2Z", f))
+
+
+@pytest.mark.parametrize("nmode", [1, 3, 7])
+def test_P13_alfven_response_with_the_exact_wavenumber(nmode):
+    """P7 with the pseudo-spectral scheme: the modified wavenumber is the physical one, for every resolved mode."""
+    nphi, c, eps = 16, 2.0, 1e-3
+    Lphi = 2 * np.pi / 100
+    o, RR, P, ZZ = make(nR=18, nphi=nphi, nZ=14, Rmin=99.0, Rmax=101.0, phi_extent=Lphi, phi_scheme=1)
+    kphys = 2 * np.pi * nmode / Lphi
+    U = np.zeros((8,) + RR.shape)
+    U[0], U[1], U[6] = 1.0, 0.3, c / RR
+    Ua = U.copy()
+    Ua[4] = eps * np.sin(kphys * P)
+    exp = (c / RR) / RR * kphys * eps * np.cos(kphys * P)
+    assert np.abs(interior(o.rhs_of(Ua)[7] - exp)).max() < 1e-10 * np.abs(exp).max()
+    Ub = U.copy()
+    Ub[7] = eps * np.sin(kphys * P)
+    assert np.abs(interior(o.rhs_of(Ub)[4] - exp)).max() < 1e-10 * np.abs(exp).max()
 
 
 # ----------------------------------------------------------------------------------------------- P8
