@@ -149,6 +149,18 @@ int clt_diagnostics(clt_ctx *ctx, clt_diag *out);
  * params.cfl.  Synchronises the stream.  Does not change the context's dt.                        */
 int clt_suggest_dt(clt_ctx *ctx, double cfl, double *dt_out);
 
+/* phi scheme [L125: "either 4th order finite difference or pseudo-spectrum method can be used"].
+ * scheme 0 (default) = 4th-order central differences; 1 = pseudo-spectral: every d/dphi and d2/dphi2 of the
+ * path (curl, gradients, divergences, Laplacians, curl E, div_c B of the diagnostics) is the exact derivative
+ * of the trigonometric interpolant through the nphi samples (Nyquist mode: first derivative 0, second
+ * derivative -(pi nphi/L)^2; reading R12).  It needs a second caller-owned DEVICE scratch buffer of
+ * clt_spectral_workspace_bytes(grid) bytes (256-byte aligned; 14 padded fields), kept alive until the scheme is
+ * set back to 0 or the context is destroyed, nphi <= 256, and the default kernel variant and tile height
+ * (clt_rhs / clt_step return CLT_EINVAL otherwise).  Synchronises the stream.
+ * Errors: CLT_EINVAL (scheme, nphi > 256), CLT_ENOMEM (scratch missing, small, misaligned, not device).   */
+size_t clt_spectral_workspace_bytes(const clt_grid *grid);
+int clt_set_phi_scheme(clt_ctx *ctx, int scheme, void *d_scratch, size_t bytes);
+
 /* Launch-shape knobs for measurement (all optional; 0 = library default): tile height in Z of the
  * fused RHS kernel, number of phi chunks per tile, use of a CUDA graph for clt_step.              */
 int clt_set_tuning(clt_ctx *ctx, int tile_z, int phi_chunks, int use_graph);
@@ -168,6 +180,7 @@ typedef struct {
     double ms_curl;  int64_t n_curl;
     double ms_rhs[5]; int64_t n_rhs[5];
     int64_t dropped;
+    double ms_phi;   int64_t n_phi;      /* pseudo-spectral phi pre-passes */
 } clt_profile;
 int clt_set_profiling(clt_ctx *ctx, int enable);
 int clt_get_profile(clt_ctx *ctx, clt_profile *out);

@@ -37,13 +37,14 @@ class clt_diag(ctypes.Structure):
 
 class clt_profile(ctypes.Structure):
     _fields_ = [("ms_curl", ctypes.c_double), ("n_curl", ctypes.c_int64), ("ms_rhs", ctypes.c_double * 5),
-                ("n_rhs", ctypes.c_int64 * 5), ("dropped", ctypes.c_int64)]
+                ("n_rhs", ctypes.c_int64 * 5), ("dropped", ctypes.c_int64), ("ms_phi", ctypes.c_double),
+                ("n_phi", ctypes.c_int64)]
 
 
 # every symbol include/clt.h declares
 EXPORTS = ["clt_workspace_bytes", "clt_create", "clt_destroy", "clt_set_equilibrium", "clt_set_state", "clt_get_state",
            "clt_rhs", "clt_curl_J1", "clt_hall_G", "clt_step", "clt_set_dt", "clt_diagnostics", "clt_suggest_dt", "clt_set_tuning",
-           "clt_set_kernel_variant", "clt_set_profiling", "clt_get_profile", "clt_launch_count", "clt_stream", "clt_strerror", "clt_last_cuda_error", "clt_version"]
+           "clt_set_kernel_variant", "clt_spectral_workspace_bytes", "clt_set_phi_scheme", "clt_set_profiling", "clt_get_profile", "clt_launch_count", "clt_stream", "clt_strerror", "clt_last_cuda_error", "clt_version"]
 
 _lib = None
 
@@ -91,6 +92,10 @@ def load():
     L.clt_set_profiling.argtypes = [vp, i]
     L.clt_get_profile.restype = i
     L.clt_get_profile.argtypes = [vp, ctypes.POINTER(clt_profile)]
+    L.clt_spectral_workspace_bytes.restype = ctypes.c_size_t
+    L.clt_spectral_workspace_bytes.argtypes = [ctypes.POINTER(clt_grid)]
+    L.clt_set_phi_scheme.restype = i
+    L.clt_set_phi_scheme.argtypes = [vp, i, vp, ctypes.c_size_t]
     L.clt_launch_count.restype = ctypes.c_int64
     L.clt_launch_count.argtypes = [vp]
     L.clt_stream.restype = vp
@@ -225,6 +230,21 @@ class Clt:
     def set_kernel_variant(self, variant=0):
         self._ck(self.L.clt_set_kernel_variant(self.h, int(variant)))
 
+    def set_phi_scheme(self, scheme=1):
+        """0 = 4th-order finite differences in phi (default), 1 = pseudo-spectral (allocates the scratch tensor)."""
+        import torch
+        if not scheme:
+            self._ck(self.L.clt_set_phi_scheme(self.h, 0, None, 0))
+            self._spec_ws = None
+            return
+        nbytes = self.L.clt_spectral_workspace_bytes(ctypes.byref(self.grid))
+        if nbytes == 0:
+            raise CltError(CLT_EINVAL, "pseudo-spectral scheme: nphi too large")
+        ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        off = (-ws.data_ptr()) % 256
+        self._ck(self.L.clt_set_phi_scheme(self.h, int(scheme), ws.data_ptr() + off, nbytes))
+        self._spec_ws = ws
+
     def set_profiling(self, enable=True):
         self._ck(self.L.clt_set_profiling(self.h, int(bool(enable))))
 
@@ -232,7 +252,7 @@ class Clt:
         p = clt_profile()
         self._ck(self.L.clt_get_profile(self.h, ctypes.byref(p)))
         return {"ms_curl": p.ms_curl, "n_curl": p.n_curl, "ms_rhs": list(p.ms_rhs), "n_rhs": list(p.n_rhs),
-                "dropped": p.dropped}
+                "dropped": p.dropped, "ms_phi": p.ms_phi, "n_phi": p.n_phi}
 
     @property
     def launch_count(self):

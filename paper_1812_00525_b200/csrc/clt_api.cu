@@ -23,6 +23,9 @@ struct clt_ctx {
     double *Un, *acc, *Ua, *Ub, *J1, *G, *tab, *Rtab, *invRtab, *cs, *partial, *result;
     int nblocks_diag;
     bool has_state, has_v0, hall;
+    bool spectral;                 // pseudo-spectral phi scheme (clt_set_phi_scheme)
+    double *spec, *spec_ctab;      // caller-provided scratch: SPEC_COUNT derivative fields + circulant weights
+    double sc1[SPEC_MAX_Q + 1], sc2[SPEC_MAX_Q + 1];
     int64_t step;
     double time;
     double dt;
@@ -200,6 +203,23 @@ void prof_end(clt_ctx *ctx, long n)
     if (n >= 0) cudaEventRecord((*ctx->ev)[2 * n + 1], ctx->stream);
 }
 
+// NEXT-2: pseudo-spectral phi derivatives of the stage state U (mode 0: what the curl needs, 1: what the RHS needs)
+int run_phi_pass(clt_ctx *ctx, int mode, const double *U)
+{
+    SpecArgs a;
+    a.L = ctx->L; a.ph = ctx->ph;
+    a.U = U; a.J1 = ctx->J1; a.tab = ctx->tab;
+    a.out = ctx->spec; a.ctab = ctx->spec_ctab;
+    a.mode = mode; a.hall = ctx->hall ? 1 : 0; a.has_v0 = ctx->has_v0 ? 1 : 0;
+    memcpy(a.c1, ctx->sc1, sizeof(a.c1));
+    memcpy(a.c2, ctx->sc2, sizeof(a.c2));
+    const long pe = prof_begin(ctx, 6);
+    CK(launch_phi_spectral(a, ctx->stream));
+    prof_end(ctx, pe);
+    ctx->launches++;
+    return CLT_OK;
+}
+
 int run_curl(clt_ctx *ctx, const double *U)
 {
     CurlArgs a;
@@ -211,15 +231,24 @@ int run_curl(clt_ctx *ctx, const double *U)
     a.R = ctx->Rtab + LP;
     a.invR = ctx->invRtab + LP;
     a.phi_chunks = effective_chunks(ctx);
+    a.spec = ctx->spec;
     alignas(64) CUtensorMap tmU;
     const bool tma = ctx->variant == 0;
+    if (ctx->spectral) {
+        if (!tma) {
+            snprintf(ctx->cuda_err, sizeof(ctx->cuda_err), "the pseudo-spectral phi scheme needs the default kernel variant");
+            return CLT_EINVAL;
+        }
+        int r = run_phi_pass(ctx, 0, U);
+        if (r) return r;
+    }
     if (tma && !make_map(ctx, U, 8, curl_tma_tile_z(), &tmU)) {
         snprintf(ctx->cuda_err, sizeof(ctx->cuda_err), "cuTensorMapEncodeTiled failed");
         return CLT_ECUDA;
     }
     const long pe = prof_begin(ctx, 5);
     if (tma)
-        CK(launch_curl_tma(a, &tmU, ctx->hall, ctx->stream));
+        CK(launch_curl_tma(a, &tmU, ctx->hall, ctx->spectral, ctx->stream));
     else
         CK(launch_curl(a, 0, ctx->stream));
     prof_end(ctx, pe);
@@ -238,11 +267,17 @@ int run_rhs(clt_ctx *ctx, int mode, const double *in, double *out, double a_next
     a.a_next = a_next; a.b_acc = b_acc;
     a.phi_chunks = effective_chunks(ctx);
     a.prefetch = 1;
+    a.spec = ctx->spec;
     const int tz = effective_tile_z(ctx);
-    const bool tma = ctx->variant == 0 && rhs_tma_supports(tz, ctx->hall);
-    if (ctx->hall && !tma) {
-        snprintf(ctx->cuda_err, sizeof(ctx->cuda_err), "the Hall term needs the default kernel variant and tile height");
+    const bool tma = ctx->variant == 0 && rhs_tma_supports(tz, ctx->hall, ctx->spectral);
+    if ((ctx->hall || ctx->spectral) && !tma) {
+        snprintf(ctx->cuda_err, sizeof(ctx->cuda_err),
+                 "the Hall term and the pseudo-spectral phi scheme need the default kernel variant and tile height");
         return CLT_EINVAL;
+    }
+    if (ctx->spectral) {
+        int r = run_phi_pass(ctx, 1, in);
+        if (r) return r;
     }
     alignas(64) CUtensorMap tmU, tmJ;
     if (tma && (!make_map(ctx, in, 8, tz, &tmU) || !make_map(ctx, ctx->J1, ctx->hall ? 6 : 3, tz, &tmJ))) {
@@ -251,7 +286,7 @@ int run_rhs(clt_ctx *ctx, int mode, const double *in, double *out, double a_next
     }
     const long pe = prof_begin(ctx, mode);
     if (tma)
-        CK(launch_rhs_tma(a, &tmU, &tmJ, mode, ctx->has_v0, ctx->hall, tz, ctx->stream));
+        CK(launch_rhs_tma(a, &tmU, &tmJ, mode, ctx->has_v0, ctx->hall, ctx->spectral, tz, ctx->stream));
     else
         CK(launch_rhs(a, mode, ctx->has_v0, tz, ctx->stream));
     prof_end(ctx, pe);
@@ -519,7 +554,7 @@ int clt_step(clt_ctx *ctx, int n)
         }
         for (int s = 0; s < n; ++s) {
             CK(cudaGraphLaunch(ctx->graph_exec, ctx->stream));
-            ctx->launches += 8;
+            ctx->launches += ctx->spectral ? 16 : 8;
         }
     } else {
         for (int s = 0; s < n; ++s) {
@@ -539,6 +574,7 @@ static int run_diag(clt_ctx *ctx, double cfl, double out6[6])
     a.U = ctx->Un; a.tab = ctx->tab;
     a.R = ctx->Rtab + LP; a.invR = ctx->invRtab + LP;
     a.cs = ctx->cs; a.partial = ctx->partial; a.cfl = cfl;
+    a.spec_c1 = ctx->spectral ? ctx->spec_ctab : nullptr;
     CK(launch_diag(a, ctx->nblocks_diag, ctx->result, ctx->stream));
     ctx->launches += 2;
     CK(cudaMemcpyAsync(out6, ctx->result, 6 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
@@ -575,6 +611,63 @@ int clt_suggest_dt(clt_ctx *ctx, double cfl, double *dt_out)
     return CLT_OK;
 }
 
+size_t clt_spectral_workspace_bytes(const clt_grid *grid)
+{
+    if (!grid_ok(grid) || grid->nphi > SPEC_MAX_NPHI) return 0;
+    return (size_t)SPEC_COUNT * carve(grid).field_b + align_up(2 * SPEC_MAX_NPHI * sizeof(double));
+}
+
+int clt_set_phi_scheme(clt_ctx *ctx, int scheme, void *d_scratch, size_t bytes)
+{
+    if (!ctx || scheme < 0 || scheme > 1) return CLT_EINVAL;
+    CK(cudaStreamSynchronize(ctx->stream));
+    destroy_graph(ctx);
+    if (scheme == 0) { ctx->spectral = false; ctx->spec = nullptr; ctx->spec_ctab = nullptr; return CLT_OK; }
+    const size_t need = clt_spectral_workspace_bytes(&ctx->grid);
+    if (need == 0) return CLT_EINVAL;                      // nphi > SPEC_MAX_NPHI
+    if (!d_scratch || bytes < need || ((uintptr_t)d_scratch % 256) != 0) return CLT_ENOMEM;
+    cudaPointerAttributes at;
+    cudaError_t e = cudaPointerGetAttributes(&at, d_scratch);
+    if (e != cudaSuccess) { cudaGetLastError(); return CLT_ECUDA; }
+    if (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeManaged) return CLT_ENOMEM;
+    // closed-form weights of the Fourier differentiation matrices on N equispaced nodes of a period L
+    // (kappa = 2 pi / L):  N even:  c1[m] = kappa/2 (-1)^(m+1) cot(pi m/N), c1[N/2] = 0;
+    //                               c2[0] = -kappa^2 (N^2+2)/12, c2[m] = -kappa^2/2 (-1)^m / sin^2(pi m/N)
+    //                      N odd:   c1[m] = kappa/2 (-1)^(m+1) / sin(pi m/N);
+    //                               c2[0] = -kappa^2 (N^2-1)/12, c2[m] = -kappa^2/2 (-1)^m cos(pi m/N) / sin^2(pi m/N)
+    const int N = ctx->grid.nphi;
+    const long double PI = 3.141592653589793238462643383279502884L;
+    const long double kap = 2.0L * PI / (long double)ctx->ph.Lphi;
+    std::vector<double> tabv(2 * SPEC_MAX_NPHI, 0.0);
+    for (int m = 0; m < N; ++m) {
+        long double c1, c2;
+        const long double th = PI * (long double)m / (long double)N, sg = (m % 2) ? -1.0L : 1.0L;
+        if (m == 0) {
+            c1 = 0.0L;
+            c2 = -kap * kap * ((N % 2 == 0) ? ((long double)N * N + 2.0L) : ((long double)N * N - 1.0L)) / 12.0L;
+        } else if (N % 2 == 0) {
+            c1 = (2 * m == N) ? 0.0L : -0.5L * kap * sg * cosl(th) / sinl(th);
+            c2 = -0.5L * kap * kap * sg / (sinl(th) * sinl(th));
+        } else {
+            c1 = -0.5L * kap * sg / sinl(th);
+            c2 = -0.5L * kap * kap * sg * cosl(th) / (sinl(th) * sinl(th));
+        }
+        tabv[m] = (double)c1;
+        tabv[SPEC_MAX_NPHI + m] = (double)c2;
+    }
+    memset(ctx->sc1, 0, sizeof(ctx->sc1));
+    memset(ctx->sc2, 0, sizeof(ctx->sc2));
+    for (int m = 0; m <= SPEC_MAX_Q && m < N; ++m) { ctx->sc1[m] = tabv[m]; ctx->sc2[m] = tabv[SPEC_MAX_NPHI + m]; }
+    const size_t fields_b = (size_t)SPEC_COUNT * carve(&ctx->grid).field_b;
+    ctx->spec = (double *)d_scratch;
+    ctx->spec_ctab = (double *)((char *)d_scratch + fields_b);
+    CK(cudaMemsetAsync(d_scratch, 0, need, ctx->stream));
+    CK(cudaMemcpyAsync(ctx->spec_ctab, tabv.data(), tabv.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    ctx->spectral = true;
+    return CLT_OK;
+}
+
 int clt_set_tuning(clt_ctx *ctx, int tile_z, int phi_chunks, int use_graph)
 {
     if (!ctx) return CLT_EINVAL;
@@ -607,6 +700,7 @@ int clt_get_profile(clt_ctx *ctx, clt_profile *out)
         CK(cudaEventElapsedTime(&ms, (*ctx->ev)[2 * n], (*ctx->ev)[2 * n + 1]));
         const int kind = (*ctx->ev_kind)[n];
         if (kind == 5) { out->ms_curl += ms; out->n_curl++; }
+        else if (kind == 6) { out->ms_phi += ms; out->n_phi++; }
         else { out->ms_rhs[kind] += ms; out->n_rhs[kind]++; }
     }
     out->dropped = ctx->ev_dropped;

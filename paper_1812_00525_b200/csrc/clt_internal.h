@@ -61,6 +61,7 @@ struct RhsArgs {
     double b_acc;         // weight of K in the accumulator (mode 2) / in U^{n+1} (mode 4)
     int phi_chunks;       // number of chunks the phi range is split into (gridDim.z)
     int prefetch;         // issue L2 prefetch hints
+    const double *spec;   // pseudo-spectral variant: SPEC_COUNT derivative fields (SpecField)
 };
 
 struct CurlArgs {
@@ -69,10 +70,37 @@ struct CurlArgs {
     const double *B;      // 3 fields (B_R, B_phi, B_Z of the stage state)
     double *J1;           // 3 fields
     double *G;            // 3 fields: Hall field (written by the Hall variant only)
+    const double *spec;   // pseudo-spectral variant: derivative fields (uses SP_DB and, with hall, SP_D1 + 1)
     const double *tab;
     const double *R;
     const double *invR;
     int phi_chunks;
+};
+
+// NEXT-2: pseudo-spectral phi derivatives.  Scratch layout: SPEC_COUNT fields.
+enum SpecField {
+    SP_D1 = 0,        // d/dphi of rho1, p1, v1_R, v1_phi, v1_Z (5 fields)
+    SP_D2 = 5,        // d2/dphi2 of the same (5 fields)
+    SP_DE = 10,       // d/dphi of E1_R, E1_Z
+    SP_DB = 12,       // d/dphi of B1_R, B1_Z
+    SPEC_COUNT = 14
+};
+constexpr int SPEC_MAX_NPHI = 256;
+constexpr int SPEC_MAX_Q = 32;       // register-resident lines: nphi in {16, 32, 64}
+
+// one phi pre-pass: mode 0 = before the curl (B_R, B_Z; p too when hall), 1 = before the fused RHS kernel
+// (rho, p, v: first and second derivative; E1_R, E1_Z: first derivative)
+struct SpecArgs {
+    Layout L;
+    Phys ph;
+    const double *U;      // stage state, 8 fields
+    const double *J1;     // 3 fields (+ G behind them when hall)
+    const double *tab;
+    double *out;          // SPEC_COUNT fields
+    const double *ctab;   // [2][SPEC_MAX_NPHI] circulant weights c1[m], c2[m] (device copy, generic path)
+    int mode, hall, has_v0;
+    double c1[SPEC_MAX_Q + 1];   // c1[m], m = 0..Q   (antisymmetric: c1[N-m] = -c1[m])
+    double c2[SPEC_MAX_Q + 1];   // c2[m], m = 0..N/2 (symmetric)
 };
 
 struct DiagArgs {
@@ -85,6 +113,7 @@ struct DiagArgs {
     const double *cs;     // cos/sin(2 pi j / nphi), [2][nphi]
     double *partial;      // [nblocks][6]
     double cfl;
+    const double *spec_c1;   // non-null: pseudo-spectral d/dphi in div_c B, weights c1[0..nphi-1]
 };
 
 enum { RHS_MODE_K = 0, RHS_MODE_S1 = 1, RHS_MODE_S2 = 2, RHS_MODE_S3 = 3, RHS_MODE_S4 = 4 };
@@ -100,12 +129,13 @@ cudaError_t launch_rhs(const RhsArgs &a, int mode, bool has_v0, int tile_z, cuda
 // TMA variant: tmU / tmJ point to CUtensorMap objects over the stage state (4-D: pR, nZ, nphi, 8) and J1 (.., 3)
 // with box (TR+4, tile_z+4, 1, 1)
 // hall: tmJ maps 6 fields (J1 then G) and the kernel adds d_i * G to E1 (default tile height only)
-cudaError_t launch_rhs_tma(const RhsArgs &a, const void *tmU, const void *tmJ, int mode, bool has_v0, bool hall, int tile_z,
-                           cudaStream_t s);
-bool rhs_tma_supports(int tile_z, bool hall);
+cudaError_t launch_rhs_tma(const RhsArgs &a, const void *tmU, const void *tmJ, int mode, bool has_v0, bool hall, bool spec,
+                           int tile_z, cudaStream_t s);
+bool rhs_tma_supports(int tile_z, bool hall, bool spec);
 // TMA variant of the curl kernel: tmU is a CUtensorMap over the 8 fields of the stage state with box
 // (TR+4, curl_tma_tile_z()+4, 1, 1); hall = also write the Hall field G
-cudaError_t launch_curl_tma(const CurlArgs &a, const void *tmU, bool hall, cudaStream_t s);
+cudaError_t launch_curl_tma(const CurlArgs &a, const void *tmU, bool hall, bool spec, cudaStream_t s);
+cudaError_t launch_phi_spectral(const SpecArgs &a, cudaStream_t s);
 int curl_tma_tile_z();
 cudaError_t launch_diag(const DiagArgs &a, int nblocks, double *result6, cudaStream_t s);
 int diag_blocks(const Layout &L);

@@ -85,11 +85,14 @@ __device__ __forceinline__ CentreTab load_centre_tab(const double *tab, long lon
 // `sync` is called once, after everything that needs no other thread's shared-memory data (centre values, the
 // phi direction from the register pipeline, the phi differences of E1 at the own node) and before the first read
 // of a neighbour's staged value: the caller puts the wait half of its split barrier there.
-template <bool V0, class Sync>
+// SPEC = true: the phi derivatives come from the pseudo-spectral pre-pass: pd1[f], pd2[f] are d/dphi and d2/dphi2 of
+// the five fluid perturbations, dP_EZ / dP_ER the true d/dphi of E1_Z / E1_R (not the unscaled stencil sums).
+template <bool V0, bool SPEC, class Sync>
 __device__ __forceinline__ void rhs_point(const double *stg, int HT, const double *eRc, const double *ePc, const double *eZc,
                                           double dP_EZ, double dP_ER, const double (&F)[3], const double (&rr)[4], int cs,
                                           const double (&q)[5][5], const CentreTab &ct, const double *tab, long long off2,
-                                          long long plane, const Phys &ph, double iR, double iR2, double (&K)[8], Sync &&sync)
+                                          long long plane, const Phys &ph, double iR, double iR2, double (&K)[8], Sync &&sync,
+                                          const double *pd1 = nullptr, const double *pd2 = nullptr)
 {
     const double rho1 = q[2][0], p1 = q[2][1], v1R = q[2][2], v1P = q[2][3], v1Z = q[2][4];
     const double rho = rho1 + ct.rho0;
@@ -106,11 +109,11 @@ __device__ __forceinline__ void rhs_point(const double *stg, int HT, const doubl
     double divv1, gRp1, gPp1, gZp1, gPvR, gPvP;
     // phi direction (register pipeline)
     {
-        const double g1 = ph.cP1 * iR, vc = vP * g1, lc = ph.cP2 * iR2;
+        const double g1 = SPEC ? iR : ph.cP1 * iR, vc = vP * g1, lc = SPEC ? iR2 : ph.cP2 * iR2;
 #pragma unroll
         for (int f = 0; f < 5; ++f) {
-            const double d1 = fd1(q[0][f], q[1][f], q[3][f], q[4][f]);
-            const double d2 = fd2(q[0][f], q[1][f], q[2][f], q[3][f], q[4][f]);
+            const double d1 = SPEC ? pd1[f] : fd1(q[0][f], q[1][f], q[3][f], q[4][f]);
+            const double d2 = SPEC ? pd2[f] : fd2(q[0][f], q[1][f], q[2][f], q[3][f], q[4][f]);
             A[f] = vc * d1;
             lap[f] = lc * d2;
             if (f == 1) gPp1 = d1 * g1;
@@ -186,7 +189,7 @@ __device__ __forceinline__ void rhs_point(const double *stg, int HT, const doubl
     const double dZ_ER = fd1(eR[-2 * SW], eR[-SW], eR[SW], eR[2 * SW]);
     const double dR_EZ = fd1(eZ[-2], eZ[-1], eZ[1], eZ[2]);
     const double dR_REP = fd1(rr[0] * eP[-2], rr[1] * eP[-1], rr[2] * eP[1], rr[3] * eP[2]);
-    const double cPi = ph.cP1 * iR;
+    const double cPi = SPEC ? iR : ph.cP1 * iR;
     K[5] = dZ_EP * ph.cZ1 - dP_EZ * cPi;
     K[6] = dR_EZ * ph.cR1 - dZ_ER * ph.cZ1;
     K[7] = dP_ER * cPi - dR_REP * (ph.cR1 * iR);
@@ -415,7 +418,7 @@ __global__ void __launch_bounds__(TR *TZ, (TZ <= 8 ? 2 : 1)) rhs_kernel(const __
             const double dP_ER = fd1(S.ering[s0][0][cs], S.ering[s1][0][cs], S.ering[s3][0][cs], S.ering[se][0][cs]);
             const double F[3] = { S.fring[sfc][0][ci], S.fring[sfc][1][ci], S.fring[sfc][2][ci] };
             const double rr[4] = { S.sR[tx], S.sR[tx + 1], S.sR[tx + 3], S.sR[tx + 4] };
-            rhs_point<V0>(&S.stage[buf][0][0], RhsSmem<TZ>::HT, &S.ering[sec][0][0], &S.ering[sec][1][0], &S.ering[sec][2][0],
+            rhs_point<V0, false>(&S.stage[buf][0][0], RhsSmem<TZ>::HT, &S.ering[sec][0][0], &S.ering[sec][1][0], &S.ering[sec][2][0],
                           dP_EZ, dP_ER, F, rr, cs, q, ct, tab, off2, L.plane, ph, iR, iR2, K, [] {});
         }
 
@@ -551,7 +554,7 @@ struct RhsTmaSmem {
     alignas(8) unsigned long long ready;       // split CTA barrier: "this plane is staged" (count = all threads)
 };
 
-template <int TZ, int NRAW, int MODE, bool V0, bool HALL>
+template <int TZ, int NRAW, int MODE, bool V0, bool HALL, bool SPEC>
 __global__ void __launch_bounds__(TR *TZ, 1)
 rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmJ)
 {
@@ -757,15 +760,27 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
 
         // ---- phase B: K at (i, k, j) -----------------------------------------------------------
         double K[8];
-        const double dP_EZ = fd1(eZ[0], eZ[1], eZ[3], eZ[4]);
-        const double dP_ER = fd1(eR[0], eR[1], eR[3], eR[4]);
-        rhs_point<V0>(&S.sring[sc][0][0], HT, &S.ering[sc][0][0], &S.ering[sc][1][0], &S.ering[sc][2][0], dP_EZ, dP_ER, Fp[0], rr,
-                      cs, q, ct, tab, off2, L.plane, ph, iR, iR2, K, [&] {
-                          if (SPLIT) {
-                              mbar_wait(&S.ready, ready_parity);
-                              refill();
-                          }
-                      });
+        double dP_EZ, dP_ER, pd1[5], pd2[5];
+        if (SPEC) {
+            // pseudo-spectral phi derivatives of this node from the pre-pass (requested with the epilogue operands)
+#pragma unroll
+            for (int f = 0; f < 5; ++f) {
+                pd1[f] = ld_stream(a.spec + (SP_D1 + f) * L.field + g);
+                pd2[f] = ld_stream(a.spec + (SP_D2 + f) * L.field + g);
+            }
+            dP_ER = ld_stream(a.spec + (SP_DE + 0) * L.field + g);
+            dP_EZ = ld_stream(a.spec + (SP_DE + 1) * L.field + g);
+        } else {
+            dP_EZ = fd1(eZ[0], eZ[1], eZ[3], eZ[4]);
+            dP_ER = fd1(eR[0], eR[1], eR[3], eR[4]);
+        }
+        rhs_point<V0, SPEC>(&S.sring[sc][0][0], HT, &S.ering[sc][0][0], &S.ering[sc][1][0], &S.ering[sc][2][0], dP_EZ, dP_ER, Fp[0],
+                            rr, cs, q, ct, tab, off2, L.plane, ph, iR, iR2, K, [&] {
+                                if (SPLIT) {
+                                    mbar_wait(&S.ready, ready_parity);
+                                    refill();
+                                }
+                            }, pd1, pd2);
         ready_parity ^= 1u;
 
         // ---- a6: RK4 stage combine in the epilogue (L125, L139) --------------------------------
@@ -774,11 +789,11 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
     }
 }
 
-template <int TZ, int NRAW, int MODE, bool V0, bool HALL>
+template <int TZ, int NRAW, int MODE, bool V0, bool HALL, bool SPEC>
 static cudaError_t launch_rhs_tma_t(const RhsArgs &a, const CUtensorMap &tmU, const CUtensorMap &tmJ, cudaStream_t s)
 {
     static bool configured = false;
-    auto kern = rhs_tma_kernel<TZ, NRAW, MODE, V0, HALL>;
+    auto kern = rhs_tma_kernel<TZ, NRAW, MODE, V0, HALL, SPEC>;
     using SM = RhsTmaSmem<TZ, NRAW, HALL ? 14 : 11>;
     const int smem = (int)sizeof(SM);
     static_assert(sizeof(SM) <= 232448, "shared memory of the TMA RHS kernel exceeds 227 KB");
@@ -793,14 +808,14 @@ static cudaError_t launch_rhs_tma_t(const RhsArgs &a, const CUtensorMap &tmU, co
     return cudaGetLastError();
 }
 
-template <int TZ, int NRAW, bool HALL>
+template <int TZ, int NRAW, bool HALL, bool SPEC>
 static cudaError_t launch_rhs_tma_tz(const RhsArgs &a, const CUtensorMap &tmU, const CUtensorMap &tmJ, int mode, bool v0,
                                      cudaStream_t s)
 {
-#define CLT_CASE(M)                                                                           \
-    case M:                                                                                   \
-        return v0 ? launch_rhs_tma_t<TZ, NRAW, M, true, HALL>(a, tmU, tmJ, s)                 \
-                  : launch_rhs_tma_t<TZ, NRAW, M, false, HALL>(a, tmU, tmJ, s);
+#define CLT_CASE(M)                                                                                 \
+    case M:                                                                                         \
+        return v0 ? launch_rhs_tma_t<TZ, NRAW, M, true, HALL, SPEC>(a, tmU, tmJ, s)                 \
+                  : launch_rhs_tma_t<TZ, NRAW, M, false, HALL, SPEC>(a, tmU, tmJ, s);
     switch (mode) {
         CLT_CASE(RHS_MODE_K)
         CLT_CASE(RHS_MODE_S1)
@@ -813,24 +828,30 @@ static cudaError_t launch_rhs_tma_tz(const RhsArgs &a, const CUtensorMap &tmU, c
 #undef CLT_CASE
 }
 
-bool rhs_tma_supports(int tile_z, bool hall)
+// the Hall and pseudo-spectral variants exist for the default tile height only
+bool rhs_tma_supports(int tile_z, bool hall, bool spec)
 {
-    if (hall) return tile_z == 8;
+    if (hall || spec) return tile_z == 8;
     return tile_z == 8 || tile_z == 10 || tile_z == 12 || tile_z == 13;
 }
 
-cudaError_t launch_rhs_tma(const RhsArgs &a, const void *tmU, const void *tmJ, int mode, bool has_v0, bool hall, int tile_z,
-                           cudaStream_t s)
+cudaError_t launch_rhs_tma(const RhsArgs &a, const void *tmU, const void *tmJ, int mode, bool has_v0, bool hall, bool spec,
+                           int tile_z, cudaStream_t s)
 {
     const CUtensorMap &mU = *reinterpret_cast<const CUtensorMap *>(tmU);
     const CUtensorMap &mJ = *reinterpret_cast<const CUtensorMap *>(tmJ);
-    if (hall) return tile_z == 8 ? launch_rhs_tma_tz<8, 2, true>(a, mU, mJ, mode, has_v0, s) : cudaErrorInvalidValue;
+    if (hall || spec) {
+        if (tile_z != 8) return cudaErrorInvalidValue;
+        if (hall && spec) return launch_rhs_tma_tz<8, 2, true, true>(a, mU, mJ, mode, has_v0, s);
+        if (hall) return launch_rhs_tma_tz<8, 2, true, false>(a, mU, mJ, mode, has_v0, s);
+        return launch_rhs_tma_tz<8, 2, false, true>(a, mU, mJ, mode, has_v0, s);
+    }
     switch (tile_z) {
     // two raw buffers (TMA two planes ahead) where shared memory allows, one otherwise
-    case 8: return launch_rhs_tma_tz<8, CLT_NRAW8, false>(a, mU, mJ, mode, has_v0, s);
-    case 10: return launch_rhs_tma_tz<10, 2, false>(a, mU, mJ, mode, has_v0, s);
-    case 12: return launch_rhs_tma_tz<12, 1, false>(a, mU, mJ, mode, has_v0, s);
-    case 13: return launch_rhs_tma_tz<13, 1, false>(a, mU, mJ, mode, has_v0, s);
+    case 8: return launch_rhs_tma_tz<8, CLT_NRAW8, false, false>(a, mU, mJ, mode, has_v0, s);
+    case 10: return launch_rhs_tma_tz<10, 2, false, false>(a, mU, mJ, mode, has_v0, s);
+    case 12: return launch_rhs_tma_tz<12, 1, false, false>(a, mU, mJ, mode, has_v0, s);
+    case 13: return launch_rhs_tma_tz<13, 1, false, false>(a, mU, mJ, mode, has_v0, s);
     default: return cudaErrorInvalidValue;
     }
 }
@@ -966,7 +987,8 @@ struct CurlTmaSmem {
 // HALL = true additionally forms the Hall field of eq (5) [L77] in its equilibrium-subtracted form (DESIGN.md
 // reading R11),  G = (J1 x B + J0 x B1 - grad p1)/rho - (rho1/rho)(v0.grad)v0,  on interior nodes: the same sweep
 // with rho and p staged next to B (p1 = p - p0 is formed before differencing, H2).  tmU maps the whole stage state.
-template <int TZ, int NS, bool HALL>
+// SPEC = true takes d/dphi of B1_R, B1_Z (and p1) from the pseudo-spectral pre-pass instead of the phi stencil.
+template <int TZ, int NS, bool HALL, bool SPEC>
 __global__ void __launch_bounds__(TR *TZ, HALL ? 1 : CLT_CURL_MINB)
 curl_tma_kernel(const __grid_constant__ CurlArgs a, const __grid_constant__ CUtensorMap tmU)
 {
@@ -1074,9 +1096,12 @@ curl_tma_kernel(const __grid_constant__ CurlArgs a, const __grid_constant__ CUte
         const double dR_BZ = fd1(sZ_[-2] - r0Z[0], sZ_[-1] - r0Z[1], sZ_[1] - r0Z[2], sZ_[2] - r0Z[3]);
         const double dR_RBP = fd1(rr[0] * (sP_[-2] - r0P[0]), rr[1] * (sP_[-1] - r0P[1]), rr[2] * (sP_[1] - r0P[2]),
                                   rr[3] * (sP_[2] - r0P[3]));
-        const double JR = dP_BZ * cPi - dZ_BP * ph.cZ1;
+        const long long gc = (long long)j * L.plane + off2;
+        const double pBZ = SPEC ? __ldg(a.spec + (SP_DB + 1) * L.field + gc) * iR : dP_BZ * cPi;     // d_phi B1_Z / R
+        const double pBR = SPEC ? __ldg(a.spec + (SP_DB + 0) * L.field + gc) * iR : dP_BR * cPi;     // d_phi B1_R / R
+        const double JR = pBZ - dZ_BP * ph.cZ1;
         const double JP = dZ_BR * ph.cZ1 - dR_BZ * ph.cR1;
-        const double JZ = dR_RBP * (ph.cR1 * iR) - dP_BR * cPi;
+        const double JZ = dR_RBP * (ph.cR1 * iR) - pBR;
         double GR = 0.0, GP = 0.0, GZ = 0.0;
         if (HALL) {
             const double *sp_ = &S.raw[st][NF - 1][cs];
@@ -1085,7 +1110,7 @@ curl_tma_kernel(const __grid_constant__ CurlArgs a, const __grid_constant__ CUte
             const double B1R = bR[2], B1P = BP - o0P, B1Z = bZ[2];
             const double gR = fd1(sp_[-2] - rp0[0], sp_[-1] - rp0[1], sp_[1] - rp0[2], sp_[2] - rp0[3]) * ph.cR1;
             const double gZ = fd1(sp_[-2 * SW] - zp0[0], sp_[-SW] - zp0[1], sp_[SW] - zp0[2], sp_[2 * SW] - zp0[3]) * ph.cZ1;
-            const double gP = fd1(pP[0], pP[1], pP[3], pP[4]) * cPi;
+            const double gP = SPEC ? __ldg(a.spec + (SP_D1 + 1) * L.field + gc) * iR : fd1(pP[0], pP[1], pP[3], pP[4]) * cPi;
             const double rinv = 1.0 / rho, r1 = (rho - rho0) * rinv;
             GR = ((JP * BZ - JZ * BP) + (j0P * B1Z - j0Z * B1P) - gR) * rinv - r1 * a0R;
             GP = ((JZ * BR - JR * BZ) + (j0Z * B1R - j0R * B1Z) - gP) * rinv - r1 * a0P;
@@ -1108,12 +1133,12 @@ curl_tma_kernel(const __grid_constant__ CurlArgs a, const __grid_constant__ CUte
     }
 }
 
-template <bool HALL>
+template <bool HALL, bool SPEC>
 static cudaError_t launch_curl_tma_t(const CurlArgs &a, const void *tmU, cudaStream_t s)
 {
     constexpr int TZ = CLT_CURL_TZ, NS = CLT_CURL_NS;
     static bool configured = false;
-    auto kern = curl_tma_kernel<TZ, NS, HALL>;
+    auto kern = curl_tma_kernel<TZ, NS, HALL, SPEC>;
     const int smem = (int)sizeof(CurlTmaSmem<TZ, NS, HALL ? 5 : 3>);
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
@@ -1126,11 +1151,126 @@ static cudaError_t launch_curl_tma_t(const CurlArgs &a, const void *tmU, cudaStr
     return cudaGetLastError();
 }
 
-cudaError_t launch_curl_tma(const CurlArgs &a, const void *tmU, bool hall, cudaStream_t s)
+cudaError_t launch_curl_tma(const CurlArgs &a, const void *tmU, bool hall, bool spec, cudaStream_t s)
 {
-    return hall ? launch_curl_tma_t<true>(a, tmU, s) : launch_curl_tma_t<false>(a, tmU, s);
+    if (spec) return hall ? launch_curl_tma_t<true, true>(a, tmU, s) : launch_curl_tma_t<false, true>(a, tmU, s);
+    return hall ? launch_curl_tma_t<true, false>(a, tmU, s) : launch_curl_tma_t<false, false>(a, tmU, s);
 }
 int curl_tma_tile_z() { return CLT_CURL_TZ; }
+
+// ---------------------------------------------------------------------------------------------
+// NEXT-2: pseudo-spectral phi derivatives ("either 4th order finite difference or
+// pseudo-spectrum method can be used" in phi; reading R12).  A phi-global operator does not fit
+// the phi-marching sweeps, so the derivatives are formed by a pre-pass and read back by the SPEC variants of
+// the curl and fused RHS kernels.  One thread owns one (R, Z) line of one quantity: it loads the N = nphi
+// samples (coalesced across the warp in R), keeps them in registers (N in {16, 32, 64}; a local array for any
+// other N <= 256) and evaluates the circulant sums in their paired form
+//   d1_j = sum_{m=1..Q} c1[m] (f_{j+m} - f_{j-m}),   Q = floor((N-1)/2)
+//   d2_j = c2[0] f_j + sum_{m=1..Q} c2[m] (f_{j+m} + f_{j-m}) [+ c2[N/2] f_{j+N/2}, N even]
+// with the closed-form weights of the Fourier differentiation matrices (clt_api.cu).  Perturbations are
+// formed before differencing (H2).  FP64-bound: about N FP64 instructions per output value.
+// ---------------------------------------------------------------------------------------------
+template <int NT>
+__global__ void __launch_bounds__(128) phi_spectral_kernel(const __grid_constant__ SpecArgs a)
+{
+    const Layout &L = a.L;
+    const int N = NT > 0 ? NT : L.nphi;
+    const int i = 2 + blockIdx.x * 32 + threadIdx.x, k = 2 + blockIdx.y * 4 + threadIdx.y;
+    if (i > L.nR - 3 || k > L.nZ - 3) return;
+    const long long o2 = (long long)k * L.pR + (LP + i);
+    const int job = blockIdx.z;
+    constexpr int NV = NT > 0 ? NT : SPEC_MAX_NPHI;
+    double v[NV];
+    int out1 = -1, out2 = -1;       // output field of the first / second derivative
+    if (a.mode == 0) {
+        // before the curl: B1_R, B1_Z (and p1 for the Hall field)
+        const int src = job == 0 ? 5 : (job == 1 ? 7 : 1);
+        const int t0 = job == 0 ? T_B0R : (job == 1 ? T_B0Z : T_P0);
+        out1 = job < 2 ? SP_DB + job : SP_D1 + 1;
+        const double f0 = __ldg(a.tab + t0 * L.plane + o2);
+#pragma unroll
+        for (int j = 0; j < NV; ++j)
+            if (j < N) v[j] = __ldg(a.U + src * L.field + (long long)j * L.plane + o2) - f0;
+    } else if (job < 5) {
+        out1 = SP_D1 + job;
+        out2 = SP_D2 + job;
+        const int t0 = job == 0 ? T_RHO0 : (job == 1 ? T_P0 : T_V0R + (job - 2));
+        const double f0 = (job < 2 || a.has_v0) ? __ldg(a.tab + t0 * L.plane + o2) : 0.0;
+#pragma unroll
+        for (int j = 0; j < NV; ++j)
+            if (j < N) v[j] = __ldg(a.U + job * L.field + (long long)j * L.plane + o2) - f0;
+    } else {
+        // E1_R (job 5) or E1_Z (job 6) = -(v x B)_c + eta J1_c (+ d_i G_c); the axisymmetric v0 x B0 drops out
+        // of the paired differences exactly and is left out
+        const int c = job == 5 ? 0 : 2;
+        out1 = SP_DE + (job - 5);
+        const int ia = c == 0 ? 3 : 2, ib = c == 0 ? 7 : 6, ic2 = c == 0 ? 4 : 3, id = c == 0 ? 6 : 5;
+        // (v x B)_R = v_phi B_Z - v_Z B_phi ; (v x B)_Z = v_R B_phi - v_phi B_R
+#pragma unroll
+        for (int j = 0; j < NV; ++j)
+            if (j < N) {
+                const long long g = (long long)j * L.plane + o2;
+                const double va = __ldg(a.U + ia * L.field + g), Bb = __ldg(a.U + ib * L.field + g);
+                const double vc = __ldg(a.U + ic2 * L.field + g), Bd = __ldg(a.U + id * L.field + g);
+                double e = a.ph.eta * __ldg(a.J1 + c * L.field + g) - (va * Bb - vc * Bd);
+                if (a.hall) e = fma(a.ph.d_i, __ldg(a.J1 + (3 + c) * L.field + g), e);
+                v[j] = e;
+            }
+    }
+    const int Q = (N - 1) / 2;
+    const bool even = (N & 1) == 0;
+    double *o1 = a.out + (long long)out1 * L.field + o2;
+    double *o2p = out2 >= 0 ? a.out + (long long)out2 * L.field + o2 : nullptr;
+    if (NT > 0) {
+#pragma unroll
+        for (int j = 0; j < NV; ++j) {
+            double s1 = 0.0, s2 = a.c2[0] * v[j];
+#pragma unroll
+            for (int m = 1; m <= (NV - 1) / 2; ++m) {
+                const double fp = v[(j + m) % NV], fm = v[(j - m + NV) % NV];
+                s1 = fma(a.c1[m], fp - fm, s1);
+                s2 = fma(a.c2[m], fp + fm, s2);
+            }
+            if ((NV & 1) == 0) s2 = fma(a.c2[NV / 2], v[(j + NV / 2) % NV], s2);
+            o1[(long long)j * L.plane] = s1;
+            if (o2p) o2p[(long long)j * L.plane] = s2;
+        }
+    } else {
+        const double *c1 = a.ctab, *c2 = a.ctab + SPEC_MAX_NPHI;
+        for (int j = 0; j < N; ++j) {
+            double s1 = 0.0, s2 = c2[0] * v[j];
+            for (int m = 1; m <= Q; ++m) {
+                int jp = j + m, jm = j - m;
+                if (jp >= N) jp -= N;
+                if (jm < 0) jm += N;
+                const double fp = v[jp], fm = v[jm];
+                s1 = fma(c1[m], fp - fm, s1);
+                s2 = fma(c2[m], fp + fm, s2);
+            }
+            if (even) {
+                int jh = j + N / 2;
+                if (jh >= N) jh -= N;
+                s2 = fma(c2[N / 2], v[jh], s2);
+            }
+            o1[(long long)j * L.plane] = s1;
+            if (o2p) o2p[(long long)j * L.plane] = s2;
+        }
+    }
+}
+
+cudaError_t launch_phi_spectral(const SpecArgs &a, cudaStream_t s)
+{
+    const int jobs = a.mode == 0 ? (a.hall ? 3 : 2) : 7;
+    dim3 block(32, 4, 1);
+    dim3 grid((a.L.nR - 4 + 31) / 32, (a.L.nZ - 4 + 3) / 4, jobs);
+    switch (a.L.nphi) {
+    case 16: phi_spectral_kernel<16><<<grid, block, 0, s>>>(a); break;
+    case 32: phi_spectral_kernel<32><<<grid, block, 0, s>>>(a); break;
+    case 64: phi_spectral_kernel<64><<<grid, block, 0, s>>>(a); break;
+    default: phi_spectral_kernel<0><<<grid, block, 0, s>>>(a); break;
+    }
+    return cudaGetLastError();
+}
 
 // ---------------------------------------------------------------------------------------------
 // Axisymmetric tables (once per clt_set_equilibrium): J0 = curl_c B0 etc.
@@ -1300,10 +1440,17 @@ __global__ void __launch_bounds__(DG_BX *DG_BY) diag_kernel(const __grid_constan
                 const double *bp = a.U + 6 * L.field + o;
                 const int n = L.nphi;
                 const double dRR = fd1(a.R[i - 2] * br[-2], a.R[i - 1] * br[-1], a.R[i + 1] * br[1], a.R[i + 2] * br[2]);
-                const double dP = fd1(bp[(long long)wrap_phi(j - 2, n) * L.plane], bp[(long long)wrap_phi(j - 1, n) * L.plane],
-                                      bp[(long long)wrap_phi(j + 1, n) * L.plane], bp[(long long)wrap_phi(j + 2, n) * L.plane]);
+                double dPs;      // d_phi B_phi
+                if (a.spec_c1) {
+                    dPs = 0.0;   // pseudo-spectral: paired circulant sum (B0_phi drops out of the differences)
+                    for (int m = 1; m <= (n - 1) / 2; ++m)
+                        dPs = fma(a.spec_c1[m], bp[(long long)wrap_phi(j + m, n) * L.plane] - bp[(long long)wrap_phi(j - m, n) * L.plane], dPs);
+                } else {
+                    dPs = fd1(bp[(long long)wrap_phi(j - 2, n) * L.plane], bp[(long long)wrap_phi(j - 1, n) * L.plane],
+                              bp[(long long)wrap_phi(j + 1, n) * L.plane], bp[(long long)wrap_phi(j + 2, n) * L.plane]) * ph.cP1;
+                }
                 const double dZ = fd1(bz[-2 * L.pR], bz[-L.pR], bz[L.pR], bz[2 * L.pR]);
-                mdiv = fmax(mdiv, fabs(dRR * ph.cR1 * iR + dP * ph.cP1 * iR + dZ * ph.cZ1));
+                mdiv = fmax(mdiv, fabs(dRR * ph.cR1 * iR + dPs * iR + dZ * ph.cZ1));
             }
         }
         const double w = Ri * ph.dR * ph.dphi * ph.dZ;

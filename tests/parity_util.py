@@ -23,7 +23,10 @@ def make_gpu(prob, set_eq=True, **over):
     c = prob.cfg
     par = dict(gamma=c.gamma, eta=c.eta, nu=c.nu, D=c.D, kappa=c.kappa, dt=prob.dt, cfl=c.cfl)
     par.update(over)
+    phi_scheme = par.pop("phi_scheme", 0)
     g = clt.Clt(c.nR, c.nphi, c.nZ, c.Rmin, c.Rmax, c.Zmin, c.Zmax, c.phi_extent, **par)
+    if phi_scheme:
+        g.set_phi_scheme(phi_scheme)
     if set_eq:
         g.set_equilibrium(np.ascontiguousarray(prob.U0))
     g.set_state(np.ascontiguousarray(prob.U))

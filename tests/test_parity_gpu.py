@@ -272,3 +272,67 @@ def test_hall_needs_the_default_kernel_variant():
     g0 = make_gpu(prob)
     with pytest.raises(clt.CltError):
         g0.hall_G()
+
+
+# ------------------------------------------------------------------------------ NEXT-2: pseudo-spectral phi scheme, L125
+SPEC_CASES = {
+    "config1": lambda: inputs.make_problem(1),                                              # nphi = 16: register-resident lines
+    "ragged-77x9x53": lambda: inputs.make_custom_problem(77, 9, 53, index=11),              # odd nphi, generic path
+    "min-9x5x9": lambda: inputs.make_custom_problem(9, 5, 9, index=12),
+    "rotating-v0-12": lambda: inputs.make_custom_problem(45, 12, 37, index=13, rotation=0.05),   # even nphi, generic path
+    "nphi32": lambda: inputs.make_custom_problem(40, 32, 24, index=17, amplitude_scale=50.0),
+    "nphi64": lambda: inputs.make_custom_problem(36, 64, 20, index=18, amplitude_scale=50.0),
+}
+
+
+@pytest.mark.parametrize("name", list(SPEC_CASES))
+@pytest.mark.parametrize("d_i", [0.0, 0.05])
+def test_spectral_curl_and_rhs_match_oracle(name, d_i):
+    prob = SPEC_CASES[name]()
+    over = dict(phi_scheme=1, d_i=d_i, eta=1e-4)
+    o, g = make_oracle(prob, **over), make_gpu(prob, **over)
+    assert_close(g.curl_J1(), o.curl_J1(prob.U), RHS_TOL, f"curl_J1, pseudo-spectral phi, {name}")
+    if d_i:
+        assert_close(g.hall_G(), o.hall_G(prob.U), RHS_TOL, f"Hall field, pseudo-spectral phi, {name}")
+    K_o, K_g = o.rhs(), g.rhs()
+    assert_close(K_g, K_o, RHS_TOL, f"rhs, pseudo-spectral phi, {name}")
+    # it is a different discretisation: the FD result differs by the FD truncation error, far above round-off
+    K_fd = make_oracle(prob, d_i=d_i, eta=1e-4).rhs()
+    assert max(rel_linf(K_fd, K_o)) > 1e-8
+    # switching back to finite differences restores the default path bit for bit
+    g.set_phi_scheme(0)
+    g_fd = make_gpu(prob, d_i=d_i, eta=1e-4)
+    assert np.array_equal(g.rhs(), g_fd.rhs())
+
+
+@pytest.mark.parametrize("name,steps", [("config1", 20), ("rotating-v0-12", 50), ("ragged-77x9x53", 30)])
+def test_spectral_steps_and_diagnostics_match_oracle(name, steps):
+    prob = SPEC_CASES[name]()
+    over = dict(phi_scheme=1, dt=0.5 * prob.dt)
+    o, g = make_oracle(prob, **over), make_gpu(prob, **over)
+    o.step(steps)
+    g.step(steps)
+    assert_close(g.get_state(), o.get_state(), STEP_TOL, f"{steps} RK4 steps, pseudo-spectral phi, {name}")
+    dg, do = g.diagnostics(), o.diagnostics()
+    for k in ("kinetic", "magnetic", "magnetic_pert", "magnetic_n1"):
+        assert abs(dg[k] - do[k]) <= 1e-12 * abs(do[k]), k
+    assert abs(dg["max_divB"] - do["max_divB"]) <= 1e-9 * do["max_divB"] + 1e-15
+
+
+def test_spectral_graph_and_errors():
+    from paper_1812_00525_b200 import clt
+    prob = inputs.make_problem(1)
+    g0 = make_gpu(prob, phi_scheme=1)
+    g0.step(3)
+    g1 = make_gpu(prob, phi_scheme=1)
+    g1.set_tuning(use_graph=1)
+    g1.step(2)
+    g1.step(1)
+    assert np.array_equal(g1.get_state(), g0.get_state())
+    g1.set_tuning(tile_z=12)
+    with pytest.raises(clt.CltError):
+        g1.step(1)
+    g1.set_tuning(tile_z=0)
+    g1.set_kernel_variant(1)
+    with pytest.raises(clt.CltError):
+        g1.rhs()
