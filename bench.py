@@ -170,7 +170,10 @@ def run_ours(args):
 
     prob = inputs.make_problem(args.config)
     cfg = prob.cfg
-    g = clt.Clt.from_config(cfg, prob.dt, device=f"cuda:{local}")
+    dt = prob.dt * args.dt_scale
+    g = clt.Clt.from_config(cfg, dt, device=f"cuda:{local}", d_i=args.d_i)
+    if args.phi_scheme:
+        g.set_phi_scheme(args.phi_scheme)
     if args.tile_z or args.phi_chunks or args.graph:
         g.set_tuning(args.tile_z, args.phi_chunks, args.graph)
     hU0 = torch.from_numpy(prob.U0).pin_memory()
@@ -245,8 +248,10 @@ def run_ours(args):
                 "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                 "traffic": args.traffic if args.traffic is not None else (profiled_traffic() if cfg.index == 4 else None),
                 "peak_source": peak_src + ", burst figure", "avg_launch_ms": ms_rhs / n_rhs,
-                "algorithmic_bytes_per_launch": bytes_per_launch, "share_of_step": ms_rhs / (ms_rhs + prof["ms_curl"]),
+                "algorithmic_bytes_per_launch": bytes_per_launch, "share_of_step": ms_rhs / (ms_rhs + prof["ms_curl"] + prof.get("ms_phi", 0.0)),
                 "per_stage": per_stage, "curl_kernel": curl,
+                "phi_prepass": ({"ms": prof["ms_phi"] / prof["n_phi"], "launches_per_step": prof["n_phi"] / args.steps}
+                                if prof.get("n_phi") else None),
                 "algorithmic_doubles_per_node": {"stage1": 19, "stage2": 35, "stage3": 27, "stage4": 35, "curl": 6,
                                                  "rk4_step": BYTES_PER_UPDATE // 8, "survey_textbook_schedule": 164},
                 "whole_step": {"GBps": BYTES_PER_UPDATE * cfg.interior / (ms_step * 1e-3) / 1e9,
@@ -265,7 +270,8 @@ def run_ours(args):
                                    f"seeded reference state + perturbations (BASELINE.json configs[{cfg.index - 1}])",
                        "parallelism": "replicas only" if world > 1 else "single GPU",
                        "l2": f"working set {g.workspace_bytes / 1e9:.2f} GB per replica, far larger than the 126 MB L2 (no flush needed)",
-                       "dt": prob.dt, "tile_z": args.tile_z, "phi_chunks": args.phi_chunks, "graph": args.graph,
+                       "dt": dt, "d_i": args.d_i, "phi_scheme": "pseudo-spectral" if args.phi_scheme else "fd4",
+                       "tile_z": args.tile_z, "phi_chunks": args.phi_chunks, "graph": args.graph,
                        "state_finite_after_run": bool(finite)},
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": state_bytes,
@@ -290,6 +296,9 @@ def main():
     ap.add_argument("--phi-chunks", dest="phi_chunks", type=int, default=0)
     ap.add_argument("--graph", type=int, default=0)
     ap.add_argument("--e2e-steps", dest="e2e_steps", type=int, default=3)
+    ap.add_argument("--d-i", dest="d_i", type=float, default=0.0, help="Hall term of eq (5) (NEXT-3); 0 = the measured config")
+    ap.add_argument("--phi-scheme", dest="phi_scheme", type=int, default=0, help="1 = pseudo-spectral phi scheme (NEXT-2)")
+    ap.add_argument("--dt-scale", dest="dt_scale", type=float, default=1.0, help="scales the recipe's CFL time step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--traffic", type=float, default=None,
                     help="dram bytes per launch of the dominant kernel from an ncu --set full capture (profiles/)")

@@ -25,7 +25,7 @@ struct clt_ctx {
     bool has_state, has_v0, hall;
     bool spectral;                 // pseudo-spectral phi scheme (clt_set_phi_scheme)
     double *spec, *spec_ctab;      // caller-provided scratch: SPEC_COUNT derivative fields + circulant weights
-    double sc1[SPEC_MAX_Q + 1], sc2[SPEC_MAX_Q + 1];
+
     int64_t step;
     double time;
     double dt;
@@ -211,12 +211,10 @@ int run_phi_pass(clt_ctx *ctx, int mode, const double *U)
     a.U = U; a.J1 = ctx->J1; a.tab = ctx->tab;
     a.out = ctx->spec; a.ctab = ctx->spec_ctab;
     a.mode = mode; a.hall = ctx->hall ? 1 : 0; a.has_v0 = ctx->has_v0 ? 1 : 0;
-    memcpy(a.c1, ctx->sc1, sizeof(a.c1));
-    memcpy(a.c2, ctx->sc2, sizeof(a.c2));
     const long pe = prof_begin(ctx, 6);
     CK(launch_phi_spectral(a, ctx->stream));
     prof_end(ctx, pe);
-    ctx->launches++;
+    ctx->launches += mode == 0 ? 1 : 2;
     return CLT_OK;
 }
 
@@ -554,7 +552,7 @@ int clt_step(clt_ctx *ctx, int n)
         }
         for (int s = 0; s < n; ++s) {
             CK(cudaGraphLaunch(ctx->graph_exec, ctx->stream));
-            ctx->launches += ctx->spectral ? 16 : 8;
+            ctx->launches += ctx->spectral ? 20 : 8;
         }
     } else {
         for (int s = 0; s < n; ++s) {
@@ -655,9 +653,6 @@ int clt_set_phi_scheme(clt_ctx *ctx, int scheme, void *d_scratch, size_t bytes)
         tabv[m] = (double)c1;
         tabv[SPEC_MAX_NPHI + m] = (double)c2;
     }
-    memset(ctx->sc1, 0, sizeof(ctx->sc1));
-    memset(ctx->sc2, 0, sizeof(ctx->sc2));
-    for (int m = 0; m <= SPEC_MAX_Q && m < N; ++m) { ctx->sc1[m] = tabv[m]; ctx->sc2[m] = tabv[SPEC_MAX_NPHI + m]; }
     const size_t fields_b = (size_t)SPEC_COUNT * carve(&ctx->grid).field_b;
     ctx->spec = (double *)d_scratch;
     ctx->spec_ctab = (double *)((char *)d_scratch + fields_b);

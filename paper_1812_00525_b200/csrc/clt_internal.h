@@ -86,7 +86,6 @@ enum SpecField {
     SPEC_COUNT = 14
 };
 constexpr int SPEC_MAX_NPHI = 256;
-constexpr int SPEC_MAX_Q = 32;       // register-resident lines: nphi in {16, 32, 64}
 
 // one phi pre-pass: mode 0 = before the curl (B_R, B_Z; p too when hall), 1 = before the fused RHS kernel
 // (rho, p, v: first and second derivative; E1_R, E1_Z: first derivative)
@@ -97,10 +96,8 @@ struct SpecArgs {
     const double *J1;     // 3 fields (+ G behind them when hall)
     const double *tab;
     double *out;          // SPEC_COUNT fields
-    const double *ctab;   // [2][SPEC_MAX_NPHI] circulant weights c1[m], c2[m] (device copy, generic path)
+    const double *ctab;   // [2][SPEC_MAX_NPHI] circulant weights c1[m] (antisymmetric in m), c2[m] (symmetric)
     int mode, hall, has_v0;
-    double c1[SPEC_MAX_Q + 1];   // c1[m], m = 0..Q   (antisymmetric: c1[N-m] = -c1[m])
-    double c2[SPEC_MAX_Q + 1];   // c2[m], m = 0..N/2 (symmetric)
 };
 
 struct DiagArgs {

@@ -1162,114 +1162,135 @@ int curl_tma_tile_z() { return CLT_CURL_TZ; }
 // NEXT-2: pseudo-spectral phi derivatives ("either 4th order finite difference or
 // pseudo-spectrum method can be used" in phi; reading R12).  A phi-global operator does not fit
 // the phi-marching sweeps, so the derivatives are formed by a pre-pass and read back by the SPEC variants of
-// the curl and fused RHS kernels.  One thread owns one (R, Z) line of one quantity: it loads the N = nphi
-// samples (coalesced across the warp in R), keeps them in registers (N in {16, 32, 64}; a local array for any
-// other N <= 256) and evaluates the circulant sums in their paired form
+// the curl and fused RHS kernels.  A CTA owns 32 neighbouring (R, Z) lines of one quantity: it stages their
+// N = nphi samples in shared memory (coalesced, perturbations formed first, H2) and evaluates the circulant sums
+// in their paired form
 //   d1_j = sum_{m=1..Q} c1[m] (f_{j+m} - f_{j-m}),   Q = floor((N-1)/2)
 //   d2_j = c2[0] f_j + sum_{m=1..Q} c2[m] (f_{j+m} + f_{j-m}) [+ c2[N/2] f_{j+N/2}, N even]
-// with the closed-form weights of the Fourier differentiation matrices (clt_api.cu).  Perturbations are
-// formed before differencing (H2).  FP64-bound: about N FP64 instructions per output value.
+// with the closed-form weights of the Fourier differentiation matrices (clt_api.cu).  A thread forms four
+// consecutive outputs of one line at a time from two sliding 4-wide register windows, so every step in m costs
+// two shared-memory loads for 8 (16 with second derivatives) FP64 operations: FP64-bound, any N <= 256.
 // ---------------------------------------------------------------------------------------------
-template <int NT>
-__global__ void __launch_bounds__(128) phi_spectral_kernel(const __grid_constant__ SpecArgs a)
+template <bool WANT2>
+__global__ void __launch_bounds__(512) phi_spectral_kernel(const __grid_constant__ SpecArgs a, int job_base)
 {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     const Layout &L = a.L;
-    const int N = NT > 0 ? NT : L.nphi;
-    const int i = 2 + blockIdx.x * 32 + threadIdx.x, k = 2 + blockIdx.y * 4 + threadIdx.y;
-    if (i > L.nR - 3 || k > L.nZ - 3) return;
-    const long long o2 = (long long)k * L.pR + (LP + i);
-    const int job = blockIdx.z;
-    constexpr int NV = NT > 0 ? NT : SPEC_MAX_NPHI;
-    double v[NV];
-    int out1 = -1, out2 = -1;       // output field of the first / second derivative
+    const int N = L.nphi;
+    double *sv = reinterpret_cast<double *>(smem_raw);        // [N][32] samples
+    double *sc1 = sv + (size_t)N * 32, *sc2 = sc1 + N;        // weights
+    const int tx = threadIdx.x, ty = threadIdx.y, TY = blockDim.y;
+    const int i = 2 + blockIdx.x * 32 + tx, k = 2 + blockIdx.y;
+    const bool valid = i <= L.nR - 3;
+    const long long o2 = (long long)k * L.pR + (LP + min(i, L.nR - 3));
+    const int job = job_base + blockIdx.z;
+    int out1, out2 = -1;       // output field of the first / second derivative
     if (a.mode == 0) {
         // before the curl: B1_R, B1_Z (and p1 for the Hall field)
         const int src = job == 0 ? 5 : (job == 1 ? 7 : 1);
         const int t0 = job == 0 ? T_B0R : (job == 1 ? T_B0Z : T_P0);
         out1 = job < 2 ? SP_DB + job : SP_D1 + 1;
         const double f0 = __ldg(a.tab + t0 * L.plane + o2);
-#pragma unroll
-        for (int j = 0; j < NV; ++j)
-            if (j < N) v[j] = __ldg(a.U + src * L.field + (long long)j * L.plane + o2) - f0;
+        for (int j = ty; j < N; j += TY) sv[j * 32 + tx] = __ldg(a.U + src * L.field + (long long)j * L.plane + o2) - f0;
     } else if (job < 5) {
         out1 = SP_D1 + job;
         out2 = SP_D2 + job;
         const int t0 = job == 0 ? T_RHO0 : (job == 1 ? T_P0 : T_V0R + (job - 2));
         const double f0 = (job < 2 || a.has_v0) ? __ldg(a.tab + t0 * L.plane + o2) : 0.0;
-#pragma unroll
-        for (int j = 0; j < NV; ++j)
-            if (j < N) v[j] = __ldg(a.U + job * L.field + (long long)j * L.plane + o2) - f0;
+        for (int j = ty; j < N; j += TY) sv[j * 32 + tx] = __ldg(a.U + job * L.field + (long long)j * L.plane + o2) - f0;
     } else {
         // E1_R (job 5) or E1_Z (job 6) = -(v x B)_c + eta J1_c (+ d_i G_c); the axisymmetric v0 x B0 drops out
         // of the paired differences exactly and is left out
         const int c = job == 5 ? 0 : 2;
         out1 = SP_DE + (job - 5);
-        const int ia = c == 0 ? 3 : 2, ib = c == 0 ? 7 : 6, ic2 = c == 0 ? 4 : 3, id = c == 0 ? 6 : 5;
         // (v x B)_R = v_phi B_Z - v_Z B_phi ; (v x B)_Z = v_R B_phi - v_phi B_R
-#pragma unroll
-        for (int j = 0; j < NV; ++j)
-            if (j < N) {
-                const long long g = (long long)j * L.plane + o2;
-                const double va = __ldg(a.U + ia * L.field + g), Bb = __ldg(a.U + ib * L.field + g);
-                const double vc = __ldg(a.U + ic2 * L.field + g), Bd = __ldg(a.U + id * L.field + g);
-                double e = a.ph.eta * __ldg(a.J1 + c * L.field + g) - (va * Bb - vc * Bd);
-                if (a.hall) e = fma(a.ph.d_i, __ldg(a.J1 + (3 + c) * L.field + g), e);
-                v[j] = e;
-            }
-    }
-    const int Q = (N - 1) / 2;
-    const bool even = (N & 1) == 0;
-    double *o1 = a.out + (long long)out1 * L.field + o2;
-    double *o2p = out2 >= 0 ? a.out + (long long)out2 * L.field + o2 : nullptr;
-    if (NT > 0) {
-#pragma unroll
-        for (int j = 0; j < NV; ++j) {
-            double s1 = 0.0, s2 = a.c2[0] * v[j];
-#pragma unroll
-            for (int m = 1; m <= (NV - 1) / 2; ++m) {
-                const double fp = v[(j + m) % NV], fm = v[(j - m + NV) % NV];
-                s1 = fma(a.c1[m], fp - fm, s1);
-                s2 = fma(a.c2[m], fp + fm, s2);
-            }
-            if ((NV & 1) == 0) s2 = fma(a.c2[NV / 2], v[(j + NV / 2) % NV], s2);
-            o1[(long long)j * L.plane] = s1;
-            if (o2p) o2p[(long long)j * L.plane] = s2;
+        const int ia = c == 0 ? 3 : 2, ib = c == 0 ? 7 : 6, ic2 = c == 0 ? 4 : 3, id = c == 0 ? 6 : 5;
+        for (int j = ty; j < N; j += TY) {
+            const long long g = (long long)j * L.plane + o2;
+            const double va = __ldg(a.U + ia * L.field + g), Bb = __ldg(a.U + ib * L.field + g);
+            const double vc = __ldg(a.U + ic2 * L.field + g), Bd = __ldg(a.U + id * L.field + g);
+            double e = a.ph.eta * __ldg(a.J1 + c * L.field + g) - (va * Bb - vc * Bd);
+            if (a.hall) e = fma(a.ph.d_i, __ldg(a.J1 + (3 + c) * L.field + g), e);
+            sv[j * 32 + tx] = e;
         }
-    } else {
-        const double *c1 = a.ctab, *c2 = a.ctab + SPEC_MAX_NPHI;
-        for (int j = 0; j < N; ++j) {
-            double s1 = 0.0, s2 = c2[0] * v[j];
-            for (int m = 1; m <= Q; ++m) {
-                int jp = j + m, jm = j - m;
-                if (jp >= N) jp -= N;
-                if (jm < 0) jm += N;
-                const double fp = v[jp], fm = v[jm];
-                s1 = fma(c1[m], fp - fm, s1);
-                s2 = fma(c2[m], fp + fm, s2);
+    }
+    for (int m = ty * 32 + tx; m < N; m += TY * 32) {
+        sc1[m] = a.ctab[m];
+        sc2[m] = a.ctab[SPEC_MAX_NPHI + m];
+    }
+    __syncthreads();
+
+    const int Q = (N - 1) / 2;
+    const bool even = (N & 1) == 0, want2 = WANT2 && out2 >= 0;
+    const double *v = sv + tx;
+    auto wrap = [N](int x) { return x >= N ? x - N : (x < 0 ? x + N : x); };
+    for (int j0 = 4 * ty; j0 < N; j0 += 4 * TY) {
+        double s1[4], s2[4], wa[4], wb[4];      // windows: wa[q] = f_{j0+q+m}, wb[q] = f_{j0+q-m}
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            s1[q] = 0.0;
+            s2[q] = WANT2 ? sc2[0] * v[wrap(j0 + q) * 32] : 0.0;
+            wa[q] = v[wrap(j0 + q + 1) * 32];
+            wb[q] = v[wrap(j0 + q - 1) * 32];
+        }
+        int pa = wrap(j0 + 5), pb = wrap(j0 - 2);
+#pragma unroll 4
+        for (int m = 1; m <= Q; ++m) {
+            const double c1 = sc1[m], c2 = sc2[m];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                s1[q] = fma(c1, wa[q] - wb[q], s1[q]);
+                if (WANT2) s2[q] = fma(c2, wa[q] + wb[q], s2[q]);
             }
-            if (even) {
-                int jh = j + N / 2;
-                if (jh >= N) jh -= N;
-                s2 = fma(c2[N / 2], v[jh], s2);
-            }
-            o1[(long long)j * L.plane] = s1;
-            if (o2p) o2p[(long long)j * L.plane] = s2;
+            wa[0] = wa[1]; wa[1] = wa[2]; wa[2] = wa[3]; wa[3] = v[pa * 32];
+            wb[3] = wb[2]; wb[2] = wb[1]; wb[1] = wb[0]; wb[0] = v[pb * 32];
+            pa = pa + 1 == N ? 0 : pa + 1;
+            pb = pb == 0 ? N - 1 : pb - 1;
+        }
+        if (WANT2 && even) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) s2[q] = fma(sc2[N / 2], v[wrap(wrap(j0 + q) + N / 2) * 32], s2[q]);
+        }
+        if (valid) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+                if (j0 + q < N) {
+                    const long long g = (long long)(j0 + q) * L.plane + o2;
+                    a.out[(long long)out1 * L.field + g] = s1[q];
+                    if (want2) a.out[(long long)out2 * L.field + g] = s2[q];
+                }
         }
     }
 }
 
+template <bool WANT2>
+static cudaError_t launch_phi_jobs(const SpecArgs &a, int job_base, int jobs, cudaStream_t s)
+{
+    static bool configured = false;
+    auto kern = phi_spectral_kernel<WANT2>;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)((SPEC_MAX_NPHI * 32 + 2 * SPEC_MAX_NPHI) * sizeof(double)));
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    const int N = a.L.nphi;
+    const int groups = (N + 3) / 4;
+    dim3 block(32, groups < 16 ? groups : 16, 1);
+    dim3 grid((a.L.nR - 4 + 31) / 32, a.L.nZ - 4, jobs);
+    const size_t smem = ((size_t)N * 32 + 2 * (size_t)N) * sizeof(double);
+    kern<<<grid, block, smem, s>>>(a, job_base);
+    return cudaGetLastError();
+}
+
+// mode 0: one launch (first derivatives of B1_R, B1_Z [, p1]); mode 1: two launches (the five fluid fields with
+// both derivatives; E1_R, E1_Z with first derivatives only)
 cudaError_t launch_phi_spectral(const SpecArgs &a, cudaStream_t s)
 {
-    const int jobs = a.mode == 0 ? (a.hall ? 3 : 2) : 7;
-    dim3 block(32, 4, 1);
-    dim3 grid((a.L.nR - 4 + 31) / 32, (a.L.nZ - 4 + 3) / 4, jobs);
-    switch (a.L.nphi) {
-    case 16: phi_spectral_kernel<16><<<grid, block, 0, s>>>(a); break;
-    case 32: phi_spectral_kernel<32><<<grid, block, 0, s>>>(a); break;
-    case 64: phi_spectral_kernel<64><<<grid, block, 0, s>>>(a); break;
-    default: phi_spectral_kernel<0><<<grid, block, 0, s>>>(a); break;
-    }
-    return cudaGetLastError();
+    if (a.mode == 0) return launch_phi_jobs<false>(a, 0, a.hall ? 3 : 2, s);
+    cudaError_t e = launch_phi_jobs<true>(a, 0, 5, s);
+    if (e != cudaSuccess) return e;
+    return launch_phi_jobs<false>(a, 5, 2, s);
 }
 
 // ---------------------------------------------------------------------------------------------
