@@ -137,6 +137,24 @@ int clt_hall_G(clt_ctx *ctx, double *G);
  * Asynchronous.                                                                                  */
 int clt_step(clt_ctx *ctx, int n);
 
+/* NEXT-4, slab decomposition [L127, L250-256, L337]: the pieces a caller needs to run one sub-domain per GPU and
+ * exchange ghost rows between RK stages (paper_1812_00525_b200/slab.py does exactly that).
+ * A sub-domain is an ordinary context whose grid is a Z-slab of the global grid with 4 ghost rows per cut; the
+ * kernels never write the two outer rows, recompute rows 2-3 (and nZ-4, nZ-3) from the ghost data, and the caller
+ * overwrites all 4 ghost rows after every stage.
+ *   clt_step_stage : stage = 1..4 of one RK4 step (curl + fused kernel), in order; stage 4 completes the step.
+ *                    The stage's output buffer is  1 (U_a), 2 (U_b), 1 (U_a), 0 (U^n)  for stage 1, 2, 3, 4.
+ *                    CLT_ESTATE if called out of order (clt_step is refused in the middle of a step).
+ *   clt_get_rows / clt_set_rows : rows k0 .. k0+nrows-1 of buffer 0 = U^n, 1 = U_a, 2 = U_b as a dense array
+ *                    double[8][nphi][nrows][nR] (host or device pointer; synchronous for host pointers).
+ *   clt_set_owned_rows : the rows the diagnostics sums / SETDT minimum run over (default 2 .. nZ-3) and the rows of
+ *                    max |div_c B| (default 4 .. nZ-5; first > last = none), so that slabs can be reduced without
+ *                    counting ghost rows twice.                                                          */
+int clt_step_stage(clt_ctx *ctx, int stage);
+int clt_get_rows(clt_ctx *ctx, int buffer, int k0, int nrows, double *dst);
+int clt_set_rows(clt_ctx *ctx, int buffer, int k0, int nrows, const double *src);
+int clt_set_owned_rows(clt_ctx *ctx, int k_first, int k_last, int deep_first, int deep_last);
+
 /* Changes the fixed time step (dt > 0, finite).                                                  */
 int clt_set_dt(clt_ctx *ctx, double dt);
 

@@ -43,7 +43,8 @@ class clt_profile(ctypes.Structure):
 
 # every symbol include/clt.h declares
 EXPORTS = ["clt_workspace_bytes", "clt_create", "clt_destroy", "clt_set_equilibrium", "clt_set_state", "clt_get_state",
-           "clt_rhs", "clt_curl_J1", "clt_hall_G", "clt_step", "clt_set_dt", "clt_diagnostics", "clt_suggest_dt", "clt_set_tuning",
+           "clt_rhs", "clt_curl_J1", "clt_hall_G", "clt_step", "clt_step_stage", "clt_get_rows", "clt_set_rows",
+           "clt_set_owned_rows", "clt_set_dt", "clt_diagnostics", "clt_suggest_dt", "clt_set_tuning",
            "clt_set_kernel_variant", "clt_spectral_workspace_bytes", "clt_set_phi_scheme", "clt_set_profiling", "clt_get_profile", "clt_launch_count", "clt_stream", "clt_strerror", "clt_last_cuda_error", "clt_version"]
 
 _lib = None
@@ -92,6 +93,13 @@ def load():
     L.clt_set_profiling.argtypes = [vp, i]
     L.clt_get_profile.restype = i
     L.clt_get_profile.argtypes = [vp, ctypes.POINTER(clt_profile)]
+    L.clt_step_stage.restype = i
+    L.clt_step_stage.argtypes = [vp, i]
+    for name in ("clt_get_rows", "clt_set_rows"):
+        getattr(L, name).restype = i
+        getattr(L, name).argtypes = [vp, i, i, i, vp]
+    L.clt_set_owned_rows.restype = i
+    L.clt_set_owned_rows.argtypes = [vp, i, i, i, i]
     L.clt_spectral_workspace_bytes.restype = ctypes.c_size_t
     L.clt_spectral_workspace_bytes.argtypes = [ctypes.POINTER(clt_grid)]
     L.clt_set_phi_scheme.restype = i
@@ -201,6 +209,20 @@ class Clt:
             out = np.empty((3,) + self.shape[1:])
         self._ck(self.L.clt_curl_J1(self.h, _addr(out)))
         return out
+
+    def step_stage(self, stage):
+        self._ck(self.L.clt_step_stage(self.h, int(stage)))
+
+    def get_rows(self, buffer, k0, nrows, out):
+        """out: numpy array or torch tensor (host or device), float64, dense [8][nphi][nrows][nR]."""
+        self._ck(self.L.clt_get_rows(self.h, int(buffer), int(k0), int(nrows), _addr(out)))
+        return out
+
+    def set_rows(self, buffer, k0, nrows, src):
+        self._ck(self.L.clt_set_rows(self.h, int(buffer), int(k0), int(nrows), _addr(src)))
+
+    def set_owned_rows(self, k_first, k_last, deep_first, deep_last):
+        self._ck(self.L.clt_set_owned_rows(self.h, int(k_first), int(k_last), int(deep_first), int(deep_last)))
 
     def hall_G(self, out=None):
         if out is None:

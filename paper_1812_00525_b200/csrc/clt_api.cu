@@ -23,6 +23,8 @@ struct clt_ctx {
     double *Un, *acc, *Ua, *Ub, *J1, *G, *tab, *Rtab, *invRtab, *cs, *partial, *result;
     int nblocks_diag;
     bool has_state, has_v0, hall;
+    int k_first, k_last, kd_first, kd_last;   // diagnostics row ranges (clt_set_owned_rows)
+    int next_stage;                // clt_step_stage: the stage expected next (1..4)
     bool spectral;                 // pseudo-spectral phi scheme (clt_set_phi_scheme)
     double *spec, *spec_ctab;      // caller-provided scratch: SPEC_COUNT derivative fields + circulant weights
 
@@ -295,18 +297,54 @@ int run_rhs(clt_ctx *ctx, int mode, const double *in, double *out, double a_next
 // a6: one classical RK4 step in the reduced-traffic accumulator form (clt_kernels.cu):
 //   s1: Ua = Un + dt/2 K1                          s2: Ub = Un + dt/2 K2, acc = Un + (Ua - Un)/3 + dt/3 K2
 //   s3: Ua = Un + dt K3                            s4: Un = acc + (Ua - Un)/3 + dt/6 K4
-int enqueue_step(clt_ctx *ctx)
+int enqueue_stage(clt_ctx *ctx, int stage)
 {
     const double dt = ctx->dt;
     int r;
-    if ((r = run_curl(ctx, ctx->Un))) return r;
-    if ((r = run_rhs(ctx, RHS_MODE_S1, ctx->Un, ctx->Ua, 0.5 * dt, 0.0))) return r;
-    if ((r = run_curl(ctx, ctx->Ua))) return r;
-    if ((r = run_rhs(ctx, RHS_MODE_S2, ctx->Ua, ctx->Ub, 0.5 * dt, dt / 3.0))) return r;
-    if ((r = run_curl(ctx, ctx->Ub))) return r;
-    if ((r = run_rhs(ctx, RHS_MODE_S3, ctx->Ub, ctx->Ua, dt, 0.0))) return r;
-    if ((r = run_curl(ctx, ctx->Ua))) return r;
-    if ((r = run_rhs(ctx, RHS_MODE_S4, ctx->Ua, ctx->Un, 0.0, dt / 6.0))) return r;
+    switch (stage) {
+    case 1:
+        if ((r = run_curl(ctx, ctx->Un))) return r;
+        return run_rhs(ctx, RHS_MODE_S1, ctx->Un, ctx->Ua, 0.5 * dt, 0.0);
+    case 2:
+        if ((r = run_curl(ctx, ctx->Ua))) return r;
+        return run_rhs(ctx, RHS_MODE_S2, ctx->Ua, ctx->Ub, 0.5 * dt, dt / 3.0);
+    case 3:
+        if ((r = run_curl(ctx, ctx->Ub))) return r;
+        return run_rhs(ctx, RHS_MODE_S3, ctx->Ub, ctx->Ua, dt, 0.0);
+    case 4:
+        if ((r = run_curl(ctx, ctx->Ua))) return r;
+        return run_rhs(ctx, RHS_MODE_S4, ctx->Ua, ctx->Un, 0.0, dt / 6.0);
+    default:
+        return CLT_EINVAL;
+    }
+}
+
+int enqueue_step(clt_ctx *ctx)
+{
+    for (int stage = 1; stage <= 4; ++stage) {
+        int r = enqueue_stage(ctx, stage);
+        if (r) return r;
+    }
+    return CLT_OK;
+}
+
+// rows k0 .. k0+nrows-1 of one 8-field buffer  <->  dense [8][nphi][nrows][nR]
+int copy_rows(clt_ctx *ctx, double *buf, int k0, int nrows, double *dense, bool to_dense)
+{
+    cudaMemcpy3DParms p;
+    memset(&p, 0, sizeof(p));
+    cudaPitchedPtr internal = make_cudaPitchedPtr(buf + (size_t)k0 * ctx->L.pR + LP, (size_t)ctx->L.pR * sizeof(double),
+                                                  (size_t)ctx->L.nR, (size_t)ctx->L.nZ);
+    cudaPitchedPtr user = make_cudaPitchedPtr(dense, (size_t)ctx->L.nR * sizeof(double), (size_t)ctx->L.nR, (size_t)nrows);
+    p.srcPtr = to_dense ? internal : user;
+    p.dstPtr = to_dense ? user : internal;
+    p.extent = make_cudaExtent((size_t)ctx->L.nR * sizeof(double), (size_t)nrows, (size_t)8 * ctx->L.nphi);
+    p.kind = cudaMemcpyDefault;
+    CK(cudaMemcpy3DAsync(&p, ctx->stream));
+    cudaPointerAttributes at;
+    cudaError_t e = cudaPointerGetAttributes(&at, dense);
+    if (e != cudaSuccess) { cudaGetLastError(); at.type = cudaMemoryTypeUnregistered; }
+    if (at.type != cudaMemoryTypeDevice) CK(cudaStreamSynchronize(ctx->stream));
     return CLT_OK;
 }
 
@@ -349,6 +387,8 @@ int clt_create(const clt_grid *grid, const clt_params *params, void *d_workspace
     ctx->L = make_layout(grid);
     ctx->stream = (cudaStream_t)cuda_stream;
     ctx->dt = params->dt;
+    ctx->k_first = 2; ctx->k_last = grid->nZ - 3; ctx->kd_first = 4; ctx->kd_last = grid->nZ - 5;
+    ctx->next_stage = 1;
     const double Lphi = grid->phi_extent == 0.0 ? 2.0 * M_PI : grid->phi_extent;
     const double dR = (grid->Rmax - grid->Rmin) / (double)(grid->nR - 1);
     const double dZ = (grid->Zmax - grid->Zmin) / (double)(grid->nZ - 1);
@@ -465,6 +505,7 @@ int clt_set_state(clt_ctx *ctx, const double *U)
     if (e != cudaSuccess) { cudaGetLastError(); at.type = cudaMemoryTypeUnregistered; }
     if (at.type != cudaMemoryTypeDevice) CK(cudaStreamSynchronize(ctx->stream));   // the caller may reuse host memory
     ctx->has_state = true;
+    ctx->next_stage = 1;
     ctx->step = 0;
     ctx->time = 0.0;
     return CLT_OK;
@@ -521,7 +562,7 @@ int clt_set_dt(clt_ctx *ctx, double dt)
 int clt_step(clt_ctx *ctx, int n)
 {
     if (!ctx || n < 0) return CLT_EINVAL;
-    if (!ctx->has_state) return CLT_ESTATE;
+    if (!ctx->has_state || ctx->next_stage != 1) return CLT_ESTATE;
     if (!(ctx->dt > 0.0)) return CLT_EINVAL;
     if (ctx->use_graph) {
         const bool stale = !ctx->graph_exec || ctx->graph_dt != ctx->dt || ctx->graph_tile_z != effective_tile_z(ctx)
@@ -573,6 +614,7 @@ static int run_diag(clt_ctx *ctx, double cfl, double out6[6])
     a.R = ctx->Rtab + LP; a.invR = ctx->invRtab + LP;
     a.cs = ctx->cs; a.partial = ctx->partial; a.cfl = cfl;
     a.spec_c1 = ctx->spectral ? ctx->spec_ctab : nullptr;
+    a.k_first = ctx->k_first; a.k_last = ctx->k_last; a.kd_first = ctx->kd_first; a.kd_last = ctx->kd_last;
     CK(launch_diag(a, ctx->nblocks_diag, ctx->result, ctx->stream));
     ctx->launches += 2;
     CK(cudaMemcpyAsync(out6, ctx->result, 6 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
@@ -660,6 +702,46 @@ int clt_set_phi_scheme(clt_ctx *ctx, int scheme, void *d_scratch, size_t bytes)
     CK(cudaMemcpyAsync(ctx->spec_ctab, tabv.data(), tabv.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
     ctx->spectral = true;
+    return CLT_OK;
+}
+
+int clt_step_stage(clt_ctx *ctx, int stage)
+{
+    if (!ctx || stage < 1 || stage > 4) return CLT_EINVAL;
+    if (!ctx->has_state || stage != ctx->next_stage) return CLT_ESTATE;
+    if (!(ctx->dt > 0.0)) return CLT_EINVAL;
+    int r = enqueue_stage(ctx, stage);
+    if (r) return r;
+    ctx->next_stage = stage == 4 ? 1 : stage + 1;
+    if (stage == 4) { ctx->step += 1; ctx->time += ctx->dt; }
+    return CLT_OK;
+}
+
+static double *stage_buffer(clt_ctx *ctx, int buffer)
+{
+    return buffer == 0 ? ctx->Un : (buffer == 1 ? ctx->Ua : (buffer == 2 ? ctx->Ub : nullptr));
+}
+
+int clt_get_rows(clt_ctx *ctx, int buffer, int k0, int nrows, double *dst)
+{
+    if (!ctx || !dst || nrows < 1 || k0 < 0 || k0 + nrows > ctx->L.nZ || !stage_buffer(ctx, buffer)) return CLT_EINVAL;
+    if (!ctx->has_state) return CLT_ESTATE;
+    return copy_rows(ctx, stage_buffer(ctx, buffer), k0, nrows, dst, true);
+}
+
+int clt_set_rows(clt_ctx *ctx, int buffer, int k0, int nrows, const double *src)
+{
+    if (!ctx || !src || nrows < 1 || k0 < 0 || k0 + nrows > ctx->L.nZ || !stage_buffer(ctx, buffer)) return CLT_EINVAL;
+    if (!ctx->has_state) return CLT_ESTATE;
+    return copy_rows(ctx, stage_buffer(ctx, buffer), k0, nrows, const_cast<double *>(src), false);
+}
+
+int clt_set_owned_rows(clt_ctx *ctx, int k_first, int k_last, int deep_first, int deep_last)
+{
+    if (!ctx) return CLT_EINVAL;
+    if (k_first < 2 || k_last > ctx->L.nZ - 3 || k_first > k_last) return CLT_EINVAL;
+    if (deep_first < 2 || deep_last > ctx->L.nZ - 3) return CLT_EINVAL;      // an empty deep range is allowed
+    ctx->k_first = k_first; ctx->k_last = k_last; ctx->kd_first = deep_first; ctx->kd_last = deep_last;
     return CLT_OK;
 }
 

@@ -111,6 +111,8 @@ struct DiagArgs {
     double *partial;      // [nblocks][6]
     double cfl;
     const double *spec_c1;   // non-null: pseudo-spectral d/dphi in div_c B, weights c1[0..nphi-1]
+    int k_first, k_last;     // rows the sums / the SETDT minimum run over (default 2 .. nZ-3; a slab's owned rows)
+    int kd_first, kd_last;   // rows of the max |div_c B| (default 4 .. nZ-5)
 };
 
 enum { RHS_MODE_K = 0, RHS_MODE_S1 = 1, RHS_MODE_S2 = 2, RHS_MODE_S3 = 3, RHS_MODE_S4 = 4 };

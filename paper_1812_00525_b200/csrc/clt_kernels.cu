@@ -1427,8 +1427,8 @@ __global__ void __launch_bounds__(DG_BX *DG_BY) diag_kernel(const __grid_constan
     const Layout &L = a.L;
     const Phys &ph = a.ph;
     const int i = 2 + blockIdx.x * DG_BX + threadIdx.x, k = 2 + blockIdx.y * DG_BY + threadIdx.y;
-    const bool valid = i <= L.nR - 3 && k <= L.nZ - 3;
-    const bool deep = i >= 4 && i <= L.nR - 5 && k >= 4 && k <= L.nZ - 5;
+    const bool valid = i <= L.nR - 3 && k >= a.k_first && k <= a.k_last;
+    const bool deep = i >= 4 && i <= L.nR - 5 && k >= a.kd_first && k <= a.kd_last;
     double ke = 0.0, me = 0.0, mep = 0.0, men1 = 0.0, mdiv = 0.0, mdt = 100.0;
     if (valid) {
         const long long o = (long long)k * L.pR + (LP + i);

@@ -336,3 +336,69 @@ def test_spectral_graph_and_errors():
     g1.set_kernel_variant(1)
     with pytest.raises(clt.CltError):
         g1.rhs()
+
+
+# ------------------------------------------------------------------------------ NEXT-4: Z-slab decomposition, L250-256
+def _single(prob, **over):
+    return make_gpu(prob, **over)
+
+
+@pytest.mark.parametrize("world", [2, 3])
+@pytest.mark.parametrize("variant", ["fd", "hall", "spectral"])
+def test_slab_decomposition_matches_single_domain_and_oracle(world, variant):
+    """Several sub-domain contexts in ONE process on one GPU (run one after the other, ghost rows handed over as
+    device tensors): same state as the undivided run (to round-off: a slab's dZ is recomputed from its own Zmin/Zmax)
+    and as the oracle."""
+    from paper_1812_00525_b200 import slab
+    prob = inputs.make_custom_problem(45, 8, 41, index=21, rotation=0.05 if variant == "fd" else 0.0)
+    kw = {"fd": {}, "hall": dict(d_i=0.03), "spectral": dict(phi_scheme=1)}[variant]
+    dt = prob.dt * (0.2 if variant == "hall" else 0.5)
+    steps = 12
+    grp = slab.SlabGroup(prob.cfg, dt, prob.U0, prob.U, world, **kw)
+    g = _single(prob, dt=dt, **kw)
+    o = make_oracle(prob, dt=dt, **kw)
+    d0 = grp.diagnostics()
+    ds = g.diagnostics()
+    for k in ("kinetic", "magnetic", "magnetic_pert", "magnetic_n1"):
+        assert abs(d0[k] - ds[k]) <= 1e-12 * abs(ds[k]), k
+    assert abs(d0["max_divB"] - ds["max_divB"]) <= 1e-9 * ds["max_divB"]
+    assert abs(grp.suggest_dt(0.5) - g.suggest_dt(0.5)) <= 1e-14
+    grp.step(steps)
+    g.step(steps)
+    o.step(steps)
+    U_s, U_g, U_o = grp.get_state(), g.get_state(), o.get_state()
+    assert_close(U_s, U_g, 1e-12, f"{world} slabs vs single domain ({variant})")
+    assert_close(U_s, U_o, STEP_TOL, f"{world} slabs vs oracle ({variant})")
+    d1 = grp.diagnostics()
+    dg = g.diagnostics()
+    assert d1["step"] == steps
+    for k in ("kinetic", "magnetic", "magnetic_pert", "magnetic_n1"):
+        assert abs(d1[k] - dg[k]) <= 1e-11 * abs(dg[k]), k
+    grp.close()
+
+
+def test_step_stage_order_and_rows_roundtrip():
+    from paper_1812_00525_b200 import clt
+    prob = inputs.make_problem(1)
+    g = make_gpu(prob)
+    ref = make_gpu(prob)
+    ref.step(1)
+    with pytest.raises(clt.CltError):
+        g.step_stage(2)                       # out of order
+    g.step_stage(1)
+    with pytest.raises(clt.CltError):
+        g.step(1)                             # refused in the middle of a step
+    for s in (2, 3, 4):
+        g.step_stage(s)
+    assert np.array_equal(g.get_state(), ref.get_state())      # four stages = one clt_step, bit for bit
+    assert g.diagnostics()["step"] == 1
+    c = prob.cfg
+    rows = np.empty((8, c.nphi, 5, c.nR))
+    g.get_rows(0, 7, 5, rows)
+    assert np.array_equal(rows, g.get_state()[:, :, 7:12])
+    g.set_rows(0, 9, 5, np.ascontiguousarray(rows * 2.0))
+    assert np.array_equal(g.get_state()[:, :, 9:14], rows * 2.0)
+    with pytest.raises(clt.CltError):
+        g.get_rows(3, 0, 1, rows)
+    with pytest.raises(clt.CltError):
+        g.get_rows(0, c.nZ - 2, 5, rows)
