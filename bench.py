@@ -21,6 +21,8 @@ import sys
 import threading
 import time
 
+import numpy as np
+
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
@@ -146,6 +148,58 @@ def run_reference(args):
             "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
+
+
+def run_slabs(args):
+    """NEXT-4 measurement: the same workload cut into Z-slabs (paper_1812_00525_b200/slab.py).  --slabs K with one
+    process = K sub-domain contexts on ONE GPU run one after the other (measures the cost of the decomposition itself:
+    redundant ghost-row work + pack/unpack, no link); under torchrun (--gpus N > 1) = one slab per rank, strong scaling,
+    ghost rows over NCCL.  Not the contract's default (north_star: replicas only)."""
+    import torch
+    import torch.distributed as dist
+    from paper_1812_00525_b200 import build as clt_build
+    from paper_1812_00525_b200 import inputs, replicas, slab
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        clt_build.build()
+    if world > 1:
+        dist.barrier()
+    prob = inputs.make_problem(args.config)
+    cfg = prob.cfg
+    nslabs = world if world > 1 else args.slabs
+    grp = slab.SlabGroup(cfg, prob.dt, prob.U0, prob.U, nslabs, devices=(f"cuda:{local}",), dist=dist if world > 1 else None,
+                         d_i=args.d_i, phi_scheme=args.phi_scheme)
+    grp.step(args.warmup)
+    replicas.barrier(f"cuda:{local}")
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    stream = grp.slabs[0].g.torch_stream
+    e0.record(stream)
+    grp.step(args.steps)
+    e1.record(stream)
+    replicas.barrier(f"cuda:{local}")
+    ms = e0.elapsed_time(e1)
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device=f"cuda:{local}")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    d = grp.diagnostics()
+    if rank == 0:
+        line = {"metric": METRIC, "value": cfg.interior * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong",
+                "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": {"workload": f"config {cfg.index}: {cfg.nR}x{cfg.nphi}x{cfg.nZ}, cut into {nslabs} Z-slabs with 4 ghost rows per cut",
+                           "parallelism": f"{nslabs} slabs, " + ("one per GPU, ghost rows over NCCL" if world > 1 else "in one process on one GPU"),
+                           "ghost_bytes_per_cut_per_step": 4 * 2 * 4 * 8 * cfg.nphi * cfg.nR * 8,
+                           "state_finite_after_run": bool(np.isfinite(d["kinetic"]) and np.isfinite(d["magnetic"]))},
+                "gpu_launches": sum(s.g.launch_count for s in grp.slabs)}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
 
 
 def run_ours(args):
@@ -298,6 +352,7 @@ def main():
     ap.add_argument("--e2e-steps", dest="e2e_steps", type=int, default=3)
     ap.add_argument("--d-i", dest="d_i", type=float, default=0.0, help="Hall term of eq (5) (NEXT-3); 0 = the measured config")
     ap.add_argument("--phi-scheme", dest="phi_scheme", type=int, default=0, help="1 = pseudo-spectral phi scheme (NEXT-2)")
+    ap.add_argument("--slabs", type=int, default=0, help="NEXT-4: cut the workload into K Z-slabs (see run_slabs)")
     ap.add_argument("--dt-scale", dest="dt_scale", type=float, default=1.0, help="scales the recipe's CFL time step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--traffic", type=float, default=None,
@@ -306,6 +361,8 @@ def main():
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         run_reference(args)
+    elif args.slabs > 1:
+        run_slabs(args)
     else:
         run_ours(args)
 
