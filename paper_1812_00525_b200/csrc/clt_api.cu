@@ -13,6 +13,11 @@
 
 using namespace clt;
 
+// L2 promotion of the TMA loads (measured choice)
+#ifndef CLT_L2_PROMO
+#define CLT_L2_PROMO CU_TENSOR_MAP_L2_PROMOTION_L2_256B
+#endif
+
 struct clt_ctx {
     clt_grid grid;
     clt_params par;
@@ -172,7 +177,7 @@ bool make_map(const clt_ctx *ctx, const double *base, int nfields, int tile_z, C
     const cuuint32_t box[4] = { 32 + 4, (cuuint32_t)tile_z + 4, 1, 1 };
     const cuuint32_t estr[4] = { 1, 1, 1, 1 };
     return enc(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, (void *)base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE)
+               CU_TENSOR_MAP_SWIZZLE_NONE, CLT_L2_PROMO, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE)
            == CUDA_SUCCESS;
 }
 int effective_chunks(const clt_ctx *ctx)

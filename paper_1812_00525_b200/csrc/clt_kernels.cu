@@ -206,6 +206,19 @@ __device__ __forceinline__ void rhs_point(const double *stg, int HT, const doubl
 // Identical to the textbook scheme up to rounding order.  Per node and step this moves 19 + 35 + 27 + 35
 // doubles through the fused kernel instead of 27 + 43 + 43 + 27.
 // ---------------------------------------------------------------------------------------------
+// output stores of the fused kernel: plain, or with the cache-streaming hint (CLT_STORE_CS, measured choice)
+#ifndef CLT_STORE_CS
+#define CLT_STORE_CS 0
+#endif
+__device__ __forceinline__ void st_out(double *p, double v)
+{
+#if CLT_STORE_CS
+    __stcs(p, v);
+#else
+    *p = v;
+#endif
+}
+
 struct EpiOperands {
     double un[8];   // U^n at the node
     double us[8];   // stage state at the node (S2: U_a of stage 1, S4: U_a of stage 3)
@@ -232,14 +245,14 @@ __device__ __forceinline__ void epilogue_store(const RhsArgs &a, long long g, lo
     for (int m = 0; m < 8; ++m) {
         const long long gm = m * field + g;
         if (MODE == RHS_MODE_K) {
-            a.out[gm] = K[m];
+            st_out(a.out + gm, K[m]);
         } else if (MODE == RHS_MODE_S1 || MODE == RHS_MODE_S3) {
-            a.out[gm] = fma(a.a_next, K[m], e.un[m]);
+            st_out(a.out + gm, fma(a.a_next, K[m], e.un[m]));
         } else if (MODE == RHS_MODE_S2) {
-            a.out[gm] = fma(a.a_next, K[m], e.un[m]);
-            a.acc[gm] = fma(a.b_acc, K[m], fma(e.us[m] - e.un[m], third, e.un[m]));
+            st_out(a.out + gm, fma(a.a_next, K[m], e.un[m]));
+            st_out(a.acc + gm, fma(a.b_acc, K[m], fma(e.us[m] - e.un[m], third, e.un[m])));
         } else {
-            a.out[gm] = fma(a.b_acc, K[m], fma(e.us[m] - e.un[m], third, e.ac[m]));
+            st_out(a.out + gm, fma(a.b_acc, K[m], fma(e.us[m] - e.un[m], third, e.ac[m])));
         }
     }
 }

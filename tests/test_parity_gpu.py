@@ -402,3 +402,32 @@ def test_step_stage_order_and_rows_roundtrip():
         g.get_rows(3, 0, 1, rows)
     with pytest.raises(clt.CltError):
         g.get_rows(0, c.nZ - 2, 5, rows)
+
+
+def test_kernels_never_write_outside_the_nodes():
+    """Bounds check of our own (compute-sanitizer is not available on this pool): clt_create zeroes the workspace; the
+    pad columns of all 38 padded fields (left of node 0, right of node nR-1) and the boundary layers of J1 / G must
+    still be zero after every kernel family has run, and the frozen layers of the RK buffers must hold the input."""
+    prob = inputs.make_custom_problem(45, 7, 37, index=23, rotation=0.03)
+    c = prob.cfg
+    g = make_gpu(prob, d_i=0.03, dt=0.2 * prob.dt)
+    g.rhs(); g.curl_J1(); g.hall_G(); g.step(3); g.diagnostics(); g.suggest_dt(0.5)
+    g.set_phi_scheme(1)
+    g.step(2); g.rhs()
+    LP = 14
+    pR = (LP + c.nR + 2 + 15) // 16 * 16
+    field = c.nphi * c.nZ * pR
+    import torch
+    torch.cuda.synchronize()
+    ws = g.workspace[:38 * field * 8].view(torch.float64).view(38, c.nphi, c.nZ, pR).cpu().numpy()
+    assert np.all(ws[..., :LP] == 0.0) and np.all(ws[..., LP + c.nR:] == 0.0)
+    nodes = ws[..., LP:LP + c.nR]
+    JG = nodes[32:38]                                     # J1 (3) and G (3): zero on the boundary layers
+    assert np.all(JG[:, :, :2] == 0) and np.all(JG[:, :, -2:] == 0) and np.all(JG[..., :2] == 0) and np.all(JG[..., -2:] == 0)
+    assert np.abs(JG[:, :, 2:-2, 2:-2]).max() > 0
+    for b in range(4):                                    # U^n, acc, U_a, U_b: frozen layers = the input state
+        buf = nodes[8 * b:8 * b + 8]
+        if b == 1:
+            continue                                      # acc's boundary layers are never read; they hold the copy too
+        assert np.array_equal(buf[:, :, :2], prob.U[:, :, :2]) and np.array_equal(buf[:, :, -2:], prob.U[:, :, -2:])
+        assert np.array_equal(buf[..., :2], prob.U[..., :2]) and np.array_equal(buf[..., -2:], prob.U[..., -2:])
