@@ -168,7 +168,9 @@ int clt_diagnostics(clt_ctx *ctx, clt_diag *out);
 int clt_suggest_dt(clt_ctx *ctx, double cfl, double *dt_out);
 
 /* phi scheme [L125: "either 4th order finite difference or pseudo-spectrum method can be used"].
- * scheme 0 (default) = 4th-order central differences; 1 = pseudo-spectral: every d/dphi and d2/dphi2 of the
+ * scheme 0 (default) = 4th-order central differences; 1 = pseudo-spectral (2 = the same, but its pre-pass uses a
+ * shared-memory radix-2 FFT instead of the circulant sums when nphi = 8, 16, .. 128; kept for A/B measurements,
+ * measured slower): every d/dphi and d2/dphi2 of the
  * path (curl, gradients, divergences, Laplacians, curl E, div_c B of the diagnostics) is the exact derivative
  * of the trigonometric interpolant through the nphi samples (Nyquist mode: first derivative 0, second
  * derivative -(pi nphi/L)^2; reading R12).  It needs a second caller-owned DEVICE scratch buffer of

@@ -30,6 +30,7 @@ struct clt_ctx {
     bool has_state, has_v0, hall;
     int k_first, k_last, kd_first, kd_last;   // diagnostics row ranges (clt_set_owned_rows)
     int next_stage;                // clt_step_stage: the stage expected next (1..4)
+    bool spec_fft;                 // pseudo-spectral pre-pass by FFT where nphi allows (scheme 2) instead of the circulant sums
     bool spectral;                 // pseudo-spectral phi scheme (clt_set_phi_scheme)
     double *spec, *spec_ctab;      // caller-provided scratch: SPEC_COUNT derivative fields + circulant weights
 
@@ -210,6 +211,14 @@ void prof_end(clt_ctx *ctx, long n)
     if (n >= 0) cudaEventRecord((*ctx->ev)[2 * n + 1], ctx->stream);
 }
 
+// kernels one phi pre-pass launches: the FFT variant does everything in one, the circulant sums need two in mode 1
+int phi_launches(const clt_ctx *ctx, int mode)
+{
+    const int N = ctx->L.nphi;
+    const bool fft = ctx->spec_fft && N >= 8 && N <= 128 && (N & (N - 1)) == 0;
+    return (mode == 0 || fft) ? 1 : 2;
+}
+
 // NEXT-2: pseudo-spectral phi derivatives of the stage state U (mode 0: what the curl needs, 1: what the RHS needs)
 int run_phi_pass(clt_ctx *ctx, int mode, const double *U)
 {
@@ -218,10 +227,11 @@ int run_phi_pass(clt_ctx *ctx, int mode, const double *U)
     a.U = U; a.J1 = ctx->J1; a.tab = ctx->tab;
     a.out = ctx->spec; a.ctab = ctx->spec_ctab;
     a.mode = mode; a.hall = ctx->hall ? 1 : 0; a.has_v0 = ctx->has_v0 ? 1 : 0;
+    a.use_fft = ctx->spec_fft ? 1 : 0;
     const long pe = prof_begin(ctx, 6);
     CK(launch_phi_spectral(a, ctx->stream));
     prof_end(ctx, pe);
-    ctx->launches += mode == 0 ? 1 : 2;
+    ctx->launches += phi_launches(ctx, mode);
     return CLT_OK;
 }
 
@@ -598,7 +608,7 @@ int clt_step(clt_ctx *ctx, int n)
         }
         for (int s = 0; s < n; ++s) {
             CK(cudaGraphLaunch(ctx->graph_exec, ctx->stream));
-            ctx->launches += ctx->spectral ? 20 : 8;
+            ctx->launches += ctx->spectral ? 8 + 4 * (phi_launches(ctx, 0) + phi_launches(ctx, 1)) : 8;
         }
     } else {
         for (int s = 0; s < n; ++s) {
@@ -659,12 +669,12 @@ int clt_suggest_dt(clt_ctx *ctx, double cfl, double *dt_out)
 size_t clt_spectral_workspace_bytes(const clt_grid *grid)
 {
     if (!grid_ok(grid) || grid->nphi > SPEC_MAX_NPHI) return 0;
-    return (size_t)SPEC_COUNT * carve(grid).field_b + align_up(2 * SPEC_MAX_NPHI * sizeof(double));
+    return (size_t)SPEC_COUNT * carve(grid).field_b + align_up(3 * SPEC_MAX_NPHI * sizeof(double));
 }
 
 int clt_set_phi_scheme(clt_ctx *ctx, int scheme, void *d_scratch, size_t bytes)
 {
-    if (!ctx || scheme < 0 || scheme > 1) return CLT_EINVAL;
+    if (!ctx || scheme < 0 || scheme > 2) return CLT_EINVAL;
     CK(cudaStreamSynchronize(ctx->stream));
     destroy_graph(ctx);
     if (scheme == 0) { ctx->spectral = false; ctx->spec = nullptr; ctx->spec_ctab = nullptr; return CLT_OK; }
@@ -683,7 +693,7 @@ int clt_set_phi_scheme(clt_ctx *ctx, int scheme, void *d_scratch, size_t bytes)
     const int N = ctx->grid.nphi;
     const long double PI = 3.141592653589793238462643383279502884L;
     const long double kap = 2.0L * PI / (long double)ctx->ph.Lphi;
-    std::vector<double> tabv(2 * SPEC_MAX_NPHI, 0.0);
+    std::vector<double> tabv(3 * SPEC_MAX_NPHI, 0.0);
     for (int m = 0; m < N; ++m) {
         long double c1, c2;
         const long double th = PI * (long double)m / (long double)N, sg = (m % 2) ? -1.0L : 1.0L;
@@ -700,6 +710,11 @@ int clt_set_phi_scheme(clt_ctx *ctx, int scheme, void *d_scratch, size_t bytes)
         tabv[m] = (double)c1;
         tabv[SPEC_MAX_NPHI + m] = (double)c2;
     }
+    if (N <= SPEC_MAX_NPHI)
+        for (int n = 0; n < N / 2 && n < SPEC_MAX_NPHI / 2; ++n) {      // FFT twiddles exp(2 pi i n/N)
+            tabv[2 * SPEC_MAX_NPHI + n] = (double)cosl(2.0L * PI * (long double)n / (long double)N);
+            tabv[2 * SPEC_MAX_NPHI + SPEC_MAX_NPHI / 2 + n] = (double)sinl(2.0L * PI * (long double)n / (long double)N);
+        }
     const size_t fields_b = (size_t)SPEC_COUNT * carve(&ctx->grid).field_b;
     ctx->spec = (double *)d_scratch;
     ctx->spec_ctab = (double *)((char *)d_scratch + fields_b);
@@ -707,6 +722,7 @@ int clt_set_phi_scheme(clt_ctx *ctx, int scheme, void *d_scratch, size_t bytes)
     CK(cudaMemcpyAsync(ctx->spec_ctab, tabv.data(), tabv.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
     ctx->spectral = true;
+    ctx->spec_fft = scheme == 2;
     return CLT_OK;
 }
 

@@ -96,8 +96,10 @@ struct SpecArgs {
     const double *J1;     // 3 fields (+ G behind them when hall)
     const double *tab;
     double *out;          // SPEC_COUNT fields
-    const double *ctab;   // [2][SPEC_MAX_NPHI] circulant weights c1[m] (antisymmetric in m), c2[m] (symmetric)
+    const double *ctab;   // [3][SPEC_MAX_NPHI]: circulant weights c1[m] (antisymmetric in m), c2[m] (symmetric), and the
+                          // FFT twiddles cos(2 pi n/N), n < N/2, then sin(2 pi n/N) at offset SPEC_MAX_NPHI/2
     int mode, hall, has_v0;
+    int use_fft;          // 1: FFT pre-pass where nphi allows (power of two, 8..128), 0: circulant sums always
 };
 
 struct DiagArgs {

@@ -1276,6 +1276,161 @@ __global__ void __launch_bounds__(512) phi_spectral_kernel(const __grid_constant
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// The same derivatives through a radix-2 Stockham FFT in shared memory, for nphi a power of two (8 .. 128): the
+// operator is diagonal in Fourier space, so two real lines f, g are packed as z = f + i g, transformed once,
+// multiplied by i kappa q (Nyquist: 0) resp. -(kappa q)^2, and transformed back: by linearity the real part is the
+// derivative of f and the imaginary part that of g -- no unpacking.  About 6x fewer FP64 operations than the
+// circulant sums at nphi = 64.  32 lines per CTA (one per lane: every shared access is conflict-free, twiddles are
+// broadcast), TY threads per line share the N/2 butterflies of a pass.
+// Line codes: 0..4 rho1, p1, v1_R, v1_phi, v1_Z (first and second derivative); 5, 6 E1_R, E1_Z; 7, 8 B1_R, B1_Z;
+// 9 p1 for the Hall field (first derivative only); -1 none.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void spec_line_setup(const SpecArgs &a, int code, long long o2, int &src, double &f0, int &out1,
+                                                int &out2)
+{
+    const Layout &L = a.L;
+    src = -1; f0 = 0.0; out1 = -1; out2 = -1;
+    if (code < 0) return;
+    if (code < 5) {
+        src = code; out1 = SP_D1 + code; out2 = SP_D2 + code;
+        const int t0 = code == 0 ? T_RHO0 : (code == 1 ? T_P0 : T_V0R + (code - 2));
+        f0 = (code < 2 || a.has_v0) ? __ldg(a.tab + t0 * L.plane + o2) : 0.0;
+    } else if (code < 7) {
+        out1 = SP_DE + (code - 5);
+    } else if (code < 9) {
+        src = code == 7 ? 5 : 7; out1 = SP_DB + (code - 7);
+        f0 = __ldg(a.tab + (code == 7 ? T_B0R : T_B0Z) * L.plane + o2);
+    } else {
+        src = 1; out1 = SP_D1 + 1;
+        f0 = __ldg(a.tab + T_P0 * L.plane + o2);
+    }
+}
+__device__ __forceinline__ double spec_line_value(const SpecArgs &a, int code, int src, double f0, long long g)
+{
+    const Layout &L = a.L;
+    if (code < 0) return 0.0;
+    if (code == 5 || code == 6) {
+        // E1_R = eta J_R - (v_phi B_Z - v_Z B_phi) ; E1_Z = eta J_Z - (v_R B_phi - v_phi B_R) (+ d_i G); v0 x B0 is axisymmetric
+        const int c = code == 5 ? 0 : 2;
+        const int ia = c == 0 ? 3 : 2, ib = c == 0 ? 7 : 6, ic2 = c == 0 ? 4 : 3, id = c == 0 ? 6 : 5;
+        const double va = __ldg(a.U + ia * L.field + g), Bb = __ldg(a.U + ib * L.field + g);
+        const double vc = __ldg(a.U + ic2 * L.field + g), Bd = __ldg(a.U + id * L.field + g);
+        double e = a.ph.eta * __ldg(a.J1 + c * L.field + g) - (va * Bb - vc * Bd);
+        if (a.hall) e = fma(a.ph.d_i, __ldg(a.J1 + (3 + c) * L.field + g), e);
+        return e;
+    }
+    return __ldg(a.U + src * L.field + g) - f0;
+}
+
+__global__ void __launch_bounds__(512) phi_fft_kernel(const __grid_constant__ SpecArgs a, int4 codesA, int4 codesB, int want2_mask)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const Layout &L = a.L;
+    const int N = L.nphi, H = N >> 1;
+    const int tx = threadIdx.x, ty = threadIdx.y, TY = blockDim.y;
+    const size_t BUF = (size_t)N * 32;
+    double *sm = reinterpret_cast<double *>(smem_raw);
+    struct Bufs { double *sm; size_t BUF; __device__ double *operator[](int b) const { return sm + 2 * (size_t)b * BUF; } };
+    const Bufs re{ sm, BUF }, im{ sm + BUF, BUF };      // three complex buffers: re[b], im[b]
+    double *twc = sm + 6 * BUF, *tws = twc + H;
+    const int i = 2 + blockIdx.x * 32 + tx, k = 2 + blockIdx.y;
+    const bool valid = i <= L.nR - 3;
+    const long long o2 = (long long)k * L.pR + (LP + min(i, L.nR - 3));
+    const int job = blockIdx.z;
+    const int codeA = job == 0 ? codesA.x : (job == 1 ? codesA.y : (job == 2 ? codesA.z : codesA.w));
+    const int codeB = job == 0 ? codesB.x : (job == 1 ? codesB.y : (job == 2 ? codesB.z : codesB.w));
+    const bool want2 = (want2_mask >> job) & 1;
+    int srcA, srcB, oA1, oA2, oB1, oB2;
+    double fA0, fB0;
+    spec_line_setup(a, codeA, o2, srcA, fA0, oA1, oA2);
+    spec_line_setup(a, codeB, o2, srcB, fB0, oB1, oB2);
+    for (int j = ty; j < N; j += TY) {
+        const long long g = (long long)j * L.plane + o2;
+        re[0][j * 32 + tx] = spec_line_value(a, codeA, srcA, fA0, g);
+        im[0][j * 32 + tx] = spec_line_value(a, codeB, srcB, fB0, g);
+    }
+    for (int n = ty * 32 + tx; n < H; n += TY * 32) {
+        twc[n] = a.ctab[2 * SPEC_MAX_NPHI + n];
+        tws[n] = a.ctab[2 * SPEC_MAX_NPHI + SPEC_MAX_NPHI / 2 + n];
+    }
+    __syncthreads();
+
+    // radix-2 Stockham passes from buffer `in` (destroyed) with scratch `other`; returns the buffer holding the result
+    auto fft = [&](int in, int other, double sign) {
+        for (int p = 1; p < N; p <<= 1) {
+            const int tstep = H / p;
+            for (int b = ty; b < H; b += TY) {
+                const int kk = b & (p - 1), j = ((b - kk) << 1) + kk;
+                const double c = twc[kk * tstep], s = sign * tws[kk * tstep];
+                const double xr = re[in][(b + H) * 32 + tx], xi = im[in][(b + H) * 32 + tx];
+                const double ur = re[in][b * 32 + tx], ui = im[in][b * 32 + tx];
+                const double vr = c * xr - s * xi, vi = c * xi + s * xr;
+                re[other][j * 32 + tx] = ur + vr;       im[other][j * 32 + tx] = ui + vi;
+                re[other][(j + p) * 32 + tx] = ur - vr; im[other][(j + p) * 32 + tx] = ui - vi;
+            }
+            __syncthreads();
+            const int t = in; in = other; other = t;
+        }
+        return in;
+    };
+    const int X = fft(0, 1, -1.0);            // spectrum of z
+    const int F1 = X == 0 ? 1 : 0, F2 = 2;    // the two free buffers
+    const double kap = 6.283185307179586476925286766559 / a.ph.Lphi, invN = 1.0 / (double)N;
+    for (int pass = 0; pass < (want2 ? 2 : 1); ++pass) {
+        for (int q = ty; q < N; q += TY) {
+            const double xr = re[X][q * 32 + tx], xi = im[X][q * 32 + tx];
+            if (pass == 0) {      // i kappa q, Nyquist mode dropped
+                const double m = kap * (double)(q < H ? q : (q == H ? 0 : q - N));
+                re[F1][q * 32 + tx] = -m * xi;
+                im[F1][q * 32 + tx] = m * xr;
+            } else {              // -(kappa q)^2, Nyquist mode kept
+                const double mq = kap * (double)(q <= H ? q : q - N), m = -mq * mq;
+                re[F1][q * 32 + tx] = m * xr;
+                im[F1][q * 32 + tx] = m * xi;
+            }
+        }
+        __syncthreads();
+        const int Y = fft(F1, F2, 1.0);
+        const int oA = pass == 0 ? oA1 : oA2, oB = pass == 0 ? oB1 : oB2;
+        if (valid)
+            for (int j = ty; j < N; j += TY) {
+                const long long g = (long long)j * L.plane + o2;
+                if (oA >= 0) a.out[(long long)oA * L.field + g] = re[Y][j * 32 + tx] * invN;
+                if (oB >= 0) a.out[(long long)oB * L.field + g] = im[Y][j * 32 + tx] * invN;
+            }
+        __syncthreads();
+    }
+}
+
+static bool phi_fft_supported(int N) { return N >= 8 && N <= 128 && (N & (N - 1)) == 0; }
+
+static cudaError_t launch_phi_fft(const SpecArgs &a, cudaStream_t s)
+{
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(phi_fft_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)((6 * 128 * 32 + 128) * sizeof(double)));
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    const int N = a.L.nphi;
+    int4 cA, cB;
+    int jobs, want2;
+    if (a.mode == 0) {
+        cA = make_int4(7, 9, -1, -1); cB = make_int4(8, -1, -1, -1);
+        jobs = a.hall ? 2 : 1; want2 = 0;
+    } else {
+        cA = make_int4(0, 2, 4, 6); cB = make_int4(1, 3, 5, -1);
+        jobs = 4; want2 = 0x7;
+    }
+    dim3 block(32, N / 2 < 16 ? N / 2 : 16, 1);
+    dim3 grid((a.L.nR - 4 + 31) / 32, a.L.nZ - 4, jobs);
+    const size_t smem = ((size_t)6 * N * 32 + N) * sizeof(double);
+    phi_fft_kernel<<<grid, block, smem, s>>>(a, cA, cB, want2);
+    return cudaGetLastError();
+}
+
 template <bool WANT2>
 static cudaError_t launch_phi_jobs(const SpecArgs &a, int job_base, int jobs, cudaStream_t s)
 {
@@ -1300,6 +1455,7 @@ static cudaError_t launch_phi_jobs(const SpecArgs &a, int job_base, int jobs, cu
 // both derivatives; E1_R, E1_Z with first derivatives only)
 cudaError_t launch_phi_spectral(const SpecArgs &a, cudaStream_t s)
 {
+    if (a.use_fft && phi_fft_supported(a.L.nphi)) return launch_phi_fft(a, s);
     if (a.mode == 0) return launch_phi_jobs<false>(a, 0, a.hall ? 3 : 2, s);
     cudaError_t e = launch_phi_jobs<true>(a, 0, 5, s);
     if (e != cudaSuccess) return e;

@@ -287,10 +287,12 @@ SPEC_CASES = {
 
 @pytest.mark.parametrize("name", list(SPEC_CASES))
 @pytest.mark.parametrize("d_i", [0.0, 0.05])
-def test_spectral_curl_and_rhs_match_oracle(name, d_i):
+@pytest.mark.parametrize("scheme", [1, 2])       # 1: circulant sums (default), 2: FFT pre-pass where nphi is a power of two
+def test_spectral_curl_and_rhs_match_oracle(name, d_i, scheme):
     prob = SPEC_CASES[name]()
     over = dict(phi_scheme=1, d_i=d_i, eta=1e-4)
-    o, g = make_oracle(prob, **over), make_gpu(prob, **over)
+    o = make_oracle(prob, **over)
+    g = make_gpu(prob, **dict(over, phi_scheme=scheme))
     assert_close(g.curl_J1(), o.curl_J1(prob.U), RHS_TOL, f"curl_J1, pseudo-spectral phi, {name}")
     if d_i:
         assert_close(g.hall_G(), o.hall_G(prob.U), RHS_TOL, f"Hall field, pseudo-spectral phi, {name}")
