@@ -107,8 +107,9 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def oracle_rate(grid, steps, warmup=0):
-    """Times the CPU oracle as it stands on a bounded sample (same recipe, smaller grid). Returns dict."""
+def oracle_rate(grid, steps, warmup=0, target_seconds=0.0):
+    """Times the CPU oracle as it stands on a bounded sample (same recipe, smaller grid). Returns dict.
+    target_seconds > 0: keep stepping (whole steps) until about that much CPU work has been timed."""
     import oracle as orc
     from paper_1812_00525_b200 import inputs
     nR, nphi, nZ = grid
@@ -123,6 +124,12 @@ def oracle_rate(grid, steps, warmup=0):
     t0 = time.perf_counter()
     o.step(steps)
     dt = time.perf_counter() - t0
+    if target_seconds > dt:
+        more = max(0, min(200, int(target_seconds / (dt / steps)) - steps))
+        if more:
+            o.step(more)
+            steps += more
+            dt = time.perf_counter() - t0
     cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
     return {"value": c.interior * steps / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": f"{steps} RK4 step(s) of the config-4 recipe on a {nR}x{nphi}x{nZ} grid ({c.interior} interior nodes), "
@@ -315,7 +322,7 @@ def run_ours(args):
     if world == 1 and not args.no_cpu_baseline:
         cores = os.cpu_count() or 1
         grid = (256, 32, 256) if cores >= 16 else (128, 16, 128)
-        cpu = oracle_rate(grid, 2 if cores >= 16 else 6)
+        cpu = oracle_rate(grid, 2, target_seconds=12.0)      # about 10-15 s of CPU work
         cpu = {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample")}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
