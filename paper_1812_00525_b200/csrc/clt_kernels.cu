@@ -27,6 +27,11 @@ namespace clt {
 #ifndef CLT_PF_DIST
 #define CLT_PF_DIST 1
 #endif
+// planes of L2-only TMA prefetch beyond the NRAW buffered ones in the fused RHS kernel (0 = none).  Measured at
+// 512x64x512: 1, 2 and 4 planes are all 3-4 % SLOWER than none (3.93 vs 3.79 ms per step), so it is off.
+#ifndef CLT_TMA_PF
+#define CLT_TMA_PF 0
+#endif
 // number of TMA raw buffers (planes in flight) of the default 32 x 8 tile
 #ifndef CLT_NRAW8
 #define CLT_NRAW8 2
@@ -552,6 +557,15 @@ __device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, i
         : "memory");
 }
 
+// TMA prefetch of a tile into L2 only (no shared memory, no barrier): used to run the HBM reads CLT_TMA_PF planes ahead
+// of the NRAW planes that have a shared-memory buffer
+__device__ __forceinline__ void tma_prefetch_4d(const CUtensorMap *map, int c0, int c1, int c2, int c3)
+{
+    asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global.tile [%0, {%1, %2, %3, %4}];" ::"l"(map), "r"(c0), "r"(c1), "r"(c2),
+                 "r"(c3)
+                 : "memory");
+}
+
 template <int TZ, int NRAW, int NF>
 struct RhsTmaSmem {
     static constexpr int HT = (TZ + 4) * SW;
@@ -628,6 +642,14 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
         for (int m = 0; m < 8; ++m) tma_load_4d(&S.raw[b][m][0], &tmU, LP + i0 - 2, k0 - 2, jw, m, &S.bar[b]);
 #pragma unroll
         for (int m = 0; m < NF - 8; ++m) tma_load_4d(&S.raw[b][8 + m][0], &tmJ, LP + i0 - 2, k0 - 2, jw, m, &S.bar[b]);
+    };
+    // L2-only prefetch of plane number n (HBM -> L2 ahead of the buffered loads)
+    auto prefetch_plane = [&](int n) {
+        const int jw = wrap_phi(ja - 2 + n, L.nphi);
+#pragma unroll
+        for (int m = 0; m < 8; ++m) tma_prefetch_4d(&tmU, LP + i0 - 2, k0 - 2, jw, m);
+#pragma unroll
+        for (int m = 0; m < NF - 8; ++m) tma_prefetch_4d(&tmJ, LP + i0 - 2, k0 - 2, jw, m);
     };
 
     // phi-invariant values of the own node and of the halo node, kept in registers for the whole sweep
@@ -722,13 +744,18 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
 
     // prologue: planes number 0 .. 3 (ja-2 .. ja+1); NRAW planes are kept in flight
     const int total = jb - ja + 4;
-    if (tid == 0)
+    if (tid == 0) {
         for (int n = 0; n < NRAW && n < total; ++n) issue(n);
+        for (int n = NRAW; n < NRAW + CLT_TMA_PF && n < total; ++n) prefetch_plane(n);
+    }
 #pragma unroll 1
     for (int n = 0; n < 4; ++n) {
         lead();
         __syncthreads();                 // every thread has read the raw tile
-        if (tid == 0 && n + NRAW < total) issue(n + NRAW);
+        if (tid == 0 && n + NRAW < total) {
+            issue(n + NRAW);
+            if (CLT_TMA_PF > 0 && n + NRAW + CLT_TMA_PF < total) prefetch_plane(n + NRAW + CLT_TMA_PF);
+        }
         advance();
     }
     unsigned ready_parity = 0;
@@ -757,7 +784,10 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
             // every thread has consumed the raw buffer of plane number j-ja+4: refill it NRAW planes ahead
             // (overlaps the rest of phase B and NRAW-1 more iterations)
             const int n = j - ja + 4 + NRAW;
-            if (tid == 0 && n < total) issue(n);
+            if (tid == 0 && n < total) {
+                issue(n);
+                if (CLT_TMA_PF > 0 && n + CLT_TMA_PF < total) prefetch_plane(n + CLT_TMA_PF);
+            }
         };
         if (SPLIT) {
             mbar_arrive(&S.ready);
