@@ -27,6 +27,12 @@ namespace clt {
 #ifndef CLT_PF_DIST
 #define CLT_PF_DIST 1
 #endif
+// distribution of the halo-node conversions over the warps of the fused RHS kernel (see rhs_tma_kernel).  Measured at
+// 512x64x512: dealing them out evenly (1) is 3 % SLOWER than packing them into the first warps (0): every warp then
+// pays the divergent halo path, and issue slots / shared-memory wavefronts, not the barrier skew, are what is short.
+#ifndef CLT_HALO_SPREAD
+#define CLT_HALO_SPREAD 0
+#endif
 // planes of L2-only TMA prefetch beyond the NRAW buffered ones in the fused RHS kernel (0 = none).  Measured at
 // 512x64x512: 1, 2 and 4 planes are all 3-4 % SLOWER than none (3.93 vs 3.79 ms per step), so it is off.
 #ifndef CLT_TMA_PF
@@ -604,17 +610,22 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
     const long long off2 = (long long)kc * L.pR + (LP + ic);
     const int cs = (ty + 2) * SW + (tx + 2);
 
+    // halo nodes: 4 full rows (Z halo) then 4 columns (R halo), NH in all.  CLT_HALO_SPREAD = 1 deals them out evenly over
+    // the warps (the first HPW lanes of every warp take one each) so that all warps carry the same conversion work and
+    // arrive at the plane barrier together; 0 = the first NH threads take them.
+    constexpr int HPW = (NH + TZ - 1) / TZ;
+    const int hid = CLT_HALO_SPREAD ? ((tid >> 5) * HPW + (tid & 31)) : tid;
+    const bool is_halo = CLT_HALO_SPREAD ? ((tid & 31) < HPW && hid < NH) : (tid < NH);
     int hx, hy;
-    if (tid < 4 * TR) {
-        const int r = tid / TR;
-        hx = tid % TR;
+    if (hid < 4 * TR) {
+        const int r = hid / TR;
+        hx = hid % TR;
         hy = (r < 2) ? r - 2 : TZ + (r - 2);
     } else {
-        const int t = tid - 4 * TR, c = t & 3;
+        const int t = hid - 4 * TR, c = t & 3;
         hy = t >> 2;
         hx = (c < 2) ? c - 2 : TR + (c - 2);
     }
-    const bool is_halo = tid < NH;
     const int hi = min(i0 + hx, L.nR - 1), hk = min(k0 + hy, L.nZ - 1);
     const long long hoff2 = (long long)hk * L.pR + (LP + hi);
     const int hs = (hy + 2) * SW + (hx + 2);
