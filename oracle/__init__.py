@@ -64,6 +64,9 @@ def lib():
             L.oracle_rhs_of.argtypes = [ctypes.c_void_p, _dp, _dp]
             L.oracle_rhs.argtypes = [ctypes.c_void_p, _dp]
             L.oracle_step.argtypes = [ctypes.c_void_p, ctypes.c_int]
+            L.oracle_step_cfl.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_double]
+            L.oracle_get_dt.restype = ctypes.c_double
+            L.oracle_get_dt.argtypes = [ctypes.c_void_p]
             L.oracle_diagnostics.argtypes = [ctypes.c_void_p, _dp]
             L.oracle_divB.argtypes = [ctypes.c_void_p, _dp, _dp]
             L.oracle_setdt.restype = ctypes.c_double
@@ -184,6 +187,14 @@ class Oracle:
 
     def step(self, n=1):
         self.L.oracle_step(self.h, int(n))
+
+    def step_cfl(self, n, cfl):
+        """n RK4 steps, each with dt = SETDT(cfl) of the state at its start (Fig. 3-4)."""
+        self.L.oracle_step_cfl(self.h, int(n), float(cfl))
+
+    @property
+    def dt(self):
+        return float(self.L.oracle_get_dt(self.h))
 
     def diagnostics(self):
         out = np.empty(5)

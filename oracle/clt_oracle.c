@@ -620,6 +620,19 @@ double oracle_setdt(const oracle *o, double cfl)
     return dt1;
 }
 
+/* NEXT-1, adaptive time step [L139: "the time step ... is calculated based on the latest rho, p, v, B"; Fig. 3:
+ * STEPON then SETDT inside the loop]: every RK4 step runs with dt = SETDT (Fig. 4) of the state at its start.  */
+void oracle_step_cfl(oracle *o, int n, double cfl)
+{
+    for (int s = 0; s < n; ++s) {
+        o->dt = oracle_setdt(o, cfl);
+        oracle_rk4(8 * o->N, o->U, o->dt, 1, mhd_rhs_thunk, o, o->K1, o->K2, o->K3, o->K4, o->Us);
+        o->step += 1;
+        o->time += o->dt;
+    }
+}
+double oracle_get_dt(const oracle *o) { return o->dt; }
+
 /* ---------------------------------------------------------------------------------------- */
 /* array-level wrappers around the point operators, so that the pins can exercise exactly the
  * functions the RHS uses.  which: 0 d1R, 1 d1P, 2 d1Z, 3 d2R, 4 d2P, 5 d2Z, 6 d1R_Rf,

@@ -13,6 +13,7 @@ P8 textbook RK4 order through oracle_rk4 and dt-halving on the MHD system   L125
 P10 SETDT closed form (Fig. 4), P11 diagnostics closed forms
 P12 Hall term of eq (5): exact whistler-type response with k*^2, momentum bracket identity, d_i = 0 reduction
     (and P3b runs with d_i != 0 against the sympy-derived continuous eq (5))
+P14 adaptive stepping (L139, Fig. 3): SETDT then one RK4 step, per step
 P13 pseudo-spectral phi scheme (L125): against numpy.fft, exact on every resolved mode, Alfven response with the
     physical wavenumber; P3b also runs with the spectral scheme
 """
@@ -619,3 +620,41 @@ def test_rounding_noise_floor_of_the_oracle_itself(tmp_path):
     assert max(physical) < 1e-9, physical
     assert per_component[3] > 1e-12, per_component      # v_phi: rounding alone already costs this much
     assert max(per_component[f] for f in (0, 1, 5, 6, 7)) < 1e-13
+
+
+# ----------------------------------------------------------------------------------------------- P14
+def test_P14_adaptive_stepping_is_setdt_then_rk4_per_step():
+    """NEXT-1 in the loop (L139, Fig. 3): oracle_step_cfl = for each step { dt = SETDT; one RK4 step }.  Composition of
+    the pinned pieces (P10 SETDT, P8 RK4), checked bit for bit against doing it by hand, plus a static state where
+    dt is the closed form of Fig. 4 and the time is n dt."""
+    prob = inputs.make_custom_problem(20, 8, 18, amplitude_scale=300.0)
+    c = prob.cfg
+    kw = dict(gamma=c.gamma, eta=c.eta, nu=c.nu, D=c.D, kappa=c.kappa)
+    a = orc.Oracle(c.nR, c.nphi, c.nZ, c.Rmin, c.Rmax, c.Zmin, c.Zmax, **kw)
+    b = orc.Oracle(c.nR, c.nphi, c.nZ, c.Rmin, c.Rmax, c.Zmin, c.Zmax, **kw)
+    for o in (a, b):
+        o.set_equilibrium(prob.U0)
+        o.set_state(prob.U)
+    a.step_cfl(4, 0.4)
+    t, dts = 0.0, []
+    for _ in range(4):
+        dt = b.setdt(0.4)
+        b.set_dt(dt)
+        b.step(1)
+        t += dt
+        dts.append(dt)
+    assert np.array_equal(a.get_state(), b.get_state())
+    assert a.time == t and a.dt == dts[-1] and a.step_count == 4
+    assert len(set(dts)) > 1                                   # the step really adapts on this state
+    # static state: U = U0 => K = 0, dt stays the closed form min over nodes of Fig. 4
+    U = np.repeat(prob.U0[:, None], c.nphi, axis=1)
+    a.set_state(U)
+    a.step_cfl(3, 0.5)
+    rho, p, B2 = U[0], U[1], (U[5:8] ** 2).sum(0)
+    cf = np.sqrt(np.abs(c.gamma * p / rho + B2 / rho))
+    dR, dZ = (c.Rmax - c.Rmin) / (c.nR - 1), (c.Zmax - c.Zmin) / (c.nZ - 1)
+    R = (c.Rmin + np.arange(c.nR) * dR)[None, None, :]
+    cand = np.minimum(np.minimum(dR, dZ), R * (2 * np.pi / c.nphi)) / cf * 0.5
+    want = cand[:, 2:-2, 2:-2].min()
+    assert abs(a.dt - want) <= 1e-14 * want and abs(a.time - 3 * a.dt) <= 1e-15
+    assert np.array_equal(a.get_state(), U)
