@@ -256,7 +256,10 @@ def run_ours(args):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     e0.record(g.torch_stream)
-    g.step(args.steps)
+    if args.adaptive:
+        g.step_cfl(args.steps, cfg.cfl)      # NEXT-1: dt = SETDT per step, on the device
+    else:
+        g.step(args.steps)
     e1.record(g.torch_stream)
     barrier()
     ms = e0.elapsed_time(e1)
@@ -332,6 +335,7 @@ def run_ours(args):
                        "parallelism": "replicas only" if world > 1 else "single GPU",
                        "l2": f"working set {g.workspace_bytes / 1e9:.2f} GB per replica, far larger than the 126 MB L2 (no flush needed)",
                        "dt": dt, "d_i": args.d_i, "phi_scheme": "pseudo-spectral" if args.phi_scheme else "fd4",
+                       "time_step": "SETDT every step (clt_step_cfl)" if args.adaptive else "fixed",
                        "tile_z": args.tile_z, "phi_chunks": args.phi_chunks, "graph": args.graph,
                        "state_finite_after_run": bool(finite)},
             "clocks": clocks,
@@ -359,6 +363,7 @@ def main():
     ap.add_argument("--e2e-steps", dest="e2e_steps", type=int, default=3)
     ap.add_argument("--d-i", dest="d_i", type=float, default=0.0, help="Hall term of eq (5) (NEXT-3); 0 = the measured config")
     ap.add_argument("--phi-scheme", dest="phi_scheme", type=int, default=0, help="1 = pseudo-spectral phi scheme (NEXT-2)")
+    ap.add_argument("--adaptive", action="store_true", help="NEXT-1: time clt_step_cfl (SETDT every step) instead of clt_step")
     ap.add_argument("--slabs", type=int, default=0, help="NEXT-4: cut the workload into K Z-slabs (see run_slabs)")
     ap.add_argument("--dt-scale", dest="dt_scale", type=float, default=1.0, help="scales the recipe's CFL time step")
     ap.add_argument("--no-cpu-baseline", action="store_true")

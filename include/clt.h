@@ -155,6 +155,15 @@ int clt_get_rows(clt_ctx *ctx, int buffer, int k0, int nrows, double *dst);
 int clt_set_rows(clt_ctx *ctx, int buffer, int k0, int nrows, const double *src);
 int clt_set_owned_rows(clt_ctx *ctx, int k_first, int k_last, int deep_first, int deep_last);
 
+/* NEXT-1 in the loop [L139 "the time step ... is calculated based on the latest rho, p, v, B"; Fig. 3: STEPON then
+ * SETDT; Fig. 4]: n RK4 steps, each with dt = SETDT(cfl) of the state at its start.  The time step lives on the
+ * device: the first one comes from the reduction kernel of clt_suggest_dt, the following ones are collected by the
+ * stage-4 epilogue of the fused kernel (no extra pass over the state, no host round trip per step).  cfl <= 0 means
+ * params.cfl.  Synchronises once at the end to report *dt_last (SETDT of the final state, i.e. the step the next call
+ * would start with) and *time_advanced (sum of the n steps); either pointer may be NULL.  params.dt is unchanged.
+ * Not available per slab (a global minimum would be needed between the slabs).                          */
+int clt_step_cfl(clt_ctx *ctx, int n, double cfl, double *dt_last, double *time_advanced);
+
 /* Changes the fixed time step (dt > 0, finite).                                                  */
 int clt_set_dt(clt_ctx *ctx, double dt);
 

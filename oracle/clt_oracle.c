@@ -50,6 +50,7 @@ typedef struct oracle {
     double gamma, eta, nu, D, kappa, dt;
     int phi_scheme;     /* 0 = 4th-order central differences in phi, 1 = pseudo-spectral (L125) */
     double *c1, *c2;    /* pseudo-spectral derivative weights, see oracle_set_phi_scheme         */
+    double last_dt;     /* dt of the last adaptive step (oracle_step_cfl); the fixed dt is untouched */
     double d_i;         /* ion inertial length of the Hall term in eq (5); 0 = resistive MHD */
     double *R;          /* R_i = Rmin + i*dR  (reading R1; hazard H1)           */
     double *Z;          /* Z_k = Zmin + k*dZ                                     */
@@ -625,13 +626,13 @@ double oracle_setdt(const oracle *o, double cfl)
 void oracle_step_cfl(oracle *o, int n, double cfl)
 {
     for (int s = 0; s < n; ++s) {
-        o->dt = oracle_setdt(o, cfl);
-        oracle_rk4(8 * o->N, o->U, o->dt, 1, mhd_rhs_thunk, o, o->K1, o->K2, o->K3, o->K4, o->Us);
+        o->last_dt = oracle_setdt(o, cfl);
+        oracle_rk4(8 * o->N, o->U, o->last_dt, 1, mhd_rhs_thunk, o, o->K1, o->K2, o->K3, o->K4, o->Us);
         o->step += 1;
-        o->time += o->dt;
+        o->time += o->last_dt;
     }
 }
-double oracle_get_dt(const oracle *o) { return o->dt; }
+double oracle_get_dt(const oracle *o) { return o->last_dt; }
 
 /* ---------------------------------------------------------------------------------------- */
 /* array-level wrappers around the point operators, so that the pins can exercise exactly the

@@ -43,7 +43,7 @@ class clt_profile(ctypes.Structure):
 
 # every symbol include/clt.h declares
 EXPORTS = ["clt_workspace_bytes", "clt_create", "clt_destroy", "clt_set_equilibrium", "clt_set_state", "clt_get_state",
-           "clt_rhs", "clt_curl_J1", "clt_hall_G", "clt_step", "clt_step_stage", "clt_get_rows", "clt_set_rows",
+           "clt_rhs", "clt_curl_J1", "clt_hall_G", "clt_step", "clt_step_cfl", "clt_step_stage", "clt_get_rows", "clt_set_rows",
            "clt_set_owned_rows", "clt_set_dt", "clt_diagnostics", "clt_suggest_dt", "clt_set_tuning",
            "clt_set_kernel_variant", "clt_spectral_workspace_bytes", "clt_set_phi_scheme", "clt_set_profiling", "clt_get_profile", "clt_launch_count", "clt_stream", "clt_strerror", "clt_last_cuda_error", "clt_version"]
 
@@ -93,6 +93,8 @@ def load():
     L.clt_set_profiling.argtypes = [vp, i]
     L.clt_get_profile.restype = i
     L.clt_get_profile.argtypes = [vp, ctypes.POINTER(clt_profile)]
+    L.clt_step_cfl.restype = i
+    L.clt_step_cfl.argtypes = [vp, i, d, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
     L.clt_step_stage.restype = i
     L.clt_step_stage.argtypes = [vp, i]
     for name in ("clt_get_rows", "clt_set_rows"):
@@ -209,6 +211,12 @@ class Clt:
             out = np.empty((3,) + self.shape[1:])
         self._ck(self.L.clt_curl_J1(self.h, _addr(out)))
         return out
+
+    def step_cfl(self, n, cfl=0.0):
+        """n adaptive RK4 steps (dt = SETDT per step, on the device); returns (dt of the next step, time advanced)."""
+        a, b = ctypes.c_double(), ctypes.c_double()
+        self._ck(self.L.clt_step_cfl(self.h, int(n), float(cfl), ctypes.byref(a), ctypes.byref(b)))
+        return a.value, b.value
 
     def step_stage(self, stage):
         self._ck(self.L.clt_step_stage(self.h, int(stage)))

@@ -29,6 +29,8 @@ struct clt_ctx {
     int nblocks_diag;
     bool has_state, has_v0, hall;
     int k_first, k_last, kd_first, kd_last;   // diagnostics row ranges (clt_set_owned_rows)
+    bool adaptive;                 // inside clt_step_cfl: stage coefficients from the device clock
+    double adaptive_cfl;
     int next_stage;                // clt_step_stage: the stage expected next (1..4)
     bool spec_fft;                 // pseudo-spectral pre-pass by FFT where nphi allows (scheme 2) instead of the circulant sums
     bool spectral;                 // pseudo-spectral phi scheme (clt_set_phi_scheme)
@@ -93,7 +95,7 @@ Carve carve(const clt_grid *g)
     c.cs_b = align_up((size_t)2 * g->nphi * sizeof(double));
     c.nblocks = diag_blocks(L);
     c.partial_b = align_up((size_t)c.nblocks * 6 * sizeof(double));
-    c.result_b = align_up(8 * sizeof(double));
+    c.result_b = align_up(32 * sizeof(double));     // 6 diagnostics + the device clock of clt_step_cfl (at +8) + dt minimum (at +16)
     c.total = 38 * c.field_b + T_COUNT * c.table_b + 2 * c.rtab_b + c.cs_b + c.partial_b + c.result_b;
     return c;
 }
@@ -283,6 +285,9 @@ int run_rhs(clt_ctx *ctx, int mode, const double *in, double *out, double a_next
     a.phi_chunks = effective_chunks(ctx);
     a.prefetch = 1;
     a.spec = ctx->spec;
+    a.coef = ctx->adaptive ? ctx->result + 8 : nullptr;
+    a.dtmin_bits = ctx->adaptive ? (unsigned long long *)(ctx->result + 16) : nullptr;
+    a.cfl = ctx->adaptive_cfl;
     const int tz = effective_tile_z(ctx);
     const bool tma = ctx->variant == 0 && rhs_tma_supports(tz, ctx->hall, ctx->spectral);
     if ((ctx->hall || ctx->spectral) && !tma) {
@@ -763,6 +768,50 @@ int clt_set_owned_rows(clt_ctx *ctx, int k_first, int k_last, int deep_first, in
     if (k_first < 2 || k_last > ctx->L.nZ - 3 || k_first > k_last) return CLT_EINVAL;
     if (deep_first < 2 || deep_last > ctx->L.nZ - 3) return CLT_EINVAL;      // an empty deep range is allowed
     ctx->k_first = k_first; ctx->k_last = k_last; ctx->kd_first = deep_first; ctx->kd_last = deep_last;
+    return CLT_OK;
+}
+
+int clt_step_cfl(clt_ctx *ctx, int n, double cfl, double *dt_last, double *time_advanced)
+{
+    if (!ctx || n < 0) return CLT_EINVAL;
+    if (!ctx->has_state || ctx->next_stage != 1) return CLT_ESTATE;
+    if (!(cfl > 0.0)) cfl = ctx->par.cfl;
+    if (!(cfl > 0.0) || !isfinite(cfl)) return CLT_EINVAL;
+    double *clock = ctx->result + 8;
+    unsigned long long *bits = (unsigned long long *)(ctx->result + 16);
+    double h[5] = { 0, 0, 0, 0, 0 };
+    if (n > 0) {
+        // dt of the first step: SETDT of the current state (the reduction kernel of clt_suggest_dt, no host round trip)
+        DiagArgs a;
+        a.L = ctx->L; a.ph = ctx->ph;
+        a.U = ctx->Un; a.tab = ctx->tab;
+        a.R = ctx->Rtab + LP; a.invR = ctx->invRtab + LP;
+        a.cs = ctx->cs; a.partial = ctx->partial; a.cfl = cfl;
+        a.spec_c1 = ctx->spectral ? ctx->spec_ctab : nullptr;
+        a.k_first = ctx->k_first; a.k_last = ctx->k_last; a.kd_first = ctx->kd_first; a.kd_last = ctx->kd_last;
+        CK(launch_diag(a, ctx->nblocks_diag, ctx->result, ctx->stream));
+        CK(launch_dt_commit(clock, bits, ctx->result, 1, ctx->stream));
+        ctx->launches += 3;
+        ctx->adaptive = true;
+        ctx->adaptive_cfl = cfl;
+        int r = CLT_OK;
+        for (int s = 0; s < n && r == CLT_OK; ++s) {
+            r = enqueue_step(ctx);                 // stage 4 collects the SETDT minimum of the new state
+            if (r == CLT_OK) {
+                cudaError_t e = launch_dt_commit(clock, bits, ctx->result, 0, ctx->stream);   // time += dt; dt = minimum
+                if (e != cudaSuccess) r = cuda_fail(ctx, e, "dt_commit_kernel");
+                ctx->launches++;
+            }
+        }
+        ctx->adaptive = false;
+        if (r) return r;
+        CK(cudaMemcpyAsync(h, clock, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
+        CK(cudaStreamSynchronize(ctx->stream));
+    }
+    ctx->step += n;
+    ctx->time += h[4];
+    if (dt_last) *dt_last = h[0];          // the SETDT value of the final state = the dt the next step would use
+    if (time_advanced) *time_advanced = h[4];
     return CLT_OK;
 }
 

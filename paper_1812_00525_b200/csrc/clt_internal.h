@@ -62,6 +62,11 @@ struct RhsArgs {
     int phi_chunks;       // number of chunks the phi range is split into (gridDim.z)
     int prefetch;         // issue L2 prefetch hints
     const double *spec;   // pseudo-spectral variant: SPEC_COUNT derivative fields (SpecField)
+    // adaptive stepping (clt_step_cfl): non-null = take the stage coefficients from the device clock
+    // { dt, dt/2, dt/3, dt/6, time } instead of a_next / b_acc; stage 4 folds the SETDT minimum into *dtmin_bits
+    const double *coef;
+    unsigned long long *dtmin_bits;
+    double cfl;
 };
 
 struct CurlArgs {
@@ -138,6 +143,7 @@ bool rhs_tma_supports(int tile_z, bool hall, bool spec);
 cudaError_t launch_curl_tma(const CurlArgs &a, const void *tmU, bool hall, bool spec, cudaStream_t s);
 cudaError_t launch_phi_spectral(const SpecArgs &a, cudaStream_t s);
 int curl_tma_tile_z();
+cudaError_t launch_dt_commit(double *clock, unsigned long long *dtmin_bits, const double *diag6, int init, cudaStream_t s);
 cudaError_t launch_diag(const DiagArgs &a, int nblocks, double *result6, cudaStream_t s);
 int diag_blocks(const Layout &L);
 cudaError_t configure_kernels();

@@ -247,25 +247,90 @@ __device__ __forceinline__ void epilogue_load(const RhsArgs &a, long long g, lon
         if (MODE == RHS_MODE_S4) e.ac[m] = ld(a.acc + gm);
     }
 }
+// SETDT of Fig. 4 [L180-215] at one node (shared by the diagnostics kernel and the stage-4 epilogue)
+__device__ __forceinline__ double setdt_node(const Phys &ph, double cfl, double Ri, double dRi, double rho, double p, double vR,
+                                             double vP, double vZ, double BR, double BP, double BZ)
+{
+    const double b2 = BR * BR + BP * BP + BZ * BZ;
+    const double cf = sqrt(fabs(ph.gamma * p / rho + b2 / rho));
+    const double dtx = dRi / ((fabs(vR) + cf) / cfl);
+    const double dtz = ph.dZ / ((fabs(vZ) + cf) / cfl);
+    const double dty = fabs(Ri * ph.dphi) / ((fabs(vP) + cf) / cfl);
+    return fmin(dty, fmin(dtx, dtz));
+}
+
+// Adaptive stepping (clt_step_cfl, NEXT-1): the stage coefficients come from device memory (a.coef = { dt, dt/2, dt/3,
+// dt/6 }, written by dt_commit_kernel) instead of the launch parameters, and stage 4 folds the SETDT minimum of the
+// new state into `rate` (Fig. 3: STEPON then SETDT, without a separate pass over the state).
 template <int MODE>
 __device__ __forceinline__ void epilogue_store(const RhsArgs &a, long long g, long long field, const EpiOperands &e,
-                                               const double (&K)[8])
+                                               const double (&K)[8], double iR, double &rate)
 {
     constexpr double third = 1.0 / 3.0;
+    double an = a.a_next, bn = a.b_acc;
+    if (a.coef) {
+        an = __ldg(a.coef + (MODE == RHS_MODE_S3 ? 0 : 1));
+        bn = __ldg(a.coef + (MODE == RHS_MODE_S2 ? 2 : 3));
+    }
+    double out[8];
 #pragma unroll
     for (int m = 0; m < 8; ++m) {
         const long long gm = m * field + g;
         if (MODE == RHS_MODE_K) {
             st_out(a.out + gm, K[m]);
         } else if (MODE == RHS_MODE_S1 || MODE == RHS_MODE_S3) {
-            st_out(a.out + gm, fma(a.a_next, K[m], e.un[m]));
+            st_out(a.out + gm, fma(an, K[m], e.un[m]));
         } else if (MODE == RHS_MODE_S2) {
-            st_out(a.out + gm, fma(a.a_next, K[m], e.un[m]));
-            st_out(a.acc + gm, fma(a.b_acc, K[m], fma(e.us[m] - e.un[m], third, e.un[m])));
+            st_out(a.out + gm, fma(an, K[m], e.un[m]));
+            st_out(a.acc + gm, fma(bn, K[m], fma(e.us[m] - e.un[m], third, e.un[m])));
         } else {
-            st_out(a.out + gm, fma(a.b_acc, K[m], fma(e.us[m] - e.un[m], third, e.ac[m])));
+            out[m] = fma(bn, K[m], fma(e.us[m] - e.un[m], third, e.ac[m]));
+            st_out(a.out + gm, out[m]);
         }
     }
+    if (MODE == RHS_MODE_S4 && a.dtmin_bits) {
+        // SETDT of Fig. 4 regrouped (rounding order only): dt = cfl / max_d (|v_d| + c) / h_d with the uniform spacings
+        // 1/dR = 12 cR1, 1/dZ = 12 cZ1, 1/(R dphi) = 12 cP1 / R; one division and one square root per node here, the
+        // division by the largest rate once per thread in dtmin_commit
+        const double b2 = out[5] * out[5] + out[6] * out[6] + out[7] * out[7];
+        const double cf = sqrt(fabs((a.ph.gamma * out[1] + b2) / out[0]));
+        const double rR = (fabs(out[2]) + cf) * a.ph.cR1, rP = (fabs(out[3]) + cf) * (a.ph.cP1 * iR),
+                     rZ = (fabs(out[4]) + cf) * a.ph.cZ1;
+        rate = fmax(rate, fmax(rP, fmax(rR, rZ)));
+    }
+}
+
+// end of a stage-4 kernel: this thread's largest signal rate -> its SETDT value -> device-wide minimum (positive doubles
+// order like their bit patterns)
+__device__ __forceinline__ void dtmin_commit(const RhsArgs &a, double rate)
+{
+    if (!a.dtmin_bits) return;
+    double dtmin = rate > 0.0 ? a.cfl / (12.0 * rate) : 100.0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) dtmin = fmin(dtmin, __shfl_xor_sync(0xffffffffu, dtmin, o));
+    if ((threadIdx.x & 31) == 0) atomicMin(a.dtmin_bits, (unsigned long long)__double_as_longlong(dtmin));
+}
+
+// one thread: opens (init = 1: dt from the SETDT reduction `diag6[5]`, time = 0) or advances (time += dt just used,
+// dt = the minimum stage 4 collected) the device-side clock of clt_step_cfl.  clock = { dt, dt/2, dt/3, dt/6, time }
+__global__ void dt_commit_kernel(double *clock, unsigned long long *dtmin_bits, const double *diag6, int init)
+{
+    double dt;
+    if (init) {
+        dt = diag6[5];
+        clock[4] = 0.0;
+    } else {
+        clock[4] += clock[0];
+        dt = fmin(100.0, __longlong_as_double((long long)*dtmin_bits));
+    }
+    clock[0] = dt; clock[1] = 0.5 * dt; clock[2] = dt / 3.0; clock[3] = dt / 6.0;
+    *dtmin_bits = (unsigned long long)__double_as_longlong(100.0);      // Fig. 4: DT1 starts at 100
+}
+
+cudaError_t launch_dt_commit(double *clock, unsigned long long *dtmin_bits, const double *diag6, int init, cudaStream_t s)
+{
+    dt_commit_kernel<<<1, 1, 0, s>>>(clock, dtmin_bits, diag6, init);
+    return cudaGetLastError();
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -394,6 +459,7 @@ __global__ void __launch_bounds__(TR *TZ, (TZ <= 8 ? 2 : 1)) rhs_kernel(const __
 
     const double iR = __ldg(a.invR + ic);
     const double iR2 = iR * iR;
+    double rate = 0.0;           // largest signal rate (|v_d| + c)/(12 h_d) at this thread's nodes (stage 4 of clt_step_cfl)
 
 #pragma unroll 1
     for (int j = ja; j < jb; ++j) {
@@ -451,10 +517,11 @@ __global__ void __launch_bounds__(TR *TZ, (TZ <= 8 ? 2 : 1)) rhs_kernel(const __
             const long long g = (long long)jw * L.plane + off2;
             EpiOperands eo;
             epilogue_load<MODE>(a, g, L.field, eo, [](const double *p) { return __ldg(p); });
-            epilogue_store<MODE>(a, g, L.field, eo, K);
+            epilogue_store<MODE>(a, g, L.field, eo, K, iR, rate);
         }
         advance();
     }
+    if (MODE == RHS_MODE_S4) dtmin_commit(a, rate);
 }
 
 template <int TZ, int MODE, bool V0>
@@ -773,6 +840,7 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
 
     const double iR = __ldg(a.invR + ic);
     const double iR2 = iR * iR;
+    double rate = 0.0;           // largest signal rate (|v_d| + c)/(12 h_d) at this thread's nodes (stage 4 of clt_step_cfl)
 
 #pragma unroll 1
     for (int j = ja; j < jb; ++j) {
@@ -838,9 +906,10 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
         ready_parity ^= 1u;
 
         // ---- a6: RK4 stage combine in the epilogue (L125, L139) --------------------------------
-        if (valid) epilogue_store<MODE>(a, g, L.field, eo, K);
+        if (valid) epilogue_store<MODE>(a, g, L.field, eo, K, iR, rate);
         advance();
     }
+    if (MODE == RHS_MODE_S4) dtmin_commit(a, rate);
 }
 
 template <int TZ, int NRAW, int MODE, bool V0, bool HALL, bool SPEC>
@@ -1660,11 +1729,7 @@ __global__ void __launch_bounds__(DG_BX *DG_BY) diag_kernel(const __grid_constan
 #pragma unroll
             for (int d = 0; d < 3; ++d) { fa[d] += b1[d] * c; fb[d] += b1[d] * s; }
             // SETDT, Fig. 4
-            const double cf = sqrt(fabs(ph.gamma * p / rho + b2 / rho));
-            const double dtx = dRi / ((fabs(vR) + cf) / a.cfl);
-            const double dtz = ph.dZ / ((fabs(vZ) + cf) / a.cfl);
-            const double dty = fabs(Ri * ph.dphi) / ((fabs(vP) + cf) / a.cfl);
-            mdt = fmin(mdt, fmin(dty, fmin(dtx, dtz)));
+            mdt = fmin(mdt, setdt_node(ph, a.cfl, Ri, dRi, rho, p, vR, vP, vZ, BR, BP, BZ));
             if (deep) {
                 // div_c B = d_R(R B_R)/R + d_phi B_phi / R + d_Z B_Z
                 const double *br = a.U + 5 * L.field + g, *bz = a.U + 7 * L.field + g;

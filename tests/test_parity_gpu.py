@@ -433,3 +433,29 @@ def test_kernels_never_write_outside_the_nodes():
             continue                                      # acc's boundary layers are never read; they hold the copy too
         assert np.array_equal(buf[:, :, :2], prob.U[:, :, :2]) and np.array_equal(buf[:, :, -2:], prob.U[:, :, -2:])
         assert np.array_equal(buf[..., :2], prob.U[..., :2]) and np.array_equal(buf[..., -2:], prob.U[..., -2:])
+
+
+# ------------------------------------------------------------------------------ NEXT-1 in the loop: clt_step_cfl
+@pytest.mark.parametrize("name,variant", [("big-amplitude", 0), ("ragged-77x9x53", 0), ("rotating-v0", 1), ("config1", 0)])
+def test_adaptive_steps_match_oracle(name, variant):
+    prob = _problems()[name]()
+    amp = dict(amplitude_scale=300.0) if name == "config1" else {}
+    if amp:
+        prob = inputs.make_custom_problem(32, 16, 32, index=1, **amp)
+    o, g = make_oracle(prob), make_gpu(prob)
+    g.set_kernel_variant(variant)
+    steps = 25
+    o.step_cfl(steps, 0.4)
+    dt_next, advanced = g.step_cfl(steps, 0.4)
+    assert_close(g.get_state(), o.get_state(), STEP_TOL, f"{steps} adaptive RK4 steps {name}")
+    assert abs(advanced - o.time) <= 1e-12 * o.time
+    assert abs(dt_next - o.setdt(0.4)) <= 1e-12 * dt_next
+    d = g.diagnostics()
+    assert d["step"] == steps and abs(d["time"] - o.time) <= 1e-12 * o.time
+    # a second call continues from the device state; fixed-dt stepping is untouched by the adaptive call
+    o.step_cfl(3, 0.4)
+    g.step_cfl(3, 0.4)
+    o.step(2)
+    g.step(2)
+    assert_close(g.get_state(), o.get_state(), STEP_TOL, f"adaptive then fixed steps {name}")
+    assert g.step_cfl(0, 0.4) == (0.0, 0.0)
