@@ -459,3 +459,39 @@ def test_adaptive_steps_match_oracle(name, variant):
     g.step(2)
     assert_close(g.get_state(), o.get_state(), STEP_TOL, f"adaptive then fixed steps {name}")
     assert g.step_cfl(0, 0.4) == (0.0, 0.0)
+
+
+# ------------------------------------------------------------------------------ more shapes: sector torus, shifted box, many planes
+EDGE_CASES = {
+    "sector-torus": lambda: inputs.make_custom_problem(40, 10, 30, index=41, phi_extent=2 * np.pi / 3),
+    "shifted-box": lambda: inputs.make_custom_problem(50, 8, 26, index=42, Rmin=0.5, Rmax=1.7, Zmin=0.2, Zmax=1.0),
+    "many-planes-144": lambda: inputs.make_custom_problem(20, 144, 13, index=43, amplitude_scale=20.0),
+    "wide-R-300": lambda: inputs.make_custom_problem(300, 6, 12, index=44),
+    "tall-Z-257": lambda: inputs.make_custom_problem(12, 6, 257, index=45),
+}
+
+
+@pytest.mark.parametrize("name", list(EDGE_CASES))
+@pytest.mark.parametrize("phi_scheme", [0, 1])
+def test_edge_shapes_rhs_and_steps_match_oracle(name, phi_scheme):
+    prob = EDGE_CASES[name]()
+    over = dict(phi_scheme=phi_scheme, dt=0.5 * prob.dt)
+    o, g = make_oracle(prob, **over), make_gpu(prob, **over)
+    assert_close(g.curl_J1(), o.curl_J1(prob.U), RHS_TOL, f"curl {name}")
+    assert_close(g.rhs(), o.rhs(), RHS_TOL, f"rhs {name} phi_scheme={phi_scheme}")
+    o.step(10)
+    g.step(10)
+    assert_close(g.get_state(), o.get_state(), STEP_TOL, f"10 steps {name} phi_scheme={phi_scheme}")
+    dg, do = g.diagnostics(), o.diagnostics()
+    for k in ("kinetic", "magnetic", "magnetic_pert", "magnetic_n1"):
+        assert abs(dg[k] - do[k]) <= 1e-12 * abs(do[k]), (name, k)
+    assert abs(g.suggest_dt(0.5) - o.setdt(0.5)) <= 1e-14 * o.setdt(0.5)
+
+
+def test_spectral_scheme_rejects_more_than_256_planes():
+    from paper_1812_00525_b200 import clt
+    prob = inputs.make_custom_problem(12, 260, 10, index=46)
+    g = make_gpu(prob)
+    assert_close(g.rhs(), make_oracle(prob).rhs(), RHS_TOL, "rhs with 260 planes (finite differences)")
+    with pytest.raises(clt.CltError):
+        g.set_phi_scheme(1)
