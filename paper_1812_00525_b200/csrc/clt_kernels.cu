@@ -33,6 +33,11 @@ namespace clt {
 #ifndef CLT_HALO_SPREAD
 #define CLT_HALO_SPREAD 0
 #endif
+// epilogue operands that equal the stage state at the own node: rebuild rho, p, v from the phi pipeline (1) or read all
+// eight fields again (0)
+#ifndef CLT_EPI_OWN
+#define CLT_EPI_OWN 1
+#endif
 // planes of L2-only TMA prefetch beyond the NRAW buffered ones in the fused RHS kernel (0 = none).  Measured at
 // 512x64x512: 1, 2 and 4 planes are all 3-4 % SLOWER than none (3.93 vs 3.79 ms per step), so it is off.
 #ifndef CLT_TMA_PF
@@ -235,15 +240,19 @@ struct EpiOperands {
     double us[8];   // stage state at the node (S2: U_a of stage 1, S4: U_a of stage 3)
     double ac[8];   // accumulator (S4)
 };
-template <int MODE, class Load>
-__device__ __forceinline__ void epilogue_load(const RhsArgs &a, long long g, long long field, EpiOperands &e, Load &&ld)
+// NOWN > 0: the caller still holds the first NOWN fields of the stage state at this node (own[m]; rho, p[, v]
+// rebuilt as perturbation + reference value, exact whenever the perturbation was formed exactly) and they are
+// taken from there instead of being read again.
+template <int MODE, int NOWN, class Load>
+__device__ __forceinline__ void epilogue_load(const RhsArgs &a, long long g, long long field, EpiOperands &e, Load &&ld,
+                                              const double *own = nullptr)
 {
 #pragma unroll
     for (int m = 0; m < 8; ++m) {
         const long long gm = m * field + g;
-        if (MODE == RHS_MODE_S1) e.un[m] = ld(a.in + gm);
+        if (MODE == RHS_MODE_S1) e.un[m] = (m < NOWN) ? own[m] : ld(a.in + gm);
         if (MODE == RHS_MODE_S2 || MODE == RHS_MODE_S3 || MODE == RHS_MODE_S4) e.un[m] = ld(a.Un + gm);
-        if (MODE == RHS_MODE_S2 || MODE == RHS_MODE_S4) e.us[m] = ld(a.in + gm);
+        if (MODE == RHS_MODE_S2 || MODE == RHS_MODE_S4) e.us[m] = (m < NOWN) ? own[m] : ld(a.in + gm);
         if (MODE == RHS_MODE_S4) e.ac[m] = ld(a.acc + gm);
     }
 }
@@ -516,7 +525,7 @@ __global__ void __launch_bounds__(TR *TZ, (TZ <= 8 ? 2 : 1)) rhs_kernel(const __
         if (valid) {
             const long long g = (long long)jw * L.plane + off2;
             EpiOperands eo;
-            epilogue_load<MODE>(a, g, L.field, eo, [](const double *p) { return __ldg(p); });
+            epilogue_load<MODE, 0>(a, g, L.field, eo, [](const double *p) { return __ldg(p); });
             epilogue_store<MODE>(a, g, L.field, eo, K, iR, rate);
         }
         advance();
@@ -878,7 +887,10 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
         // ---- a6 inputs: U^n / stage state / acc of this node, requested now so that they arrive during phase B ---
         const long long g = (long long)j * L.plane + off2;
         EpiOperands eo;
-        epilogue_load<MODE>(a, g, L.field, eo, [](const double *p) { return ld_stream(p); });
+        // rho, p (and v when the reference state is static) of the centre plane are still in the phi pipeline
+        constexpr int NOWN = CLT_EPI_OWN ? (V0 ? 2 : 5) : 0;
+        const double own[5] = { q[2][0] + ct.rho0, q[2][1] + ct.p0, q[2][2], q[2][3], q[2][4] };
+        epilogue_load<MODE, NOWN>(a, g, L.field, eo, [](const double *p) { return ld_stream(p); }, own);
 
         // ---- phase B: K at (i, k, j) -----------------------------------------------------------
         double K[8];
