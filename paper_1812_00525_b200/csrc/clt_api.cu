@@ -13,6 +13,10 @@
 
 using namespace clt;
 
+// prefetch.global.L2 hints for the next plane's epilogue operands (measured choice)
+#ifndef CLT_PREFETCH
+#define CLT_PREFETCH 1
+#endif
 // L2 promotion of the TMA loads (measured choice)
 #ifndef CLT_L2_PROMO
 #define CLT_L2_PROMO CU_TENSOR_MAP_L2_PROMOTION_L2_256B
@@ -283,7 +287,7 @@ int run_rhs(clt_ctx *ctx, int mode, const double *in, double *out, double a_next
     a.invR = ctx->invRtab + LP;
     a.a_next = a_next; a.b_acc = b_acc;
     a.phi_chunks = effective_chunks(ctx);
-    a.prefetch = 1;
+    a.prefetch = CLT_PREFETCH;
     a.spec = ctx->spec;
     a.coef = ctx->adaptive ? ctx->result + 8 : nullptr;
     a.dtmin_bits = ctx->adaptive ? (unsigned long long *)(ctx->result + 16) : nullptr;
