@@ -161,7 +161,7 @@ int clt_set_owned_rows(clt_ctx *ctx, int k_first, int k_last, int deep_first, in
  * stage-4 epilogue of the fused kernel (no extra pass over the state, no host round trip per step).  cfl <= 0 means
  * params.cfl.  Synchronises once at the end to report *dt_last (SETDT of the final state, i.e. the step the next call
  * would start with) and *time_advanced (sum of the n steps); either pointer may be NULL.  params.dt is unchanged.
- * Not available per slab (a global minimum would be needed between the slabs).                          */
+ * Slabs need the global minimum instead: slab.py's step_cfl reduces clt_suggest_dt over the slabs every step.  */
 int clt_step_cfl(clt_ctx *ctx, int n, double cfl, double *dt_last, double *time_advanced);
 
 /* Changes the fixed time step (dt > 0, finite).                                                  */

@@ -173,6 +173,19 @@ class SlabGroup:
                     s.g.step_stage(stage)
                 exchange(self.slabs, self.extents, STAGE_BUFFER[stage], self.dist, _make_buffer)
 
+    def step_cfl(self, n=1, cfl=0.0):
+        """n adaptive RK4 steps (Fig. 3-4): every step runs with the global SETDT minimum of the state at
+        its start -- the minimum of the slabs' reductions (one MIN all-reduce and one host round trip per step; the
+        device-resident clock of clt_step_cfl needs a single context).  Returns the time advanced."""
+        t = 0.0
+        for _ in range(n):
+            dt = self.suggest_dt(cfl)
+            for s in self.slabs:
+                s.g.set_dt(dt)
+            self.step(1)
+            t += dt
+        return t
+
     def diagnostics(self):
         """Global diagnostics: sums over the slabs' owned rows, max of the div B maxima."""
         parts = [s.g.diagnostics() for s in self.slabs]

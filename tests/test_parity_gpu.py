@@ -495,3 +495,17 @@ def test_spectral_scheme_rejects_more_than_256_planes():
     assert_close(g.rhs(), make_oracle(prob).rhs(), RHS_TOL, "rhs with 260 planes (finite differences)")
     with pytest.raises(clt.CltError):
         g.set_phi_scheme(1)
+
+
+def test_slab_adaptive_steps_match_single_domain_and_oracle():
+    from paper_1812_00525_b200 import slab
+    prob = inputs.make_custom_problem(40, 8, 45, index=24, amplitude_scale=200.0)
+    grp = slab.SlabGroup(prob.cfg, prob.dt, prob.U0, prob.U, 3)
+    g, o = make_gpu(prob), make_oracle(prob)
+    t_s = grp.step_cfl(10, 0.4)
+    _, t_g = g.step_cfl(10, 0.4)
+    o.step_cfl(10, 0.4)
+    assert abs(t_s - o.time) <= 1e-12 * o.time and abs(t_g - o.time) <= 1e-12 * o.time
+    assert_close(grp.get_state(), g.get_state(), 1e-11, "3 slabs vs single domain, adaptive steps")
+    assert_close(grp.get_state(), o.get_state(), STEP_TOL, "3 slabs vs oracle, adaptive steps")
+    grp.close()
