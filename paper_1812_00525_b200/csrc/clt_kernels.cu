@@ -38,6 +38,10 @@ namespace clt {
 #ifndef CLT_EPI_OWN
 #define CLT_EPI_OWN 1
 #endif
+// outputs per thread (= width of the sliding register windows) of the pseudo-spectral pre-pass
+#ifndef CLT_SPEC_NQ
+#define CLT_SPEC_NQ 8
+#endif
 // planes of L2-only TMA prefetch beyond the NRAW buffered ones in the fused RHS kernel (0 = none).  Measured at
 // 512x64x512: 1, 2 and 4 planes are all 3-4 % SLOWER than none (3.93 vs 3.79 ms per step), so it is off.
 #ifndef CLT_TMA_PF
@@ -1302,9 +1306,9 @@ int curl_tma_tile_z() { return CLT_CURL_TZ; }
 // in their paired form
 //   d1_j = sum_{m=1..Q} c1[m] (f_{j+m} - f_{j-m}),   Q = floor((N-1)/2)
 //   d2_j = c2[0] f_j + sum_{m=1..Q} c2[m] (f_{j+m} + f_{j-m}) [+ c2[N/2] f_{j+N/2}, N even]
-// with the closed-form weights of the Fourier differentiation matrices (clt_api.cu).  A thread forms four
-// consecutive outputs of one line at a time from two sliding 4-wide register windows, so every step in m costs
-// two shared-memory loads for 8 (16 with second derivatives) FP64 operations: FP64-bound, any N <= 256.
+// with the closed-form weights of the Fourier differentiation matrices (clt_api.cu).  A thread forms CLT_SPEC_NQ = 8
+// consecutive outputs of one line at a time from two sliding register windows, so every step in m costs two
+// shared-memory loads for 16 (32 with second derivatives) FP64 operations: FP64-bound, any N <= 256.
 // ---------------------------------------------------------------------------------------------
 template <bool WANT2>
 __global__ void __launch_bounds__(512) phi_spectral_kernel(const __grid_constant__ SpecArgs a, int job_base)
@@ -1358,37 +1362,42 @@ __global__ void __launch_bounds__(512) phi_spectral_kernel(const __grid_constant
     const int Q = (N - 1) / 2;
     const bool even = (N & 1) == 0, want2 = WANT2 && out2 >= 0;
     const double *v = sv + tx;
-    auto wrap = [N](int x) { return x >= N ? x - N : (x < 0 ? x + N : x); };
-    for (int j0 = 4 * ty; j0 < N; j0 += 4 * TY) {
-        double s1[4], s2[4], wa[4], wb[4];      // windows: wa[q] = f_{j0+q+m}, wb[q] = f_{j0+q-m}
+    auto wrap = [N](int x) { x %= N; return x < 0 ? x + N : x; };
+    constexpr int NQ = CLT_SPEC_NQ;             // outputs per thread and window width
+    for (int j0 = NQ * ty; j0 < N; j0 += NQ * TY) {
+        double s1[NQ], s2[NQ], wa[NQ], wb[NQ];  // windows: wa[q] = f_{j0+q+m}, wb[q] = f_{j0+q-m}
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
+        for (int q = 0; q < NQ; ++q) {
             s1[q] = 0.0;
             s2[q] = WANT2 ? sc2[0] * v[wrap(j0 + q) * 32] : 0.0;
             wa[q] = v[wrap(j0 + q + 1) * 32];
             wb[q] = v[wrap(j0 + q - 1) * 32];
         }
-        int pa = wrap(j0 + 5), pb = wrap(j0 - 2);
+        int pa = wrap(j0 + NQ + 1), pb = wrap(j0 - 2);
 #pragma unroll 4
         for (int m = 1; m <= Q; ++m) {
             const double c1 = sc1[m], c2 = sc2[m];
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
+            for (int q = 0; q < NQ; ++q) {
                 s1[q] = fma(c1, wa[q] - wb[q], s1[q]);
                 if (WANT2) s2[q] = fma(c2, wa[q] + wb[q], s2[q]);
             }
-            wa[0] = wa[1]; wa[1] = wa[2]; wa[2] = wa[3]; wa[3] = v[pa * 32];
-            wb[3] = wb[2]; wb[2] = wb[1]; wb[1] = wb[0]; wb[0] = v[pb * 32];
+#pragma unroll
+            for (int q = 0; q < NQ - 1; ++q) wa[q] = wa[q + 1];
+            wa[NQ - 1] = v[pa * 32];
+#pragma unroll
+            for (int q = NQ - 1; q > 0; --q) wb[q] = wb[q - 1];
+            wb[0] = v[pb * 32];
             pa = pa + 1 == N ? 0 : pa + 1;
             pb = pb == 0 ? N - 1 : pb - 1;
         }
         if (WANT2 && even) {
 #pragma unroll
-            for (int q = 0; q < 4; ++q) s2[q] = fma(sc2[N / 2], v[wrap(wrap(j0 + q) + N / 2) * 32], s2[q]);
+            for (int q = 0; q < NQ; ++q) s2[q] = fma(sc2[N / 2], v[wrap(j0 + q + N / 2) * 32], s2[q]);
         }
         if (valid) {
 #pragma unroll
-            for (int q = 0; q < 4; ++q)
+            for (int q = 0; q < NQ; ++q)
                 if (j0 + q < N) {
                     const long long g = (long long)(j0 + q) * L.plane + o2;
                     a.out[(long long)out1 * L.field + g] = s1[q];
@@ -1565,7 +1574,7 @@ static cudaError_t launch_phi_jobs(const SpecArgs &a, int job_base, int jobs, cu
         configured = true;
     }
     const int N = a.L.nphi;
-    const int groups = (N + 3) / 4;
+    const int groups = (N + CLT_SPEC_NQ - 1) / CLT_SPEC_NQ;
     dim3 block(32, groups < 16 ? groups : 16, 1);
     dim3 grid((a.L.nR - 4 + 31) / 32, a.L.nZ - 4, jobs);
     const size_t smem = ((size_t)N * 32 + 2 * (size_t)N) * sizeof(double);
