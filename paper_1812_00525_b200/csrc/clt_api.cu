@@ -35,6 +35,7 @@ struct clt_ctx {
     int k_first, k_last, kd_first, kd_last;   // diagnostics row ranges (clt_set_owned_rows)
     bool adaptive;                 // inside clt_step_cfl: stage coefficients from the device clock
     double adaptive_cfl;
+    int device;                    // the device the workspace lives on (every call runs with it current)
     int next_stage;                // clt_step_stage: the stage expected next (1..4)
     bool spec_fft;                 // pseudo-spectral pre-pass by FFT where nphi allows (scheme 2) instead of the circulant sums
     bool spectral;                 // pseudo-spectral phi scheme (clt_set_phi_scheme)
@@ -60,6 +61,18 @@ struct clt_ctx {
 };
 
 namespace {
+
+// makes the context's device current for the duration of an API call (callers with several GPUs in one process)
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(const clt_ctx *ctx)
+    {
+        if (!ctx) return;
+        if (cudaGetDevice(&prev) != cudaSuccess) { cudaGetLastError(); prev = -1; return; }
+        if (prev != ctx->device) cudaSetDevice(ctx->device); else prev = -1;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
 
 constexpr size_t ALIGN = 128;   // every field and table base is 128-byte aligned
 inline size_t align_up(size_t n) { return (n + ALIGN - 1) / ALIGN * ALIGN; }
@@ -410,6 +423,8 @@ int clt_create(const clt_grid *grid, const clt_params *params, void *d_workspace
     ctx->par = *params;
     ctx->L = make_layout(grid);
     ctx->stream = (cudaStream_t)cuda_stream;
+    ctx->device = at.device;
+    DeviceGuard device_guard(ctx);
     ctx->dt = params->dt;
     ctx->k_first = 2; ctx->k_last = grid->nZ - 3; ctx->kd_first = 4; ctx->kd_last = grid->nZ - 5;
     ctx->next_stage = 1;
@@ -480,6 +495,7 @@ int clt_create(const clt_grid *grid, const clt_params *params, void *d_workspace
 
 int clt_destroy(clt_ctx *ctx)
 {
+    DeviceGuard device_guard(ctx);
     if (!ctx) return CLT_OK;
     cudaError_t e = cudaStreamSynchronize(ctx->stream);
     destroy_graph(ctx);
@@ -491,6 +507,7 @@ int clt_destroy(clt_ctx *ctx)
 
 int clt_set_equilibrium(clt_ctx *ctx, const double *U0)
 {
+    DeviceGuard device_guard(ctx);
     if (!ctx) return CLT_EINVAL;
     ctx->has_state = false;
     const size_t rows = (size_t)8 * ctx->L.nZ;
@@ -518,6 +535,7 @@ int clt_set_equilibrium(clt_ctx *ctx, const double *U0)
 
 int clt_set_state(clt_ctx *ctx, const double *U)
 {
+    DeviceGuard device_guard(ctx);
     if (!ctx || !U) return CLT_EINVAL;
     int r = copy_in(ctx, ctx->Un, U, (size_t)8 * ctx->L.nphi * ctx->L.nZ);
     if (r) return r;
@@ -537,6 +555,7 @@ int clt_set_state(clt_ctx *ctx, const double *U)
 
 int clt_get_state(clt_ctx *ctx, double *U)
 {
+    DeviceGuard device_guard(ctx);
     if (!ctx || !U) return CLT_EINVAL;
     if (!ctx->has_state) return CLT_ESTATE;
     return copy_out(ctx, U, ctx->Un, (size_t)8 * ctx->L.nphi * ctx->L.nZ);
@@ -544,6 +563,7 @@ int clt_get_state(clt_ctx *ctx, double *U)
 
 int clt_rhs(clt_ctx *ctx, double *dUdt)
 {
+    DeviceGuard device_guard(ctx);
     if (!ctx || !dUdt) return CLT_EINVAL;
     if (!ctx->has_state) return CLT_ESTATE;
     int r;
@@ -559,6 +579,7 @@ int clt_rhs(clt_ctx *ctx, double *dUdt)
 
 int clt_curl_J1(clt_ctx *ctx, double *J1)
 {
+    DeviceGuard device_guard(ctx);
     if (!ctx || !J1) return CLT_EINVAL;
     if (!ctx->has_state) return CLT_ESTATE;
     int r;
@@ -568,6 +589,7 @@ int clt_curl_J1(clt_ctx *ctx, double *J1)
 
 int clt_hall_G(clt_ctx *ctx, double *G)
 {
+    DeviceGuard device_guard(ctx);
     if (!ctx || !G) return CLT_EINVAL;
     if (!ctx->has_state) return CLT_ESTATE;
     if (!ctx->hall) return CLT_EINVAL;
@@ -585,6 +607,7 @@ int clt_set_dt(clt_ctx *ctx, double dt)
 
 int clt_step(clt_ctx *ctx, int n)
 {
+    DeviceGuard device_guard(ctx);
     if (!ctx || n < 0) return CLT_EINVAL;
     if (!ctx->has_state || ctx->next_stage != 1) return CLT_ESTATE;
     if (!(ctx->dt > 0.0)) return CLT_EINVAL;
@@ -648,6 +671,7 @@ static int run_diag(clt_ctx *ctx, double cfl, double out6[6])
 
 int clt_diagnostics(clt_ctx *ctx, clt_diag *out)
 {
+    DeviceGuard device_guard(ctx);
     if (!ctx || !out) return CLT_EINVAL;
     if (!ctx->has_state) return CLT_ESTATE;
     double r6[6];
@@ -664,6 +688,7 @@ int clt_diagnostics(clt_ctx *ctx, clt_diag *out)
 
 int clt_suggest_dt(clt_ctx *ctx, double cfl, double *dt_out)
 {
+    DeviceGuard device_guard(ctx);
     if (!ctx || !dt_out) return CLT_EINVAL;
     if (!ctx->has_state) return CLT_ESTATE;
     if (!(cfl > 0.0)) cfl = ctx->par.cfl;
@@ -683,6 +708,7 @@ size_t clt_spectral_workspace_bytes(const clt_grid *grid)
 
 int clt_set_phi_scheme(clt_ctx *ctx, int scheme, void *d_scratch, size_t bytes)
 {
+    DeviceGuard device_guard(ctx);
     if (!ctx || scheme < 0 || scheme > 2) return CLT_EINVAL;
     CK(cudaStreamSynchronize(ctx->stream));
     destroy_graph(ctx);
@@ -737,6 +763,7 @@ int clt_set_phi_scheme(clt_ctx *ctx, int scheme, void *d_scratch, size_t bytes)
 
 int clt_step_stage(clt_ctx *ctx, int stage)
 {
+    DeviceGuard device_guard(ctx);
     if (!ctx || stage < 1 || stage > 4) return CLT_EINVAL;
     if (!ctx->has_state || stage != ctx->next_stage) return CLT_ESTATE;
     if (!(ctx->dt > 0.0)) return CLT_EINVAL;
@@ -754,6 +781,7 @@ static double *stage_buffer(clt_ctx *ctx, int buffer)
 
 int clt_get_rows(clt_ctx *ctx, int buffer, int k0, int nrows, double *dst)
 {
+    DeviceGuard device_guard(ctx);
     if (!ctx || !dst || nrows < 1 || k0 < 0 || k0 + nrows > ctx->L.nZ || !stage_buffer(ctx, buffer)) return CLT_EINVAL;
     if (!ctx->has_state) return CLT_ESTATE;
     return copy_rows(ctx, stage_buffer(ctx, buffer), k0, nrows, dst, true);
@@ -761,6 +789,7 @@ int clt_get_rows(clt_ctx *ctx, int buffer, int k0, int nrows, double *dst)
 
 int clt_set_rows(clt_ctx *ctx, int buffer, int k0, int nrows, const double *src)
 {
+    DeviceGuard device_guard(ctx);
     if (!ctx || !src || nrows < 1 || k0 < 0 || k0 + nrows > ctx->L.nZ || !stage_buffer(ctx, buffer)) return CLT_EINVAL;
     if (!ctx->has_state) return CLT_ESTATE;
     return copy_rows(ctx, stage_buffer(ctx, buffer), k0, nrows, const_cast<double *>(src), false);
@@ -777,6 +806,7 @@ int clt_set_owned_rows(clt_ctx *ctx, int k_first, int k_last, int deep_first, in
 
 int clt_step_cfl(clt_ctx *ctx, int n, double cfl, double *dt_last, double *time_advanced)
 {
+    DeviceGuard device_guard(ctx);
     if (!ctx || n < 0) return CLT_EINVAL;
     if (!ctx->has_state || ctx->next_stage != 1) return CLT_ESTATE;
     if (!(cfl > 0.0)) cfl = ctx->par.cfl;
@@ -833,6 +863,7 @@ int clt_set_tuning(clt_ctx *ctx, int tile_z, int phi_chunks, int use_graph)
 
 int clt_set_profiling(clt_ctx *ctx, int enable)
 {
+    DeviceGuard device_guard(ctx);
     if (!ctx) return CLT_EINVAL;
     CK(cudaStreamSynchronize(ctx->stream));
     ctx->profiling = enable != 0;
@@ -843,6 +874,7 @@ int clt_set_profiling(clt_ctx *ctx, int enable)
 
 int clt_get_profile(clt_ctx *ctx, clt_profile *out)
 {
+    DeviceGuard device_guard(ctx);
     if (!ctx || !out) return CLT_EINVAL;
     CK(cudaStreamSynchronize(ctx->stream));
     memset(out, 0, sizeof(*out));

@@ -55,6 +55,14 @@ namespace clt {
 constexpr int TR = 32;        // tile width in R = one warp per tile row
 constexpr int SW = TR + 4;    // shared row width with the radius-2 halo
 
+// index of the current device (0..63) for the per-device "shared-memory opt-in done" flags of the launchers
+static int current_device()
+{
+    int d = 0;
+    if (cudaGetDevice(&d) != cudaSuccess) { cudaGetLastError(); d = 0; }
+    return d & 63;
+}
+
 __device__ __forceinline__ void prefetch_l2(const void *p)
 {
     asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
@@ -540,7 +548,8 @@ __global__ void __launch_bounds__(TR *TZ, (TZ <= 8 ? 2 : 1)) rhs_kernel(const __
 template <int TZ, int MODE, bool V0>
 static cudaError_t launch_rhs_t(const RhsArgs &a, cudaStream_t s)
 {
-    static bool configured = false;
+    static bool configured_dev[64] = {};     // per device: the opt-in is a per-device function attribute
+    bool &configured = configured_dev[current_device()];
     auto kern = rhs_kernel<TZ, MODE, V0>;
     const int smem = (int)sizeof(RhsSmem<TZ>);
     if (!configured) {
@@ -931,7 +940,8 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
 template <int TZ, int NRAW, int MODE, bool V0, bool HALL, bool SPEC>
 static cudaError_t launch_rhs_tma_t(const RhsArgs &a, const CUtensorMap &tmU, const CUtensorMap &tmJ, cudaStream_t s)
 {
-    static bool configured = false;
+    static bool configured_dev[64] = {};     // per device: the opt-in is a per-device function attribute
+    bool &configured = configured_dev[current_device()];
     auto kern = rhs_tma_kernel<TZ, NRAW, MODE, V0, HALL, SPEC>;
     using SM = RhsTmaSmem<TZ, NRAW, HALL ? 14 : 11>;
     const int smem = (int)sizeof(SM);
@@ -1276,7 +1286,8 @@ template <bool HALL, bool SPEC>
 static cudaError_t launch_curl_tma_t(const CurlArgs &a, const void *tmU, cudaStream_t s)
 {
     constexpr int TZ = CLT_CURL_TZ, NS = CLT_CURL_NS;
-    static bool configured = false;
+    static bool configured_dev[64] = {};     // per device: the opt-in is a per-device function attribute
+    bool &configured = configured_dev[current_device()];
     auto kern = curl_tma_kernel<TZ, NS, HALL, SPEC>;
     const int smem = (int)sizeof(CurlTmaSmem<TZ, NS, HALL ? 5 : 3>);
     if (!configured) {
@@ -1538,7 +1549,8 @@ static bool phi_fft_supported(int N) { return N >= 8 && N <= 128 && (N & (N - 1)
 
 static cudaError_t launch_phi_fft(const SpecArgs &a, cudaStream_t s)
 {
-    static bool configured = false;
+    static bool configured_dev[64] = {};     // per device: the opt-in is a per-device function attribute
+    bool &configured = configured_dev[current_device()];
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(phi_fft_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              (int)((6 * 128 * 32 + 128) * sizeof(double)));
@@ -1565,7 +1577,8 @@ static cudaError_t launch_phi_fft(const SpecArgs &a, cudaStream_t s)
 template <bool WANT2>
 static cudaError_t launch_phi_jobs(const SpecArgs &a, int job_base, int jobs, cudaStream_t s)
 {
-    static bool configured = false;
+    static bool configured_dev[64] = {};     // per device: the opt-in is a per-device function attribute
+    bool &configured = configured_dev[current_device()];
     auto kern = phi_spectral_kernel<WANT2>;
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
