@@ -49,15 +49,29 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def profiled_pipes(kernel="rhs_tma"):
+    """FP64-pipe and L1/shared-memory utilisation of the dominant kernel from the same committed ncu capture (mean over
+    its launches), or None."""
+    p = os.path.join(ROOT, "profiles", "traffic.csv")
+    try:
+        for line in open(p).read().splitlines()[1:]:
+            f = line.split(",")
+            if f[0] == kernel and len(f) >= 5:
+                return {"fp64_pipe_pct": float(f[3]), "l1tex_throughput_pct": float(f[4]), "source": f[2]}
+    except Exception:
+        pass
+    return None
+
+
 def profiled_traffic(kernel="rhs_tma"):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed ncu --set full
     summary (profiles/traffic.csv names the source file); None if there is no capture."""
     p = os.path.join(ROOT, "profiles", "traffic.csv")
     try:
         for line in open(p).read().splitlines()[1:]:
-            k, v, _src = line.split(",", 2)
-            if k == kernel:
-                return float(v)
+            f = line.split(",")
+            if f[0] == kernel:
+                return float(f[1])
     except Exception:
         pass
     return None
@@ -311,6 +325,7 @@ def run_ours(args):
         roof = {"bound": "hbm", "kernel": "rhs_tma_kernel (fused RHS + RK4 stage combine, its 4 stage variants pooled)",
                 "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                 "traffic": args.traffic if args.traffic is not None else (profiled_traffic() if cfg.index == 4 else None),
+                "ncu_pipes": profiled_pipes() if cfg.index == 4 else None,
                 "peak_source": peak_src + ", burst figure", "avg_launch_ms": ms_rhs / n_rhs,
                 "algorithmic_bytes_per_launch": bytes_per_launch, "share_of_step": ms_rhs / (ms_rhs + prof["ms_curl"] + prof.get("ms_phi", 0.0)),
                 "per_stage": per_stage, "curl_kernel": curl,
