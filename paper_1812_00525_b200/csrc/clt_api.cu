@@ -56,6 +56,8 @@ struct clt_ctx {
     bool profiling;
     std::vector<cudaEvent_t> *ev;      // pairs: start, stop
     std::vector<int> *ev_kind;         // 0..4 rhs mode, 5 curl
+    std::vector<long> *ev_start;       // index of the event that marks the start of launch n (its own, or the previous end)
+    bool prof_chain;                   // the last operation on the stream was the end event of the previous profiled launch
     size_t ev_used;
     int64_t ev_dropped;
 };
@@ -65,9 +67,10 @@ namespace {
 // makes the context's device current for the duration of an API call (callers with several GPUs in one process)
 struct DeviceGuard {
     int prev = -1;
-    explicit DeviceGuard(const clt_ctx *ctx)
+    explicit DeviceGuard(clt_ctx *ctx)
     {
         if (!ctx) return;
+        ctx->prof_chain = false;       // whatever this call enqueues first does not follow a profiled launch back to back
         if (cudaGetDevice(&prev) != cudaSuccess) { cudaGetLastError(); prev = -1; return; }
         if (prev != ctx->device) cudaSetDevice(ctx->device); else prev = -1;
     }
@@ -155,6 +158,8 @@ void free_profile(clt_ctx *ctx)
     }
     delete ctx->ev_kind;
     ctx->ev_kind = nullptr;
+    delete ctx->ev_start;
+    ctx->ev_start = nullptr;
 }
 
 void destroy_graph(clt_ctx *ctx)
@@ -212,22 +217,35 @@ constexpr size_t MAX_PROFILED = 8192;
 // returns the index of the event pair to use for this launch, or -1
 long prof_begin(clt_ctx *ctx, int kind)
 {
-    if (!ctx->profiling || ctx->use_graph) return -1;
-    if (ctx->ev_used >= MAX_PROFILED) { ctx->ev_dropped++; return -1; }
+    if (!ctx->profiling || ctx->use_graph) { ctx->prof_chain = false; return -1; }
+    if (ctx->ev_used >= MAX_PROFILED) { ctx->ev_dropped++; ctx->prof_chain = false; return -1; }
     if (ctx->ev->size() < 2 * (ctx->ev_used + 1)) {
         cudaEvent_t a, b;
-        if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) { cudaGetLastError(); return -1; }
+        if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) {
+            cudaGetLastError();
+            ctx->prof_chain = false;
+            return -1;
+        }
         ctx->ev->push_back(a); ctx->ev->push_back(b);
         ctx->ev_kind->push_back(kind);
+        ctx->ev_start->push_back(0);
     }
     const long n = (long)ctx->ev_used++;
     (*ctx->ev_kind)[n] = kind;
-    cudaEventRecord((*ctx->ev)[2 * n], ctx->stream);
+    if (ctx->prof_chain && n > 0) {
+        (*ctx->ev_start)[n] = 2 * (n - 1) + 1;      // back-to-back launches: the previous end event is this start
+    } else {
+        (*ctx->ev_start)[n] = 2 * n;
+        cudaEventRecord((*ctx->ev)[2 * n], ctx->stream);
+    }
     return n;
 }
 void prof_end(clt_ctx *ctx, long n)
 {
-    if (n >= 0) cudaEventRecord((*ctx->ev)[2 * n + 1], ctx->stream);
+    if (n >= 0) {
+        cudaEventRecord((*ctx->ev)[2 * n + 1], ctx->stream);
+        ctx->prof_chain = true;
+    }
 }
 
 // kernels one phi pre-pass launches: the FFT variant does everything in one, the circulant sums need two in mode 1
@@ -419,6 +437,7 @@ int clt_create(const clt_grid *grid, const clt_params *params, void *d_workspace
     memset(ctx, 0, sizeof(*ctx));
     ctx->ev = new std::vector<cudaEvent_t>();
     ctx->ev_kind = new std::vector<int>();
+    ctx->ev_start = new std::vector<long>();
     ctx->grid = *grid;
     ctx->par = *params;
     ctx->L = make_layout(grid);
@@ -833,6 +852,7 @@ int clt_step_cfl(clt_ctx *ctx, int n, double cfl, double *dt_last, double *time_
             r = enqueue_step(ctx);                 // stage 4 collects the SETDT minimum of the new state
             if (r == CLT_OK) {
                 cudaError_t e = launch_dt_commit(clock, bits, ctx->result, 0, ctx->stream);   // time += dt; dt = minimum
+                ctx->prof_chain = false;
                 if (e != cudaSuccess) r = cuda_fail(ctx, e, "dt_commit_kernel");
                 ctx->launches++;
             }
@@ -880,7 +900,7 @@ int clt_get_profile(clt_ctx *ctx, clt_profile *out)
     memset(out, 0, sizeof(*out));
     for (size_t n = 0; n < ctx->ev_used; ++n) {
         float ms = 0.f;
-        CK(cudaEventElapsedTime(&ms, (*ctx->ev)[2 * n], (*ctx->ev)[2 * n + 1]));
+        CK(cudaEventElapsedTime(&ms, (*ctx->ev)[(*ctx->ev_start)[n]], (*ctx->ev)[2 * n + 1]));
         const int kind = (*ctx->ev_kind)[n];
         if (kind == 5) { out->ms_curl += ms; out->n_curl++; }
         else if (kind == 6) { out->ms_phi += ms; out->n_phi++; }
