@@ -42,6 +42,12 @@ namespace clt {
 #ifndef CLT_SPEC_NQ
 #define CLT_SPEC_NQ 8
 #endif
+// circular phi pipelines with a five times unrolled plane loop in the fused RHS kernel (1) or shifting pipelines (0).
+// Measured at 512x64x512: no difference (3.715 vs 3.712 ms per step; the 70 register moves per node it removes are not
+// what the kernel waits for) at twice the code size, so it is off; parity-tested once with it on.
+#ifndef CLT_ROT
+#define CLT_ROT 0
+#endif
 // planes of L2-only TMA prefetch beyond the NRAW buffered ones in the fused RHS kernel (0 = none).  Measured at
 // 512x64x512: 1, 2 and 4 planes are all 3-4 % SLOWER than none (3.93 vs 3.79 ms per step), so it is off.
 #ifndef CLT_TMA_PF
@@ -51,6 +57,9 @@ namespace clt {
 #ifndef CLT_NRAW8
 #define CLT_NRAW8 2
 #endif
+
+template <int V>
+struct IC { static constexpr int value = V; };      // compile-time integer passed to generic lambdas
 
 constexpr int TR = 32;        // tile width in R = one warp per tile row
 constexpr int SW = TR + 4;    // shared row width with the radius-2 halo
@@ -115,14 +124,15 @@ __device__ __forceinline__ CentreTab load_centre_tab(const double *tab, long lon
 // of a neighbour's staged value: the caller puts the wait half of its split barrier there.
 // SPEC = true: the phi derivatives come from the pseudo-spectral pre-pass: pd1[f], pd2[f] are d/dphi and d2/dphi2 of
 // the five fluid perturbations, dP_EZ / dP_ER the true d/dphi of E1_Z / E1_R (not the unscaled stencil sums).
-template <bool V0, bool SPEC, class Sync>
+// P = phase of the circular phi pipeline: plane j-2+d sits in q[(P + d) % 5] (P = 0: q[d] is plane j-2+d)
+template <bool V0, bool SPEC, int P, class Sync>
 __device__ __forceinline__ void rhs_point(const double *stg, int HT, const double *eRc, const double *ePc, const double *eZc,
                                           double dP_EZ, double dP_ER, const double (&F)[3], const double (&rr)[4], int cs,
                                           const double (&q)[5][5], const CentreTab &ct, const double *tab, long long off2,
                                           long long plane, const Phys &ph, double iR, double iR2, double (&K)[8], Sync &&sync,
                                           const double *pd1 = nullptr, const double *pd2 = nullptr)
 {
-    const double rho1 = q[2][0], p1 = q[2][1], v1R = q[2][2], v1P = q[2][3], v1Z = q[2][4];
+    const double rho1 = q[(P + 2) % 5][0], p1 = q[(P + 2) % 5][1], v1R = q[(P + 2) % 5][2], v1P = q[(P + 2) % 5][3], v1Z = q[(P + 2) % 5][4];
     const double rho = rho1 + ct.rho0;
     const double p = p1 + ct.p0;
     double vR = v1R, vP = v1P, vZ = v1Z;
@@ -140,8 +150,8 @@ __device__ __forceinline__ void rhs_point(const double *stg, int HT, const doubl
         const double g1 = SPEC ? iR : ph.cP1 * iR, vc = vP * g1, lc = SPEC ? iR2 : ph.cP2 * iR2;
 #pragma unroll
         for (int f = 0; f < 5; ++f) {
-            const double d1 = SPEC ? pd1[f] : fd1(q[0][f], q[1][f], q[3][f], q[4][f]);
-            const double d2 = SPEC ? pd2[f] : fd2(q[0][f], q[1][f], q[2][f], q[3][f], q[4][f]);
+            const double d1 = SPEC ? pd1[f] : fd1(q[(P + 0) % 5][f], q[(P + 1) % 5][f], q[(P + 3) % 5][f], q[(P + 4) % 5][f]);
+            const double d2 = SPEC ? pd2[f] : fd2(q[(P + 0) % 5][f], q[(P + 1) % 5][f], q[(P + 2) % 5][f], q[(P + 3) % 5][f], q[(P + 4) % 5][f]);
             A[f] = vc * d1;
             lap[f] = lc * d2;
             if (f == 1) gPp1 = d1 * g1;
@@ -160,7 +170,7 @@ __device__ __forceinline__ void rhs_point(const double *stg, int HT, const doubl
         for (int f = 0; f < 5; ++f) {
             const double *s = stg + f * HT + cs;
             const double m2 = s[-2], m1 = s[-1], p1_ = s[1], p2 = s[2];
-            const double d1 = fd1(m2, m1, p1_, p2), d2 = fd2(m2, m1, q[2][f], p1_, p2);
+            const double d1 = fd1(m2, m1, p1_, p2), d2 = fd2(m2, m1, q[(P + 2) % 5][f], p1_, p2);
             A[f] += vc * d1;
             lap[f] += d2 * ph.cR2 + lc * d1;
             if (f == 1) gRp1 = d1 * ph.cR1;
@@ -174,7 +184,7 @@ __device__ __forceinline__ void rhs_point(const double *stg, int HT, const doubl
         for (int f = 0; f < 5; ++f) {
             const double *s = stg + f * HT + cs;
             const double m2 = s[-2 * SW], m1 = s[-SW], p1_ = s[SW], p2 = s[2 * SW];
-            const double d1 = fd1(m2, m1, p1_, p2), d2 = fd2(m2, m1, q[2][f], p1_, p2);
+            const double d1 = fd1(m2, m1, p1_, p2), d2 = fd2(m2, m1, q[(P + 2) % 5][f], p1_, p2);
             A[f] += vc * d1;
             lap[f] += d2 * ph.cZ2;
             if (f == 1) gZp1 = d1 * ph.cZ1;
@@ -529,7 +539,7 @@ __global__ void __launch_bounds__(TR *TZ, (TZ <= 8 ? 2 : 1)) rhs_kernel(const __
             const double dP_ER = fd1(S.ering[s0][0][cs], S.ering[s1][0][cs], S.ering[s3][0][cs], S.ering[se][0][cs]);
             const double F[3] = { S.fring[sfc][0][ci], S.fring[sfc][1][ci], S.fring[sfc][2][ci] };
             const double rr[4] = { S.sR[tx], S.sR[tx + 1], S.sR[tx + 3], S.sR[tx + 4] };
-            rhs_point<V0, false>(&S.stage[buf][0][0], RhsSmem<TZ>::HT, &S.ering[sec][0][0], &S.ering[sec][1][0], &S.ering[sec][2][0],
+            rhs_point<V0, false, 0>(&S.stage[buf][0][0], RhsSmem<TZ>::HT, &S.ering[sec][0][0], &S.ering[sec][1][0], &S.ering[sec][2][0],
                           dP_EZ, dP_ER, F, rr, cs, q, ct, tab, off2, L.plane, ph, iR, iR2, K, [] {});
         }
 
@@ -805,21 +815,26 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
     double eR[5], eZ[5];   // E1_R, E1_Z of planes j-2 .. j+2
     double Fp[3][3];       // F = J1 x B + J0 x B1 of planes j .. j+2
     int sl = 0;            // ring slot that receives the plane being consumed (plane j+2)
+    const int total = jb - ja + 4;
 
-    // consume the raw tile of plane number nlead (the plane that becomes plane j+2)
-    auto lead = [&]() {
+    // The fluid and E pipelines are CIRCULAR with a compile-time phase (CLT_ROT = 1): plane number n (counted from
+    // ja-2) lives in slot n % 5, the main loop is unrolled five times, and nothing is ever shifted (the shifts were
+    // 70 of about 530 instructions per node).  CLT_ROT = 0 keeps the shifting pipelines (slot 4 = newest plane).
+    // consume the raw tile of plane number nlead (the plane that becomes plane j+2) into pipeline slot SLOT
+    auto lead = [&](auto slot_c) {
+        constexpr int SLOT = decltype(slot_c)::value;
         const int b = nlead % NRAW;
         mbar_wait(&S.bar[b], (unsigned)((nlead / NRAW) & 1));
         ++nlead;
         const double (*raw)[SM::HTP] = S.raw[b];
         double E[3];
-        node(raw, cs, off2, ct.rho0, ct.p0, q[4], E, Fp[2], true);
-        eR[4] = E[0];
-        eZ[4] = E[2];
+        node(raw, cs, off2, ct.rho0, ct.p0, q[SLOT], E, Fp[2], true);
+        eR[SLOT] = E[0];
+        eZ[SLOT] = E[2];
 #pragma unroll
         for (int c = 0; c < 3; ++c) S.ering[sl][c][cs] = E[c];
 #pragma unroll
-        for (int f = 0; f < 5; ++f) S.sring[sl][f][cs] = q[4][f];
+        for (int f = 0; f < 5; ++f) S.sring[sl][f][cs] = q[SLOT][f];
         if (is_halo) {
             double hq[5], hE[3], hF[3];
             node(raw, hs, hoff2, h_rho0, h_p0, hq, hE, hF, false);
@@ -830,33 +845,44 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
         }
     };
     auto advance = [&]() {
+        if (!CLT_ROT) {
 #pragma unroll
-        for (int d = 0; d < 4; ++d) {
+            for (int d = 0; d < 4; ++d) {
 #pragma unroll
-            for (int f = 0; f < 5; ++f) q[d][f] = q[d + 1][f];
-            eR[d] = eR[d + 1];
-            eZ[d] = eZ[d + 1];
+                for (int f = 0; f < 5; ++f) q[d][f] = q[d + 1][f];
+                eR[d] = eR[d + 1];
+                eZ[d] = eZ[d + 1];
+            }
         }
 #pragma unroll
         for (int c = 0; c < 3; ++c) { Fp[0][c] = Fp[1][c]; Fp[1][c] = Fp[2][c]; }
         sl = (sl + 1) & 3;
     };
-
-    // prologue: planes number 0 .. 3 (ja-2 .. ja+1); NRAW planes are kept in flight
-    const int total = jb - ja + 4;
-    if (tid == 0) {
-        for (int n = 0; n < NRAW && n < total; ++n) issue(n);
-        for (int n = NRAW; n < NRAW + CLT_TMA_PF && n < total; ++n) prefetch_plane(n);
-    }
-#pragma unroll 1
-    for (int n = 0; n < 4; ++n) {
-        lead();
+    auto after_lead = [&](int n) {
         __syncthreads();                 // every thread has read the raw tile
         if (tid == 0 && n + NRAW < total) {
             issue(n + NRAW);
             if (CLT_TMA_PF > 0 && n + NRAW + CLT_TMA_PF < total) prefetch_plane(n + NRAW + CLT_TMA_PF);
         }
         advance();
+    };
+
+    // prologue: planes number 0 .. 3 (ja-2 .. ja+1); NRAW planes are kept in flight
+    if (tid == 0) {
+        for (int n = 0; n < NRAW && n < total; ++n) issue(n);
+        for (int n = NRAW; n < NRAW + CLT_TMA_PF && n < total; ++n) prefetch_plane(n);
+    }
+    if (CLT_ROT) {
+        lead(IC<0>{}); after_lead(0);
+        lead(IC<1>{}); after_lead(1);
+        lead(IC<2>{}); after_lead(2);
+        lead(IC<3>{}); after_lead(3);
+    } else {
+#pragma unroll 1
+        for (int n = 0; n < 4; ++n) {
+            lead(IC<4>{});
+            after_lead(n);
+        }
     }
     unsigned ready_parity = 0;
 
@@ -864,8 +890,9 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
     const double iR2 = iR * iR;
     double rate = 0.0;           // largest signal rate (|v_d| + c)/(12 h_d) at this thread's nodes (stage 4 of clt_step_cfl)
 
-#pragma unroll 1
-    for (int j = ja; j < jb; ++j) {
+    // one plane: P = phase of the circular pipelines = (j - ja) % 5 (always 0 with CLT_ROT = 0)
+    auto plane = [&](auto phase_c, int j) {
+        constexpr int P = decltype(phase_c)::value;
         // ---- phase A: consume plane j+2 --------------------------------------------------------
         if (a.prefetch && MODE != RHS_MODE_K && (tx & 15) == 0 && j + CLT_PF_DIST < jb) {
             const long long g1 = (long long)(j + CLT_PF_DIST) * L.plane + off2;
@@ -875,7 +902,7 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
                 if (MODE == RHS_MODE_S4) prefetch_l2(a.acc + m * L.field + g1);
             }
         }
-        lead();
+        lead(IC<(P + 4) % 5>{});
         const int sc = (sl + 2) & 3;                              // ring slot of the centre plane
         // split barrier: announce "my part of plane j+2 is in the rings", keep working on what needs nobody else's
         // data (epilogue operand loads, the phi direction), and only then wait for the other warps.  Which stage
@@ -902,7 +929,8 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
         EpiOperands eo;
         // rho, p (and v when the reference state is static) of the centre plane are still in the phi pipeline
         constexpr int NOWN = CLT_EPI_OWN ? (V0 ? 2 : 5) : 0;
-        const double own[5] = { q[2][0] + ct.rho0, q[2][1] + ct.p0, q[2][2], q[2][3], q[2][4] };
+        const double own[5] = { q[(P + 2) % 5][0] + ct.rho0, q[(P + 2) % 5][1] + ct.p0, q[(P + 2) % 5][2], q[(P + 2) % 5][3],
+                                q[(P + 2) % 5][4] };
         epilogue_load<MODE, NOWN>(a, g, L.field, eo, [](const double *p) { return ld_stream(p); }, own);
 
         // ---- phase B: K at (i, k, j) -----------------------------------------------------------
@@ -918,10 +946,10 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
             dP_ER = ld_stream(a.spec + (SP_DE + 0) * L.field + g);
             dP_EZ = ld_stream(a.spec + (SP_DE + 1) * L.field + g);
         } else {
-            dP_EZ = fd1(eZ[0], eZ[1], eZ[3], eZ[4]);
-            dP_ER = fd1(eR[0], eR[1], eR[3], eR[4]);
+            dP_EZ = fd1(eZ[P % 5], eZ[(P + 1) % 5], eZ[(P + 3) % 5], eZ[(P + 4) % 5]);
+            dP_ER = fd1(eR[P % 5], eR[(P + 1) % 5], eR[(P + 3) % 5], eR[(P + 4) % 5]);
         }
-        rhs_point<V0, SPEC>(&S.sring[sc][0][0], HT, &S.ering[sc][0][0], &S.ering[sc][1][0], &S.ering[sc][2][0], dP_EZ, dP_ER, Fp[0],
+        rhs_point<V0, SPEC, P>(&S.sring[sc][0][0], HT, &S.ering[sc][0][0], &S.ering[sc][1][0], &S.ering[sc][2][0], dP_EZ, dP_ER, Fp[0],
                             rr, cs, q, ct, tab, off2, L.plane, ph, iR, iR2, K, [&] {
                                 if (SPLIT) {
                                     mbar_wait(&S.ready, ready_parity);
@@ -933,6 +961,23 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
         // ---- a6: RK4 stage combine in the epilogue (L125, L139) --------------------------------
         if (valid) epilogue_store<MODE>(a, g, L.field, eo, K, iR, rate);
         advance();
+    };
+    if (CLT_ROT) {
+#pragma unroll 1
+        for (int j = ja; j < jb; j += 5) {
+            plane(IC<0>{}, j);
+            if (j + 1 >= jb) break;
+            plane(IC<1>{}, j + 1);
+            if (j + 2 >= jb) break;
+            plane(IC<2>{}, j + 2);
+            if (j + 3 >= jb) break;
+            plane(IC<3>{}, j + 3);
+            if (j + 4 >= jb) break;
+            plane(IC<4>{}, j + 4);
+        }
+    } else {
+#pragma unroll 1
+        for (int j = ja; j < jb; ++j) plane(IC<0>{}, j);
     }
     if (MODE == RHS_MODE_S4) dtmin_commit(a, rate);
 }
