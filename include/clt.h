@@ -191,7 +191,8 @@ size_t clt_spectral_workspace_bytes(const clt_grid *grid);
 int clt_set_phi_scheme(clt_ctx *ctx, int scheme, void *d_scratch, size_t bytes);
 
 /* Launch-shape knobs for measurement (all optional; 0 = library default): tile height in Z of the
- * fused RHS kernel, number of phi chunks per tile, use of a CUDA graph for clt_step.              */
+ * fused RHS kernel, number of phi chunks per tile (default: 1, more on grids with fewer tiles than the
+ * device has SMs), use of a CUDA graph for clt_step.  None of them changes a bit of the result.   */
 int clt_set_tuning(clt_ctx *ctx, int tile_z, int phi_chunks, int use_graph);
 
 /* Selects the implementation of the fused RHS kernel: 0 (default) = shared-memory tiles fed by TMA
