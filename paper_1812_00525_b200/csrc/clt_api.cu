@@ -599,7 +599,7 @@ int clt_rhs(clt_ctx *ctx, double *dUdt)
 {
     DeviceGuard device_guard(ctx);
     if (!ctx || !dUdt) return CLT_EINVAL;
-    if (!ctx->has_state) return CLT_ESTATE;
+    if (!ctx->has_state || ctx->next_stage != 1) return CLT_ESTATE;      // U_b is the scratch buffer: not inside a step
     int r;
     if ((r = run_curl(ctx, ctx->Un))) return r;
     CK(launch_zero_boundary(ctx->L, 8, ctx->Ub, ctx->stream));     // K = 0 on the boundary layers

@@ -390,6 +390,8 @@ def test_step_stage_order_and_rows_roundtrip():
     g.step_stage(1)
     with pytest.raises(clt.CltError):
         g.step(1)                             # refused in the middle of a step
+    with pytest.raises(clt.CltError):
+        g.rhs()                               # ... and so is clt_rhs (it uses U_b as scratch)
     for s in (2, 3, 4):
         g.step_stage(s)
     assert np.array_equal(g.get_state(), ref.get_state())      # four stages = one clt_step, bit for bit
