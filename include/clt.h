@@ -122,7 +122,8 @@ int clt_set_state(clt_ctx *ctx, const double *U);
 int clt_get_state(clt_ctx *ctx, double *U);
 
 /* dUdt[8][nphi][nZ][nR] = right-hand side of eqs (11)-(14) at the current state; exactly 0 on the
- * boundary layers.  Does not change the state.  Synchronous if dUdt is host memory.               */
+ * boundary layers.  Does not change the state.  Synchronous if dUdt is host memory.  CLT_ESTATE
+ * between clt_step_stage(1) and clt_step_stage(4) (the call uses U_b as scratch).                  */
 int clt_rhs(clt_ctx *ctx, double *dUdt);
 
 /* J1[3][nphi][nZ][nR] = curl(B - B0) of the current state (eq (6)); 0 on the boundary layers.     */
