@@ -193,7 +193,8 @@ int clt_set_phi_scheme(clt_ctx *ctx, int scheme, void *d_scratch, size_t bytes);
 
 /* Launch-shape knobs for measurement (all optional; 0 = library default): tile height in Z of the
  * fused RHS kernel, number of phi chunks per tile (default: 1, more on grids with fewer tiles than the
- * device has SMs), use of a CUDA graph for clt_step.  None of them changes a bit of the result.   */
+ * device has SMs), use of a CUDA graph for the 8 launches of a clt_step step (0 = default: yes, unless
+ * per-kernel profiling is on; 1 = always; 2 = never).  None of them changes a bit of the result.   */
 int clt_set_tuning(clt_ctx *ctx, int tile_z, int phi_chunks, int use_graph);
 
 /* Selects the implementation of the fused RHS kernel: 0 (default) = shared-memory tiles fed by TMA
@@ -202,7 +203,7 @@ int clt_set_tuning(clt_ctx *ctx, int tile_z, int phi_chunks, int use_graph);
  * two are bit-identical.                                                                          */
 int clt_set_kernel_variant(clt_ctx *ctx, int variant);
 
-/* Per-kernel device timing for the roofline report.  With profiling enabled (and use_graph = 0)
+/* Per-kernel device timing for the roofline report.  With profiling enabled (and use_graph != 1)
  * every hot-path launch of clt_step / clt_rhs is bracketed by CUDA events on the context's stream;
  * clt_get_profile() synchronises, sums the elapsed times per kernel kind since profiling was
  * (re-)enabled, and resets the record.  rhs index = RK4 stage 1..4, 0 = clt_rhs' K-only variant.

@@ -228,7 +228,7 @@ constexpr size_t MAX_PROFILED = 8192;
 // returns the index of the event pair to use for this launch, or -1
 long prof_begin(clt_ctx *ctx, int kind)
 {
-    if (!ctx->profiling || ctx->use_graph) { ctx->prof_chain = false; return -1; }
+    if (!ctx->profiling || ctx->use_graph == 1) { ctx->prof_chain = false; return -1; }
     if (ctx->ev_used >= MAX_PROFILED) { ctx->ev_dropped++; ctx->prof_chain = false; return -1; }
     if (ctx->ev->size() < 2 * (ctx->ev_used + 1)) {
         cudaEvent_t a, b;
@@ -645,7 +645,8 @@ int clt_step(clt_ctx *ctx, int n)
     if (!ctx || n < 0) return CLT_EINVAL;
     if (!ctx->has_state || ctx->next_stage != 1) return CLT_ESTATE;
     if (!(ctx->dt > 0.0)) return CLT_EINVAL;
-    if (ctx->use_graph) {
+    // CUDA graph of the 8-launch step: 1 = always, 2 = never, 0 (default) = unless per-kernel profiling is on
+    if (ctx->use_graph == 1 || (ctx->use_graph == 0 && !ctx->profiling)) {
         const bool stale = !ctx->graph_exec || ctx->graph_dt != ctx->dt || ctx->graph_tile_z != effective_tile_z(ctx)
                            || ctx->graph_chunks != effective_chunks(ctx) || ctx->graph_v0 != ctx->has_v0;
         if (stale) {
@@ -889,10 +890,10 @@ int clt_set_tuning(clt_ctx *ctx, int tile_z, int phi_chunks, int use_graph)
     if (!ctx) return CLT_EINVAL;
     if (tile_z != 0 && tile_z != 7 && tile_z != 8 && tile_z != 10 && tile_z != 12 && tile_z != 13 && tile_z != 14 && tile_z != 16)
         return CLT_EINVAL;
-    if (phi_chunks < 0 || phi_chunks > 64) return CLT_EINVAL;
+    if (phi_chunks < 0 || phi_chunks > 64 || use_graph < 0 || use_graph > 2) return CLT_EINVAL;
     ctx->tile_z = tile_z;
     ctx->phi_chunks = phi_chunks;
-    ctx->use_graph = use_graph ? 1 : 0;
+    ctx->use_graph = use_graph;
     return CLT_OK;
 }
 

@@ -91,9 +91,10 @@ def test_config2_100_steps_match_oracle():
     assert_close(g.get_state(), o.get_state(), STEP_TOL, "config 2, 100 RK4 steps")
 
 
-@pytest.mark.parametrize("chunks,graph,variant,tile_z", [(2, 0, 0, 0), (4, 0, 0, 0), (1, 1, 0, 0), (2, 1, 0, 0), (3, 1, 1, 12)])
+@pytest.mark.parametrize("chunks,graph,variant,tile_z", [(2, 2, 0, 0), (4, 2, 0, 0), (1, 1, 0, 0), (2, 1, 0, 0), (3, 1, 1, 12), (1, 2, 0, 0)])
 def test_phi_chunks_and_graph_give_identical_bits(chunks, graph, variant, tile_z):
-    """The launch shape along phi and the CUDA-graph path do not change a single bit of the result."""
+    """The launch shape along phi and the CUDA-graph path (0 = default: on, 1 = on, 2 = off) do not change a single bit of
+    the result."""
     prob = inputs.make_problem(1)
     g0 = make_gpu(prob)
     g0.set_kernel_variant(variant)
