@@ -4,4 +4,4 @@ The product is the C-ABI library ``libclt.so`` (``include/clt.h``; CUDA sources 
 ``clt`` is the thin ctypes binding with the same names; ``inputs`` is the seeded synthetic workload
 recipe shared with the tests of the CPU oracle.  Nothing here imports ``oracle``.
 """
-__all__ = ["inputs", "clt"]
+__all__ = ["inputs", "clt", "slab", "replicas", "build"]
