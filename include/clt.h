@@ -162,10 +162,13 @@ int clt_set_owned_rows(clt_ctx *ctx, int k_first, int k_last, int deep_first, in
  * stage-4 epilogue of the fused kernel (no extra pass over the state, no host round trip per step).  cfl <= 0 means
  * params.cfl.  Synchronises once at the end to report *dt_last (SETDT of the final state, i.e. the step the next call
  * would start with) and *time_advanced (sum of the n steps); either pointer may be NULL.  params.dt is unchanged.
- * Slabs need the global minimum instead: slab.py's step_cfl reduces clt_suggest_dt over the slabs every step.  */
+ * Slabs need the global minimum instead: slab.py's step_cfl reduces clt_suggest_dt over the slabs every step.
+ * CLT_ENONFINITE if a state of the call had a non-finite signal speed (NaN / Inf in rho, p, v or B): the device
+ * clock then holds dt = 0 for the remaining steps of the call instead of stepping on with a meaningless dt.  */
 int clt_step_cfl(clt_ctx *ctx, int n, double cfl, double *dt_last, double *time_advanced);
 
-/* Changes the fixed time step (dt > 0, finite).                                                  */
+/* Changes the fixed time step (dt > 0, finite).  Stream-ordered: steps already enqueued keep their dt; the CUDA
+ * graph of the step is kept (the kernels read dt/2, dt/3, dt/6 from device memory).             */
 int clt_set_dt(clt_ctx *ctx, double dt);
 
 /* Reductions over the current state; synchronises the stream.  CLT_ENONFINITE if a sum is not
@@ -178,29 +181,28 @@ int clt_diagnostics(clt_ctx *ctx, clt_diag *out);
 int clt_suggest_dt(clt_ctx *ctx, double cfl, double *dt_out);
 
 /* phi scheme [L125: "either 4th order finite difference or pseudo-spectrum method can be used"].
- * scheme 0 (default) = 4th-order central differences; 1 = pseudo-spectral (2 = the same, but its pre-pass uses a
- * shared-memory radix-2 FFT instead of the circulant sums when nphi = 8, 16, .. 128; kept for A/B measurements,
- * measured slower): every d/dphi and d2/dphi2 of the
+ * scheme 0 (default) = 4th-order central differences; 1 = pseudo-spectral: every d/dphi and d2/dphi2 of the
  * path (curl, gradients, divergences, Laplacians, curl E, div_c B of the diagnostics) is the exact derivative
  * of the trigonometric interpolant through the nphi samples (Nyquist mode: first derivative 0, second
  * derivative -(pi nphi/L)^2; reading R12).  It needs a second caller-owned DEVICE scratch buffer of
  * clt_spectral_workspace_bytes(grid) bytes (256-byte aligned; 14 padded fields), kept alive until the scheme is
- * set back to 0 or the context is destroyed, nphi <= 256, and the default kernel variant and tile height
+ * set back to 0 or the context is destroyed, nphi <= 256, and the default kernel variant
  * (clt_rhs / clt_step return CLT_EINVAL otherwise).  Synchronises the stream.
  * Errors: CLT_EINVAL (scheme, nphi > 256), CLT_ENOMEM (scratch missing, small, misaligned, not device).   */
 size_t clt_spectral_workspace_bytes(const clt_grid *grid);
 int clt_set_phi_scheme(clt_ctx *ctx, int scheme, void *d_scratch, size_t bytes);
 
 /* Launch-shape knobs for measurement (all optional; 0 = library default): tile height in Z of the
- * fused RHS kernel, number of phi chunks per tile (default: 1, more on grids with fewer tiles than the
+ * fused RHS kernel (one shape is built: 0 or 8, anything else is CLT_EINVAL), number of phi chunks per tile
+ * (default: 1, more on grids with fewer tiles than the
  * device has SMs), use of a CUDA graph for the 8 launches of a clt_step step (0 = default: yes, unless
  * per-kernel profiling is on; 1 = always; 2 = never).  None of them changes a bit of the result.   */
 int clt_set_tuning(clt_ctx *ctx, int tile_z, int phi_chunks, int use_graph);
 
 /* Selects the implementation of the fused RHS kernel: 0 (default) = shared-memory tiles fed by TMA
- * (cp.async.bulk.tensor + mbarrier), 1 = the same arithmetic fed by plain global loads (kept for A/B
- * measurements; also used for tile heights the TMA variant has no shared memory for).  Results of the
- * two are bit-identical.                                                                          */
+ * (cp.async.bulk.tensor + mbarrier), 1 = the same arithmetic fed by plain global loads (kept as the A/B
+ * measurement and as a parity cross-check; no Hall term, no pseudo-spectral scheme).  The two agree to
+ * round-off (separate template instantiations: the compiler may contract FMAs differently).       */
 int clt_set_kernel_variant(clt_ctx *ctx, int variant);
 
 /* Per-kernel device timing for the roofline report.  With profiling enabled (and use_graph != 1)

@@ -38,7 +38,6 @@ struct clt_ctx {
     int sm_count;                  // multiprocessors of that device (automatic phi chunking of small grids)
     int device;                    // the device the workspace lives on (every call runs with it current)
     int next_stage;                // clt_step_stage: the stage expected next (1..4)
-    bool spec_fft;                 // pseudo-spectral pre-pass by FFT where nphi allows (scheme 2) instead of the circulant sums
     bool spectral;                 // pseudo-spectral phi scheme (clt_set_phi_scheme)
     double *spec, *spec_ctab;      // caller-provided scratch: SPEC_COUNT derivative fields + circulant weights
 
@@ -46,12 +45,16 @@ struct clt_ctx {
     double time;
     double dt;
     int64_t launches;
-    int tile_z, phi_chunks, use_graph;
+    int phi_chunks, use_graph;
     int variant;      // 0 = TMA-fed fused RHS kernel (default), 1 = plain-load variant
     cudaGraphExec_t graph_exec;
-    double graph_dt;
-    int graph_tile_z, graph_chunks;
+    int graph_chunks;
     bool graph_v0;
+    // "does the reference state move?" is decided on the device (any_nonzero_kernel) and read back lazily, so that
+    // clt_set_equilibrium stays asynchronous: pinned flag + the event that marks its copy
+    int *v0_flag_host;
+    cudaEvent_t v0_event;
+    bool v0_pending;
     char cuda_err[256];
     // per-kernel event timing (clt_set_profiling)
     bool profiling;
@@ -116,7 +119,9 @@ Carve carve(const clt_grid *g)
     c.cs_b = align_up((size_t)2 * g->nphi * sizeof(double));
     c.nblocks = diag_blocks(L);
     c.partial_b = align_up((size_t)c.nblocks * 6 * sizeof(double));
-    c.result_b = align_up(32 * sizeof(double));     // 6 diagnostics + the device clock of clt_step_cfl (at +8) + dt minimum (at +16)
+    // 6 diagnostics + the device clock of clt_step_cfl (6 doubles at +8) + dt minimum (at +16) + the fixed-dt stage
+    // coefficients (4 doubles at +24) + the "v0 != 0" flag (at +28)
+    c.result_b = align_up(32 * sizeof(double));
     c.total = 38 * c.field_b + T_COUNT * c.table_b + 2 * c.rtab_b + c.cs_b + c.partial_b + c.result_b;
     return c;
 }
@@ -152,6 +157,8 @@ int copy_out(clt_ctx *ctx, double *dst, const double *src_padded, size_t rows)
 
 void free_profile(clt_ctx *ctx)
 {
+    if (ctx->v0_flag_host) { cudaFreeHost(ctx->v0_flag_host); ctx->v0_flag_host = nullptr; }
+    if (ctx->v0_event) { cudaEventDestroy(ctx->v0_event); ctx->v0_event = nullptr; }
     if (ctx->ev) {
         for (cudaEvent_t e : *ctx->ev) cudaEventDestroy(e);
         delete ctx->ev;
@@ -171,7 +178,16 @@ void destroy_graph(clt_ctx *ctx)
     }
 }
 
-int effective_tile_z(const clt_ctx *ctx) { return ctx->tile_z ? ctx->tile_z : rhs_default_tile_z(); }
+// the kernels' v0 = 0 specialisation is chosen on the host: wait (once) for the flag clt_set_equilibrium requested
+int resolve_v0(clt_ctx *ctx)
+{
+    if (!ctx->v0_pending) return CLT_OK;
+    cudaError_t e = cudaEventSynchronize(ctx->v0_event);
+    if (e != cudaSuccess) { snprintf(ctx->cuda_err, sizeof(ctx->cuda_err), "v0 flag: %s", cudaGetErrorString(e)); return CLT_ECUDA; }
+    ctx->has_v0 = *ctx->v0_flag_host != 0;
+    ctx->v0_pending = false;
+    return CLT_OK;
+}
 
 // cuTensorMapEncodeTiled through the runtime's driver entry point (no link-time dependency on libcuda)
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
@@ -200,7 +216,7 @@ bool make_map(const clt_ctx *ctx, const double *base, int nfields, int tile_z, C
     const Layout &L = ctx->L;
     const cuuint64_t dims[4] = { (cuuint64_t)L.pR, (cuuint64_t)L.nZ, (cuuint64_t)L.nphi, (cuuint64_t)nfields };
     const cuuint64_t strides[3] = { (cuuint64_t)L.pR * 8, (cuuint64_t)L.plane * 8, (cuuint64_t)L.field * 8 };
-    const cuuint32_t box[4] = { 32 + 4, (cuuint32_t)tile_z + 4, 1, 1 };
+    const cuuint32_t box[4] = { 32 + 4, (cuuint32_t)tile_z + 4, 1, 1 };      // tile with the radius-2 halo
     const cuuint32_t estr[4] = { 1, 1, 1, 1 };
     return enc(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, (void *)base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                CU_TENSOR_MAP_SWIZZLE_NONE, CLT_L2_PROMO, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE)
@@ -214,7 +230,7 @@ int effective_chunks(const clt_ctx *ctx)
 {
     int c = ctx->phi_chunks;
     if (c == 0) {
-        const int tiles = ((ctx->L.nR - 4 + 31) / 32) * ((ctx->L.nZ - 4 + 7) / 8);
+        const int tiles = ((ctx->L.nR - 4 + 31) / 32) * ((ctx->L.nZ - 4 + rhs_tile_z() - 1) / rhs_tile_z());
         c = ctx->sm_count / (tiles > 0 ? tiles : 1);
         if (c > ctx->L.nphi / 8) c = ctx->L.nphi / 8;
         if (c < 1) c = 1;
@@ -259,13 +275,8 @@ void prof_end(clt_ctx *ctx, long n)
     }
 }
 
-// kernels one phi pre-pass launches: the FFT variant does everything in one, the circulant sums need two in mode 1
-int phi_launches(const clt_ctx *ctx, int mode)
-{
-    const int N = ctx->L.nphi;
-    const bool fft = ctx->spec_fft && N >= 8 && N <= 128 && (N & (N - 1)) == 0;
-    return (mode == 0 || fft) ? 1 : 2;
-}
+// kernels one phi pre-pass launches
+int phi_launches(const clt_ctx *, int mode) { return mode == 0 ? 1 : 2; }
 
 // NEXT-2: pseudo-spectral phi derivatives of the stage state U (mode 0: what the curl needs, 1: what the RHS needs)
 int run_phi_pass(clt_ctx *ctx, int mode, const double *U)
@@ -275,7 +286,6 @@ int run_phi_pass(clt_ctx *ctx, int mode, const double *U)
     a.U = U; a.J1 = ctx->J1; a.tab = ctx->tab;
     a.out = ctx->spec; a.ctab = ctx->spec_ctab;
     a.mode = mode; a.hall = ctx->hall ? 1 : 0; a.has_v0 = ctx->has_v0 ? 1 : 0;
-    a.use_fft = ctx->spec_fft ? 1 : 0;
     const long pe = prof_begin(ctx, 6);
     CK(launch_phi_spectral(a, ctx->stream));
     prof_end(ctx, pe);
@@ -313,13 +323,13 @@ int run_curl(clt_ctx *ctx, const double *U)
     if (tma)
         CK(launch_curl_tma(a, &tmU, ctx->hall, ctx->spectral, ctx->stream));
     else
-        CK(launch_curl(a, 0, ctx->stream));
+        CK(launch_curl(a, ctx->stream));
     prof_end(ctx, pe);
     ctx->launches++;
     return CLT_OK;
 }
 
-int run_rhs(clt_ctx *ctx, int mode, const double *in, double *out, double a_next, double b_acc)
+int run_rhs(clt_ctx *ctx, int mode, const double *in, double *out)
 {
     RhsArgs a;
     a.L = ctx->L; a.ph = ctx->ph;
@@ -327,18 +337,17 @@ int run_rhs(clt_ctx *ctx, int mode, const double *in, double *out, double a_next
     a.tab = ctx->tab;
     a.R = ctx->Rtab + LP;
     a.invR = ctx->invRtab + LP;
-    a.a_next = a_next; a.b_acc = b_acc;
     a.phi_chunks = effective_chunks(ctx);
     a.prefetch = CLT_PREFETCH;
     a.spec = ctx->spec;
-    a.coef = ctx->adaptive ? ctx->result + 8 : nullptr;
+    // stage coefficients: the device clock inside clt_step_cfl, else the fixed-dt table clt_set_dt keeps up to date
+    a.coef = ctx->adaptive ? ctx->result + 8 : ctx->result + 24;
     a.dtmin_bits = ctx->adaptive ? (unsigned long long *)(ctx->result + 16) : nullptr;
     a.cfl = ctx->adaptive_cfl;
-    const int tz = effective_tile_z(ctx);
-    const bool tma = ctx->variant == 0 && rhs_tma_supports(tz, ctx->hall, ctx->spectral);
+    const bool tma = ctx->variant == 0;
     if ((ctx->hall || ctx->spectral) && !tma) {
         snprintf(ctx->cuda_err, sizeof(ctx->cuda_err),
-                 "the Hall term and the pseudo-spectral phi scheme need the default kernel variant and tile height");
+                 "the Hall term and the pseudo-spectral phi scheme need the default kernel variant");
         return CLT_EINVAL;
     }
     if (ctx->spectral) {
@@ -346,15 +355,15 @@ int run_rhs(clt_ctx *ctx, int mode, const double *in, double *out, double a_next
         if (r) return r;
     }
     alignas(64) CUtensorMap tmU, tmJ;
-    if (tma && (!make_map(ctx, in, 8, tz, &tmU) || !make_map(ctx, ctx->J1, ctx->hall ? 6 : 3, tz, &tmJ))) {
+    if (tma && (!make_map(ctx, in, 8, rhs_tile_z(), &tmU) || !make_map(ctx, ctx->J1, ctx->hall ? 6 : 3, rhs_tile_z(), &tmJ))) {
         snprintf(ctx->cuda_err, sizeof(ctx->cuda_err), "cuTensorMapEncodeTiled failed");
         return CLT_ECUDA;
     }
     const long pe = prof_begin(ctx, mode);
     if (tma)
-        CK(launch_rhs_tma(a, &tmU, &tmJ, mode, ctx->has_v0, ctx->hall, ctx->spectral, tz, ctx->stream));
+        CK(launch_rhs_tma(a, &tmU, &tmJ, mode, ctx->has_v0, ctx->hall, ctx->spectral, ctx->stream));
     else
-        CK(launch_rhs(a, mode, ctx->has_v0, tz, ctx->stream));
+        CK(launch_rhs(a, mode, ctx->has_v0, ctx->stream));
     prof_end(ctx, pe);
     ctx->launches++;
     return CLT_OK;
@@ -365,21 +374,21 @@ int run_rhs(clt_ctx *ctx, int mode, const double *in, double *out, double a_next
 //   s3: Ua = Un + dt K3                            s4: Un = acc + (Ua - Un)/3 + dt/6 K4
 int enqueue_stage(clt_ctx *ctx, int stage)
 {
-    const double dt = ctx->dt;
     int r;
+    if ((r = resolve_v0(ctx))) return r;
     switch (stage) {
     case 1:
         if ((r = run_curl(ctx, ctx->Un))) return r;
-        return run_rhs(ctx, RHS_MODE_S1, ctx->Un, ctx->Ua, 0.5 * dt, 0.0);
+        return run_rhs(ctx, RHS_MODE_S1, ctx->Un, ctx->Ua);
     case 2:
         if ((r = run_curl(ctx, ctx->Ua))) return r;
-        return run_rhs(ctx, RHS_MODE_S2, ctx->Ua, ctx->Ub, 0.5 * dt, dt / 3.0);
+        return run_rhs(ctx, RHS_MODE_S2, ctx->Ua, ctx->Ub);
     case 3:
         if ((r = run_curl(ctx, ctx->Ub))) return r;
-        return run_rhs(ctx, RHS_MODE_S3, ctx->Ub, ctx->Ua, dt, 0.0);
+        return run_rhs(ctx, RHS_MODE_S3, ctx->Ub, ctx->Ua);
     case 4:
         if ((r = run_curl(ctx, ctx->Ua))) return r;
-        return run_rhs(ctx, RHS_MODE_S4, ctx->Ua, ctx->Un, 0.0, dt / 6.0);
+        return run_rhs(ctx, RHS_MODE_S4, ctx->Ua, ctx->Un);
     default:
         return CLT_EINVAL;
     }
@@ -514,8 +523,15 @@ int clt_create(const clt_grid *grid, const clt_params *params, void *d_workspace
         if ((e = cudaMemcpyAsync(ctx->invRtab, iR.data(), iR.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream))) break;
         if ((e = cudaMemcpyAsync(ctx->cs, cs.data(), cs.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream))) break;
         if ((e = cudaStreamSynchronize(ctx->stream))) break;     // the host vectors go out of scope
+        if ((e = configure_kernels())) break;                    // shared-memory opt-in of this context's device
+        if ((e = cudaHostAlloc((void **)&ctx->v0_flag_host, sizeof(int), cudaHostAllocDefault))) break;
+        if ((e = cudaEventCreateWithFlags(&ctx->v0_event, cudaEventDisableTiming))) break;
         if ((e = launch_tables(ctx->L, ctx->ph, ctx->tab, ctx->Rtab + LP, ctx->invRtab + LP, ctx->stream))) break;
         ctx->launches++;
+        if (ctx->dt > 0.0) {
+            const double dt = ctx->dt, c4[4] = { dt, 0.5 * dt, dt / 3.0, dt / 6.0 };
+            if ((e = cudaMemcpyAsync(ctx->result + 24, c4, sizeof(c4), cudaMemcpyHostToDevice, ctx->stream))) break;
+        }
     } while (0);
     if (e != cudaSuccess) {
         free_profile(ctx);
@@ -545,23 +561,26 @@ int clt_set_equilibrium(clt_ctx *ctx, const double *U0)
     if (!ctx) return CLT_EINVAL;
     ctx->has_state = false;
     const size_t rows = (size_t)8 * ctx->L.nZ;
-    bool v0 = false;
+    ctx->has_v0 = false;
+    ctx->v0_pending = false;
     if (U0) {
         int r = copy_in(ctx, ctx->tab, U0, rows);          // tables 0..7 are U0 itself
         if (r) return r;
-        // does the reference state move?  (selects the v0 = 0 specialisation of the kernels)
-        const size_t n = (size_t)3 * ctx->L.nZ * ctx->L.nR;
-        std::vector<double> h(n);
-        CK(cudaMemcpy2DAsync(h.data(), (size_t)ctx->L.nR * sizeof(double), ctx->tab + T_V0R * ctx->L.plane + LP,
-                             (size_t)ctx->L.pR * sizeof(double), (size_t)ctx->L.nR * sizeof(double), (size_t)3 * ctx->L.nZ,
-                             cudaMemcpyDeviceToHost, ctx->stream));
-        CK(cudaStreamSynchronize(ctx->stream));
-        for (size_t q = 0; q < n; ++q)
-            if (h[q] != 0.0) { v0 = true; break; }
+        // does the reference state move?  (selects the v0 = 0 specialisation of the kernels)  Decided on the device; the
+        // flag is read back when the first kernel that needs it is launched (resolve_v0), so this call stays asynchronous
+        int *flag = (int *)(ctx->result + 28);
+        CK(launch_any_nonzero(ctx->tab + T_V0R * ctx->L.plane, 3 * ctx->L.plane, flag, ctx->stream));
+        ctx->launches++;
+        CK(cudaMemcpyAsync(ctx->v0_flag_host, flag, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+        CK(cudaEventRecord(ctx->v0_event, ctx->stream));
+        ctx->v0_pending = true;
+        cudaPointerAttributes at;
+        cudaError_t e = cudaPointerGetAttributes(&at, U0);
+        if (e != cudaSuccess) { cudaGetLastError(); at.type = cudaMemoryTypeUnregistered; }
+        if (at.type != cudaMemoryTypeDevice) CK(cudaStreamSynchronize(ctx->stream));   // the caller may reuse host memory
     } else {
         CK(cudaMemsetAsync(ctx->tab, 0, (size_t)8 * ctx->L.plane * sizeof(double), ctx->stream));
     }
-    ctx->has_v0 = v0;
     CK(launch_tables(ctx->L, ctx->ph, ctx->tab, ctx->Rtab + LP, ctx->invRtab + LP, ctx->stream));
     ctx->launches++;
     return CLT_OK;
@@ -574,7 +593,7 @@ int clt_set_state(clt_ctx *ctx, const double *U)
     int r = copy_in(ctx, ctx->Un, U, (size_t)8 * ctx->L.nphi * ctx->L.nZ);
     if (r) return r;
     // a1: freeze the two boundary layers per R/Z side in every RK buffer
-    CK(launch_copy_boundary(ctx->L, 8, ctx->Un, ctx->acc, ctx->Ua, ctx->Ub, ctx->stream));
+    CK(launch_copy_boundary(ctx->L, 8, ctx->Un, ctx->acc, ctx->Ua, ctx->Ub, ctx->sm_count, ctx->stream));
     ctx->launches++;
     cudaPointerAttributes at;
     cudaError_t e = cudaPointerGetAttributes(&at, U);
@@ -601,12 +620,13 @@ int clt_rhs(clt_ctx *ctx, double *dUdt)
     if (!ctx || !dUdt) return CLT_EINVAL;
     if (!ctx->has_state || ctx->next_stage != 1) return CLT_ESTATE;      // U_b is the scratch buffer: not inside a step
     int r;
+    if ((r = resolve_v0(ctx))) return r;
     if ((r = run_curl(ctx, ctx->Un))) return r;
-    CK(launch_zero_boundary(ctx->L, 8, ctx->Ub, ctx->stream));     // K = 0 on the boundary layers
+    CK(launch_zero_boundary(ctx->L, 8, ctx->Ub, ctx->sm_count, ctx->stream));     // K = 0 on the boundary layers
     ctx->launches++;
-    if ((r = run_rhs(ctx, RHS_MODE_K, ctx->Un, ctx->Ub, 0.0, 0.0))) return r;
+    if ((r = run_rhs(ctx, RHS_MODE_K, ctx->Un, ctx->Ub))) return r;
     if ((r = copy_out(ctx, dUdt, ctx->Ub, (size_t)8 * ctx->L.nphi * ctx->L.nZ))) return r;
-    CK(launch_copy_boundary(ctx->L, 8, ctx->Un, ctx->Ub, nullptr, nullptr, ctx->stream));   // restore the scratch buffer
+    CK(launch_copy_boundary(ctx->L, 8, ctx->Un, ctx->Ub, nullptr, nullptr, ctx->sm_count, ctx->stream));   // restore the scratch buffer
     ctx->launches++;
     return CLT_OK;
 }
@@ -617,6 +637,7 @@ int clt_curl_J1(clt_ctx *ctx, double *J1)
     if (!ctx || !J1) return CLT_EINVAL;
     if (!ctx->has_state) return CLT_ESTATE;
     int r;
+    if ((r = resolve_v0(ctx))) return r;
     if ((r = run_curl(ctx, ctx->Un))) return r;
     return copy_out(ctx, J1, ctx->J1, (size_t)3 * ctx->L.nphi * ctx->L.nZ);
 }
@@ -628,15 +649,27 @@ int clt_hall_G(clt_ctx *ctx, double *G)
     if (!ctx->has_state) return CLT_ESTATE;
     if (!ctx->hall) return CLT_EINVAL;
     int r;
+    if ((r = resolve_v0(ctx))) return r;
     if ((r = run_curl(ctx, ctx->Un))) return r;
     return copy_out(ctx, G, ctx->G, (size_t)3 * ctx->L.nphi * ctx->L.nZ);
 }
 
+// { dt, dt/2, dt/3, dt/6 } -> the fixed-dt coefficient table in device memory (stream-ordered: steps already enqueued
+// keep the dt they were enqueued with; a captured graph of the step stays valid)
+static int upload_dt(clt_ctx *ctx)
+{
+    const double dt = ctx->dt;
+    const double c[4] = { dt, 0.5 * dt, dt / 3.0, dt / 6.0 };
+    CK(cudaMemcpyAsync(ctx->result + 24, c, sizeof(c), cudaMemcpyHostToDevice, ctx->stream));   // pageable source: staged before the call returns
+    return CLT_OK;
+}
+
 int clt_set_dt(clt_ctx *ctx, double dt)
 {
+    DeviceGuard device_guard(ctx);
     if (!ctx || !(dt > 0.0) || !isfinite(dt)) return CLT_EINVAL;
     ctx->dt = dt;
-    return CLT_OK;
+    return upload_dt(ctx);
 }
 
 int clt_step(clt_ctx *ctx, int n)
@@ -647,8 +680,10 @@ int clt_step(clt_ctx *ctx, int n)
     if (!(ctx->dt > 0.0)) return CLT_EINVAL;
     // CUDA graph of the 8-launch step: 1 = always, 2 = never, 0 (default) = unless per-kernel profiling is on
     if (ctx->use_graph == 1 || (ctx->use_graph == 0 && !ctx->profiling)) {
-        const bool stale = !ctx->graph_exec || ctx->graph_dt != ctx->dt || ctx->graph_tile_z != effective_tile_z(ctx)
-                           || ctx->graph_chunks != effective_chunks(ctx) || ctx->graph_v0 != ctx->has_v0;
+        int rv = resolve_v0(ctx);
+        if (rv) return rv;
+        // dt is not part of the graph: the kernels read the stage coefficients from device memory (clt_set_dt)
+        const bool stale = !ctx->graph_exec || ctx->graph_chunks != effective_chunks(ctx) || ctx->graph_v0 != ctx->has_v0;
         if (stale) {
             destroy_graph(ctx);
             cudaGraph_t g = nullptr;
@@ -670,7 +705,6 @@ int clt_step(clt_ctx *ctx, int n)
             e = cudaGraphInstantiate(&ctx->graph_exec, g, 0);
             cudaGraphDestroy(g);
             if (e != cudaSuccess) return cuda_fail(ctx, e, "cudaGraphInstantiate");
-            ctx->graph_dt = ctx->dt; ctx->graph_tile_z = effective_tile_z(ctx);
             ctx->graph_chunks = effective_chunks(ctx); ctx->graph_v0 = ctx->has_v0;
         }
         for (int s = 0; s < n; ++s) {
@@ -694,7 +728,7 @@ static int run_diag(clt_ctx *ctx, double cfl, double out6[6])
     a.L = ctx->L; a.ph = ctx->ph;
     a.U = ctx->Un; a.tab = ctx->tab;
     a.R = ctx->Rtab + LP; a.invR = ctx->invRtab + LP;
-    a.cs = ctx->cs; a.partial = ctx->partial; a.cfl = cfl;
+    a.cs = ctx->cs; a.partial = ctx->partial; a.cfl = cfl; a.ihZ = 1.0 / ctx->ph.dZ;
     a.spec_c1 = ctx->spectral ? ctx->spec_ctab : nullptr;
     a.k_first = ctx->k_first; a.k_last = ctx->k_last; a.kd_first = ctx->kd_first; a.kd_last = ctx->kd_last;
     CK(launch_diag(a, ctx->nblocks_diag, ctx->result, ctx->stream));
@@ -732,19 +766,20 @@ int clt_suggest_dt(clt_ctx *ctx, double cfl, double *dt_out)
     int r = run_diag(ctx, cfl, r6);
     if (r) return r;
     *dt_out = r6[5];
+    if (!(r6[5] > 0.0)) return CLT_ENONFINITE;      // a non-finite signal speed somewhere in the state
     return CLT_OK;
 }
 
 size_t clt_spectral_workspace_bytes(const clt_grid *grid)
 {
     if (!grid_ok(grid) || grid->nphi > SPEC_MAX_NPHI) return 0;
-    return (size_t)SPEC_COUNT * carve(grid).field_b + align_up(3 * SPEC_MAX_NPHI * sizeof(double));
+    return (size_t)SPEC_COUNT * carve(grid).field_b + align_up(2 * SPEC_MAX_NPHI * sizeof(double));
 }
 
 int clt_set_phi_scheme(clt_ctx *ctx, int scheme, void *d_scratch, size_t bytes)
 {
     DeviceGuard device_guard(ctx);
-    if (!ctx || scheme < 0 || scheme > 2) return CLT_EINVAL;
+    if (!ctx || scheme < 0 || scheme > 1) return CLT_EINVAL;
     CK(cudaStreamSynchronize(ctx->stream));
     destroy_graph(ctx);
     if (scheme == 0) { ctx->spectral = false; ctx->spec = nullptr; ctx->spec_ctab = nullptr; return CLT_OK; }
@@ -763,7 +798,7 @@ int clt_set_phi_scheme(clt_ctx *ctx, int scheme, void *d_scratch, size_t bytes)
     const int N = ctx->grid.nphi;
     const long double PI = 3.141592653589793238462643383279502884L;
     const long double kap = 2.0L * PI / (long double)ctx->ph.Lphi;
-    std::vector<double> tabv(3 * SPEC_MAX_NPHI, 0.0);
+    std::vector<double> tabv(2 * SPEC_MAX_NPHI, 0.0);
     for (int m = 0; m < N; ++m) {
         long double c1, c2;
         const long double th = PI * (long double)m / (long double)N, sg = (m % 2) ? -1.0L : 1.0L;
@@ -780,11 +815,6 @@ int clt_set_phi_scheme(clt_ctx *ctx, int scheme, void *d_scratch, size_t bytes)
         tabv[m] = (double)c1;
         tabv[SPEC_MAX_NPHI + m] = (double)c2;
     }
-    if (N <= SPEC_MAX_NPHI)
-        for (int n = 0; n < N / 2 && n < SPEC_MAX_NPHI / 2; ++n) {      // FFT twiddles exp(2 pi i n/N)
-            tabv[2 * SPEC_MAX_NPHI + n] = (double)cosl(2.0L * PI * (long double)n / (long double)N);
-            tabv[2 * SPEC_MAX_NPHI + SPEC_MAX_NPHI / 2 + n] = (double)sinl(2.0L * PI * (long double)n / (long double)N);
-        }
     const size_t fields_b = (size_t)SPEC_COUNT * carve(&ctx->grid).field_b;
     ctx->spec = (double *)d_scratch;
     ctx->spec_ctab = (double *)((char *)d_scratch + fields_b);
@@ -792,7 +822,6 @@ int clt_set_phi_scheme(clt_ctx *ctx, int scheme, void *d_scratch, size_t bytes)
     CK(cudaMemcpyAsync(ctx->spec_ctab, tabv.data(), tabv.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
     ctx->spectral = true;
-    ctx->spec_fft = scheme == 2;
     return CLT_OK;
 }
 
@@ -848,14 +877,14 @@ int clt_step_cfl(clt_ctx *ctx, int n, double cfl, double *dt_last, double *time_
     if (!(cfl > 0.0) || !isfinite(cfl)) return CLT_EINVAL;
     double *clock = ctx->result + 8;
     unsigned long long *bits = (unsigned long long *)(ctx->result + 16);
-    double h[5] = { 0, 0, 0, 0, 0 };
+    double h[6] = { 0, 0, 0, 0, 0, 0 };
     if (n > 0) {
         // dt of the first step: SETDT of the current state (the reduction kernel of clt_suggest_dt, no host round trip)
         DiagArgs a;
         a.L = ctx->L; a.ph = ctx->ph;
         a.U = ctx->Un; a.tab = ctx->tab;
         a.R = ctx->Rtab + LP; a.invR = ctx->invRtab + LP;
-        a.cs = ctx->cs; a.partial = ctx->partial; a.cfl = cfl;
+        a.cs = ctx->cs; a.partial = ctx->partial; a.cfl = cfl; a.ihZ = 1.0 / ctx->ph.dZ;
         a.spec_c1 = ctx->spectral ? ctx->spec_ctab : nullptr;
         a.k_first = ctx->k_first; a.k_last = ctx->k_last; a.kd_first = ctx->kd_first; a.kd_last = ctx->kd_last;
         CK(launch_diag(a, ctx->nblocks_diag, ctx->result, ctx->stream));
@@ -882,16 +911,17 @@ int clt_step_cfl(clt_ctx *ctx, int n, double cfl, double *dt_last, double *time_
     ctx->time += h[4];
     if (dt_last) *dt_last = h[0];          // the SETDT value of the final state = the dt the next step would use
     if (time_advanced) *time_advanced = h[4];
+    // a state whose signal speed is not finite (NaN / Inf anywhere in rho, p, B, or a NaN velocity) raised the clock's
+    // mark and froze dt at 0: the call reports it instead of stepping on with a meaningless dt
+    if (h[5] != 0.0) return CLT_ENONFINITE;
     return CLT_OK;
 }
 
 int clt_set_tuning(clt_ctx *ctx, int tile_z, int phi_chunks, int use_graph)
 {
     if (!ctx) return CLT_EINVAL;
-    if (tile_z != 0 && tile_z != 7 && tile_z != 8 && tile_z != 10 && tile_z != 12 && tile_z != 13 && tile_z != 14 && tile_z != 16)
-        return CLT_EINVAL;
+    if (tile_z != 0 && tile_z != rhs_tile_z()) return CLT_EINVAL;     // one tile shape is built (32 x 8); 0 = default
     if (phi_chunks < 0 || phi_chunks > 64 || use_graph < 0 || use_graph > 2) return CLT_EINVAL;
-    ctx->tile_z = tile_z;
     ctx->phi_chunks = phi_chunks;
     ctx->use_graph = use_graph;
     return CLT_OK;

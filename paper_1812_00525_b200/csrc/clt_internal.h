@@ -57,14 +57,13 @@ struct RhsArgs {
     const double *tab;    // T_COUNT tables
     const double *R;      // R_i, i = -LP .. : pointer already offset so that R[i] is node i; padded with valid numbers
     const double *invR;   // 1/R_i, same indexing
-    double a_next;        // out = U^n + a_next * K   (modes 1-3)
-    double b_acc;         // weight of K in the accumulator (mode 2) / in U^{n+1} (mode 4)
     int phi_chunks;       // number of chunks the phi range is split into (gridDim.z)
     int prefetch;         // issue L2 prefetch hints
     const double *spec;   // pseudo-spectral variant: SPEC_COUNT derivative fields (SpecField)
-    // adaptive stepping (clt_step_cfl): non-null = take the stage coefficients from the device clock
-    // { dt, dt/2, dt/3, dt/6, time } instead of a_next / b_acc; stage 4 folds the SETDT minimum into *dtmin_bits
+    // stage coefficients { dt, dt/2, dt/3, dt/6 } in device memory: the fixed-dt table of clt_set_dt or the device clock of
+    // clt_step_cfl (so a captured CUDA graph of the step does not bake dt in)
     const double *coef;
+    // adaptive stepping (clt_step_cfl): non-null = stage 4 folds the SETDT minimum of the new state into *dtmin_bits
     unsigned long long *dtmin_bits;
     double cfl;
 };
@@ -101,10 +100,8 @@ struct SpecArgs {
     const double *J1;     // 3 fields (+ G behind them when hall)
     const double *tab;
     double *out;          // SPEC_COUNT fields
-    const double *ctab;   // [3][SPEC_MAX_NPHI]: circulant weights c1[m] (antisymmetric in m), c2[m] (symmetric), and the
-                          // FFT twiddles cos(2 pi n/N), n < N/2, then sin(2 pi n/N) at offset SPEC_MAX_NPHI/2
+    const double *ctab;   // [2][SPEC_MAX_NPHI]: circulant weights c1[m] (antisymmetric in m), c2[m] (symmetric)
     int mode, hall, has_v0;
-    int use_fft;          // 1: FFT pre-pass where nphi allows (power of two, 8..128), 0: circulant sums always
 };
 
 struct DiagArgs {
@@ -118,35 +115,38 @@ struct DiagArgs {
     double *partial;      // [nblocks][6]
     double cfl;
     const double *spec_c1;   // non-null: pseudo-spectral d/dphi in div_c B, weights c1[0..nphi-1]
+    double ihZ;              // 1 / dZ
     int k_first, k_last;     // rows the sums / the SETDT minimum run over (default 2 .. nZ-3; a slab's owned rows)
     int kd_first, kd_last;   // rows of the max |div_c B| (default 4 .. nZ-5)
 };
 
 enum { RHS_MODE_K = 0, RHS_MODE_S1 = 1, RHS_MODE_S2 = 2, RHS_MODE_S3 = 3, RHS_MODE_S4 = 4 };
 
-// kernel launchers (clt_kernels.cu); each returns the cudaGetLastError() of its launch
+// kernel launchers (clt_kernels.cu); each returns the cudaGetLastError() of its launch.  configure = true: do not
+// launch, only opt the kernel in to its dynamic shared-memory size on the current device (configure_kernels)
 cudaError_t launch_tables(const Layout &L, const Phys &ph, double *tab, const double *R, const double *invR,
                           cudaStream_t s);
+cudaError_t launch_any_nonzero(const double *x, long long n, int *flag, cudaStream_t s);
 cudaError_t launch_copy_boundary(const Layout &L, int nfields, const double *src, double *d0, double *d1, double *d2,
-                                 cudaStream_t s);
-cudaError_t launch_zero_boundary(const Layout &L, int nfields, double *dst, cudaStream_t s);
-cudaError_t launch_curl(const CurlArgs &a, int tile_z, cudaStream_t s);
-cudaError_t launch_rhs(const RhsArgs &a, int mode, bool has_v0, int tile_z, cudaStream_t s);
+                                 int sm_count, cudaStream_t s);
+cudaError_t launch_zero_boundary(const Layout &L, int nfields, double *dst, int sm_count, cudaStream_t s);
+// plain-load variants (kernel variant 1: A/B and parity cross-check of the TMA-fed default)
+cudaError_t launch_curl(const CurlArgs &a, cudaStream_t s);
+cudaError_t launch_rhs(const RhsArgs &a, int mode, bool has_v0, cudaStream_t s, bool configure = false);
 // TMA variant: tmU / tmJ point to CUtensorMap objects over the stage state (4-D: pR, nZ, nphi, 8) and J1 (.., 3)
-// with box (TR+4, tile_z+4, 1, 1)
-// hall: tmJ maps 6 fields (J1 then G) and the kernel adds d_i * G to E1 (default tile height only)
+// with box (TR+4, rhs_tile_z()+4, 1, 1)
+// hall: tmJ maps 6 fields (J1 then G) and the kernel adds d_i * G to E1
 cudaError_t launch_rhs_tma(const RhsArgs &a, const void *tmU, const void *tmJ, int mode, bool has_v0, bool hall, bool spec,
-                           int tile_z, cudaStream_t s);
-bool rhs_tma_supports(int tile_z, bool hall, bool spec);
+                           cudaStream_t s, bool configure = false);
 // TMA variant of the curl kernel: tmU is a CUtensorMap over the 8 fields of the stage state with box
 // (TR+4, curl_tma_tile_z()+4, 1, 1); hall = also write the Hall field G
-cudaError_t launch_curl_tma(const CurlArgs &a, const void *tmU, bool hall, bool spec, cudaStream_t s);
-cudaError_t launch_phi_spectral(const SpecArgs &a, cudaStream_t s);
+cudaError_t launch_curl_tma(const CurlArgs &a, const void *tmU, bool hall, bool spec, cudaStream_t s, bool configure = false);
+cudaError_t launch_phi_spectral(const SpecArgs &a, cudaStream_t s, bool configure = false);
 int curl_tma_tile_z();
+int rhs_tile_z();
 cudaError_t launch_dt_commit(double *clock, unsigned long long *dtmin_bits, const double *diag6, int init, cudaStream_t s);
 cudaError_t launch_diag(const DiagArgs &a, int nblocks, double *result6, cudaStream_t s);
 int diag_blocks(const Layout &L);
 cudaError_t configure_kernels();
-int rhs_default_tile_z();
 
 }  // namespace clt

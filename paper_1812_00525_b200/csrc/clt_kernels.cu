@@ -13,64 +13,19 @@
 
 namespace clt {
 
-// bit m set: the rhs_tma_kernel instantiation of mode m (0 = K only, 1..4 = RK4 stage) uses the split CTA barrier
-#ifndef CLT_SPLIT_MASK
-#define CLT_SPLIT_MASK 0x1F
-#endif
 // launch shape of curl_tma_kernel: tile height, ring depth (planes), CTAs per SM
 #ifndef CLT_CURL_TZ
 #define CLT_CURL_TZ 10
 #define CLT_CURL_NS 6
 #define CLT_CURL_MINB 2
 #endif
-// how many planes ahead of their use the epilogue operands (U^n, acc) are prefetched into L2
-#ifndef CLT_PF_DIST
-#define CLT_PF_DIST 1
-#endif
-// distribution of the halo-node conversions over the warps of the fused RHS kernel (see rhs_tma_kernel).  Measured at
-// 512x64x512: dealing them out evenly (1) is 3 % SLOWER than packing them into the first warps (0): every warp then
-// pays the divergent halo path, and issue slots / shared-memory wavefronts, not the barrier skew, are what is short.
-#ifndef CLT_HALO_SPREAD
-#define CLT_HALO_SPREAD 0
-#endif
-// epilogue operands that equal the stage state at the own node: rebuild rho, p, v from the phi pipeline (1) or read all
-// eight fields again (0)
-#ifndef CLT_EPI_OWN
-#define CLT_EPI_OWN 1
-#endif
 // outputs per thread (= width of the sliding register windows) of the pseudo-spectral pre-pass
 #ifndef CLT_SPEC_NQ
 #define CLT_SPEC_NQ 8
 #endif
-// circular phi pipelines with a five times unrolled plane loop in the fused RHS kernel (1) or shifting pipelines (0).
-// Measured at 512x64x512: no difference (3.715 vs 3.712 ms per step; the 70 register moves per node it removes are not
-// what the kernel waits for) at twice the code size, so it is off; parity-tested once with it on.
-#ifndef CLT_ROT
-#define CLT_ROT 0
-#endif
-// planes of L2-only TMA prefetch beyond the NRAW buffered ones in the fused RHS kernel (0 = none).  Measured at
-// 512x64x512: 1, 2 and 4 planes are all 3-4 % SLOWER than none (3.93 vs 3.79 ms per step), so it is off.
-#ifndef CLT_TMA_PF
-#define CLT_TMA_PF 0
-#endif
-// number of TMA raw buffers (planes in flight) of the default 32 x 8 tile
-#ifndef CLT_NRAW8
-#define CLT_NRAW8 2
-#endif
-
-template <int V>
-struct IC { static constexpr int value = V; };      // compile-time integer passed to generic lambdas
 
 constexpr int TR = 32;        // tile width in R = one warp per tile row
 constexpr int SW = TR + 4;    // shared row width with the radius-2 halo
-
-// index of the current device (0..63) for the per-device "shared-memory opt-in done" flags of the launchers
-static int current_device()
-{
-    int d = 0;
-    if (cudaGetDevice(&d) != cudaSuccess) { cudaGetLastError(); d = 0; }
-    return d & 63;
-}
 
 __device__ __forceinline__ void prefetch_l2(const void *p)
 {
@@ -124,15 +79,14 @@ __device__ __forceinline__ CentreTab load_centre_tab(const double *tab, long lon
 // of a neighbour's staged value: the caller puts the wait half of its split barrier there.
 // SPEC = true: the phi derivatives come from the pseudo-spectral pre-pass: pd1[f], pd2[f] are d/dphi and d2/dphi2 of
 // the five fluid perturbations, dP_EZ / dP_ER the true d/dphi of E1_Z / E1_R (not the unscaled stencil sums).
-// P = phase of the circular phi pipeline: plane j-2+d sits in q[(P + d) % 5] (P = 0: q[d] is plane j-2+d)
-template <bool V0, bool SPEC, int P, class Sync>
+template <bool V0, bool SPEC, class Sync>
 __device__ __forceinline__ void rhs_point(const double *stg, int HT, const double *eRc, const double *ePc, const double *eZc,
                                           double dP_EZ, double dP_ER, const double (&F)[3], const double (&rr)[4], int cs,
                                           const double (&q)[5][5], const CentreTab &ct, const double *tab, long long off2,
                                           long long plane, const Phys &ph, double iR, double iR2, double (&K)[8], Sync &&sync,
                                           const double *pd1 = nullptr, const double *pd2 = nullptr)
 {
-    const double rho1 = q[(P + 2) % 5][0], p1 = q[(P + 2) % 5][1], v1R = q[(P + 2) % 5][2], v1P = q[(P + 2) % 5][3], v1Z = q[(P + 2) % 5][4];
+    const double rho1 = q[2][0], p1 = q[2][1], v1R = q[2][2], v1P = q[2][3], v1Z = q[2][4];
     const double rho = rho1 + ct.rho0;
     const double p = p1 + ct.p0;
     double vR = v1R, vP = v1P, vZ = v1Z;
@@ -150,8 +104,8 @@ __device__ __forceinline__ void rhs_point(const double *stg, int HT, const doubl
         const double g1 = SPEC ? iR : ph.cP1 * iR, vc = vP * g1, lc = SPEC ? iR2 : ph.cP2 * iR2;
 #pragma unroll
         for (int f = 0; f < 5; ++f) {
-            const double d1 = SPEC ? pd1[f] : fd1(q[(P + 0) % 5][f], q[(P + 1) % 5][f], q[(P + 3) % 5][f], q[(P + 4) % 5][f]);
-            const double d2 = SPEC ? pd2[f] : fd2(q[(P + 0) % 5][f], q[(P + 1) % 5][f], q[(P + 2) % 5][f], q[(P + 3) % 5][f], q[(P + 4) % 5][f]);
+            const double d1 = SPEC ? pd1[f] : fd1(q[0][f], q[1][f], q[3][f], q[4][f]);
+            const double d2 = SPEC ? pd2[f] : fd2(q[0][f], q[1][f], q[2][f], q[3][f], q[4][f]);
             A[f] = vc * d1;
             lap[f] = lc * d2;
             if (f == 1) gPp1 = d1 * g1;
@@ -170,7 +124,7 @@ __device__ __forceinline__ void rhs_point(const double *stg, int HT, const doubl
         for (int f = 0; f < 5; ++f) {
             const double *s = stg + f * HT + cs;
             const double m2 = s[-2], m1 = s[-1], p1_ = s[1], p2 = s[2];
-            const double d1 = fd1(m2, m1, p1_, p2), d2 = fd2(m2, m1, q[(P + 2) % 5][f], p1_, p2);
+            const double d1 = fd1(m2, m1, p1_, p2), d2 = fd2(m2, m1, q[2][f], p1_, p2);
             A[f] += vc * d1;
             lap[f] += d2 * ph.cR2 + lc * d1;
             if (f == 1) gRp1 = d1 * ph.cR1;
@@ -184,7 +138,7 @@ __device__ __forceinline__ void rhs_point(const double *stg, int HT, const doubl
         for (int f = 0; f < 5; ++f) {
             const double *s = stg + f * HT + cs;
             const double m2 = s[-2 * SW], m1 = s[-SW], p1_ = s[SW], p2 = s[2 * SW];
-            const double d1 = fd1(m2, m1, p1_, p2), d2 = fd2(m2, m1, q[(P + 2) % 5][f], p1_, p2);
+            const double d1 = fd1(m2, m1, p1_, p2), d2 = fd2(m2, m1, q[2][f], p1_, p2);
             A[f] += vc * d1;
             lap[f] += d2 * ph.cZ2;
             if (f == 1) gZp1 = d1 * ph.cZ1;
@@ -244,18 +198,7 @@ __device__ __forceinline__ void rhs_point(const double *stg, int HT, const doubl
 // Identical to the textbook scheme up to rounding order.  Per node and step this moves 19 + 35 + 27 + 35
 // doubles through the fused kernel instead of 27 + 43 + 43 + 27.
 // ---------------------------------------------------------------------------------------------
-// output stores of the fused kernel: plain, or with the cache-streaming hint (CLT_STORE_CS, measured choice)
-#ifndef CLT_STORE_CS
-#define CLT_STORE_CS 0
-#endif
-__device__ __forceinline__ void st_out(double *p, double v)
-{
-#if CLT_STORE_CS
-    __stcs(p, v);
-#else
-    *p = v;
-#endif
-}
+__device__ __forceinline__ void st_out(double *p, double v) { *p = v; }
 
 struct EpiOperands {
     double un[8];   // U^n at the node
@@ -278,28 +221,17 @@ __device__ __forceinline__ void epilogue_load(const RhsArgs &a, long long g, lon
         if (MODE == RHS_MODE_S4) e.ac[m] = ld(a.acc + gm);
     }
 }
-// SETDT of Fig. 4 [L180-215] at one node (shared by the diagnostics kernel and the stage-4 epilogue)
-__device__ __forceinline__ double setdt_node(const Phys &ph, double cfl, double Ri, double dRi, double rho, double p, double vR,
-                                             double vP, double vZ, double BR, double BP, double BZ)
-{
-    const double b2 = BR * BR + BP * BP + BZ * BZ;
-    const double cf = sqrt(fabs(ph.gamma * p / rho + b2 / rho));
-    const double dtx = dRi / ((fabs(vR) + cf) / cfl);
-    const double dtz = ph.dZ / ((fabs(vZ) + cf) / cfl);
-    const double dty = fabs(Ri * ph.dphi) / ((fabs(vP) + cf) / cfl);
-    return fmin(dty, fmin(dtx, dtz));
-}
-
-// Adaptive stepping (clt_step_cfl, NEXT-1): the stage coefficients come from device memory (a.coef = { dt, dt/2, dt/3,
-// dt/6 }, written by dt_commit_kernel) instead of the launch parameters, and stage 4 folds the SETDT minimum of the
+// The stage coefficients come from device memory (a.coef = { dt, dt/2, dt/3, dt/6 }: the fixed-dt table, or the clock
+// that dt_commit_kernel advances).  Adaptive stepping (clt_step_cfl, NEXT-1): stage 4 folds the SETDT minimum of the
 // new state into `rate` (Fig. 3: STEPON then SETDT, without a separate pass over the state).
 template <int MODE>
 __device__ __forceinline__ void epilogue_store(const RhsArgs &a, long long g, long long field, const EpiOperands &e,
                                                const double (&K)[8], double iR, double &rate)
 {
     constexpr double third = 1.0 / 3.0;
-    double an = a.a_next, bn = a.b_acc;
-    if (a.coef) {
+    // out = U^n + an K (stages 1-3: dt/2, dt/2, dt); bn = weight of K in the accumulator (stage 2: dt/3) / in U^{n+1} (stage 4: dt/6)
+    double an = 0.0, bn = 0.0;
+    if (MODE != RHS_MODE_K) {
         an = __ldg(a.coef + (MODE == RHS_MODE_S3 ? 0 : 1));
         bn = __ldg(a.coef + (MODE == RHS_MODE_S2 ? 2 : 3));
     }
@@ -328,6 +260,9 @@ __device__ __forceinline__ void epilogue_store(const RhsArgs &a, long long g, lo
         const double rR = (fabs(out[2]) + cf) * a.ph.cR1, rP = (fabs(out[3]) + cf) * (a.ph.cP1 * iR),
                      rZ = (fabs(out[4]) + cf) * a.ph.cZ1;
         rate = fmax(rate, fmax(rP, fmax(rR, rZ)));
+        // fmax drops NaN: a non-finite new state must not pass for "no signal" (dt = 100).  An infinite rate gives
+        // dt = 0, which dt_commit_kernel turns into the clock's non-finite mark and clt_step_cfl into CLT_ENONFINITE.
+        if (!(rR + rP + rZ <= 1.79769313486231570815e308)) rate = __longlong_as_double(0x7ff0000000000000LL);
     }
 }
 
@@ -343,16 +278,24 @@ __device__ __forceinline__ void dtmin_commit(const RhsArgs &a, double rate)
 }
 
 // one thread: opens (init = 1: dt from the SETDT reduction `diag6[5]`, time = 0) or advances (time += dt just used,
-// dt = the minimum stage 4 collected) the device-side clock of clt_step_cfl.  clock = { dt, dt/2, dt/3, dt/6, time }
+// dt = the minimum stage 4 collected) the device-side clock of clt_step_cfl.
+// clock = { dt, dt/2, dt/3, dt/6, time, non-finite mark }.  A state with a non-finite signal speed yields dt = 0 (stage 4) or
+// a NaN / non-positive SETDT value (init): the mark is raised, dt stays 0 (the remaining steps of the call change
+// nothing) and clt_step_cfl returns CLT_ENONFINITE.
 __global__ void dt_commit_kernel(double *clock, unsigned long long *dtmin_bits, const double *diag6, int init)
 {
     double dt;
     if (init) {
         dt = diag6[5];
         clock[4] = 0.0;
+        clock[5] = 0.0;
     } else {
         clock[4] += clock[0];
         dt = fmin(100.0, __longlong_as_double((long long)*dtmin_bits));
+    }
+    if (!(dt > 0.0) || clock[5] != 0.0) {
+        clock[5] = 1.0;
+        dt = 0.0;
     }
     clock[0] = dt; clock[1] = 0.5 * dt; clock[2] = dt / 3.0; clock[3] = dt / 6.0;
     *dtmin_bits = (unsigned long long)__double_as_longlong(100.0);      // Fig. 4: DT1 starts at 100
@@ -378,7 +321,7 @@ struct RhsSmem {
 };
 
 template <int TZ, int MODE, bool V0>
-__global__ void __launch_bounds__(TR *TZ, (TZ <= 8 ? 2 : 1)) rhs_kernel(const __grid_constant__ RhsArgs a)
+__global__ void __launch_bounds__(TR *TZ, 1) rhs_kernel(const __grid_constant__ RhsArgs a)
 {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     RhsSmem<TZ> &S = *reinterpret_cast<RhsSmem<TZ> *>(smem_raw);
@@ -539,7 +482,7 @@ __global__ void __launch_bounds__(TR *TZ, (TZ <= 8 ? 2 : 1)) rhs_kernel(const __
             const double dP_ER = fd1(S.ering[s0][0][cs], S.ering[s1][0][cs], S.ering[s3][0][cs], S.ering[se][0][cs]);
             const double F[3] = { S.fring[sfc][0][ci], S.fring[sfc][1][ci], S.fring[sfc][2][ci] };
             const double rr[4] = { S.sR[tx], S.sR[tx + 1], S.sR[tx + 3], S.sR[tx + 4] };
-            rhs_point<V0, false, 0>(&S.stage[buf][0][0], RhsSmem<TZ>::HT, &S.ering[sec][0][0], &S.ering[sec][1][0], &S.ering[sec][2][0],
+            rhs_point<V0, false>(&S.stage[buf][0][0], RhsSmem<TZ>::HT, &S.ering[sec][0][0], &S.ering[sec][1][0], &S.ering[sec][2][0],
                           dP_EZ, dP_ER, F, rr, cs, q, ct, tab, off2, L.plane, ph, iR, iR2, K, [] {});
         }
 
@@ -547,7 +490,8 @@ __global__ void __launch_bounds__(TR *TZ, (TZ <= 8 ? 2 : 1)) rhs_kernel(const __
         if (valid) {
             const long long g = (long long)jw * L.plane + off2;
             EpiOperands eo;
-            epilogue_load<MODE, 0>(a, g, L.field, eo, [](const double *p) { return __ldg(p); });
+            // plain coherent loads: stage 4 updates U^n in place through a.out, so the non-coherent path is not allowed here
+            epilogue_load<MODE, 0>(a, g, L.field, eo, [](const double *p) { return *p; });
             epilogue_store<MODE>(a, g, L.field, eo, K, iR, rate);
         }
         advance();
@@ -555,30 +499,28 @@ __global__ void __launch_bounds__(TR *TZ, (TZ <= 8 ? 2 : 1)) rhs_kernel(const __
     if (MODE == RHS_MODE_S4) dtmin_commit(a, rate);
 }
 
+// configure = true: only opt the kernel in to its dynamic shared-memory size on the current device (clt_create)
 template <int TZ, int MODE, bool V0>
-static cudaError_t launch_rhs_t(const RhsArgs &a, cudaStream_t s)
+static cudaError_t launch_rhs_t(const RhsArgs &a, cudaStream_t s, bool configure)
 {
-    static bool configured_dev[64] = {};     // per device: the opt-in is a per-device function attribute
-    bool &configured = configured_dev[current_device()];
     auto kern = rhs_kernel<TZ, MODE, V0>;
     const int smem = (int)sizeof(RhsSmem<TZ>);
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    if (configure) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     dim3 block(TR, TZ, 1);
     dim3 grid((a.L.nR - 4 + TR - 1) / TR, (a.L.nZ - 4 + TZ - 1) / TZ, a.phi_chunks);
     kern<<<grid, block, smem, s>>>(a);
     return cudaGetLastError();
 }
 
-template <int TZ>
-static cudaError_t launch_rhs_tz(const RhsArgs &a, int mode, bool v0, cudaStream_t s)
+constexpr int RHS_TZ = 8;     // tile height of both fused-kernel variants (32 x 8 nodes, one node per thread)
+int rhs_tile_z() { return RHS_TZ; }
+
+// plain-load variant (variant 1): the A/B and parity cross-check of the TMA-fed default
+cudaError_t launch_rhs(const RhsArgs &a, int mode, bool has_v0, cudaStream_t s, bool configure)
 {
 #define CLT_CASE(M)                                                      \
     case M:                                                              \
-        return v0 ? launch_rhs_t<TZ, M, true>(a, s) : launch_rhs_t<TZ, M, false>(a, s);
+        return has_v0 ? launch_rhs_t<RHS_TZ, M, true>(a, s, configure) : launch_rhs_t<RHS_TZ, M, false>(a, s, configure);
     switch (mode) {
         CLT_CASE(RHS_MODE_K)
         CLT_CASE(RHS_MODE_S1)
@@ -589,22 +531,6 @@ static cudaError_t launch_rhs_tz(const RhsArgs &a, int mode, bool v0, cudaStream
         return cudaErrorInvalidValue;
     }
 #undef CLT_CASE
-}
-
-int rhs_default_tile_z() { return 8; }
-
-cudaError_t launch_rhs(const RhsArgs &a, int mode, bool has_v0, int tile_z, cudaStream_t s)
-{
-    switch (tile_z) {
-    case 7: return launch_rhs_tz<7>(a, mode, has_v0, s);
-    case 13: return launch_rhs_tz<13>(a, mode, has_v0, s);
-    case 8: return launch_rhs_tz<8>(a, mode, has_v0, s);
-    case 10: return launch_rhs_tz<10>(a, mode, has_v0, s);
-    case 12: return launch_rhs_tz<12>(a, mode, has_v0, s);
-    case 14: return launch_rhs_tz<14>(a, mode, has_v0, s);
-    case 16: return launch_rhs_tz<16>(a, mode, has_v0, s);
-    default: return cudaErrorInvalidValue;
-    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -662,15 +588,6 @@ __device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, i
         : "memory");
 }
 
-// TMA prefetch of a tile into L2 only (no shared memory, no barrier): used to run the HBM reads CLT_TMA_PF planes ahead
-// of the NRAW planes that have a shared-memory buffer
-__device__ __forceinline__ void tma_prefetch_4d(const CUtensorMap *map, int c0, int c1, int c2, int c3)
-{
-    asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global.tile [%0, {%1, %2, %3, %4}];" ::"l"(map), "r"(c0), "r"(c1), "r"(c2),
-                 "r"(c3)
-                 : "memory");
-}
-
 template <int TZ, int NRAW, int NF>
 struct RhsTmaSmem {
     static constexpr int HT = (TZ + 4) * SW;
@@ -709,19 +626,16 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
     const long long off2 = (long long)kc * L.pR + (LP + ic);
     const int cs = (ty + 2) * SW + (tx + 2);
 
-    // halo nodes: 4 full rows (Z halo) then 4 columns (R halo), NH in all.  CLT_HALO_SPREAD = 1 deals them out evenly over
-    // the warps (the first HPW lanes of every warp take one each) so that all warps carry the same conversion work and
-    // arrive at the plane barrier together; 0 = the first NH threads take them.
-    constexpr int HPW = (NH + TZ - 1) / TZ;
-    const int hid = CLT_HALO_SPREAD ? ((tid >> 5) * HPW + (tid & 31)) : tid;
-    const bool is_halo = CLT_HALO_SPREAD ? ((tid & 31) < HPW && hid < NH) : (tid < NH);
+    // halo nodes: 4 full rows (Z halo) then 4 columns (R halo), NH in all; the first NH threads take one each (dealing
+    // them out evenly over the warps was measured 3 % slower: every warp then pays the divergent halo path)
+    const bool is_halo = tid < NH;
     int hx, hy;
-    if (hid < 4 * TR) {
-        const int r = hid / TR;
-        hx = hid % TR;
+    if (tid < 4 * TR) {
+        const int r = tid / TR;
+        hx = tid % TR;
         hy = (r < 2) ? r - 2 : TZ + (r - 2);
     } else {
-        const int t = hid - 4 * TR, c = t & 3;
+        const int t = tid - 4 * TR, c = t & 3;
         hy = t >> 2;
         hx = (c < 2) ? c - 2 : TR + (c - 2);
     }
@@ -752,14 +666,6 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
         for (int m = 0; m < 8; ++m) tma_load_4d(&S.raw[b][m][0], &tmU, LP + i0 - 2, k0 - 2, jw, m, &S.bar[b]);
 #pragma unroll
         for (int m = 0; m < NF - 8; ++m) tma_load_4d(&S.raw[b][8 + m][0], &tmJ, LP + i0 - 2, k0 - 2, jw, m, &S.bar[b]);
-    };
-    // L2-only prefetch of plane number n (HBM -> L2 ahead of the buffered loads)
-    auto prefetch_plane = [&](int n) {
-        const int jw = wrap_phi(ja - 2 + n, L.nphi);
-#pragma unroll
-        for (int m = 0; m < 8; ++m) tma_prefetch_4d(&tmU, LP + i0 - 2, k0 - 2, jw, m);
-#pragma unroll
-        for (int m = 0; m < NF - 8; ++m) tma_prefetch_4d(&tmJ, LP + i0 - 2, k0 - 2, jw, m);
     };
 
     // phi-invariant values of the own node and of the halo node, kept in registers for the whole sweep
@@ -810,31 +716,27 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
         }
     };
 
-    // thread-private phi pipelines at the own node
+    // thread-private phi pipelines at the own node (slot 4 = newest plane; shifted once per plane)
     double q[5][5];        // rho1, p1, v1 of planes j-2 .. j+2
     double eR[5], eZ[5];   // E1_R, E1_Z of planes j-2 .. j+2
     double Fp[3][3];       // F = J1 x B + J0 x B1 of planes j .. j+2
     int sl = 0;            // ring slot that receives the plane being consumed (plane j+2)
     const int total = jb - ja + 4;
 
-    // The fluid and E pipelines are CIRCULAR with a compile-time phase (CLT_ROT = 1): plane number n (counted from
-    // ja-2) lives in slot n % 5, the main loop is unrolled five times, and nothing is ever shifted (the shifts were
-    // 70 of about 530 instructions per node).  CLT_ROT = 0 keeps the shifting pipelines (slot 4 = newest plane).
-    // consume the raw tile of plane number nlead (the plane that becomes plane j+2) into pipeline slot SLOT
-    auto lead = [&](auto slot_c) {
-        constexpr int SLOT = decltype(slot_c)::value;
+    // consume the raw tile of plane number nlead (the plane that becomes plane j+2)
+    auto lead = [&]() {
         const int b = nlead % NRAW;
         mbar_wait(&S.bar[b], (unsigned)((nlead / NRAW) & 1));
         ++nlead;
         const double (*raw)[SM::HTP] = S.raw[b];
         double E[3];
-        node(raw, cs, off2, ct.rho0, ct.p0, q[SLOT], E, Fp[2], true);
-        eR[SLOT] = E[0];
-        eZ[SLOT] = E[2];
+        node(raw, cs, off2, ct.rho0, ct.p0, q[4], E, Fp[2], true);
+        eR[4] = E[0];
+        eZ[4] = E[2];
 #pragma unroll
         for (int c = 0; c < 3; ++c) S.ering[sl][c][cs] = E[c];
 #pragma unroll
-        for (int f = 0; f < 5; ++f) S.sring[sl][f][cs] = q[SLOT][f];
+        for (int f = 0; f < 5; ++f) S.sring[sl][f][cs] = q[4][f];
         if (is_halo) {
             double hq[5], hE[3], hF[3];
             node(raw, hs, hoff2, h_rho0, h_p0, hq, hE, hF, false);
@@ -845,44 +747,27 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
         }
     };
     auto advance = [&]() {
-        if (!CLT_ROT) {
 #pragma unroll
-            for (int d = 0; d < 4; ++d) {
+        for (int d = 0; d < 4; ++d) {
 #pragma unroll
-                for (int f = 0; f < 5; ++f) q[d][f] = q[d + 1][f];
-                eR[d] = eR[d + 1];
-                eZ[d] = eZ[d + 1];
-            }
+            for (int f = 0; f < 5; ++f) q[d][f] = q[d + 1][f];
+            eR[d] = eR[d + 1];
+            eZ[d] = eZ[d + 1];
         }
 #pragma unroll
         for (int c = 0; c < 3; ++c) { Fp[0][c] = Fp[1][c]; Fp[1][c] = Fp[2][c]; }
         sl = (sl + 1) & 3;
     };
-    auto after_lead = [&](int n) {
-        __syncthreads();                 // every thread has read the raw tile
-        if (tid == 0 && n + NRAW < total) {
-            issue(n + NRAW);
-            if (CLT_TMA_PF > 0 && n + NRAW + CLT_TMA_PF < total) prefetch_plane(n + NRAW + CLT_TMA_PF);
-        }
-        advance();
-    };
 
     // prologue: planes number 0 .. 3 (ja-2 .. ja+1); NRAW planes are kept in flight
-    if (tid == 0) {
+    if (tid == 0)
         for (int n = 0; n < NRAW && n < total; ++n) issue(n);
-        for (int n = NRAW; n < NRAW + CLT_TMA_PF && n < total; ++n) prefetch_plane(n);
-    }
-    if (CLT_ROT) {
-        lead(IC<0>{}); after_lead(0);
-        lead(IC<1>{}); after_lead(1);
-        lead(IC<2>{}); after_lead(2);
-        lead(IC<3>{}); after_lead(3);
-    } else {
 #pragma unroll 1
-        for (int n = 0; n < 4; ++n) {
-            lead(IC<4>{});
-            after_lead(n);
-        }
+    for (int n = 0; n < 4; ++n) {
+        lead();
+        __syncthreads();                 // every thread has read the raw tile
+        if (tid == 0 && n + NRAW < total) issue(n + NRAW);
+        advance();
     }
     unsigned ready_parity = 0;
 
@@ -890,47 +775,29 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
     const double iR2 = iR * iR;
     double rate = 0.0;           // largest signal rate (|v_d| + c)/(12 h_d) at this thread's nodes (stage 4 of clt_step_cfl)
 
-    // one plane: P = phase of the circular pipelines = (j - ja) % 5 (always 0 with CLT_ROT = 0)
-    auto plane = [&](auto phase_c, int j) {
-        constexpr int P = decltype(phase_c)::value;
+#pragma unroll 1
+    for (int j = ja; j < jb; ++j) {
         // ---- phase A: consume plane j+2 --------------------------------------------------------
-        if (a.prefetch && MODE != RHS_MODE_K && (tx & 15) == 0 && j + CLT_PF_DIST < jb) {
-            const long long g1 = (long long)(j + CLT_PF_DIST) * L.plane + off2;
+        if (a.prefetch && MODE != RHS_MODE_K && (tx & 15) == 0 && j + 1 < jb) {
+            const long long g1 = (long long)(j + 1) * L.plane + off2;
 #pragma unroll
             for (int m = 0; m < 8; ++m) {
                 if (MODE != RHS_MODE_S1) prefetch_l2(a.Un + m * L.field + g1);
                 if (MODE == RHS_MODE_S4) prefetch_l2(a.acc + m * L.field + g1);
             }
         }
-        lead(IC<(P + 4) % 5>{});
+        lead();
         const int sc = (sl + 2) & 3;                              // ring slot of the centre plane
         // split barrier: announce "my part of plane j+2 is in the rings", keep working on what needs nobody else's
-        // data (epilogue operand loads, the phi direction), and only then wait for the other warps.  Which stage
-        // variants use it is a measured choice (CLT_SPLIT_MASK); the others keep the plain barrier right here.
-        constexpr bool SPLIT = ((CLT_SPLIT_MASK >> MODE) & 1) != 0;
-        auto refill = [&]() {
-            // every thread has consumed the raw buffer of plane number j-ja+4: refill it NRAW planes ahead
-            // (overlaps the rest of phase B and NRAW-1 more iterations)
-            const int n = j - ja + 4 + NRAW;
-            if (tid == 0 && n < total) {
-                issue(n);
-                if (CLT_TMA_PF > 0 && n + CLT_TMA_PF < total) prefetch_plane(n + CLT_TMA_PF);
-            }
-        };
-        if (SPLIT) {
-            mbar_arrive(&S.ready);
-        } else {
-            __syncthreads();
-            refill();
-        }
+        // data (epilogue operand loads, the phi direction), and only then wait for the other warps
+        mbar_arrive(&S.ready);
 
         // ---- a6 inputs: U^n / stage state / acc of this node, requested now so that they arrive during phase B ---
         const long long g = (long long)j * L.plane + off2;
         EpiOperands eo;
         // rho, p (and v when the reference state is static) of the centre plane are still in the phi pipeline
-        constexpr int NOWN = CLT_EPI_OWN ? (V0 ? 2 : 5) : 0;
-        const double own[5] = { q[(P + 2) % 5][0] + ct.rho0, q[(P + 2) % 5][1] + ct.p0, q[(P + 2) % 5][2], q[(P + 2) % 5][3],
-                                q[(P + 2) % 5][4] };
+        constexpr int NOWN = V0 ? 2 : 5;
+        const double own[5] = { q[2][0] + ct.rho0, q[2][1] + ct.p0, q[2][2], q[2][3], q[2][4] };
         epilogue_load<MODE, NOWN>(a, g, L.field, eo, [](const double *p) { return ld_stream(p); }, own);
 
         // ---- phase B: K at (i, k, j) -----------------------------------------------------------
@@ -946,70 +813,49 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
             dP_ER = ld_stream(a.spec + (SP_DE + 0) * L.field + g);
             dP_EZ = ld_stream(a.spec + (SP_DE + 1) * L.field + g);
         } else {
-            dP_EZ = fd1(eZ[P % 5], eZ[(P + 1) % 5], eZ[(P + 3) % 5], eZ[(P + 4) % 5]);
-            dP_ER = fd1(eR[P % 5], eR[(P + 1) % 5], eR[(P + 3) % 5], eR[(P + 4) % 5]);
+            dP_EZ = fd1(eZ[0], eZ[1], eZ[3], eZ[4]);
+            dP_ER = fd1(eR[0], eR[1], eR[3], eR[4]);
         }
-        rhs_point<V0, SPEC, P>(&S.sring[sc][0][0], HT, &S.ering[sc][0][0], &S.ering[sc][1][0], &S.ering[sc][2][0], dP_EZ, dP_ER, Fp[0],
+        rhs_point<V0, SPEC>(&S.sring[sc][0][0], HT, &S.ering[sc][0][0], &S.ering[sc][1][0], &S.ering[sc][2][0], dP_EZ, dP_ER, Fp[0],
                             rr, cs, q, ct, tab, off2, L.plane, ph, iR, iR2, K, [&] {
-                                if (SPLIT) {
-                                    mbar_wait(&S.ready, ready_parity);
-                                    refill();
-                                }
+                                mbar_wait(&S.ready, ready_parity);
+                                // every thread has consumed the raw buffer of plane number j-ja+4: refill it NRAW planes
+                                // ahead (overlaps the rest of phase B and NRAW-1 more iterations)
+                                const int n = j - ja + 4 + NRAW;
+                                if (tid == 0 && n < total) issue(n);
                             }, pd1, pd2);
         ready_parity ^= 1u;
 
         // ---- a6: RK4 stage combine in the epilogue (L125, L139) --------------------------------
         if (valid) epilogue_store<MODE>(a, g, L.field, eo, K, iR, rate);
         advance();
-    };
-    if (CLT_ROT) {
-#pragma unroll 1
-        for (int j = ja; j < jb; j += 5) {
-            plane(IC<0>{}, j);
-            if (j + 1 >= jb) break;
-            plane(IC<1>{}, j + 1);
-            if (j + 2 >= jb) break;
-            plane(IC<2>{}, j + 2);
-            if (j + 3 >= jb) break;
-            plane(IC<3>{}, j + 3);
-            if (j + 4 >= jb) break;
-            plane(IC<4>{}, j + 4);
-        }
-    } else {
-#pragma unroll 1
-        for (int j = ja; j < jb; ++j) plane(IC<0>{}, j);
     }
     if (MODE == RHS_MODE_S4) dtmin_commit(a, rate);
 }
 
-template <int TZ, int NRAW, int MODE, bool V0, bool HALL, bool SPEC>
-static cudaError_t launch_rhs_tma_t(const RhsArgs &a, const CUtensorMap &tmU, const CUtensorMap &tmJ, cudaStream_t s)
+template <int MODE, bool V0, bool HALL, bool SPEC>
+static cudaError_t launch_rhs_tma_t(const RhsArgs &a, const CUtensorMap &tmU, const CUtensorMap &tmJ, cudaStream_t s, bool configure)
 {
-    static bool configured_dev[64] = {};     // per device: the opt-in is a per-device function attribute
-    bool &configured = configured_dev[current_device()];
+    constexpr int TZ = RHS_TZ, NRAW = 2;
     auto kern = rhs_tma_kernel<TZ, NRAW, MODE, V0, HALL, SPEC>;
     using SM = RhsTmaSmem<TZ, NRAW, HALL ? 14 : 11>;
     const int smem = (int)sizeof(SM);
     static_assert(sizeof(SM) <= 232448, "shared memory of the TMA RHS kernel exceeds 227 KB");
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    if (configure) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     dim3 block(TR, TZ, 1);
     dim3 grid((a.L.nR - 4 + TR - 1) / TR, (a.L.nZ - 4 + TZ - 1) / TZ, a.phi_chunks);
     kern<<<grid, block, smem, s>>>(a, tmU, tmJ);
     return cudaGetLastError();
 }
 
-template <int TZ, int NRAW, bool HALL, bool SPEC>
-static cudaError_t launch_rhs_tma_tz(const RhsArgs &a, const CUtensorMap &tmU, const CUtensorMap &tmJ, int mode, bool v0,
-                                     cudaStream_t s)
+template <bool HALL, bool SPEC>
+static cudaError_t launch_rhs_tma_hs(const RhsArgs &a, const CUtensorMap &tmU, const CUtensorMap &tmJ, int mode, bool v0,
+                                     cudaStream_t s, bool configure)
 {
 #define CLT_CASE(M)                                                                                 \
     case M:                                                                                         \
-        return v0 ? launch_rhs_tma_t<TZ, NRAW, M, true, HALL, SPEC>(a, tmU, tmJ, s)                 \
-                  : launch_rhs_tma_t<TZ, NRAW, M, false, HALL, SPEC>(a, tmU, tmJ, s);
+        return v0 ? launch_rhs_tma_t<M, true, HALL, SPEC>(a, tmU, tmJ, s, configure)                \
+                  : launch_rhs_tma_t<M, false, HALL, SPEC>(a, tmU, tmJ, s, configure);
     switch (mode) {
         CLT_CASE(RHS_MODE_K)
         CLT_CASE(RHS_MODE_S1)
@@ -1022,32 +868,15 @@ static cudaError_t launch_rhs_tma_tz(const RhsArgs &a, const CUtensorMap &tmU, c
 #undef CLT_CASE
 }
 
-// the Hall and pseudo-spectral variants exist for the default tile height only
-bool rhs_tma_supports(int tile_z, bool hall, bool spec)
-{
-    if (hall || spec) return tile_z == 8;
-    return tile_z == 8 || tile_z == 10 || tile_z == 12 || tile_z == 13;
-}
-
 cudaError_t launch_rhs_tma(const RhsArgs &a, const void *tmU, const void *tmJ, int mode, bool has_v0, bool hall, bool spec,
-                           int tile_z, cudaStream_t s)
+                           cudaStream_t s, bool configure)
 {
     const CUtensorMap &mU = *reinterpret_cast<const CUtensorMap *>(tmU);
     const CUtensorMap &mJ = *reinterpret_cast<const CUtensorMap *>(tmJ);
-    if (hall || spec) {
-        if (tile_z != 8) return cudaErrorInvalidValue;
-        if (hall && spec) return launch_rhs_tma_tz<8, 2, true, true>(a, mU, mJ, mode, has_v0, s);
-        if (hall) return launch_rhs_tma_tz<8, 2, true, false>(a, mU, mJ, mode, has_v0, s);
-        return launch_rhs_tma_tz<8, 2, false, true>(a, mU, mJ, mode, has_v0, s);
-    }
-    switch (tile_z) {
-    // two raw buffers (TMA two planes ahead) where shared memory allows, one otherwise
-    case 8: return launch_rhs_tma_tz<8, CLT_NRAW8, false, false>(a, mU, mJ, mode, has_v0, s);
-    case 10: return launch_rhs_tma_tz<10, 2, false, false>(a, mU, mJ, mode, has_v0, s);
-    case 12: return launch_rhs_tma_tz<12, 1, false, false>(a, mU, mJ, mode, has_v0, s);
-    case 13: return launch_rhs_tma_tz<13, 1, false, false>(a, mU, mJ, mode, has_v0, s);
-    default: return cudaErrorInvalidValue;
-    }
+    if (hall && spec) return launch_rhs_tma_hs<true, true>(a, mU, mJ, mode, has_v0, s, configure);
+    if (hall) return launch_rhs_tma_hs<true, false>(a, mU, mJ, mode, has_v0, s, configure);
+    if (spec) return launch_rhs_tma_hs<false, true>(a, mU, mJ, mode, has_v0, s, configure);
+    return launch_rhs_tma_hs<false, false>(a, mU, mJ, mode, has_v0, s, configure);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -1153,9 +982,8 @@ __global__ void __launch_bounds__(TR *TZ, 2) curl_kernel(const __grid_constant__
     }
 }
 
-cudaError_t launch_curl(const CurlArgs &a, int tile_z, cudaStream_t s)
+cudaError_t launch_curl(const CurlArgs &a, cudaStream_t s)
 {
-    (void)tile_z;
     constexpr int TZ = 8;
     dim3 block(TR, TZ, 1);
     dim3 grid((a.L.nR - 4 + TR - 1) / TR, (a.L.nZ - 4 + TZ - 1) / TZ, a.phi_chunks);
@@ -1328,28 +1156,22 @@ curl_tma_kernel(const __grid_constant__ CurlArgs a, const __grid_constant__ CUte
 }
 
 template <bool HALL, bool SPEC>
-static cudaError_t launch_curl_tma_t(const CurlArgs &a, const void *tmU, cudaStream_t s)
+static cudaError_t launch_curl_tma_t(const CurlArgs &a, const void *tmU, cudaStream_t s, bool configure)
 {
     constexpr int TZ = CLT_CURL_TZ, NS = CLT_CURL_NS;
-    static bool configured_dev[64] = {};     // per device: the opt-in is a per-device function attribute
-    bool &configured = configured_dev[current_device()];
     auto kern = curl_tma_kernel<TZ, NS, HALL, SPEC>;
     const int smem = (int)sizeof(CurlTmaSmem<TZ, NS, HALL ? 5 : 3>);
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    if (configure) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     dim3 block(TR, TZ, 1);
     dim3 grid((a.L.nR - 4 + TR - 1) / TR, (a.L.nZ - 4 + TZ - 1) / TZ, a.phi_chunks);
     kern<<<grid, block, smem, s>>>(a, *reinterpret_cast<const CUtensorMap *>(tmU));
     return cudaGetLastError();
 }
 
-cudaError_t launch_curl_tma(const CurlArgs &a, const void *tmU, bool hall, bool spec, cudaStream_t s)
+cudaError_t launch_curl_tma(const CurlArgs &a, const void *tmU, bool hall, bool spec, cudaStream_t s, bool configure)
 {
-    if (spec) return hall ? launch_curl_tma_t<true, true>(a, tmU, s) : launch_curl_tma_t<false, true>(a, tmU, s);
-    return hall ? launch_curl_tma_t<true, false>(a, tmU, s) : launch_curl_tma_t<false, false>(a, tmU, s);
+    if (spec) return hall ? launch_curl_tma_t<true, true>(a, tmU, s, configure) : launch_curl_tma_t<false, true>(a, tmU, s, configure);
+    return hall ? launch_curl_tma_t<true, false>(a, tmU, s, configure) : launch_curl_tma_t<false, false>(a, tmU, s, configure);
 }
 int curl_tma_tile_z() { return CLT_CURL_TZ; }
 
@@ -1463,174 +1285,13 @@ __global__ void __launch_bounds__(512) phi_spectral_kernel(const __grid_constant
     }
 }
 
-// ---------------------------------------------------------------------------------------------
-// The same derivatives through a radix-2 Stockham FFT in shared memory, for nphi a power of two (8 .. 128): the
-// operator is diagonal in Fourier space, so two real lines f, g are packed as z = f + i g, transformed once,
-// multiplied by i kappa q (Nyquist: 0) resp. -(kappa q)^2, and transformed back: by linearity the real part is the
-// derivative of f and the imaginary part that of g -- no unpacking.  About 6x fewer FP64 operations than the
-// circulant sums at nphi = 64.  32 lines per CTA (one per lane: every shared access is conflict-free, twiddles are
-// broadcast), TY threads per line share the N/2 butterflies of a pass.
-// Line codes: 0..4 rho1, p1, v1_R, v1_phi, v1_Z (first and second derivative); 5, 6 E1_R, E1_Z; 7, 8 B1_R, B1_Z;
-// 9 p1 for the Hall field (first derivative only); -1 none.
-// ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ void spec_line_setup(const SpecArgs &a, int code, long long o2, int &src, double &f0, int &out1,
-                                                int &out2)
-{
-    const Layout &L = a.L;
-    src = -1; f0 = 0.0; out1 = -1; out2 = -1;
-    if (code < 0) return;
-    if (code < 5) {
-        src = code; out1 = SP_D1 + code; out2 = SP_D2 + code;
-        const int t0 = code == 0 ? T_RHO0 : (code == 1 ? T_P0 : T_V0R + (code - 2));
-        f0 = (code < 2 || a.has_v0) ? __ldg(a.tab + t0 * L.plane + o2) : 0.0;
-    } else if (code < 7) {
-        out1 = SP_DE + (code - 5);
-    } else if (code < 9) {
-        src = code == 7 ? 5 : 7; out1 = SP_DB + (code - 7);
-        f0 = __ldg(a.tab + (code == 7 ? T_B0R : T_B0Z) * L.plane + o2);
-    } else {
-        src = 1; out1 = SP_D1 + 1;
-        f0 = __ldg(a.tab + T_P0 * L.plane + o2);
-    }
-}
-__device__ __forceinline__ double spec_line_value(const SpecArgs &a, int code, int src, double f0, long long g)
-{
-    const Layout &L = a.L;
-    if (code < 0) return 0.0;
-    if (code == 5 || code == 6) {
-        // E1_R = eta J_R - (v_phi B_Z - v_Z B_phi) ; E1_Z = eta J_Z - (v_R B_phi - v_phi B_R) (+ d_i G); v0 x B0 is axisymmetric
-        const int c = code == 5 ? 0 : 2;
-        const int ia = c == 0 ? 3 : 2, ib = c == 0 ? 7 : 6, ic2 = c == 0 ? 4 : 3, id = c == 0 ? 6 : 5;
-        const double va = __ldg(a.U + ia * L.field + g), Bb = __ldg(a.U + ib * L.field + g);
-        const double vc = __ldg(a.U + ic2 * L.field + g), Bd = __ldg(a.U + id * L.field + g);
-        double e = a.ph.eta * __ldg(a.J1 + c * L.field + g) - (va * Bb - vc * Bd);
-        if (a.hall) e = fma(a.ph.d_i, __ldg(a.J1 + (3 + c) * L.field + g), e);
-        return e;
-    }
-    return __ldg(a.U + src * L.field + g) - f0;
-}
-
-__global__ void __launch_bounds__(512) phi_fft_kernel(const __grid_constant__ SpecArgs a, int4 codesA, int4 codesB, int want2_mask)
-{
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    const Layout &L = a.L;
-    const int N = L.nphi, H = N >> 1;
-    const int tx = threadIdx.x, ty = threadIdx.y, TY = blockDim.y;
-    const size_t BUF = (size_t)N * 32;
-    double *sm = reinterpret_cast<double *>(smem_raw);
-    struct Bufs { double *sm; size_t BUF; __device__ double *operator[](int b) const { return sm + 2 * (size_t)b * BUF; } };
-    const Bufs re{ sm, BUF }, im{ sm + BUF, BUF };      // three complex buffers: re[b], im[b]
-    double *twc = sm + 6 * BUF, *tws = twc + H;
-    const int i = 2 + blockIdx.x * 32 + tx, k = 2 + blockIdx.y;
-    const bool valid = i <= L.nR - 3;
-    const long long o2 = (long long)k * L.pR + (LP + min(i, L.nR - 3));
-    const int job = blockIdx.z;
-    const int codeA = job == 0 ? codesA.x : (job == 1 ? codesA.y : (job == 2 ? codesA.z : codesA.w));
-    const int codeB = job == 0 ? codesB.x : (job == 1 ? codesB.y : (job == 2 ? codesB.z : codesB.w));
-    const bool want2 = (want2_mask >> job) & 1;
-    int srcA, srcB, oA1, oA2, oB1, oB2;
-    double fA0, fB0;
-    spec_line_setup(a, codeA, o2, srcA, fA0, oA1, oA2);
-    spec_line_setup(a, codeB, o2, srcB, fB0, oB1, oB2);
-    for (int j = ty; j < N; j += TY) {
-        const long long g = (long long)j * L.plane + o2;
-        re[0][j * 32 + tx] = spec_line_value(a, codeA, srcA, fA0, g);
-        im[0][j * 32 + tx] = spec_line_value(a, codeB, srcB, fB0, g);
-    }
-    for (int n = ty * 32 + tx; n < H; n += TY * 32) {
-        twc[n] = a.ctab[2 * SPEC_MAX_NPHI + n];
-        tws[n] = a.ctab[2 * SPEC_MAX_NPHI + SPEC_MAX_NPHI / 2 + n];
-    }
-    __syncthreads();
-
-    // radix-2 Stockham passes from buffer `in` (destroyed) with scratch `other`; returns the buffer holding the result
-    auto fft = [&](int in, int other, double sign) {
-        for (int p = 1; p < N; p <<= 1) {
-            const int tstep = H / p;
-            for (int b = ty; b < H; b += TY) {
-                const int kk = b & (p - 1), j = ((b - kk) << 1) + kk;
-                const double c = twc[kk * tstep], s = sign * tws[kk * tstep];
-                const double xr = re[in][(b + H) * 32 + tx], xi = im[in][(b + H) * 32 + tx];
-                const double ur = re[in][b * 32 + tx], ui = im[in][b * 32 + tx];
-                const double vr = c * xr - s * xi, vi = c * xi + s * xr;
-                re[other][j * 32 + tx] = ur + vr;       im[other][j * 32 + tx] = ui + vi;
-                re[other][(j + p) * 32 + tx] = ur - vr; im[other][(j + p) * 32 + tx] = ui - vi;
-            }
-            __syncthreads();
-            const int t = in; in = other; other = t;
-        }
-        return in;
-    };
-    const int X = fft(0, 1, -1.0);            // spectrum of z
-    const int F1 = X == 0 ? 1 : 0, F2 = 2;    // the two free buffers
-    const double kap = 6.283185307179586476925286766559 / a.ph.Lphi, invN = 1.0 / (double)N;
-    for (int pass = 0; pass < (want2 ? 2 : 1); ++pass) {
-        for (int q = ty; q < N; q += TY) {
-            const double xr = re[X][q * 32 + tx], xi = im[X][q * 32 + tx];
-            if (pass == 0) {      // i kappa q, Nyquist mode dropped
-                const double m = kap * (double)(q < H ? q : (q == H ? 0 : q - N));
-                re[F1][q * 32 + tx] = -m * xi;
-                im[F1][q * 32 + tx] = m * xr;
-            } else {              // -(kappa q)^2, Nyquist mode kept
-                const double mq = kap * (double)(q <= H ? q : q - N), m = -mq * mq;
-                re[F1][q * 32 + tx] = m * xr;
-                im[F1][q * 32 + tx] = m * xi;
-            }
-        }
-        __syncthreads();
-        const int Y = fft(F1, F2, 1.0);
-        const int oA = pass == 0 ? oA1 : oA2, oB = pass == 0 ? oB1 : oB2;
-        if (valid)
-            for (int j = ty; j < N; j += TY) {
-                const long long g = (long long)j * L.plane + o2;
-                if (oA >= 0) a.out[(long long)oA * L.field + g] = re[Y][j * 32 + tx] * invN;
-                if (oB >= 0) a.out[(long long)oB * L.field + g] = im[Y][j * 32 + tx] * invN;
-            }
-        __syncthreads();
-    }
-}
-
-static bool phi_fft_supported(int N) { return N >= 8 && N <= 128 && (N & (N - 1)) == 0; }
-
-static cudaError_t launch_phi_fft(const SpecArgs &a, cudaStream_t s)
-{
-    static bool configured_dev[64] = {};     // per device: the opt-in is a per-device function attribute
-    bool &configured = configured_dev[current_device()];
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(phi_fft_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)((6 * 128 * 32 + 128) * sizeof(double)));
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
-    const int N = a.L.nphi;
-    int4 cA, cB;
-    int jobs, want2;
-    if (a.mode == 0) {
-        cA = make_int4(7, 9, -1, -1); cB = make_int4(8, -1, -1, -1);
-        jobs = a.hall ? 2 : 1; want2 = 0;
-    } else {
-        cA = make_int4(0, 2, 4, 6); cB = make_int4(1, 3, 5, -1);
-        jobs = 4; want2 = 0x7;
-    }
-    dim3 block(32, N / 2 < 16 ? N / 2 : 16, 1);
-    dim3 grid((a.L.nR - 4 + 31) / 32, a.L.nZ - 4, jobs);
-    const size_t smem = ((size_t)6 * N * 32 + N) * sizeof(double);
-    phi_fft_kernel<<<grid, block, smem, s>>>(a, cA, cB, want2);
-    return cudaGetLastError();
-}
-
 template <bool WANT2>
-static cudaError_t launch_phi_jobs(const SpecArgs &a, int job_base, int jobs, cudaStream_t s)
+static cudaError_t launch_phi_jobs(const SpecArgs &a, int job_base, int jobs, cudaStream_t s, bool configure)
 {
-    static bool configured_dev[64] = {};     // per device: the opt-in is a per-device function attribute
-    bool &configured = configured_dev[current_device()];
     auto kern = phi_spectral_kernel<WANT2>;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)((SPEC_MAX_NPHI * 32 + 2 * SPEC_MAX_NPHI) * sizeof(double)));
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    if (configure)
+        return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    (int)((SPEC_MAX_NPHI * 32 + 2 * SPEC_MAX_NPHI) * sizeof(double)));
     const int N = a.L.nphi;
     const int groups = (N + CLT_SPEC_NQ - 1) / CLT_SPEC_NQ;
     dim3 block(32, groups < 16 ? groups : 16, 1);
@@ -1642,13 +1303,16 @@ static cudaError_t launch_phi_jobs(const SpecArgs &a, int job_base, int jobs, cu
 
 // mode 0: one launch (first derivatives of B1_R, B1_Z [, p1]); mode 1: two launches (the five fluid fields with
 // both derivatives; E1_R, E1_Z with first derivatives only)
-cudaError_t launch_phi_spectral(const SpecArgs &a, cudaStream_t s)
+cudaError_t launch_phi_spectral(const SpecArgs &a, cudaStream_t s, bool configure)
 {
-    if (a.use_fft && phi_fft_supported(a.L.nphi)) return launch_phi_fft(a, s);
-    if (a.mode == 0) return launch_phi_jobs<false>(a, 0, a.hall ? 3 : 2, s);
-    cudaError_t e = launch_phi_jobs<true>(a, 0, 5, s);
+    if (configure) {
+        cudaError_t e = launch_phi_jobs<true>(a, 0, 0, s, true);
+        return e != cudaSuccess ? e : launch_phi_jobs<false>(a, 0, 0, s, true);
+    }
+    if (a.mode == 0) return launch_phi_jobs<false>(a, 0, a.hall ? 3 : 2, s, false);
+    cudaError_t e = launch_phi_jobs<true>(a, 0, 5, s, false);
     if (e != cudaSuccess) return e;
-    return launch_phi_jobs<false>(a, 5, 2, s);
+    return launch_phi_jobs<false>(a, 5, 2, s, false);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -1701,6 +1365,22 @@ cudaError_t launch_tables(const Layout &L, const Phys &ph, double *tab, const do
     return cudaGetLastError();
 }
 
+// Does the reference state move?  One block scans v0 (three tables) and raises *flag: selects the v0 = 0
+// specialisation of the kernels without a synchronous copy of the tables to the host.
+__global__ void __launch_bounds__(1024) any_nonzero_kernel(const double *x, long long n, int *flag)
+{
+    int mine = 0;
+    for (long long q = threadIdx.x; q < n; q += blockDim.x) mine |= (x[q] != 0.0);
+    const int any = __syncthreads_or(mine);
+    if (threadIdx.x == 0) *flag = any;
+}
+
+cudaError_t launch_any_nonzero(const double *x, long long n, int *flag, cudaStream_t s)
+{
+    any_nonzero_kernel<<<1, 1024, 0, s>>>(x, n, flag);
+    return cudaGetLastError();
+}
+
 // ---------------------------------------------------------------------------------------------
 // a1: boundary layers.  The two outer node layers in R and Z hold the values given to
 // clt_set_state in every RK buffer (L123, L187-189); the step kernels never write them.
@@ -1740,26 +1420,34 @@ __global__ void copy_boundary_kernel(Layout L, long long total, const double *sr
 }
 
 cudaError_t launch_copy_boundary(const Layout &L, int nfields, const double *src, double *d0, double *d1, double *d2,
-                                 cudaStream_t s)
+                                 int sm_count, cudaStream_t s)
 {
     const long long total = (long long)nfields * L.nphi * (4LL * L.nR + 4LL * (L.nZ - 4));
     const int block = 256;
-    const int grid = (int)((total + block - 1) / block < 148 * 16 ? (total + block - 1) / block : 148 * 16);
+    const long long want = (total + block - 1) / block, cap = (long long)(sm_count > 0 ? sm_count : 148) * 16;
+    const int grid = (int)(want < cap ? want : cap);
     copy_boundary_kernel<<<grid, block, 0, s>>>(L, total, src, d0, d1, d2);
     return cudaGetLastError();
 }
 
-cudaError_t launch_zero_boundary(const Layout &L, int nfields, double *dst, cudaStream_t s)
+cudaError_t launch_zero_boundary(const Layout &L, int nfields, double *dst, int sm_count, cudaStream_t s)
 {
-    return launch_copy_boundary(L, nfields, nullptr, dst, nullptr, nullptr, s);
+    return launch_copy_boundary(L, nfields, nullptr, dst, nullptr, nullptr, sm_count, s);
 }
 
 // ---------------------------------------------------------------------------------------------
 // a7 diagnostics (L139, L149, L430) and the SETDT minimum (Fig. 4).
-// One thread per interior (i, k) column; warp-shuffle + shared-memory block reduction; the block
-// partials are combined in a fixed order by a second, single-block kernel (deterministic).
+// A CTA owns 32 neighbouring R nodes of one Z row and all nphi planes: thread (tx, g) marches the g-th of DG_G
+// contiguous phi chunks (so 8 x more threads stream than one per (R, Z) column, and B_phi's phi neighbours for
+// div_c B come from a 5-deep register pipeline instead of being read five times).  The chunk partials -- the
+// Fourier sums of the n = 1 harmonic have to be complete before they are squared -- meet in shared memory and
+// are combined in a fixed order; warp shuffles reduce over R; the block partials are combined in a fixed order
+// by a second, single-block kernel (deterministic).
+// SETDT is regrouped (rounding order only): a node's three cell-crossing times become the rates (|v_d| + c)/h_d with
+// h_R = |R_i - R_{i-1}| as in Fig. 4; the maximum is taken over the nodes and dt = min(100, cfl / max rate) once.
 // ---------------------------------------------------------------------------------------------
-constexpr int DG_BX = 32, DG_BY = 8, DG_N = 6;   // kinetic, magnetic, magnetic_pert, magnetic_n1, max divB, min dt
+constexpr int DG_BX = 32, DG_G = 8, DG_N = 6;   // kinetic, magnetic, magnetic_pert, magnetic_n1, max divB, max rate
+constexpr int DG_Q = 11;                        // per-thread partials: ke, me, mep, fa[3], fb[3], mdiv, rate
 
 __device__ __forceinline__ double warp_sum(double v)
 {
@@ -1773,132 +1461,189 @@ __device__ __forceinline__ double warp_max(double v)
     for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
     return v;
 }
-__device__ __forceinline__ double warp_min(double v)
-{
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
-    return v;
-}
 
-__global__ void __launch_bounds__(DG_BX *DG_BY) diag_kernel(const __grid_constant__ DiagArgs a)
+__global__ void __launch_bounds__(DG_BX *DG_G, 2) diag_kernel(const __grid_constant__ DiagArgs a)
 {
     const Layout &L = a.L;
     const Phys &ph = a.ph;
-    const int i = 2 + blockIdx.x * DG_BX + threadIdx.x, k = 2 + blockIdx.y * DG_BY + threadIdx.y;
+    const int tx = threadIdx.x, g = threadIdx.y, n = L.nphi;
+    const int i = 2 + blockIdx.x * DG_BX + tx, k = 2 + blockIdx.y;
+    const int ja = (int)(((long long)n * g) / DG_G), jb = (int)(((long long)n * (g + 1)) / DG_G);
     const bool valid = i <= L.nR - 3 && k >= a.k_first && k <= a.k_last;
-    const bool deep = i >= 4 && i <= L.nR - 5 && k >= a.kd_first && k <= a.kd_last;
-    double ke = 0.0, me = 0.0, mep = 0.0, men1 = 0.0, mdiv = 0.0, mdt = 100.0;
-    if (valid) {
+    const bool deep = valid && i >= 4 && i <= L.nR - 5 && k >= a.kd_first && k <= a.kd_last;
+    const double inf = __longlong_as_double(0x7ff0000000000000LL);
+    double ke = 0.0, me = 0.0, mep = 0.0, mdiv = 0.0, rate = 0.0;
+    double fa[3] = { 0, 0, 0 }, fb[3] = { 0, 0, 0 };
+    if (valid && ja < jb) {
         const long long o = (long long)k * L.pR + (LP + i);
         const double Ri = a.R[i], iR = a.invR[i];
         const double b0R = a.tab[T_B0R * L.plane + o], b0P = a.tab[T_B0P * L.plane + o], b0Z = a.tab[T_B0Z * L.plane + o];
-        double fa[3] = { 0, 0, 0 }, fb[3] = { 0, 0, 0 };
-        const double dRi = fabs(Ri - a.R[i - 1]);
-        for (int j = 0; j < L.nphi; ++j) {
-            const long long g = (long long)j * L.plane + o;
-            const double rho = a.U[g], p = a.U[L.field + g];
-            const double vR = a.U[2 * L.field + g], vP = a.U[3 * L.field + g], vZ = a.U[4 * L.field + g];
-            const double BR = a.U[5 * L.field + g], BP = a.U[6 * L.field + g], BZ = a.U[7 * L.field + g];
+        const double ihR = 1.0 / fabs(Ri - a.R[i - 1]), ihP = 1.0 / fabs(Ri * ph.dphi);
+        const double *Bp = a.U + 6 * L.field + o;
+        const bool pipe = a.spec_c1 == nullptr;     // finite differences: B_phi of planes j-2 .. j+2 in registers
+        double bp[5] = { 0, 0, 0, 0, 0 };
+        if (pipe) {
+#pragma unroll
+            for (int d = 0; d < 4; ++d) bp[d + 1] = Bp[(long long)wrap_phi(ja - 2 + d, n) * L.plane];
+        }
+#pragma unroll 1
+        for (int j = ja; j < jb; ++j) {
+            const long long gq = (long long)j * L.plane + o;
+            const double rho = a.U[gq], p = a.U[L.field + gq];
+            const double vR = a.U[2 * L.field + gq], vP = a.U[3 * L.field + gq], vZ = a.U[4 * L.field + gq];
+            const double BR = a.U[5 * L.field + gq], BZ = a.U[7 * L.field + gq];
+            double BP;
+            if (pipe) {
+#pragma unroll
+                for (int d = 0; d < 4; ++d) bp[d] = bp[d + 1];
+                bp[4] = Bp[(long long)wrap_phi(j + 2, n) * L.plane];
+                BP = bp[2];
+            } else {
+                BP = Bp[(long long)j * L.plane];
+            }
             const double b2 = BR * BR + BP * BP + BZ * BZ;
             ke += 0.5 * rho * (vR * vR + vP * vP + vZ * vZ);
             me += 0.5 * b2;
             const double b1[3] = { BR - b0R, BP - b0P, BZ - b0Z };
             mep += 0.5 * (b1[0] * b1[0] + b1[1] * b1[1] + b1[2] * b1[2]);
-            const double c = a.cs[j], s = a.cs[L.nphi + j];
+            const double c = a.cs[j], s = a.cs[n + j];
 #pragma unroll
             for (int d = 0; d < 3; ++d) { fa[d] += b1[d] * c; fb[d] += b1[d] * s; }
-            // SETDT, Fig. 4
-            mdt = fmin(mdt, setdt_node(ph, a.cfl, Ri, dRi, rho, p, vR, vP, vZ, BR, BP, BZ));
+            // SETDT, Fig. 4: signal speed and the three rates
+            const double cf = sqrt(fabs((ph.gamma * p + b2) / rho));
+            const double rR = (fabs(vR) + cf) * ihR, rZ = (fabs(vZ) + cf) * a.ihZ, rP = (fabs(vP) + cf) * ihP;
+            rate = fmax(rate, fmax(rP, fmax(rR, rZ)));
+            if (!(rR + rP + rZ <= 1.79769313486231570815e308)) rate = inf;     // fmax drops NaN: mark a non-finite state
             if (deep) {
                 // div_c B = d_R(R B_R)/R + d_phi B_phi / R + d_Z B_Z
-                const double *br = a.U + 5 * L.field + g, *bz = a.U + 7 * L.field + g;
-                const double *bp = a.U + 6 * L.field + o;
-                const int n = L.nphi;
+                const double *br = a.U + 5 * L.field + gq, *bz = a.U + 7 * L.field + gq;
                 const double dRR = fd1(a.R[i - 2] * br[-2], a.R[i - 1] * br[-1], a.R[i + 1] * br[1], a.R[i + 2] * br[2]);
                 double dPs;      // d_phi B_phi
-                if (a.spec_c1) {
+                if (pipe) {
+                    dPs = fd1(bp[0], bp[1], bp[3], bp[4]) * ph.cP1;
+                } else {
                     dPs = 0.0;   // pseudo-spectral: paired circulant sum (B0_phi drops out of the differences)
                     for (int m = 1; m <= (n - 1) / 2; ++m)
-                        dPs = fma(a.spec_c1[m], bp[(long long)wrap_phi(j + m, n) * L.plane] - bp[(long long)wrap_phi(j - m, n) * L.plane], dPs);
-                } else {
-                    dPs = fd1(bp[(long long)wrap_phi(j - 2, n) * L.plane], bp[(long long)wrap_phi(j - 1, n) * L.plane],
-                              bp[(long long)wrap_phi(j + 1, n) * L.plane], bp[(long long)wrap_phi(j + 2, n) * L.plane]) * ph.cP1;
+                        dPs = fma(a.spec_c1[m], Bp[(long long)wrap_phi(j + m, n) * L.plane] - Bp[(long long)wrap_phi(j - m, n) * L.plane], dPs);
                 }
                 const double dZ = fd1(bz[-2 * L.pR], bz[-L.pR], bz[L.pR], bz[2 * L.pR]);
                 mdiv = fmax(mdiv, fabs(dRR * ph.cR1 * iR + dPs * iR + dZ * ph.cZ1));
             }
         }
-        const double w = Ri * ph.dR * ph.dphi * ph.dZ;
-        ke *= w; me *= w; mep *= w;
-        const double sc = 2.0 / (double)L.nphi;
-        double e1 = 0.0;
-#pragma unroll
-        for (int d = 0; d < 3; ++d) { const double A = fa[d] * sc, B = fb[d] * sc; e1 += A * A + B * B; }
-        men1 = 0.25 * e1 * (Ri * ph.dR * ph.dZ * ph.Lphi);
     }
-    __shared__ double red[DG_BY][DG_N];
-    ke = warp_sum(ke); me = warp_sum(me); mep = warp_sum(mep); men1 = warp_sum(men1);
-    mdiv = warp_max(mdiv); mdt = warp_min(mdt);
-    if (threadIdx.x == 0) {
-        double *r = red[threadIdx.y];
-        r[0] = ke; r[1] = me; r[2] = mep; r[3] = men1; r[4] = mdiv; r[5] = mdt;
+    // phi chunks meet in shared memory; chunk 0's warp combines them in a fixed order
+    __shared__ double sh[DG_G][DG_Q][DG_BX];
+    {
+        double (*m)[DG_BX] = sh[g];
+        m[0][tx] = ke; m[1][tx] = me; m[2][tx] = mep;
+#pragma unroll
+        for (int d = 0; d < 3; ++d) { m[3 + d][tx] = fa[d]; m[6 + d][tx] = fb[d]; }
+        m[9][tx] = mdiv; m[10][tx] = rate;
     }
     __syncthreads();
-    if (threadIdx.x == 0 && threadIdx.y == 0) {
-        double acc[DG_N] = { 0, 0, 0, 0, 0, 100.0 };
-        for (int w = 0; w < DG_BY; ++w) {
-            for (int q = 0; q < 4; ++q) acc[q] += red[w][q];
-            acc[4] = fmax(acc[4], red[w][4]);
-            acc[5] = fmin(acc[5], red[w][5]);
-        }
+    if (g != 0) return;
+    auto sum_chunks = [&](int q) {
+        double v = sh[0][q][tx];
+#pragma unroll
+        for (int w = 1; w < DG_G; ++w) v += sh[w][q][tx];
+        return v;
+    };
+    auto max_chunks = [&](int q) {
+        double v = sh[0][q][tx];
+#pragma unroll
+        for (int w = 1; w < DG_G; ++w) v = fmax(v, sh[w][q][tx]);
+        return v;
+    };
+    double out[DG_N] = { 0, 0, 0, 0, 0, 0 };
+    if (valid) {
+        const double Ri = a.R[i];
+        const double w = Ri * ph.dR * ph.dphi * ph.dZ;
+        out[0] = sum_chunks(0) * w; out[1] = sum_chunks(1) * w; out[2] = sum_chunks(2) * w;
+        const double sc = 2.0 / (double)n;
+        double e1 = 0.0;
+#pragma unroll
+        for (int d = 0; d < 3; ++d) { const double A = sum_chunks(3 + d) * sc, B = sum_chunks(6 + d) * sc; e1 += A * A + B * B; }
+        out[3] = 0.25 * e1 * (Ri * ph.dR * ph.dZ * ph.Lphi);
+        out[4] = max_chunks(9); out[5] = max_chunks(10);
+    }
+#pragma unroll
+    for (int q = 0; q < 4; ++q) out[q] = warp_sum(out[q]);
+    out[4] = warp_max(out[4]); out[5] = warp_max(out[5]);
+    if (tx == 0) {
         double *dst = a.partial + (long long)(blockIdx.y * gridDim.x + blockIdx.x) * DG_N;
-        for (int q = 0; q < DG_N; ++q) dst[q] = acc[q];
+#pragma unroll
+        for (int q = 0; q < DG_N; ++q) dst[q] = out[q];
     }
 }
 
-__global__ void __launch_bounds__(256) diag_final_kernel(const double *partial, int nblocks, double *result)
+// result = { kinetic, magnetic, magnetic_pert, magnetic_n1, max |div_c B|, dt = min(100, cfl / max rate) }; an infinite
+// rate (non-finite state) gives dt = 0
+__global__ void __launch_bounds__(256) diag_final_kernel(const double *partial, int nblocks, double cfl, double *result)
 {
     __shared__ double red[8][DG_N];
-    double acc[DG_N] = { 0, 0, 0, 0, 0, 100.0 };
+    double acc[DG_N] = { 0, 0, 0, 0, 0, 0 };
     for (int b = threadIdx.x; b < nblocks; b += 256) {
         const double *p = partial + (long long)b * DG_N;
         for (int q = 0; q < 4; ++q) acc[q] += p[q];
         acc[4] = fmax(acc[4], p[4]);
-        acc[5] = fmin(acc[5], p[5]);
+        acc[5] = fmax(acc[5], p[5]);
     }
     for (int q = 0; q < 4; ++q) acc[q] = warp_sum(acc[q]);
     acc[4] = warp_max(acc[4]);
-    acc[5] = warp_min(acc[5]);
+    acc[5] = warp_max(acc[5]);
     const int w = threadIdx.x >> 5;
     if ((threadIdx.x & 31) == 0)
         for (int q = 0; q < DG_N; ++q) red[w][q] = acc[q];
     __syncthreads();
     if (threadIdx.x == 0) {
-        double out[DG_N] = { 0, 0, 0, 0, 0, 100.0 };
+        double out[DG_N] = { 0, 0, 0, 0, 0, 0 };
         for (int ww = 0; ww < 8; ++ww) {
             for (int q = 0; q < 4; ++q) out[q] += red[ww][q];
             out[4] = fmax(out[4], red[ww][4]);
-            out[5] = fmin(out[5], red[ww][5]);
+            out[5] = fmax(out[5], red[ww][5]);
         }
+        out[5] = out[5] > 0.0 ? fmin(100.0, cfl / out[5]) : 100.0;      // Fig. 4: DT1 starts at 100
         for (int q = 0; q < DG_N; ++q) result[q] = out[q];
     }
 }
 
 int diag_blocks(const Layout &L)
 {
-    return ((L.nR - 4 + DG_BX - 1) / DG_BX) * ((L.nZ - 4 + DG_BY - 1) / DG_BY);
+    return ((L.nR - 4 + DG_BX - 1) / DG_BX) * (L.nZ - 4);
 }
 
 cudaError_t launch_diag(const DiagArgs &a, int nblocks, double *result6, cudaStream_t s)
 {
-    dim3 block(DG_BX, DG_BY), grid((a.L.nR - 4 + DG_BX - 1) / DG_BX, (a.L.nZ - 4 + DG_BY - 1) / DG_BY);
+    dim3 block(DG_BX, DG_G), grid((a.L.nR - 4 + DG_BX - 1) / DG_BX, a.L.nZ - 4);
     diag_kernel<<<grid, block, 0, s>>>(a);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    diag_final_kernel<<<1, 256, 0, s>>>(a.partial, nblocks, result6);
+    diag_final_kernel<<<1, 256, 0, s>>>(a.partial, nblocks, a.cfl, result6);
     return cudaGetLastError();
 }
 
-cudaError_t configure_kernels() { return cudaSuccess; }
+// Opts every kernel with more than 48 KB of dynamic shared memory in on the CURRENT device (the attribute is per
+// function and device).  Called by clt_create under the context's device, so nothing about it is process-global state.
+cudaError_t configure_kernels()
+{
+    const RhsArgs ra{};
+    const CurlArgs ca{};
+    const SpecArgs sa{};
+    const CUtensorMap tm{};
+    for (int mode = RHS_MODE_K; mode <= RHS_MODE_S4; ++mode)
+        for (int v0 = 0; v0 < 2; ++v0) {
+            cudaError_t e = launch_rhs(ra, mode, v0 != 0, nullptr, true);
+            if (e != cudaSuccess) return e;
+            for (int hs = 0; hs < 4; ++hs) {
+                e = launch_rhs_tma(ra, &tm, &tm, mode, v0 != 0, (hs & 1) != 0, (hs & 2) != 0, nullptr, true);
+                if (e != cudaSuccess) return e;
+            }
+        }
+    for (int hs = 0; hs < 4; ++hs) {
+        cudaError_t e = launch_curl_tma(ca, &tm, (hs & 1) != 0, (hs & 2) != 0, nullptr, true);
+        if (e != cudaSuccess) return e;
+    }
+    return launch_phi_spectral(sa, nullptr, true);
+}
 
 }  // namespace clt
