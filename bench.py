@@ -7,7 +7,8 @@
 One "step" = one classical RK4 step = 4 x (curl_J1 + fused RHS) over the whole grid = all rows of SURVEY 8(a).
 Multi-GPU: the path does not shard in this round (north_star: one GPU, no halo exchange) -- "replicas only":
 N ranks run N independent replicas, value = sum of the replicas' updates / max-over-ranks time.
---impl reference times the CPU oracle (oracle/) on a bounded sample of the same workload, rank 0 only.
+--impl reference times the CPU oracle (oracle/) on the same configuration (whole RK4 steps of config 4; the number of
+timed steps is cut if the box's cores would need more than a few minutes), rank 0 only.
 Prints ONE JSON line.
 """
 from __future__ import annotations
@@ -121,50 +122,69 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def oracle_rate(grid, steps, warmup=0, target_seconds=0.0):
-    """Times the CPU oracle as it stands on a bounded sample (same recipe, smaller grid). Returns dict.
-    target_seconds > 0: keep stepping (whole steps) until about that much CPU work has been timed."""
+def oracle_rate(index, steps, warmup=0, budget_seconds=0.0):
+    """Times the CPU oracle as it stands on BASELINE.json config `index` (same seeded inputs as the GPU arm).
+    budget_seconds > 0: the first step is timed alone and the number of timed steps is cut so that the whole call stays
+    within the budget (the grid is never shrunk: the sample is whole RK4 steps of the named configuration)."""
     import oracle as orc
     from paper_1812_00525_b200 import inputs
-    nR, nphi, nZ = grid
-    prob = inputs.make_custom_problem(nR, nphi, nZ, index=4)
+    prob = inputs.make_problem(index)
     c = prob.cfg
     o = orc.Oracle(c.nR, c.nphi, c.nZ, c.Rmin, c.Rmax, c.Zmin, c.Zmax, c.phi_extent, gamma=c.gamma, eta=c.eta, nu=c.nu,
                    D=c.D, kappa=c.kappa, dt=prob.dt)
     o.set_equilibrium(prob.U0)
     o.set_state(prob.U)
+    asked = steps
     if warmup:
-        o.step(warmup)
+        t0 = time.perf_counter()
+        o.step(1)
+        t1 = time.perf_counter() - t0
+        if budget_seconds > 0:
+            warmup = max(1, min(warmup, int(0.15 * budget_seconds / t1)))
+        if warmup > 1:
+            o.step(warmup - 1)
     t0 = time.perf_counter()
-    o.step(steps)
+    o.step(1)
+    first = time.perf_counter() - t0
+    if budget_seconds > 0:
+        steps = max(1, min(steps, int(0.8 * budget_seconds / first)))
+    if steps > 1:
+        o.step(steps - 1)
     dt = time.perf_counter() - t0
-    if target_seconds > dt:
-        more = max(0, min(200, int(target_seconds / (dt / steps)) - steps))
-        if more:
-            o.step(more)
-            steps += more
-            dt = time.perf_counter() - t0
     cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
-    return {"value": c.interior * steps / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": f"{steps} RK4 step(s) of the config-4 recipe on a {nR}x{nphi}x{nZ} grid ({c.interior} interior nodes), "
-                      f"oracle/clt_oracle.c as it stands (gcc -O2, OpenMP over nodes)", "seconds": dt, "ms_per_step": 1e3 * dt / steps}
+    cut = "" if steps == asked else f" (of {asked} asked: cut to stay within {budget_seconds:.0f} s)"
+    return {"value": c.interior * steps / dt, "unit": UNIT, "cores": cores, "kind": "oracle", "config_index": index,
+            "sample": f"{steps} RK4 step(s){cut} of config {index} itself, {c.nR}x{c.nphi}x{c.nZ} ({c.interior} interior nodes), "
+                      f"oracle/clt_oracle.c as it stands (gcc -O2 -ffp-contract=off, OpenMP over nodes, {cores} thread(s))",
+            "seconds": dt, "ms_per_step": 1e3 * dt / steps, "steps": steps}
+
+
+def oracle_rate_single_thread(index, steps):
+    """The same measurement with OMP_NUM_THREADS=1 (single-threaded on config 2), in a worker process
+    because the OpenMP runtime reads the variable once."""
+    env = dict(os.environ, OMP_NUM_THREADS="1")
+    try:
+        r = subprocess.run([sys.executable, os.path.abspath(__file__), "--oracle-worker", f"{index},{steps}"], env=env,
+                           capture_output=True, text=True, timeout=600)
+        return json.loads(r.stdout.strip().splitlines()[-1])
+    except Exception as e:      # a baseline figure, never a reason to lose the bench line
+        return {"error": repr(e)}
 
 
 def run_reference(args):
+    """--impl reference: the CPU oracle, as it stands, on the configuration the GPU arm measures (config 4 by default)."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    cores = os.cpu_count() or 1
-    # bounded sample: about (K+W) steps within ~2-3 minutes at ~0.05 M updates/s/core
-    budget_updates = 0.05e6 * cores * 150.0 / max(1, args.steps + args.warmup)
-    grid = (128, 16, 128) if budget_updates < 2.0e6 else (256, 32, 256)
-    if budget_updates < 0.25e6:
-        grid = (64, 16, 64)
-    r = oracle_rate(grid, args.steps, args.warmup)
+    r = oracle_rate(args.config, args.steps, args.warmup, budget_seconds=args.reference_budget)
+    from paper_1812_00525_b200 import inputs
+    cfg = inputs.CONFIGS[args.config]
     line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "config 4 recipe (512x64x512 box, seeded perturbations), bounded sample: " + r["sample"]},
+            "config": {"workload": f"config {cfg.index}: {cfg.nR}x{cfg.nphi}x{cfg.nZ} (R x phi x Z), {cfg.interior} interior nodes, "
+                                   f"seeded reference state + perturbations (BASELINE.json configs[{cfg.index - 1}])",
+                       "timed_steps": r["steps"], "sample": r["sample"]},
             "cpu_baseline": {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")},
             "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -260,12 +280,11 @@ def run_ours(args):
     def barrier():
         replicas.barrier(f"cuda:{local}")
 
-    # ---- device-resident throughput -------------------------------------------------------------
+    # ---- device-resident throughput: the library's default path (clt_step replays the step as a CUDA graph) ---------
     g.step(args.warmup)
     barrier()
     sampler = ClockSampler(local)
     sampler.start()
-    g.set_profiling(not args.graph)
     launches0 = g.launch_count
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
@@ -278,9 +297,22 @@ def run_ours(args):
     barrier()
     ms = e0.elapsed_time(e1)
     launches = g.launch_count - launches0
+    clocks = sampler.stop()
+    # ---- second, separately reported region: the same steps with a CUDA event pair around every launch (no graph), for
+    # the per-kernel roofline; `value` above never comes from it ----------------------------------------------------
+    prof_steps = max(1, min(args.steps, args.profile_steps))
+    g.set_profiling(True)
+    p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    p0.record(g.torch_stream)
+    if args.adaptive:
+        g.step_cfl(prof_steps, cfg.cfl)
+    else:
+        g.step(prof_steps)
+    p1.record(g.torch_stream)
+    barrier()
+    prof_ms_step = p0.elapsed_time(p1) / prof_steps
     prof = g.get_profile()
     g.set_profiling(False)
-    clocks = sampler.stop()
     total_updates, secs, value = replicas.aggregate(cfg.interior * args.steps, ms * 1e-3, device=f"cuda:{local}")
     ms = secs * 1e3
     d = g.diagnostics()
@@ -325,11 +357,16 @@ def run_ours(args):
         roof = {"bound": "hbm", "kernel": "rhs_tma_kernel (fused RHS + RK4 stage combine, its 4 stage variants pooled)",
                 "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                 "traffic": args.traffic if args.traffic is not None else (profiled_traffic() if cfg.index == 4 else None),
+                "traffic_source": ("--traffic argument" if args.traffic is not None else
+                                   ("committed ncu --set full capture, profiles/traffic.csv (not measured in this run)"
+                                    if cfg.index == 4 else None)),
+                "profiled_region": {"steps": prof_steps, "ms_per_step": prof_ms_step,
+                                    "note": "per-kernel CUDA events, no graph; `value` is timed on the default graph path"},
                 "ncu_pipes": profiled_pipes() if cfg.index == 4 else None,
                 "peak_source": peak_src + ", burst figure", "avg_launch_ms": ms_rhs / n_rhs,
                 "algorithmic_bytes_per_launch": bytes_per_launch, "share_of_step": ms_rhs / (ms_rhs + prof["ms_curl"] + prof.get("ms_phi", 0.0)),
                 "per_stage": per_stage, "curl_kernel": curl,
-                "phi_prepass": ({"ms": prof["ms_phi"] / prof["n_phi"], "launches_per_step": prof["n_phi"] / args.steps}
+                "phi_prepass": ({"ms": prof["ms_phi"] / prof["n_phi"], "launches_per_step": prof["n_phi"] / prof_steps}
                                 if prof.get("n_phi") else None),
                 "algorithmic_doubles_per_node": {"stage1": 19, "stage2": 35, "stage3": 27, "stage4": 35, "curl": 6,
                                                  "rk4_step": BYTES_PER_UPDATE // 8, "survey_textbook_schedule": 164},
@@ -338,10 +375,12 @@ def run_ours(args):
                                "survey_equivalent_GBps": SURVEY_BYTES_PER_UPDATE * cfg.interior / (ms_step * 1e-3) / 1e9}}
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
-        cores = os.cpu_count() or 1
-        grid = (256, 32, 256) if cores >= 16 else (128, 16, 128)
-        cpu = oracle_rate(grid, 2, target_seconds=12.0)      # about 10-15 s of CPU work
-        cpu = {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        # the oracle on the measured configuration itself (>= 2 steps of config 4, about 10-30 s on the box's
+        # cores) and once single-threaded on config 2
+        r = oracle_rate(cfg.index, 2, budget_seconds=60.0)
+        cpu = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        one = oracle_rate_single_thread(2, 2)
+        cpu["single_thread_config2"] = {k: one[k] for k in ("value", "unit", "cores", "sample") if k in one} or one
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic",
@@ -374,7 +413,12 @@ def main():
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--tile-z", dest="tile_z", type=int, default=0)
     ap.add_argument("--phi-chunks", dest="phi_chunks", type=int, default=0)
-    ap.add_argument("--graph", type=int, default=0)
+    ap.add_argument("--graph", type=int, default=0, help="clt_set_tuning use_graph: 0 = library default (graph), 1 = always, 2 = never")
+    ap.add_argument("--profile-steps", dest="profile_steps", type=int, default=10,
+                    help="steps of the second, per-kernel-profiled region (roofline object)")
+    ap.add_argument("--reference-budget", dest="reference_budget", type=float, default=280.0,
+                    help="--impl reference: seconds of oracle time the run may take (timed steps are cut to fit)")
+    ap.add_argument("--oracle-worker", dest="oracle_worker", default=None, help=argparse.SUPPRESS)
     ap.add_argument("--e2e-steps", dest="e2e_steps", type=int, default=3)
     ap.add_argument("--d-i", dest="d_i", type=float, default=0.0, help="Hall term of eq (5) (NEXT-3); 0 = the measured config")
     ap.add_argument("--phi-scheme", dest="phi_scheme", type=int, default=0, help="1 = pseudo-spectral phi scheme (NEXT-2)")
@@ -385,6 +429,10 @@ def main():
     ap.add_argument("--traffic", type=float, default=None,
                     help="dram bytes per launch of the dominant kernel from an ncu --set full capture (profiles/)")
     args = ap.parse_args()
+    if args.oracle_worker:
+        idx, n = (int(x) for x in args.oracle_worker.split(","))
+        print(json.dumps(oracle_rate(idx, n)), flush=True)
+        return
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         run_reference(args)

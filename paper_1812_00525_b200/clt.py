@@ -47,7 +47,9 @@ EXPORTS = ["clt_workspace_bytes", "clt_create", "clt_destroy", "clt_set_equilibr
            "clt_set_owned_rows", "clt_set_dt", "clt_diagnostics", "clt_suggest_dt", "clt_set_tuning",
            "clt_set_kernel_variant", "clt_spectral_workspace_bytes", "clt_set_phi_scheme", "clt_set_profiling", "clt_get_profile", "clt_launch_count", "clt_stream", "clt_strerror", "clt_last_cuda_error", "clt_version"]
 
+LIB_TEXTBOOK_PATH = os.path.join(_HERE, "libclt_textbook.so")
 _lib = None
+_libs = {}
 
 
 class CltError(RuntimeError):
@@ -56,15 +58,17 @@ class CltError(RuntimeError):
         self.code = code
 
 
-def load():
-    """Loads libclt.so (loudly).  Building is a separate, explicit step: ``python -m paper_1812_00525_b200.build``."""
+def load(path=None):
+    """Loads libclt.so (loudly).  Building is a separate, explicit step: ``python -m paper_1812_00525_b200.build``.
+    ``path`` selects another build of the same ABI (libclt_textbook.so, the textbook-RK4-schedule A/B)."""
     global _lib
-    if _lib is not None:
-        return _lib
-    if not os.path.exists(LIB_PATH):
-        raise ImportError(f"{LIB_PATH} not found: build it with `python -m paper_1812_00525_b200.build` "
+    path = path or LIB_PATH
+    if path in _libs:
+        return _libs[path]
+    if not os.path.exists(path):
+        raise ImportError(f"{path} not found: build it with `python -m paper_1812_00525_b200.build` "
                           "(there is no CPU fallback)")
-    L = ctypes.CDLL(LIB_PATH)
+    L = ctypes.CDLL(path)
     vp, i, d = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
     L.clt_workspace_bytes.restype = ctypes.c_size_t
     L.clt_workspace_bytes.argtypes = [ctypes.POINTER(clt_grid)]
@@ -116,7 +120,9 @@ def load():
     L.clt_last_cuda_error.argtypes = [vp]
     L.clt_version.restype = ctypes.c_char_p
     L.clt_version.argtypes = []
-    _lib = L
+    _libs[path] = L
+    if path == LIB_PATH:
+        _lib = L
     return L
 
 
@@ -140,9 +146,9 @@ class Clt:
     """One libclt context.  Method names and semantics are those of include/clt.h."""
 
     def __init__(self, nR, nphi, nZ, Rmin, Rmax, Zmin, Zmax, phi_extent=0.0, gamma=5.0 / 3.0, eta=0.0, nu=0.0, D=0.0,
-                 kappa=0.0, dt=0.0, cfl=0.5, d_i=0.0, device="cuda:0", stream=None):
+                 kappa=0.0, dt=0.0, cfl=0.5, d_i=0.0, device="cuda:0", stream=None, lib_path=None):
         import torch
-        self.L = load()
+        self.L = load(lib_path)
         if not torch.cuda.is_available():
             raise RuntimeError("libclt needs a CUDA device (no CPU fallback)")
         self.device = torch.device(device)

@@ -197,7 +197,16 @@ __device__ __forceinline__ void rhs_point(const double *stg, int HT, const doubl
 //   S4: U^{n+1} = acc + (U_a - U^n)/3 + dt/6 K4                     ((U_a - U^n)/3 = dt/3 K3)
 // Identical to the textbook scheme up to rounding order.  Per node and step this moves 19 + 35 + 27 + 35
 // doubles through the fused kernel instead of 27 + 43 + 43 + 27.
+// -DCLT_TEXTBOOK_RK4 builds the textbook accumulator schedule instead (libclt_textbook.so; the A/B that shows what
+// the reduced schedule costs in round-off -- BASELINE.md section 4 -- never the product's default):
+//   S1: U_a = U^n + dt/2 K1, acc = U^n + dt/6 K1      S2: U_b = U^n + dt/2 K2, acc += dt/3 K2
+//   S3: U_a = U^n + dt K3,   acc += dt/3 K3           S4: U^{n+1} = acc + dt/6 K4
 // ---------------------------------------------------------------------------------------------
+#ifdef CLT_TEXTBOOK_RK4
+constexpr bool TEXTBOOK_RK4 = true;
+#else
+constexpr bool TEXTBOOK_RK4 = false;
+#endif
 __device__ __forceinline__ void st_out(double *p, double v) { *p = v; }
 
 struct EpiOperands {
@@ -216,6 +225,11 @@ __device__ __forceinline__ void epilogue_load(const RhsArgs &a, long long g, lon
     for (int m = 0; m < 8; ++m) {
         const long long gm = m * field + g;
         if (MODE == RHS_MODE_S1) e.un[m] = (m < NOWN) ? own[m] : ld(a.in + gm);
+        if (TEXTBOOK_RK4) {
+            if (MODE == RHS_MODE_S2 || MODE == RHS_MODE_S3) e.un[m] = ld(a.Un + gm);
+            if (MODE == RHS_MODE_S2 || MODE == RHS_MODE_S3 || MODE == RHS_MODE_S4) e.ac[m] = ld(a.acc + gm);
+            continue;
+        }
         if (MODE == RHS_MODE_S2 || MODE == RHS_MODE_S3 || MODE == RHS_MODE_S4) e.un[m] = ld(a.Un + gm);
         if (MODE == RHS_MODE_S2 || MODE == RHS_MODE_S4) e.us[m] = (m < NOWN) ? own[m] : ld(a.in + gm);
         if (MODE == RHS_MODE_S4) e.ac[m] = ld(a.acc + gm);
@@ -233,7 +247,7 @@ __device__ __forceinline__ void epilogue_store(const RhsArgs &a, long long g, lo
     double an = 0.0, bn = 0.0;
     if (MODE != RHS_MODE_K) {
         an = __ldg(a.coef + (MODE == RHS_MODE_S3 ? 0 : 1));
-        bn = __ldg(a.coef + (MODE == RHS_MODE_S2 ? 2 : 3));
+        bn = __ldg(a.coef + ((MODE == RHS_MODE_S2 || (TEXTBOOK_RK4 && MODE == RHS_MODE_S3)) ? 2 : 3));
     }
     double out[8];
 #pragma unroll
@@ -241,6 +255,17 @@ __device__ __forceinline__ void epilogue_store(const RhsArgs &a, long long g, lo
         const long long gm = m * field + g;
         if (MODE == RHS_MODE_K) {
             st_out(a.out + gm, K[m]);
+        } else if (TEXTBOOK_RK4) {
+            if (MODE == RHS_MODE_S1) {
+                st_out(a.out + gm, fma(an, K[m], e.un[m]));
+                st_out(a.acc + gm, fma(bn, K[m], e.un[m]));
+            } else if (MODE == RHS_MODE_S2 || MODE == RHS_MODE_S3) {
+                st_out(a.out + gm, fma(an, K[m], e.un[m]));
+                st_out(a.acc + gm, fma(bn, K[m], e.ac[m]));
+            } else {
+                out[m] = fma(bn, K[m], e.ac[m]);
+                st_out(a.out + gm, out[m]);
+            }
         } else if (MODE == RHS_MODE_S1 || MODE == RHS_MODE_S3) {
             st_out(a.out + gm, fma(an, K[m], e.un[m]));
         } else if (MODE == RHS_MODE_S2) {

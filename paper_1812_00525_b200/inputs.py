@@ -201,14 +201,24 @@ def custom_config(nR, nphi, nZ, index=99, steps=1, **kw) -> Config:
     return Config(index, f"custom-{nR}x{nphi}x{nZ}", nR, nphi, nZ, steps, **kw)
 
 
-def make_custom_problem(nR, nphi, nZ, index=99, rotation=0.0, amplitude_scale=1.0, **kw) -> Problem:
+def make_custom_problem(nR, nphi, nZ, index=99, rotation=0.0, amplitude_scale=1.0, poloidal=None, **kw) -> Problem:
     """Same recipe on an arbitrary grid.  ``rotation`` = Omega adds a rigid toroidal rotation
-    v0 = Omega R phi^ to the reference state (exercises the v0 terms of eqs (11)-(13))."""
+    v0 = Omega R phi^ to the reference state (exercises the toroidal v0 terms of eqs (11)-(13)).
+    ``poloidal`` = (a, b) adds a compressible poloidal flow  v0_R = a sin(pi x) cos(pi z),
+    v0_Z = b cos(2 pi x) sin(pi z) + b/2  (x, z = box coordinates in [0, 1]): div v0, grad v0_R, grad v0_Z,
+    (v0.grad)v0 and the R/Z parts of v0 x B0 are all non-zero, on the frozen layers too."""
     cfg = custom_config(nR, nphi, nZ, index=index, **kw)
     U0 = reference_state(cfg)
     if rotation != 0.0:
         R, _, _ = grid_axes(cfg)
         U0[3] = rotation * R[None, :]
+    if poloidal is not None:
+        a, b = poloidal
+        R, Z, _ = grid_axes(cfg)
+        x = ((R - cfg.Rmin) / (cfg.Rmax - cfg.Rmin))[None, :]
+        z = ((Z - cfg.Zmin) / (cfg.Zmax - cfg.Zmin))[:, None]
+        U0[2] = a * np.sin(np.pi * x) * np.cos(np.pi * z)
+        U0[4] = b * np.cos(2.0 * np.pi * x) * np.sin(np.pi * z) + 0.5 * b
     U = initial_state(cfg, U0)
     if amplitude_scale != 1.0:
         U = U0[:, None] + amplitude_scale * (U - U0[:, None])

@@ -4,7 +4,8 @@ import numpy as np
 import pytest
 
 from paper_1812_00525_b200 import inputs
-from parity_util import RHS_TOL, STEP_TOL, assert_close, assert_close_physical, make_gpu, make_oracle, rel_linf
+from parity_util import (RHS_TOL, STEP_TOL, assert_close, assert_close_physical, fma_oracle, make_gpu, make_oracle, oracle_run,
+                         record_margin, rel_linf)
 
 pytestmark = pytest.mark.gpu
 
@@ -17,6 +18,10 @@ def _problems():
         "min-9x5x9": lambda: inputs.make_custom_problem(9, 5, 9, index=12),
         "rotating-v0": lambda: inputs.make_custom_problem(45, 8, 37, index=13, rotation=0.05),
         "big-amplitude": lambda: inputs.make_custom_problem(40, 12, 40, index=14, amplitude_scale=200.0),
+        # a moving reference state with poloidal, compressible flow (and rotation): every v0 term of eqs (11)-(13) and of
+        # E1 = -v x B + v0 x B0 is non-zero (rigid rotation alone leaves div v0, grad v0_R/Z, v0_R, v0_Z at zero)
+        "poloidal-v0": lambda: inputs.make_custom_problem(45, 8, 37, index=19, rotation=0.04, poloidal=(0.03, -0.02),
+                                                          amplitude_scale=20.0),
     }
 
 
@@ -65,7 +70,8 @@ def test_rhs_with_large_dissipation_matches_oracle():
     assert_close(g.rhs(), o.rhs(), RHS_TOL, "rhs, large dissipation")
 
 
-@pytest.mark.parametrize("name,steps", [("config1", 10), ("ragged-77x9x53", 100), ("rotating-v0", 100), ("min-9x5x9", 20)])
+@pytest.mark.parametrize("name,steps", [("config1", 10), ("ragged-77x9x53", 100), ("rotating-v0", 100), ("min-9x5x9", 20),
+                                        ("poloidal-v0", 100)])
 def test_steps_match_oracle(name, steps):
     prob = _problems()[name]()
     o, g = make_oracle(prob), make_gpu(prob)
@@ -84,11 +90,10 @@ def test_steps_match_oracle(name, steps):
 
 
 def test_config2_100_steps_match_oracle():
-    prob = inputs.make_problem(2)
-    o, g = make_oracle(prob), make_gpu(prob)
-    o.step(prob.cfg.steps)
-    g.step(prob.cfg.steps)
-    assert_close(g.get_state(), o.get_state(), STEP_TOL, "config 2, 100 RK4 steps")
+    ref = oracle_run(2, 100)
+    g = make_gpu(ref["prob"])
+    g.step(100)
+    record_margin("config2_100_steps", assert_close(g.get_state(), ref["U"], STEP_TOL, "config 2, 100 RK4 steps"))
 
 
 @pytest.mark.parametrize("chunks,graph,variant,tile_z", [(2, 2, 0, 0), (4, 2, 0, 0), (1, 1, 0, 0), (2, 1, 0, 0), (3, 1, 1, 0), (1, 2, 0, 0)])
@@ -171,28 +176,39 @@ def test_device_pointers_and_call_order():
 # BASELINE.json configs at full size (the oracle needs about a minute per 100 steps of 256x32x256 on 16 cores)
 
 def test_config3_100_steps_match_oracle():
-    prob = inputs.make_problem(3)
-    o, g = make_oracle(prob), make_gpu(prob)
-    assert_close(g.rhs(), o.rhs(), RHS_TOL, "config 3, rhs")
-    o.step(prob.cfg.steps)
-    g.step(prob.cfg.steps)
-    assert_close(g.get_state(), o.get_state(), STEP_TOL, "config 3, 100 RK4 steps")
-
-
-def test_config5_first_100_steps_match_oracle_and_2000_step_trace():
-    prob = inputs.make_problem(5)
-    o, g = make_oracle(prob), make_gpu(prob)
-    assert_close(g.rhs(), o.rhs(), RHS_TOL, "config 5, rhs")
-    d0 = g.diagnostics()
-    o.step(100)
+    ref = oracle_run(3, 100)
+    g = make_gpu(ref["prob"])
+    record_margin("config3_rhs", assert_close(g.rhs(), ref["K"], RHS_TOL, "config 3, rhs"))
     g.step(100)
-    # v_phi is ~1e-7 here, five orders below p: per-component relative error is dominated by the 1-ulp noise of the
-    # stored total p (reading R10); the vector v as a whole and every other field meet 1e-9
-    U_g, U_o = g.get_state(), o.get_state()
-    assert_close_physical(U_g, U_o, STEP_TOL, "config 5, first 100 RK4 steps")
+    record_margin("config3_100_steps", assert_close(g.get_state(), ref["U"], STEP_TOL, "config 3, 100 RK4 steps"))
+
+
+def test_config5_first_100_steps_match_oracle_against_the_measured_rounding_floor_and_2000_step_trace(tmp_path):
+    """Config 5 (north_star: compared with the oracle on the first 100 steps).  Seven of the eight fields meet the 1e-9
+    bar per component.  v_phi stays ~1e-7 beside p ~1e-2 and B_phi ~1, and round-off alone moves it by more than
+    1e-9 of itself: the floor is MEASURED here on this very run as the distance between two builds of the oracle
+    (with and without FMA contraction -- same arithmetic, other rounding), and the GPU's v_phi error has to stay
+    within 3x that floor (reading R10)."""
+    ref = oracle_run(5, 100)
+    prob, U_o, do = ref["prob"], ref["U"], ref["diag"]
+    g = make_gpu(prob)
+    record_margin("config5_rhs", assert_close(g.rhs(), ref["K"], RHS_TOL, "config 5, rhs"))
+    d0 = g.diagnostics()
+    g.step(100)
+    U_g = g.get_state()
     errs = rel_linf(U_g, U_o)
-    assert max(errs[f] for f in (0, 1, 2, 4, 5, 6, 7)) <= STEP_TOL and errs[3] <= 5e-8, errs
-    do, dg = o.diagnostics(), g.diagnostics()
+    record_margin("config5_100_steps_gpu_vs_oracle", errs)
+    assert_close_physical(U_g, U_o, STEP_TOL, "config 5, first 100 RK4 steps")
+    assert max(errs[f] for f in (0, 1, 2, 4, 5, 6, 7)) <= STEP_TOL, errs
+    of = fma_oracle(prob, tmp_path)
+    if of is None:
+        pytest.skip("no FMA-capable host compiler/CPU: the rounding floor of v_phi cannot be measured here")
+    of.step(100)
+    floor = rel_linf(of.get_state(), U_o)
+    record_margin("config5_100_steps_oracle_fma_vs_oracle", floor)
+    assert max(floor[f] for f in (0, 1, 2, 4, 5, 6, 7)) <= STEP_TOL, floor      # the floor of the other fields is far below the bar
+    assert errs[3] <= max(STEP_TOL, 3.0 * floor[3]), (errs[3], floor[3])
+    dg = g.diagnostics()
     for k in ("kinetic", "magnetic", "magnetic_pert", "magnetic_n1"):
         assert abs(dg[k] - do[k]) <= 1e-9 * abs(do[k]), (k, dg[k], do[k])
     # the rest of the 2000-step run on the GPU alone: the n = 1 magnetic energy trace stays finite and smooth, the
@@ -212,24 +228,49 @@ def test_config5_first_100_steps_match_oracle_and_2000_step_trace():
     assert np.array_equal(U[:, :, :2], prob.U[:, :, :2]) and np.array_equal(U[..., -2:], prob.U[..., -2:])
 
 
-def test_config4_rhs_and_2_steps_match_oracle_in_the_bench_launch_configuration():
-    prob = inputs.make_problem(4)
-    o, g = make_oracle(prob), make_gpu(prob)          # default tuning = what bench.py times
-    assert_close(g.rhs(), o.rhs(), RHS_TOL, "config 4, rhs")
-    o.step(2)
-    g.step(2)
-    assert_close(g.get_state(), o.get_state(), STEP_TOL, "config 4, 2 RK4 steps")
-    # properties that hold at any size after the bench's 50 steps: frozen layers, finite, div_c B invariant
-    d2 = g.diagnostics()
-    g.step(48)
+def test_config4_rhs_and_50_steps_match_oracle_in_the_bench_launch_configuration():
+    """BASELINE.json config 4 at its own step count (the paper's validation is a full-length CPU-vs-GPU run, L430-436):
+    all 8 fields, element by element, after 50 RK4 steps -- default tuning = exactly what bench.py times."""
+    ref = oracle_run(4, 50)
+    prob = ref["prob"]
+    g = make_gpu(prob)
+    record_margin("config4_rhs", assert_close(g.rhs(), ref["K"], RHS_TOL, "config 4, rhs"))
+    d0 = g.diagnostics()
+    g.step(50)
+    U_g = g.get_state()
+    record_margin("config4_50_steps", assert_close(U_g, ref["U"], STEP_TOL, "config 4, 50 RK4 steps"))
+    assert np.array_equal(U_g[:, :, :2], prob.U[:, :, :2]) and np.array_equal(U_g[..., -2:], prob.U[..., -2:])
     d = g.diagnostics()
-    assert d["step"] == 50 and all(np.isfinite(d[k]) for k in ("kinetic", "magnetic", "magnetic_pert", "magnetic_n1", "max_divB"))
-    assert abs(d["max_divB"] - d2["max_divB"]) <= 1e-6 * d2["max_divB"] + 1e-12
-    assert abs(d["magnetic"] - d2["magnetic"]) <= 1e-6 * d2["magnetic"]
+    assert d["step"] == 50
+    for k in ("kinetic", "magnetic", "magnetic_pert", "magnetic_n1"):
+        assert abs(d[k] - ref["diag"][k]) <= 1e-9 * abs(ref["diag"][k]), (k, d[k], ref["diag"][k])
+    assert abs(d["max_divB"] - d0["max_divB"]) <= 1e-6 * d0["max_divB"] + 1e-12
+
+
+@pytest.mark.parametrize("index,steps", [(2, 100), (3, 100), (5, 100)])
+def test_textbook_rk4_schedule_build_against_the_reduced_schedule(index, steps):
+    """A/B of the RK4 buffer schedule: libclt_textbook.so is the same source built with
+    -DCLT_TEXTBOOK_RK4 (27/43/43/27 doubles per node, the accumulator written every stage).  Both schedules must meet the
+    same bars against the oracle; the observed margins of both go to BASELINE.md section 4, and the reduced schedule
+    may not be more than 4x further from the oracle than the textbook one on any field (it re-derives dt/6 K1 and
+    dt/3 K3 from rounded stage states: a few ulp of the state, not a change of the method)."""
+    ref = oracle_run(index, steps)
+    out = {}
+    for name, tb in (("reduced", False), ("textbook", True)):
+        g = make_gpu(ref["prob"], textbook_rk4=tb)
+        g.step(steps)
+        out[name] = rel_linf(g.get_state(), ref["U"])
+        g.close()
+    record_margin(f"config{index}_{steps}_steps_schedules", out)
+    fields = (0, 1, 2, 4, 5, 6, 7) if index == 5 else range(8)
+    for name in out:
+        assert max(out[name][f] for f in fields) <= STEP_TOL, (name, out[name])
+    for f in range(8):
+        assert out["reduced"][f] <= 4.0 * out["textbook"][f] + 1e-13, (f, out)
 
 
 # ------------------------------------------------------------------------------ NEXT-3: Hall term of eq (5), L77
-HALL_CASES = ["config1", "ragged-77x9x53", "rotating-v0", "min-9x5x9", "big-amplitude"]
+HALL_CASES = ["config1", "ragged-77x9x53", "rotating-v0", "min-9x5x9", "big-amplitude", "poloidal-v0"]
 
 
 @pytest.mark.parametrize("name", HALL_CASES)
@@ -248,7 +289,7 @@ def test_hall_field_and_rhs_match_oracle(name):
     assert np.abs(K_o[5:] - K_0[5:]).max() > 1e-3 * np.abs(K_0[5:]).max()
 
 
-@pytest.mark.parametrize("name,steps", [("config1", 20), ("rotating-v0", 50), ("ragged-77x9x53", 30)])
+@pytest.mark.parametrize("name,steps", [("config1", 20), ("rotating-v0", 50), ("ragged-77x9x53", 30), ("poloidal-v0", 40)])
 def test_hall_steps_match_oracle(name, steps):
     prob = _problems()[name]()
     over = dict(d_i=0.03, dt=0.2 * prob.dt)       # whistler CFL: d_i k^2 B dt stays well below the RK4 limit
@@ -283,6 +324,8 @@ SPEC_CASES = {
     "rotating-v0-12": lambda: inputs.make_custom_problem(45, 12, 37, index=13, rotation=0.05),   # even nphi, generic path
     "nphi32": lambda: inputs.make_custom_problem(40, 32, 24, index=17, amplitude_scale=50.0),
     "nphi64": lambda: inputs.make_custom_problem(36, 64, 20, index=18, amplitude_scale=50.0),
+    "poloidal-v0-16": lambda: inputs.make_custom_problem(45, 16, 37, index=19, rotation=0.04, poloidal=(0.03, -0.02),
+                                                         amplitude_scale=20.0),
 }
 
 
@@ -307,7 +350,7 @@ def test_spectral_curl_and_rhs_match_oracle(name, d_i, scheme=1):
     assert np.array_equal(g.rhs(), g_fd.rhs())
 
 
-@pytest.mark.parametrize("name,steps", [("config1", 20), ("rotating-v0-12", 50), ("ragged-77x9x53", 30)])
+@pytest.mark.parametrize("name,steps", [("config1", 20), ("rotating-v0-12", 50), ("ragged-77x9x53", 30), ("poloidal-v0-16", 30)])
 def test_spectral_steps_and_diagnostics_match_oracle(name, steps):
     prob = SPEC_CASES[name]()
     over = dict(phi_scheme=1, dt=0.5 * prob.dt)
@@ -350,7 +393,8 @@ def test_slab_decomposition_matches_single_domain_and_oracle(world, variant):
     device tensors): same state as the undivided run (to round-off: a slab's dZ is recomputed from its own Zmin/Zmax)
     and as the oracle."""
     from paper_1812_00525_b200 import slab
-    prob = inputs.make_custom_problem(45, 8, 41, index=21, rotation=0.05 if variant == "fd" else 0.0)
+    prob = inputs.make_custom_problem(45, 8, 41, index=21, rotation=0.05 if variant == "fd" else 0.0,
+                                      poloidal=(0.03, -0.02) if variant != "spectral" else None)
     kw = {"fd": {}, "hall": dict(d_i=0.03), "spectral": dict(phi_scheme=1)}[variant]
     dt = prob.dt * (0.2 if variant == "hall" else 0.5)
     steps = 12
@@ -436,7 +480,8 @@ def test_kernels_never_write_outside_the_nodes():
 
 
 # ------------------------------------------------------------------------------ NEXT-1 in the loop: clt_step_cfl
-@pytest.mark.parametrize("name,variant", [("big-amplitude", 0), ("ragged-77x9x53", 0), ("rotating-v0", 1), ("config1", 0)])
+@pytest.mark.parametrize("name,variant", [("big-amplitude", 0), ("ragged-77x9x53", 0), ("rotating-v0", 1), ("config1", 0),
+                                          ("poloidal-v0", 0), ("poloidal-v0", 1)])
 def test_adaptive_steps_match_oracle(name, variant):
     prob = _problems()[name]()
     amp = dict(amplitude_scale=300.0) if name == "config1" else {}
