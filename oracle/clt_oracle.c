@@ -28,6 +28,8 @@
  * exact discrete whistler-type response with the squared modified wavenumber, d_i = 0 reduction, and the
  * sympy convergence pin P3b run with d_i != 0.  P13 pseudo-spectral phi scheme: against numpy.fft, exact on
  * resolved Fourier modes, the Alfven identity with the exact wavenumber, P3b with the spectral scheme.
+ * P10 oracle_setdt against the closed form of Fig. 4 on a uniform state; P11 oracle_diagnostics (all five
+ * outputs) against closed forms; P14 oracle_step_cfl = SETDT + one RK4 step with that dt, step by step.
  * Parity unpinned: none of the exported functions (each is covered by at least one pin); the
  * absolute value of a generic RHS has no paper-printed number to compare with (PAPER.md prints
  * no worked example), so the pins above are mathematical ones.

@@ -209,14 +209,15 @@ EncodeTiledFn encode_tiled()
 }
 
 // 4-D map (R column, Z row, phi plane, field) over nfields consecutive padded fields; box = tile with halo
-bool make_map(const clt_ctx *ctx, const double *base, int nfields, int tile_z, CUtensorMap *out)
+// box_fields = 1: one field per copy; = nfields: one copy brings the tiles of all fields (stored field after field)
+bool make_map(const clt_ctx *ctx, const double *base, int nfields, int tile_z, CUtensorMap *out, int box_fields = 1)
 {
     EncodeTiledFn enc = encode_tiled();
     if (!enc) return false;
     const Layout &L = ctx->L;
     const cuuint64_t dims[4] = { (cuuint64_t)L.pR, (cuuint64_t)L.nZ, (cuuint64_t)L.nphi, (cuuint64_t)nfields };
     const cuuint64_t strides[3] = { (cuuint64_t)L.pR * 8, (cuuint64_t)L.plane * 8, (cuuint64_t)L.field * 8 };
-    const cuuint32_t box[4] = { 32 + 4, (cuuint32_t)tile_z + 4, 1, 1 };      // tile with the radius-2 halo
+    const cuuint32_t box[4] = { 32 + 4, (cuuint32_t)tile_z + 4, 1, (cuuint32_t)box_fields };      // tile with the radius-2 halo
     const cuuint32_t estr[4] = { 1, 1, 1, 1 };
     return enc(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, (void *)base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                CU_TENSOR_MAP_SWIZZLE_NONE, CLT_L2_PROMO, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE)
@@ -355,7 +356,8 @@ int run_rhs(clt_ctx *ctx, int mode, const double *in, double *out)
         if (r) return r;
     }
     alignas(64) CUtensorMap tmU, tmJ;
-    if (tma && (!make_map(ctx, in, 8, rhs_tile_z(), &tmU) || !make_map(ctx, ctx->J1, ctx->hall ? 6 : 3, rhs_tile_z(), &tmJ))) {
+    const int nJ = ctx->hall ? 6 : 3;
+    if (tma && (!make_map(ctx, in, 8, rhs_tile_z(), &tmU, 8) || !make_map(ctx, ctx->J1, nJ, rhs_tile_z(), &tmJ, nJ))) {
         snprintf(ctx->cuda_err, sizeof(ctx->cuda_err), "cuTensorMapEncodeTiled failed");
         return CLT_ECUDA;
     }

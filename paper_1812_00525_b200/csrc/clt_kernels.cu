@@ -189,18 +189,21 @@ __device__ __forceinline__ void rhs_point(const double *stg, int HT, const doubl
 
 // ---------------------------------------------------------------------------------------------
 // a6: RK4 stage combine (L125, L139) in a reduced-traffic accumulator form.
-// Classical RK4, U^{n+1} = U^n + dt/6 (K1 + 2 K2 + 2 K3 + K4); the partial sums are rebuilt from stage
-// states that are read anyway instead of being written and re-read through a separate array:
+// Classical RK4, U^{n+1} = U^n + dt/6 (K1 + 2 K2 + 2 K3 + K4).  The accumulator holds the INCREMENT
+// dt/6 K1 + dt/3 K2 (+ ...), never the state: U^n is added once, in stage 4, so a step rounds the state once at the
+// size of U -- like the literal formula above -- instead of once per stage (for B_phi ~ 1 next to v_phi ~ 1e-7 every
+// extra rounding of the state is visible in v_phi after 100 steps: DESIGN.md reading R10).  The partial sums are
+// rebuilt from stage states that are read anyway instead of being written and re-read through a separate array:
 //   S1: U_a = U^n + dt/2 K1                                        (no accumulator write)
-//   S2: U_b = U^n + dt/2 K2,  acc = U^n + (U_a - U^n)/3 + dt/3 K2   ((U_a - U^n)/3 = dt/6 K1)
+//   S2: U_b = U^n + dt/2 K2,  acc = (U_a - U^n)/3 + dt/3 K2         ((U_a - U^n)/3 = dt/6 K1)
 //   S3: U_a = U^n + dt K3                                          (no accumulator traffic)
-//   S4: U^{n+1} = acc + (U_a - U^n)/3 + dt/6 K4                     ((U_a - U^n)/3 = dt/3 K3)
+//   S4: U^{n+1} = U^n + [acc + (U_a - U^n)/3 + dt/6 K4]             ((U_a - U^n)/3 = dt/3 K3)
 // Identical to the textbook scheme up to rounding order.  Per node and step this moves 19 + 35 + 27 + 35
 // doubles through the fused kernel instead of 27 + 43 + 43 + 27.
 // -DCLT_TEXTBOOK_RK4 builds the textbook accumulator schedule instead (libclt_textbook.so; the A/B that shows what
 // the reduced schedule costs in round-off -- BASELINE.md section 4 -- never the product's default):
-//   S1: U_a = U^n + dt/2 K1, acc = U^n + dt/6 K1      S2: U_b = U^n + dt/2 K2, acc += dt/3 K2
-//   S3: U_a = U^n + dt K3,   acc += dt/3 K3           S4: U^{n+1} = acc + dt/6 K4
+//   S1: U_a = U^n + dt/2 K1, acc = dt/6 K1            S2: U_b = U^n + dt/2 K2, acc += dt/3 K2
+//   S3: U_a = U^n + dt K3,   acc += dt/3 K3           S4: U^{n+1} = U^n + (acc + dt/6 K4)
 // ---------------------------------------------------------------------------------------------
 #ifdef CLT_TEXTBOOK_RK4
 constexpr bool TEXTBOOK_RK4 = true;
@@ -226,8 +229,10 @@ __device__ __forceinline__ void epilogue_load(const RhsArgs &a, long long g, lon
         const long long gm = m * field + g;
         if (MODE == RHS_MODE_S1) e.un[m] = (m < NOWN) ? own[m] : ld(a.in + gm);
         if (TEXTBOOK_RK4) {
-            if (MODE == RHS_MODE_S2 || MODE == RHS_MODE_S3) e.un[m] = ld(a.Un + gm);
-            if (MODE == RHS_MODE_S2 || MODE == RHS_MODE_S3 || MODE == RHS_MODE_S4) e.ac[m] = ld(a.acc + gm);
+            if (MODE == RHS_MODE_S2 || MODE == RHS_MODE_S3 || MODE == RHS_MODE_S4) {
+                e.un[m] = ld(a.Un + gm);
+                e.ac[m] = ld(a.acc + gm);
+            }
             continue;
         }
         if (MODE == RHS_MODE_S2 || MODE == RHS_MODE_S3 || MODE == RHS_MODE_S4) e.un[m] = ld(a.Un + gm);
@@ -238,17 +243,27 @@ __device__ __forceinline__ void epilogue_load(const RhsArgs &a, long long g, lon
 // The stage coefficients come from device memory (a.coef = { dt, dt/2, dt/3, dt/6 }: the fixed-dt table, or the clock
 // that dt_commit_kernel advances).  Adaptive stepping (clt_step_cfl, NEXT-1): stage 4 folds the SETDT minimum of the
 // new state into `rate` (Fig. 3: STEPON then SETDT, without a separate pass over the state).
+// out = U^n + an K (stages 1-3: dt/2, dt/2, dt); bn = weight of K in the accumulator (stage 2: dt/3) / in U^{n+1}
+// (stage 4: dt/6).  Read once per thread, before the sweep.
+struct StageCoef {
+    double an, bn;
+};
+template <int MODE>
+__device__ __forceinline__ StageCoef load_stage_coef(const RhsArgs &a)
+{
+    StageCoef c = { 0.0, 0.0 };
+    if (MODE != RHS_MODE_K) {
+        c.an = __ldg(a.coef + (MODE == RHS_MODE_S3 ? 0 : 1));
+        c.bn = __ldg(a.coef + ((MODE == RHS_MODE_S2 || (TEXTBOOK_RK4 && MODE == RHS_MODE_S3)) ? 2 : 3));
+    }
+    return c;
+}
 template <int MODE>
 __device__ __forceinline__ void epilogue_store(const RhsArgs &a, long long g, long long field, const EpiOperands &e,
-                                               const double (&K)[8], double iR, double &rate)
+                                               const double (&K)[8], double iR, double &rate, const StageCoef &sc)
 {
     constexpr double third = 1.0 / 3.0;
-    // out = U^n + an K (stages 1-3: dt/2, dt/2, dt); bn = weight of K in the accumulator (stage 2: dt/3) / in U^{n+1} (stage 4: dt/6)
-    double an = 0.0, bn = 0.0;
-    if (MODE != RHS_MODE_K) {
-        an = __ldg(a.coef + (MODE == RHS_MODE_S3 ? 0 : 1));
-        bn = __ldg(a.coef + ((MODE == RHS_MODE_S2 || (TEXTBOOK_RK4 && MODE == RHS_MODE_S3)) ? 2 : 3));
-    }
+    const double an = sc.an, bn = sc.bn;
     double out[8];
 #pragma unroll
     for (int m = 0; m < 8; ++m) {
@@ -258,21 +273,21 @@ __device__ __forceinline__ void epilogue_store(const RhsArgs &a, long long g, lo
         } else if (TEXTBOOK_RK4) {
             if (MODE == RHS_MODE_S1) {
                 st_out(a.out + gm, fma(an, K[m], e.un[m]));
-                st_out(a.acc + gm, fma(bn, K[m], e.un[m]));
+                st_out(a.acc + gm, bn * K[m]);
             } else if (MODE == RHS_MODE_S2 || MODE == RHS_MODE_S3) {
                 st_out(a.out + gm, fma(an, K[m], e.un[m]));
                 st_out(a.acc + gm, fma(bn, K[m], e.ac[m]));
             } else {
-                out[m] = fma(bn, K[m], e.ac[m]);
+                out[m] = e.un[m] + fma(bn, K[m], e.ac[m]);
                 st_out(a.out + gm, out[m]);
             }
         } else if (MODE == RHS_MODE_S1 || MODE == RHS_MODE_S3) {
             st_out(a.out + gm, fma(an, K[m], e.un[m]));
         } else if (MODE == RHS_MODE_S2) {
             st_out(a.out + gm, fma(an, K[m], e.un[m]));
-            st_out(a.acc + gm, fma(bn, K[m], fma(e.us[m] - e.un[m], third, e.un[m])));
+            st_out(a.acc + gm, fma(bn, K[m], (e.us[m] - e.un[m]) * third));
         } else {
-            out[m] = fma(bn, K[m], fma(e.us[m] - e.un[m], third, e.ac[m]));
+            out[m] = e.un[m] + fma(bn, K[m], fma(e.us[m] - e.un[m], third, e.ac[m]));
             st_out(a.out + gm, out[m]);
         }
     }
@@ -459,6 +474,7 @@ __global__ void __launch_bounds__(TR *TZ, 1) rhs_kernel(const __grid_constant__ 
     const double iR = __ldg(a.invR + ic);
     const double iR2 = iR * iR;
     double rate = 0.0;           // largest signal rate (|v_d| + c)/(12 h_d) at this thread's nodes (stage 4 of clt_step_cfl)
+    const StageCoef coef = load_stage_coef<MODE>(a);
 
 #pragma unroll 1
     for (int j = ja; j < jb; ++j) {
@@ -517,7 +533,7 @@ __global__ void __launch_bounds__(TR *TZ, 1) rhs_kernel(const __grid_constant__ 
             EpiOperands eo;
             // plain coherent loads: stage 4 updates U^n in place through a.out, so the non-coherent path is not allowed here
             epilogue_load<MODE, 0>(a, g, L.field, eo, [](const double *p) { return *p; });
-            epilogue_store<MODE>(a, g, L.field, eo, K, iR, rate);
+            epilogue_store<MODE>(a, g, L.field, eo, K, iR, rate, coef);
         }
         advance();
     }
@@ -625,7 +641,7 @@ struct RhsTmaSmem {
     double sring[4][5][HT];            // rho1, p1, v1
     double ering[4][3][HT];            // E1
     alignas(8) unsigned long long bar[NRAW];   // TMA completion, one per raw buffer
-    alignas(8) unsigned long long ready;       // split CTA barrier: "this plane is staged" (count = all threads)
+    alignas(8) unsigned long long ready;       // split CTA barrier: "this plane is staged" (one arrival per warp)
 };
 
 template <int TZ, int NRAW, int MODE, bool V0, bool HALL, bool SPEC>
@@ -670,7 +686,7 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
 
     if (tid == 0) {
         for (int b = 0; b < NRAW; ++b) mbar_init(&S.bar[b], 1);
-        mbar_init(&S.ready, TR * TZ);
+        mbar_init(&S.ready, TZ);         // one arrival per warp (lane 0, after __syncwarp)
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmU) : "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmJ) : "memory");
@@ -687,11 +703,18 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
         const int jw = wrap_phi(ja - 2 + n, L.nphi);
         const int b = n % NRAW;
         mbar_expect_tx(&S.bar[b], (unsigned)(NF * HT * sizeof(double)));
-#pragma unroll
-        for (int m = 0; m < 8; ++m) tma_load_4d(&S.raw[b][m][0], &tmU, LP + i0 - 2, k0 - 2, jw, m, &S.bar[b]);
-#pragma unroll
-        for (int m = 0; m < NF - 8; ++m) tma_load_4d(&S.raw[b][8 + m][0], &tmJ, LP + i0 - 2, k0 - 2, jw, m, &S.bar[b]);
+        // two bulk copies per plane: the boxes span the field axis (8 fields of U; J1 [and G]), so the one thread that
+        // issues them -- and the warp that waits for it at the next barrier -- loses a dozen instructions, not a hundred
+        static_assert(SM::HTP == HT, "a box that spans the field axis fills the raw buffer densely");
+        tma_load_4d(&S.raw[b][0][0], &tmU, LP + i0 - 2, k0 - 2, jw, 0, &S.bar[b]);
+        tma_load_4d(&S.raw[b][8][0], &tmJ, LP + i0 - 2, k0 - 2, jw, 0, &S.bar[b]);
     };
+
+    // NRAW planes are kept in flight; the first ones are requested before anything else so that the table reads below
+    // overlap their latency
+    const int total = jb - ja + 4;
+    if (tid == 0)
+        for (int n = 0; n < NRAW && n < total; ++n) issue(n);
 
     // phi-invariant values of the own node and of the halo node, kept in registers for the whole sweep
     const CentreTab ct = load_centre_tab(tab, L.plane, off2);
@@ -746,7 +769,6 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
     double eR[5], eZ[5];   // E1_R, E1_Z of planes j-2 .. j+2
     double Fp[3][3];       // F = J1 x B + J0 x B1 of planes j .. j+2
     int sl = 0;            // ring slot that receives the plane being consumed (plane j+2)
-    const int total = jb - ja + 4;
 
     // consume the raw tile of plane number nlead (the plane that becomes plane j+2)
     auto lead = [&]() {
@@ -784,9 +806,7 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
         sl = (sl + 1) & 3;
     };
 
-    // prologue: planes number 0 .. 3 (ja-2 .. ja+1); NRAW planes are kept in flight
-    if (tid == 0)
-        for (int n = 0; n < NRAW && n < total; ++n) issue(n);
+    // prologue: planes number 0 .. 3 (ja-2 .. ja+1)
 #pragma unroll 1
     for (int n = 0; n < 4; ++n) {
         lead();
@@ -794,11 +814,11 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
         if (tid == 0 && n + NRAW < total) issue(n + NRAW);
         advance();
     }
-    unsigned ready_parity = 0;
 
     const double iR = __ldg(a.invR + ic);
     const double iR2 = iR * iR;
     double rate = 0.0;           // largest signal rate (|v_d| + c)/(12 h_d) at this thread's nodes (stage 4 of clt_step_cfl)
+    const StageCoef coef = load_stage_coef<MODE>(a);
 
 #pragma unroll 1
     for (int j = ja; j < jb; ++j) {
@@ -811,11 +831,13 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
                 if (MODE == RHS_MODE_S4) prefetch_l2(a.acc + m * L.field + g1);
             }
         }
+        const int it = j - ja;                                    // iteration number: consumes plane number it + 4
         lead();
         const int sc = (sl + 2) & 3;                              // ring slot of the centre plane
         // split barrier: announce "my part of plane j+2 is in the rings", keep working on what needs nobody else's
         // data (epilogue operand loads, the phi direction), and only then wait for the other warps
-        mbar_arrive(&S.ready);
+        __syncwarp();
+        if (tx == 0) mbar_arrive(&S.ready);
 
         // ---- a6 inputs: U^n / stage state / acc of this node, requested now so that they arrive during phase B ---
         const long long g = (long long)j * L.plane + off2;
@@ -843,16 +865,15 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
         }
         rhs_point<V0, SPEC>(&S.sring[sc][0][0], HT, &S.ering[sc][0][0], &S.ering[sc][1][0], &S.ering[sc][2][0], dP_EZ, dP_ER, Fp[0],
                             rr, cs, q, ct, tab, off2, L.plane, ph, iR, iR2, K, [&] {
-                                mbar_wait(&S.ready, ready_parity);
-                                // every thread has consumed the raw buffer of plane number j-ja+4: refill it NRAW planes
+                                mbar_wait(&S.ready, (unsigned)(it & 1));
+                                // every thread has consumed the raw buffer of plane number it+4: refill it NRAW planes
                                 // ahead (overlaps the rest of phase B and NRAW-1 more iterations)
-                                const int n = j - ja + 4 + NRAW;
+                                const int n = it + 4 + NRAW;
                                 if (tid == 0 && n < total) issue(n);
                             }, pd1, pd2);
-        ready_parity ^= 1u;
 
         // ---- a6: RK4 stage combine in the epilogue (L125, L139) --------------------------------
-        if (valid) epilogue_store<MODE>(a, g, L.field, eo, K, iR, rate);
+        if (valid) epilogue_store<MODE>(a, g, L.field, eo, K, iR, rate, coef);
         advance();
     }
     if (MODE == RHS_MODE_S4) dtmin_commit(a, rate);
