@@ -1239,33 +1239,28 @@ int curl_tma_tile_z() { return CLT_CURL_TZ; }
 // consecutive outputs of one line at a time from two sliding register windows, so every step in m costs two
 // shared-memory loads for 16 (32 with second derivatives) FP64 operations: FP64-bound, any N <= 256.
 // ---------------------------------------------------------------------------------------------
-template <bool WANT2>
-__global__ void __launch_bounds__(512) phi_spectral_kernel(const __grid_constant__ SpecArgs a, int job_base)
+// Stages the N = nphi samples of the quantity pre-pass job `job` differentiates, for the (R, Z) line at table offset o2,
+// into sv[j * pitch + tx] (thread (tx, ty) of TY rows takes planes ty, ty + TY, ..: coalesced along R), and names the
+// output fields.  Perturbations are formed first (H2).
+__device__ __forceinline__ void spec_stage(const SpecArgs &a, int job, long long o2, double *sv, int pitch, int tx, int ty, int TY,
+                                           int &out1, int &out2)
 {
-    extern __shared__ __align__(128) unsigned char smem_raw[];
     const Layout &L = a.L;
     const int N = L.nphi;
-    double *sv = reinterpret_cast<double *>(smem_raw);        // [N][32] samples
-    double *sc1 = sv + (size_t)N * 32, *sc2 = sc1 + N;        // weights
-    const int tx = threadIdx.x, ty = threadIdx.y, TY = blockDim.y;
-    const int i = 2 + blockIdx.x * 32 + tx, k = 2 + blockIdx.y;
-    const bool valid = i <= L.nR - 3;
-    const long long o2 = (long long)k * L.pR + (LP + min(i, L.nR - 3));
-    const int job = job_base + blockIdx.z;
-    int out1, out2 = -1;       // output field of the first / second derivative
+    out2 = -1;
     if (a.mode == 0) {
         // before the curl: B1_R, B1_Z (and p1 for the Hall field)
         const int src = job == 0 ? 5 : (job == 1 ? 7 : 1);
         const int t0 = job == 0 ? T_B0R : (job == 1 ? T_B0Z : T_P0);
         out1 = job < 2 ? SP_DB + job : SP_D1 + 1;
         const double f0 = __ldg(a.tab + t0 * L.plane + o2);
-        for (int j = ty; j < N; j += TY) sv[j * 32 + tx] = __ldg(a.U + src * L.field + (long long)j * L.plane + o2) - f0;
+        for (int j = ty; j < N; j += TY) sv[j * pitch + tx] = __ldg(a.U + src * L.field + (long long)j * L.plane + o2) - f0;
     } else if (job < 5) {
         out1 = SP_D1 + job;
         out2 = SP_D2 + job;
         const int t0 = job == 0 ? T_RHO0 : (job == 1 ? T_P0 : T_V0R + (job - 2));
         const double f0 = (job < 2 || a.has_v0) ? __ldg(a.tab + t0 * L.plane + o2) : 0.0;
-        for (int j = ty; j < N; j += TY) sv[j * 32 + tx] = __ldg(a.U + job * L.field + (long long)j * L.plane + o2) - f0;
+        for (int j = ty; j < N; j += TY) sv[j * pitch + tx] = __ldg(a.U + job * L.field + (long long)j * L.plane + o2) - f0;
     } else {
         // E1_R (job 5) or E1_Z (job 6) = -(v x B)_c + eta J1_c (+ d_i G_c); the axisymmetric v0 x B0 drops out
         // of the paired differences exactly and is left out
@@ -1279,9 +1274,26 @@ __global__ void __launch_bounds__(512) phi_spectral_kernel(const __grid_constant
             const double vc = __ldg(a.U + ic2 * L.field + g), Bd = __ldg(a.U + id * L.field + g);
             double e = a.ph.eta * __ldg(a.J1 + c * L.field + g) - (va * Bb - vc * Bd);
             if (a.hall) e = fma(a.ph.d_i, __ldg(a.J1 + (3 + c) * L.field + g), e);
-            sv[j * 32 + tx] = e;
+            sv[j * pitch + tx] = e;
         }
     }
+}
+
+template <bool WANT2>
+__global__ void __launch_bounds__(512) phi_spectral_kernel(const __grid_constant__ SpecArgs a, int job_base)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const Layout &L = a.L;
+    const int N = L.nphi;
+    double *sv = reinterpret_cast<double *>(smem_raw);        // [N][32] samples
+    double *sc1 = sv + (size_t)N * 32, *sc2 = sc1 + N;        // weights
+    const int tx = threadIdx.x, ty = threadIdx.y, TY = blockDim.y;
+    const int i = 2 + blockIdx.x * 32 + tx, k = 2 + blockIdx.y;
+    const bool valid = i <= L.nR - 3;
+    const long long o2 = (long long)k * L.pR + (LP + min(i, L.nR - 3));
+    const int job = job_base + blockIdx.z;
+    int out1, out2;            // output field of the first / second derivative (-1: none)
+    spec_stage(a, job, o2, sv, 32, tx, ty, TY, out1, out2);
     for (int m = ty * 32 + tx; m < N; m += TY * 32) {
         sc1[m] = a.ctab[m];
         sc2[m] = a.ctab[SPEC_MAX_NPHI + m];
@@ -1336,6 +1348,144 @@ __global__ void __launch_bounds__(512) phi_spectral_kernel(const __grid_constant
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// N = nphi = 64: the same derivatives through a register-resident FFT (about 6 x fewer FP64 operations than the circulant
+// sums; the pre-pass becomes HBM-bound).  Two neighbouring real lines a, b are packed as z = a + i b: the derivative is
+// a real-linear operator, so multiplying the spectrum of z by i kappa q (resp. -(kappa q)^2) and transforming back gives
+// a' + i b' (a'' + i b'') directly -- no unpacking.  Eight threads share one packed line: thread t holds the samples
+// n = t + 8 n2, does a radix-8 DFT in registers, exchanges through shared memory (__syncwarp only: the eight threads sit
+// in one warp), does the second radix-8 pass and ends up with the modes k = t + 8 k1 -- the same stride-8 layout, so the
+// inverse transforms are the same routine with conjugated twiddles.  Reading R12: modes q = -31 .. 31 and the Nyquist
+// mode (first derivative 0, second derivative -(32 kappa)^2).
+// ---------------------------------------------------------------------------------------------
+struct cpx {
+    double x, y;
+};
+__device__ __forceinline__ cpx operator+(cpx a, cpx b) { return { a.x + b.x, a.y + b.y }; }
+__device__ __forceinline__ cpx operator-(cpx a, cpx b) { return { a.x - b.x, a.y - b.y }; }
+__device__ __forceinline__ cpx cmul(cpx a, cpx b) { return { a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x }; }
+// multiplication by exp(S i pi/2) = S i  (S = -1: forward transform, +1: inverse)
+template <int S>
+__device__ __forceinline__ cpx mul_si(cpx a)
+{
+    return S > 0 ? cpx{ -a.y, a.x } : cpx{ a.y, -a.x };
+}
+// 4-point DFT in place, natural order: X[k] = sum_n c_n exp(S 2 pi i n k / 4)
+template <int S>
+__device__ __forceinline__ void dft4(cpx &c0, cpx &c1, cpx &c2, cpx &c3)
+{
+    const cpx e0 = c0 + c2, e1 = c0 - c2, o0 = c1 + c3, o1 = mul_si<S>(c1 - c3);
+    c0 = e0 + o0; c2 = e0 - o0; c1 = e1 + o1; c3 = e1 - o1;
+}
+// 8-point DFT in place, natural order: X[k] = sum_n x_n exp(S 2 pi i n k / 8)
+template <int S>
+__device__ __forceinline__ void dft8(cpx (&x)[8])
+{
+    constexpr double h = 0.70710678118654752440;      // sqrt(1/2)
+    cpx a0 = x[0] + x[4], a1 = x[1] + x[5], a2 = x[2] + x[6], a3 = x[3] + x[7];
+    const cpx d0 = x[0] - x[4], d1 = x[1] - x[5], d2 = x[2] - x[6], d3 = x[3] - x[7];
+    // b_j = d_j W8^j, W8 = exp(S i pi/4) = h (1 + S i)
+    cpx b0 = d0;
+    cpx b1 = { h * (d1.x - S * d1.y), h * (d1.y + S * d1.x) };
+    cpx b2 = mul_si<S>(d2);
+    cpx b3 = { h * (-d3.x - S * d3.y), h * (-d3.y + S * d3.x) };
+    dft4<S>(a0, a1, a2, a3);
+    dft4<S>(b0, b1, b2, b3);
+    x[0] = a0; x[2] = a1; x[4] = a2; x[6] = a3;
+    x[1] = b0; x[3] = b1; x[5] = b2; x[7] = b3;
+}
+// 64-point transform of one packed line shared by 8 threads; in and out: thread t holds elements t + 8 m, m = 0..7.
+// tw[m] = exp(-2 pi i t m / 64) (forward twiddles of this thread); ex = this line's exchange buffer (8 x 9 cpx).
+template <int S>
+__device__ __forceinline__ void fft64(cpx (&x)[8], const cpx (&tw)[8], cpx *ex, int t)
+{
+    dft8<S>(x);
+#pragma unroll
+    for (int k2 = 0; k2 < 8; ++k2) {
+        const cpx w = S < 0 ? tw[k2] : cpx{ tw[k2].x, -tw[k2].y };
+        ex[k2 * 9 + t] = k2 == 0 ? x[0] : cmul(x[k2], w);
+    }
+    __syncwarp();
+#pragma unroll
+    for (int n1 = 0; n1 < 8; ++n1) x[n1] = ex[t * 9 + n1];
+    __syncwarp();
+    dft8<S>(x);
+}
+
+constexpr int FFT_N = 64, FFT_PITCH = 33, FFT_LINES = 32;     // lines per CTA; staging rows padded against bank conflicts
+// Grid: (R tile, Z row, job).  Measured alternatives, both slower: the job index fastest (so that the quantities of the
+// same lines run together and share their reads in L2: 9.15 ms per step against 8.87) and one CTA working through all
+// quantities of its lines (9.69 ms).
+template <bool WANT2>
+__global__ void __launch_bounds__(128) phi_fft64_kernel(const __grid_constant__ SpecArgs a, int job_base)
+{
+    __shared__ double sv[FFT_N * FFT_PITCH];                  // samples, then the first derivative
+    // exchange buffers, one per packed line (8 x 9 cpx); once the transforms are done the same storage takes the
+    // second derivative (FFT_N * FFT_PITCH doubles)
+    __shared__ __align__(16) double sbuf[(FFT_LINES / 2) * 72 * 2];
+    static_assert((FFT_LINES / 2) * 72 * 2 >= FFT_N * FFT_PITCH, "second-derivative staging fits the exchange storage");
+    cpx *sex = reinterpret_cast<cpx *>(sbuf);
+    double *s2 = sbuf;
+    const Layout &L = a.L;
+    const int tid = threadIdx.x, tx = tid & 31, ty = tid >> 5;
+    const int i = 2 + blockIdx.x * 32 + tx, k = 2 + blockIdx.y;
+    const bool valid = i <= L.nR - 3;
+    const long long o2 = (long long)k * L.pR + (LP + min(i, L.nR - 3));
+    const int job = job_base + blockIdx.z;
+    const int pair = tid >> 3, t = tid & 7;                   // packed line (R nodes 2 pair, 2 pair + 1) and slot in it
+    cpx tw[8];
+#pragma unroll
+    for (int m = 0; m < 8; ++m) {
+        double sn, cs;
+        sincospi(-(double)(t * m) / 32.0, &sn, &cs);
+        tw[m] = { cs, sn };
+    }
+    const double kap = 6.283185307179586476925286766559 / a.ph.Lphi;
+    int out1, out2;
+    spec_stage(a, job, o2, sv, FFT_PITCH, tx, ty, 4, out1, out2);
+    const bool want2 = WANT2 && out2 >= 0;
+    __syncthreads();
+
+    cpx z[8];
+#pragma unroll
+    for (int m = 0; m < 8; ++m) {
+        z[m].x = sv[(t + 8 * m) * FFT_PITCH + 2 * pair];
+        z[m].y = sv[(t + 8 * m) * FFT_PITCH + 2 * pair + 1];
+    }
+    cpx *ex = sex + pair * 72;
+    fft64<-1>(z, tw, ex, t);
+    // mode k = t + 8 m: signed wavenumber q (Nyquist: first derivative 0); 1/N of the inverse transform folded in
+    cpx d1[8], d2[8];
+#pragma unroll
+    for (int m = 0; m < 8; ++m) {
+        const int kk = t + 8 * m;
+        const double q = kap * (double)(kk < 32 ? kk : kk - 64);
+        const double w1 = kk == 32 ? 0.0 : q * (1.0 / 64.0), w2 = -(q * q) * (1.0 / 64.0);
+        d1[m] = { -w1 * z[m].y, w1 * z[m].x };
+        if (WANT2) d2[m] = { w2 * z[m].x, w2 * z[m].y };
+    }
+    fft64<1>(d1, tw, ex, t);
+    if (WANT2) fft64<1>(d2, tw, ex, t);
+    __syncthreads();                                          // every thread has taken its samples out of sv
+#pragma unroll
+    for (int m = 0; m < 8; ++m) {
+        sv[(t + 8 * m) * FFT_PITCH + 2 * pair] = d1[m].x;
+        sv[(t + 8 * m) * FFT_PITCH + 2 * pair + 1] = d1[m].y;
+        if (WANT2) {
+            s2[(t + 8 * m) * FFT_PITCH + 2 * pair] = d2[m].x;
+            s2[(t + 8 * m) * FFT_PITCH + 2 * pair + 1] = d2[m].y;
+        }
+    }
+    __syncthreads();
+    if (valid) {
+        for (int j = ty; j < FFT_N; j += 4) {
+            const long long g = (long long)j * L.plane + o2;
+            a.out[(long long)out1 * L.field + g] = sv[j * FFT_PITCH + tx];
+            if (want2) a.out[(long long)out2 * L.field + g] = s2[j * FFT_PITCH + tx];
+        }
+    }
+}
+
 template <bool WANT2>
 static cudaError_t launch_phi_jobs(const SpecArgs &a, int job_base, int jobs, cudaStream_t s, bool configure)
 {
@@ -1344,6 +1494,11 @@ static cudaError_t launch_phi_jobs(const SpecArgs &a, int job_base, int jobs, cu
         return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     (int)((SPEC_MAX_NPHI * 32 + 2 * SPEC_MAX_NPHI) * sizeof(double)));
     const int N = a.L.nphi;
+    if (N == FFT_N) {
+        dim3 grid((a.L.nR - 4 + 31) / 32, a.L.nZ - 4, jobs);
+        phi_fft64_kernel<WANT2><<<grid, 128, 0, s>>>(a, job_base);
+        return cudaGetLastError();
+    }
     const int groups = (N + CLT_SPEC_NQ - 1) / CLT_SPEC_NQ;
     dim3 block(32, groups < 16 ? groups : 16, 1);
     dim3 grid((a.L.nR - 4 + 31) / 32, a.L.nZ - 4, jobs);
