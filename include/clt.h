@@ -156,6 +156,20 @@ int clt_get_rows(clt_ctx *ctx, int buffer, int k0, int nrows, double *dst);
 int clt_set_rows(clt_ctx *ctx, int buffer, int k0, int nrows, const double *src);
 int clt_set_owned_rows(clt_ctx *ctx, int k_first, int k_last, int deep_first, int deep_last);
 
+/* A slab of a larger grid carries the GLOBAL spacing: dZ replaces (Zmax - Zmin)/(nZ - 1) of this context's own grid in
+ * every stencil weight, table and diagnostic weight, so that a decomposed run reproduces the undivided run bit for bit
+ * (the method has no other use for Z than its spacing).  Call it right after clt_create: it invalidates the
+ * equilibrium tables and the state (set them again).  dZ must be finite and > 0.  Asynchronous.            */
+int clt_set_z_spacing(clt_ctx *ctx, double dZ);
+
+/* Ghost-row hand-over between two contexts of one process [L127 "message passing between every two neighboring
+ * blocks"]: rows k0_src .. k0_src+nrows-1 of `buffer` (0 = U^n, 1 = U_a, 2 = U_b; all 8 fields, all planes) of `src`
+ * are written straight into rows k0_dst .. of the same buffer of `dst` by ONE kernel -- no dense staging array, no host
+ * wait.  Both contexts must have the same nR and nphi.  Stream order: the copy runs on dst's stream after everything
+ * enqueued on src's stream so far, and src's stream waits for it (events; nothing to do when both contexts share one
+ * stream).  Contexts on different devices need peer access (CLT_ECUDA otherwise).                         */
+int clt_push_rows(clt_ctx *src, int buffer, int k0_src, int nrows, clt_ctx *dst, int k0_dst);
+
 /* NEXT-1 in the loop [L139 "the time step ... is calculated based on the latest rho, p, v, B"; Fig. 3: STEPON then
  * SETDT; Fig. 4]: n RK4 steps, each with dt = SETDT(cfl) of the state at its start.  The time step lives on the
  * device: the first one comes from the reduction kernel of clt_suggest_dt, the following ones are collected by the

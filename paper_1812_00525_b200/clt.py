@@ -44,7 +44,7 @@ class clt_profile(ctypes.Structure):
 # every symbol include/clt.h declares
 EXPORTS = ["clt_workspace_bytes", "clt_create", "clt_destroy", "clt_set_equilibrium", "clt_set_state", "clt_get_state",
            "clt_rhs", "clt_curl_J1", "clt_hall_G", "clt_step", "clt_step_cfl", "clt_step_stage", "clt_get_rows", "clt_set_rows",
-           "clt_set_owned_rows", "clt_set_dt", "clt_diagnostics", "clt_suggest_dt", "clt_set_tuning",
+           "clt_set_owned_rows", "clt_set_z_spacing", "clt_push_rows", "clt_set_dt", "clt_diagnostics", "clt_suggest_dt", "clt_set_tuning",
            "clt_set_kernel_variant", "clt_spectral_workspace_bytes", "clt_set_phi_scheme", "clt_set_profiling", "clt_get_profile", "clt_launch_count", "clt_stream", "clt_strerror", "clt_last_cuda_error", "clt_version"]
 
 LIB_TEXTBOOK_PATH = os.path.join(_HERE, "libclt_textbook.so")
@@ -106,6 +106,10 @@ def load(path=None):
         getattr(L, name).argtypes = [vp, i, i, i, vp]
     L.clt_set_owned_rows.restype = i
     L.clt_set_owned_rows.argtypes = [vp, i, i, i, i]
+    L.clt_set_z_spacing.restype = i
+    L.clt_set_z_spacing.argtypes = [vp, d]
+    L.clt_push_rows.restype = i
+    L.clt_push_rows.argtypes = [vp, i, i, i, vp, i]
     L.clt_spectral_workspace_bytes.restype = ctypes.c_size_t
     L.clt_spectral_workspace_bytes.argtypes = [ctypes.POINTER(clt_grid)]
     L.clt_set_phi_scheme.restype = i
@@ -237,6 +241,16 @@ class Clt:
 
     def set_owned_rows(self, k_first, k_last, deep_first, deep_last):
         self._ck(self.L.clt_set_owned_rows(self.h, int(k_first), int(k_last), int(deep_first), int(deep_last)))
+
+    def set_z_spacing(self, dZ):
+        """A slab of a larger grid: the global dZ, bit for bit (call before set_equilibrium / set_state)."""
+        self._ck(self.L.clt_set_z_spacing(self.h, float(dZ)))
+
+    def push_rows(self, buffer, k0, nrows, dst, k0_dst):
+        """Rows k0 .. k0+nrows-1 of `buffer` of this context -> rows k0_dst .. of the same buffer of context `dst`."""
+        rc = self.L.clt_push_rows(self.h, int(buffer), int(k0), int(nrows), dst.h, int(k0_dst))
+        if rc != 0:
+            dst._ck(rc)
 
     def hall_G(self, out=None):
         if out is None:

@@ -861,6 +861,71 @@ int clt_set_rows(clt_ctx *ctx, int buffer, int k0, int nrows, const double *src)
     return copy_rows(ctx, stage_buffer(ctx, buffer), k0, nrows, const_cast<double *>(src), false);
 }
 
+int clt_set_z_spacing(clt_ctx *ctx, double dZ)
+{
+    DeviceGuard device_guard(ctx);
+    if (!ctx || !(dZ > 0.0) || !isfinite(dZ)) return CLT_EINVAL;
+    Phys &ph = ctx->ph;
+    ph.dZ = dZ;
+    ph.cZ1 = 1.0 / (12.0 * dZ);
+    ph.cZ2 = 1.0 / (12.0 * dZ * dZ);
+    // everything derived from the old spacing goes: tables of the reference state, the state, a captured step
+    ctx->has_state = false;
+    ctx->has_v0 = false;
+    ctx->v0_pending = false;
+    destroy_graph(ctx);
+    CK(cudaMemsetAsync(ctx->tab, 0, (size_t)T_COUNT * ctx->L.plane * sizeof(double), ctx->stream));
+    CK(launch_tables(ctx->L, ctx->ph, ctx->tab, ctx->Rtab + LP, ctx->invRtab + LP, ctx->stream));
+    ctx->launches++;
+    return CLT_OK;
+}
+
+int clt_push_rows(clt_ctx *src, int buffer, int k0_src, int nrows, clt_ctx *dst, int k0_dst)
+{
+    if (!src || !dst || src == dst || nrows < 1 || !stage_buffer(src, buffer)) return CLT_EINVAL;
+    if (k0_src < 0 || k0_src + nrows > src->L.nZ || k0_dst < 0 || k0_dst + nrows > dst->L.nZ) return CLT_EINVAL;
+    if (src->L.nR != dst->L.nR || src->L.nphi != dst->L.nphi) return CLT_EINVAL;
+    if (!src->has_state || !dst->has_state) return CLT_ESTATE;
+    clt_ctx *ctx = dst;                                          // CK reports into the destination context
+    DeviceGuard device_guard(dst);
+    if (src->device != dst->device) {
+        int can = 0;
+        CK(cudaDeviceCanAccessPeer(&can, dst->device, src->device));
+        if (!can) { snprintf(dst->cuda_err, sizeof(dst->cuda_err), "clt_push_rows: no peer access between devices %d and %d", dst->device, src->device); return CLT_ECUDA; }
+        cudaError_t pe = cudaDeviceEnablePeerAccess(src->device, 0);
+        if (pe != cudaSuccess && pe != cudaErrorPeerAccessAlreadyEnabled) return cuda_fail(dst, pe, "cudaDeviceEnablePeerAccess");
+        cudaGetLastError();
+    }
+    const bool two_streams = src->stream != dst->stream || src->device != dst->device;
+    cudaEvent_t ready = nullptr, done = nullptr;
+    if (two_streams) {
+        // order: src's stage kernel -> copy on dst's stream -> whatever src enqueues next (it will overwrite these rows)
+        CK(cudaEventCreateWithFlags(&done, cudaEventDisableTiming));
+        {
+            DeviceGuard src_guard(src);
+            cudaError_t e = cudaEventCreateWithFlags(&ready, cudaEventDisableTiming);
+            if (e == cudaSuccess) e = cudaEventRecord(ready, src->stream);
+            if (e != cudaSuccess) { cudaEventDestroy(done); if (ready) cudaEventDestroy(ready); return cuda_fail(dst, e, "clt_push_rows: event on the source stream"); }
+        }
+        CK(cudaStreamWaitEvent(dst->stream, ready, 0));
+    }
+    cudaError_t e = launch_push_rows(src->L, stage_buffer(src, buffer), k0_src, dst->L, stage_buffer(dst, buffer), k0_dst, nrows,
+                                     dst->sm_count, dst->stream);
+    dst->launches++;
+    dst->prof_chain = false;
+    if (two_streams) {
+        if (e == cudaSuccess) e = cudaEventRecord(done, dst->stream);
+        if (e == cudaSuccess) {
+            DeviceGuard src_guard(src);
+            e = cudaStreamWaitEvent(src->stream, done, 0);
+        }
+        cudaEventDestroy(ready);      // destruction is deferred until the events have completed
+        cudaEventDestroy(done);
+    }
+    if (e != cudaSuccess) return cuda_fail(dst, e, "clt_push_rows");
+    return CLT_OK;
+}
+
 int clt_set_owned_rows(clt_ctx *ctx, int k_first, int k_last, int deep_first, int deep_last)
 {
     if (!ctx) return CLT_EINVAL;

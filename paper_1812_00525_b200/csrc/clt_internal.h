@@ -129,6 +129,9 @@ cudaError_t launch_tables(const Layout &L, const Phys &ph, double *tab, const do
 cudaError_t launch_any_nonzero(const double *x, long long n, int *flag, cudaStream_t s);
 cudaError_t launch_copy_boundary(const Layout &L, int nfields, const double *src, double *d0, double *d1, double *d2,
                                  int sm_count, cudaStream_t s);
+// rows k0s .. k0s+nrows-1 of nfp = fields * planes slices of `src` (layout Ls) -> rows k0d .. of `dst` (layout Ld)
+cudaError_t launch_push_rows(const Layout &Ls, const double *src, int k0s, const Layout &Ld, double *dst, int k0d, int nrows,
+                             int sm_count, cudaStream_t s);
 cudaError_t launch_zero_boundary(const Layout &L, int nfields, double *dst, int sm_count, cudaStream_t s);
 // plain-load variants (kernel variant 1: A/B and parity cross-check of the TMA-fed default)
 cudaError_t launch_curl(const CurlArgs &a, cudaStream_t s);

@@ -1636,6 +1636,31 @@ cudaError_t launch_copy_boundary(const Layout &L, int nfields, const double *src
     return cudaGetLastError();
 }
 
+// NEXT-4: ghost rows of a neighbouring slab, straight from its buffer into this one (8 fields x nphi planes x nrows rows
+// of nR nodes; the two layouts differ only in nZ)
+__global__ void push_rows_kernel(Layout Ls, const double *src, int k0s, Layout Ld, double *dst, int k0d, int nrows, long long total)
+{
+    const int nR = Ls.nR;
+    for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < total; n += (long long)gridDim.x * blockDim.x) {
+        const int i = (int)(n % nR);
+        const long long r = n / nR;
+        const int row = (int)(r % nrows);
+        const long long slice = r / nrows;                   // field * nphi + plane
+        dst[slice * Ld.plane + (long long)(k0d + row) * Ld.pR + (LP + i)] =
+            src[slice * Ls.plane + (long long)(k0s + row) * Ls.pR + (LP + i)];
+    }
+}
+
+cudaError_t launch_push_rows(const Layout &Ls, const double *src, int k0s, const Layout &Ld, double *dst, int k0d, int nrows,
+                             int sm_count, cudaStream_t s)
+{
+    const long long total = 8LL * Ls.nphi * nrows * Ls.nR;
+    const int block = 256;
+    const long long want = (total + block - 1) / block, cap = (long long)(sm_count > 0 ? sm_count : 148) * 8;
+    push_rows_kernel<<<(int)(want < cap ? want : cap), block, 0, s>>>(Ls, src, k0s, Ld, dst, k0d, nrows, total);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_zero_boundary(const Layout &L, int nfields, double *dst, int sm_count, cudaStream_t s)
 {
     return launch_copy_boundary(L, nfields, nullptr, dst, nullptr, nullptr, sm_count, s);

@@ -83,6 +83,11 @@ def exchange(backends, extents, buffer, dist=None, make_buffer=None):
     [8][nphi][n][nR] float64 tensor on the transfer device."""
     if dist is None:
         for lo, hi, elo, ehi in zip(backends[:-1], backends[1:], extents[:-1], extents[1:]):
+            if hasattr(lo, "push_rows"):
+                # one kernel per direction, straight from the owner's buffer into the neighbour's ghost rows, stream-ordered
+                lo.push_rows(buffer, *elo.send_up(), hi, ehi.recv_from_lower()[0])
+                hi.push_rows(buffer, *ehi.send_down(), lo, elo.recv_from_upper()[0])
+                continue
             up = make_buffer(lo, GHOST)
             lo.get_rows(buffer, *elo.send_up(), up)
             down = make_buffer(hi, GHOST)
@@ -121,6 +126,7 @@ class Slab:
         Zmax = cfg.Zmin + (ex.z1 - 1) * dZ
         self.g = clt.Clt(cfg.nR, cfg.nphi, ex.nZ_local, cfg.Rmin, cfg.Rmax, Zmin, Zmax, cfg.phi_extent, cfg.gamma, cfg.eta,
                          cfg.nu, cfg.D, cfg.kappa, dt, cfg.cfl, d_i=d_i, device=device)
+        self.g.set_z_spacing(dZ)      # the global spacing itself, not (Zmax - Zmin)/(nZ_local - 1): slabs == undivided run, bit for bit
         if phi_scheme:
             self.g.set_phi_scheme(phi_scheme)
         self.device = torch.device(device)
@@ -135,6 +141,9 @@ class Slab:
 
     def set_rows(self, buffer, k0, n, src):
         self.g.set_rows(buffer, k0, n, src)
+
+    def push_rows(self, buffer, k0, n, dst, k0_dst):
+        self.g.push_rows(buffer, k0, n, dst.g, k0_dst)
 
     def new_rows(self, n=GHOST):
         import torch

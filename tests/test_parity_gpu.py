@@ -389,9 +389,9 @@ def _single(prob, **over):
 @pytest.mark.parametrize("world", [2, 3])
 @pytest.mark.parametrize("variant", ["fd", "hall", "spectral"])
 def test_slab_decomposition_matches_single_domain_and_oracle(world, variant):
-    """Several sub-domain contexts in ONE process on one GPU (run one after the other, ghost rows handed over as
-    device tensors): same state as the undivided run (to round-off: a slab's dZ is recomputed from its own Zmin/Zmax)
-    and as the oracle."""
+    """Several sub-domain contexts in ONE process on one GPU (run one after the other, ghost rows pushed from buffer to
+    buffer by clt_push_rows): the SAME BITS as the undivided run (a slab carries the global dZ, clt_set_z_spacing) and
+    the oracle's state within the step tolerance."""
     from paper_1812_00525_b200 import slab
     prob = inputs.make_custom_problem(45, 8, 41, index=21, rotation=0.05 if variant == "fd" else 0.0,
                                       poloidal=(0.03, -0.02) if variant != "spectral" else None)
@@ -411,7 +411,7 @@ def test_slab_decomposition_matches_single_domain_and_oracle(world, variant):
     g.step(steps)
     o.step(steps)
     U_s, U_g, U_o = grp.get_state(), g.get_state(), o.get_state()
-    assert_close(U_s, U_g, 1e-12, f"{world} slabs vs single domain ({variant})")
+    assert np.array_equal(U_s, U_g), f"{world} slabs vs single domain ({variant}): {rel_linf(U_s, U_g)}"
     assert_close(U_s, U_o, STEP_TOL, f"{world} slabs vs oracle ({variant})")
     d1 = grp.diagnostics()
     dg = g.diagnostics()
@@ -419,6 +419,50 @@ def test_slab_decomposition_matches_single_domain_and_oracle(world, variant):
     for k in ("kinetic", "magnetic", "magnetic_pert", "magnetic_n1"):
         assert abs(d1[k] - dg[k]) <= 1e-11 * abs(dg[k]), k
     grp.close()
+
+
+def test_push_rows_and_z_spacing():
+    """clt_push_rows = clt_get_rows + clt_set_rows without the dense staging array; clt_set_z_spacing replaces the
+    spacing in every weight (a context built with a wrong Z extent and the right dZ reproduces the reference bits)."""
+    import torch
+    from paper_1812_00525_b200 import clt
+    prob = inputs.make_custom_problem(40, 6, 30, index=23, amplitude_scale=30.0)
+    c = prob.cfg
+    a, b = make_gpu(prob), make_gpu(prob)
+    a.step(1)
+    rows = torch.empty((8, c.nphi, 5, c.nR), dtype=torch.float64, device="cuda")
+    a.get_rows(0, 7, 5, rows)
+    a.push_rows(0, 7, 5, b, 11)
+    got = torch.empty_like(rows)
+    b.get_rows(0, 11, 5, got)
+    torch.cuda.synchronize()
+    assert torch.equal(got, rows)
+    before = torch.empty((8, c.nphi, 11, c.nR), dtype=torch.float64, device="cuda")
+    b.get_rows(0, 0, 11, before)
+    torch.cuda.synchronize()
+    assert np.array_equal(before.cpu().numpy(), prob.U[:, :, :11])          # nothing else was touched
+    with pytest.raises(clt.CltError):
+        a.push_rows(0, 27, 5, b, 0)                                          # rows past the end
+    with pytest.raises(clt.CltError):
+        a.push_rows(3, 0, 4, b, 0)                                           # no such buffer
+    # the same problem through a context whose box is 3 x too tall, corrected by the true spacing
+    dZ = (c.Zmax - c.Zmin) / (c.nZ - 1)
+    g = clt.Clt(c.nR, c.nphi, c.nZ, c.Rmin, c.Rmax, c.Zmin, c.Zmin + 3.0 * (c.Zmax - c.Zmin), c.phi_extent, c.gamma, c.eta,
+                c.nu, c.D, c.kappa, prob.dt, c.cfl)
+    g.set_z_spacing(dZ)
+    with pytest.raises(clt.CltError):
+        g.step(1)                                                            # the call invalidates the state
+    g.set_equilibrium(np.ascontiguousarray(prob.U0))
+    g.set_state(np.ascontiguousarray(prob.U))
+    ref = make_gpu(prob)
+    assert np.array_equal(g.rhs(), ref.rhs())
+    g.step(3)
+    ref.step(3)
+    assert np.array_equal(g.get_state(), ref.get_state())
+    dg, dr = g.diagnostics(), ref.diagnostics()
+    assert dg["kinetic"] == dr["kinetic"] and dg["max_divB"] == dr["max_divB"]
+    with pytest.raises(clt.CltError):
+        g.set_z_spacing(0.0)
 
 
 def test_step_stage_order_and_rows_roundtrip():
