@@ -355,15 +355,18 @@ int run_rhs(clt_ctx *ctx, int mode, const double *in, double *out)
         int r = run_phi_pass(ctx, 1, in);
         if (r) return r;
     }
-    alignas(64) CUtensorMap tmU, tmJ;
+    alignas(64) CUtensorMap tmU, tmJ, tmV;
     const int nJ = ctx->hall ? 6 : 3;
-    if (tma && (!make_map(ctx, in, 8, rhs_tile_z(), &tmU, 8) || !make_map(ctx, ctx->J1, nJ, rhs_tile_z(), &tmJ, nJ))) {
+    // static reference state: rho, p and B land in the raw buffer, v in a ring of its own (three boxes over the stage state)
+    const int nU = ctx->has_v0 ? 8 : 2;
+    if (tma && (!make_map(ctx, in, 8, rhs_tile_z(), &tmU, nU) || !make_map(ctx, in, 8, rhs_tile_z(), &tmV, 3)
+                || !make_map(ctx, ctx->J1, nJ, rhs_tile_z(), &tmJ, nJ))) {
         snprintf(ctx->cuda_err, sizeof(ctx->cuda_err), "cuTensorMapEncodeTiled failed");
         return CLT_ECUDA;
     }
     const long pe = prof_begin(ctx, mode);
     if (tma)
-        CK(launch_rhs_tma(a, &tmU, &tmJ, mode, ctx->has_v0, ctx->hall, ctx->spectral, ctx->stream));
+        CK(launch_rhs_tma(a, &tmU, &tmJ, &tmV, mode, ctx->has_v0, ctx->hall, ctx->spectral, ctx->stream));
     else
         CK(launch_rhs(a, mode, ctx->has_v0, ctx->stream));
     prof_end(ctx, pe);

@@ -50,7 +50,9 @@ __device__ __forceinline__ int wrap_phi(int j, int n)
 
 // ---------------------------------------------------------------------------------------------
 // a3-a5 at one node: K of eqs (11)-(14) from
-//   stg  [5][HT]    centre-plane tile (with halo) of rho1, p1, v1_R, v1_phi, v1_Z; field f at stg + f*HT
+//   stg  [2][HT]    centre-plane tile (with halo) of rho1, p1; field f at stg + f*HT
+//   stgV [3][HT]    centre-plane tile (with halo) of v1_R, v1_phi, v1_Z (the TMA-fed kernel with a static reference state
+//                   reads the velocity tiles as they arrived: v1 = v)
 //   eRc, ePc, eZc   E1_R / E1_phi / E1_Z tiles (with halo) of the centre plane
 //   dP_EZ, dP_ER    unscaled phi differences (fd1) of E1_Z, E1_R at the own node
 //   F    [3]        J1 x B + J0 x B1 at the own node of the centre plane
@@ -80,7 +82,7 @@ __device__ __forceinline__ CentreTab load_centre_tab(const double *tab, long lon
 // SPEC = true: the phi derivatives come from the pseudo-spectral pre-pass: pd1[f], pd2[f] are d/dphi and d2/dphi2 of
 // the five fluid perturbations, dP_EZ / dP_ER the true d/dphi of E1_Z / E1_R (not the unscaled stencil sums).
 template <bool V0, bool SPEC, class Sync>
-__device__ __forceinline__ void rhs_point(const double *stg, int HT, const double *eRc, const double *ePc, const double *eZc,
+__device__ __forceinline__ void rhs_point(const double *stg, const double *stgV, int HT, const double *eRc, const double *ePc, const double *eZc,
                                           double dP_EZ, double dP_ER, const double (&F)[3], const double (&rr)[4], int cs,
                                           const double (&q)[5][5], const CentreTab &ct, const double *tab, long long off2,
                                           long long plane, const Phys &ph, double iR, double iR2, double (&K)[8], Sync &&sync,
@@ -122,7 +124,7 @@ __device__ __forceinline__ void rhs_point(const double *stg, int HT, const doubl
         const double vc = vR * ph.cR1, lc = iR * ph.cR1;
 #pragma unroll
         for (int f = 0; f < 5; ++f) {
-            const double *s = stg + f * HT + cs;
+            const double *s = (f < 2 ? stg + f * HT : stgV + (f - 2) * HT) + cs;
             const double m2 = s[-2], m1 = s[-1], p1_ = s[1], p2 = s[2];
             const double d1 = fd1(m2, m1, p1_, p2), d2 = fd2(m2, m1, q[2][f], p1_, p2);
             A[f] += vc * d1;
@@ -136,7 +138,7 @@ __device__ __forceinline__ void rhs_point(const double *stg, int HT, const doubl
         const double vc = vZ * ph.cZ1;
 #pragma unroll
         for (int f = 0; f < 5; ++f) {
-            const double *s = stg + f * HT + cs;
+            const double *s = (f < 2 ? stg + f * HT : stgV + (f - 2) * HT) + cs;
             const double m2 = s[-2 * SW], m1 = s[-SW], p1_ = s[SW], p2 = s[2 * SW];
             const double d1 = fd1(m2, m1, p1_, p2), d2 = fd2(m2, m1, q[2][f], p1_, p2);
             A[f] += vc * d1;
@@ -523,7 +525,7 @@ __global__ void __launch_bounds__(TR *TZ, 1) rhs_kernel(const __grid_constant__ 
             const double dP_ER = fd1(S.ering[s0][0][cs], S.ering[s1][0][cs], S.ering[s3][0][cs], S.ering[se][0][cs]);
             const double F[3] = { S.fring[sfc][0][ci], S.fring[sfc][1][ci], S.fring[sfc][2][ci] };
             const double rr[4] = { S.sR[tx], S.sR[tx + 1], S.sR[tx + 3], S.sR[tx + 4] };
-            rhs_point<V0, false>(&S.stage[buf][0][0], RhsSmem<TZ>::HT, &S.ering[sec][0][0], &S.ering[sec][1][0], &S.ering[sec][2][0],
+            rhs_point<V0, false>(&S.stage[buf][0][0], &S.stage[buf][2][0], RhsSmem<TZ>::HT, &S.ering[sec][0][0], &S.ering[sec][1][0], &S.ering[sec][2][0],
                           dP_EZ, dP_ER, F, rr, cs, q, ct, tab, off2, L.plane, ph, iR, iR2, K, [] {});
         }
 
@@ -634,16 +636,24 @@ __device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, i
         : "memory");
 }
 
-template <int TZ, int NRAW, int NF>
+// VR = true (static reference state, v1 = v): the velocity tiles are not converted at all -- they land in a 5-slot ring of
+// their own and the stencils read them where TMA put them (planes j .. j+4 are alive: the centre plane, the two that
+// wait for their turn, the one being converted and the one in flight); raw and sring hold the other fields only.
+template <int TZ, int NRAW, int NF, bool VR>
 struct RhsTmaSmem {
     static constexpr int HT = (TZ + 4) * SW;
     static constexpr int NH = 4 * TR + 4 * TZ;
     static constexpr int HTP = (HT + 15) / 16 * 16;   // every TMA destination 128-byte aligned
-    alignas(128) double raw[NRAW][NF][HTP];  // TMA destinations: U (8), J1 (3) [and G (3), Hall] of one plane, tile with halo
+    static constexpr int NFR = VR ? NF - 3 : NF;      // fields per raw buffer
+    static constexpr int NV = VR ? 5 : 1;             // slots of the velocity ring
+    static constexpr int NS = VR ? 2 : 5;             // fields of sring
+    // TMA destinations of one plane, tile with halo.  VR: rho, p, B (3), J1 (3) [, G (3)]; else U (8), J1 (3) [, G (3)]
+    alignas(128) double raw[NRAW][NFR][HTP];
+    alignas(128) double vring[NV][3][HTP];            // VR: v_R, v_phi, v_Z of planes n % 5 (TMA destinations)
     // 4-slot rings, tile with halo, written once when a plane arrives (as plane j+2) and read by the in-plane
     // stencils when it is the centre plane (two iterations later).  Four slots, not three: the slot that receives
     // plane j+2 held plane j-2, whose last readers are separated from this write by the barrier of iteration j-1.
-    double sring[4][5][HT];            // rho1, p1, v1
+    double sring[4][NS][HT];           // rho1, p1 (, v1)
     double ering[4][3][HT];            // E1
     alignas(8) unsigned long long bar[NRAW];   // TMA completion, one per raw buffer
     alignas(8) unsigned long long ready;       // split CTA barrier: "this plane is staged" (one arrival per warp)
@@ -651,13 +661,18 @@ struct RhsTmaSmem {
 
 template <int TZ, int NRAW, int MODE, bool V0, bool HALL, bool SPEC>
 __global__ void __launch_bounds__(TR *TZ, 1)
-rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmJ)
+rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmJ,
+               const __grid_constant__ CUtensorMap tmV)
 {
+    // tmU: box over the field axis of the stage state -- all 8 fields (moving reference state) or 2 (rho, p; VR);
+    // tmV: box of 3 fields (VR: v at field 2, B at field 5); tmJ: J1 [and G]
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int NF = HALL ? 14 : 11;
-    using SM = RhsTmaSmem<TZ, NRAW, NF>;
+    constexpr bool VR = !V0;
+    using SM = RhsTmaSmem<TZ, NRAW, NF, VR>;
     SM &S = *reinterpret_cast<SM *>(smem_raw);
     constexpr int HT = SM::HT, NH = SM::NH;
+    constexpr int IB = VR ? 2 : 5, IJ = VR ? 5 : 8;      // where B and J1 sit in a raw buffer
     static_assert(NH <= TR * TZ, "tile too small for one halo node per thread");
     const Layout &L = a.L;
     const Phys &ph = a.ph;
@@ -695,6 +710,7 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmU) : "memory");
         asm volatile("prefetch.tensormap [%0];" ::"l"(&tmJ) : "memory");
+        if (VR) asm volatile("prefetch.tensormap [%0];" ::"l"(&tmV) : "memory");
     }
     __syncthreads();
 
@@ -708,11 +724,15 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
         const int jw = wrap_phi(ja - 2 + n, L.nphi);
         const int b = n % NRAW;
         mbar_expect_tx(&S.bar[b], (unsigned)(NF * HT * sizeof(double)));
-        // two bulk copies per plane: the boxes span the field axis (8 fields of U; J1 [and G]), so the one thread that
+        // two (VR: four) bulk copies per plane: the boxes span the field axis (fields of U; J1 [and G]), so the one thread that
         // issues them -- and the warp that waits for it at the next barrier -- loses a dozen instructions, not a hundred
         static_assert(SM::HTP == HT, "a box that spans the field axis fills the raw buffer densely");
         tma_load_4d(&S.raw[b][0][0], &tmU, LP + i0 - 2, k0 - 2, jw, 0, &S.bar[b]);
-        tma_load_4d(&S.raw[b][8][0], &tmJ, LP + i0 - 2, k0 - 2, jw, 0, &S.bar[b]);
+        if (VR) {
+            tma_load_4d(&S.vring[n % SM::NV][0][0], &tmV, LP + i0 - 2, k0 - 2, jw, 2, &S.bar[b]);
+            tma_load_4d(&S.raw[b][IB][0], &tmV, LP + i0 - 2, k0 - 2, jw, 5, &S.bar[b]);
+        }
+        tma_load_4d(&S.raw[b][IJ][0], &tmJ, LP + i0 - 2, k0 - 2, jw, 0, &S.bar[b]);
     };
 
     // NRAW planes are kept in flight; the first ones are requested before anything else so that the table reads below
@@ -732,12 +752,12 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
                            __ldg(a.R + min(i + 2, L.nR - 1)) };
 
     // forms perturbations, E1 and (optionally) F from the raw tile at slot s; o2 = table offset of the node
-    auto node = [&](const double (*raw)[SM::HTP], int s, long long o2, double rho0, double p0, double q[5], double E[3],
-                    double F[3], bool wantF) {
+    auto node = [&](const double (*raw)[SM::HTP], const double (*vel)[SM::HTP], int s, long long o2, double rho0, double p0,
+                    double q[5], double E[3], double F[3], bool wantF) {
         const double rho = raw[0][s], p = raw[1][s];
-        const double vR = raw[2][s], vP = raw[3][s], vZ = raw[4][s];
-        const double BR = raw[5][s], BP = raw[6][s], BZ = raw[7][s];
-        const double JR = raw[8][s], JP = raw[9][s], JZ = raw[10][s];
+        const double vR = vel[0][s], vP = vel[1][s], vZ = vel[2][s];
+        const double BR = raw[IB][s], BP = raw[IB + 1][s], BZ = raw[IB + 2][s];
+        const double JR = raw[IJ][s], JP = raw[IJ + 1][s], JZ = raw[IJ + 2][s];
         q[0] = rho - rho0;
         q[1] = p - p0;
         if (V0) {
@@ -757,9 +777,9 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
             E[2] += __ldg(tab + T_E0Z * L.plane + o2);
         }
         if (HALL) {      // Hall term of eq (5): + d_i G (reading R11); G = 0 on the boundary layers
-            E[0] = fma(ph.d_i, raw[NF - 3][s], E[0]);
-            E[1] = fma(ph.d_i, raw[NF - 2][s], E[1]);
-            E[2] = fma(ph.d_i, raw[NF - 1][s], E[2]);
+            E[0] = fma(ph.d_i, raw[IJ + 3][s], E[0]);
+            E[1] = fma(ph.d_i, raw[IJ + 4][s], E[1]);
+            E[2] = fma(ph.d_i, raw[IJ + 5][s], E[2]);
         }
         if (wantF) {
             const double B1R = BR - b0R, B1P = BP - b0P, B1Z = BZ - b0Z;
@@ -779,23 +799,24 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
     auto lead = [&]() {
         const int b = nlead % NRAW;
         mbar_wait(&S.bar[b], (unsigned)((nlead / NRAW) & 1));
-        ++nlead;
         const double (*raw)[SM::HTP] = S.raw[b];
+        const double (*vel)[SM::HTP] = VR ? S.vring[nlead % SM::NV] : S.raw[b] + 2;
+        ++nlead;
         double E[3];
-        node(raw, cs, off2, ct.rho0, ct.p0, q[4], E, Fp[2], true);
+        node(raw, vel, cs, off2, ct.rho0, ct.p0, q[4], E, Fp[2], true);
         eR[4] = E[0];
         eZ[4] = E[2];
 #pragma unroll
         for (int c = 0; c < 3; ++c) S.ering[sl][c][cs] = E[c];
 #pragma unroll
-        for (int f = 0; f < 5; ++f) S.sring[sl][f][cs] = q[4][f];
+        for (int f = 0; f < SM::NS; ++f) S.sring[sl][f][cs] = q[4][f];
         if (is_halo) {
             double hq[5], hE[3], hF[3];
-            node(raw, hs, hoff2, h_rho0, h_p0, hq, hE, hF, false);
+            node(raw, vel, hs, hoff2, h_rho0, h_p0, hq, hE, hF, false);
 #pragma unroll
             for (int c = 0; c < 3; ++c) S.ering[sl][c][hs] = hE[c];
 #pragma unroll
-            for (int f = 0; f < 5; ++f) S.sring[sl][f][hs] = hq[f];
+            for (int f = 0; f < SM::NS; ++f) S.sring[sl][f][hs] = hq[f];
         }
     };
     auto advance = [&]() {
@@ -868,7 +889,9 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
             dP_EZ = fd1(eZ[0], eZ[1], eZ[3], eZ[4]);
             dP_ER = fd1(eR[0], eR[1], eR[3], eR[4]);
         }
-        rhs_point<V0, SPEC>(&S.sring[sc][0][0], HT, &S.ering[sc][0][0], &S.ering[sc][1][0], &S.ering[sc][2][0], dP_EZ, dP_ER, Fp[0],
+        // velocity tiles of the centre plane (plane number it + 2): as they arrived (VR), or converted (sring fields 2-4)
+        const double *velc = VR ? &S.vring[(it + 2) % SM::NV][0][0] : &S.sring[sc][SM::NS - 3][0];
+        rhs_point<V0, SPEC>(&S.sring[sc][0][0], velc, HT, &S.ering[sc][0][0], &S.ering[sc][1][0], &S.ering[sc][2][0], dP_EZ, dP_ER, Fp[0],
                             rr, cs, q, ct, tab, off2, L.plane, ph, iR, iR2, K, [&] {
                                 mbar_wait(&S.ready, (unsigned)(it & 1));
                                 // every thread has consumed the raw buffer of plane number it+4: refill it NRAW planes
@@ -885,28 +908,29 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
 }
 
 template <int MODE, bool V0, bool HALL, bool SPEC>
-static cudaError_t launch_rhs_tma_t(const RhsArgs &a, const CUtensorMap &tmU, const CUtensorMap &tmJ, cudaStream_t s, bool configure)
+static cudaError_t launch_rhs_tma_t(const RhsArgs &a, const CUtensorMap &tmU, const CUtensorMap &tmJ, const CUtensorMap &tmV,
+                                    cudaStream_t s, bool configure)
 {
     constexpr int TZ = RHS_TZ, NRAW = 2;
     auto kern = rhs_tma_kernel<TZ, NRAW, MODE, V0, HALL, SPEC>;
-    using SM = RhsTmaSmem<TZ, NRAW, HALL ? 14 : 11>;
+    using SM = RhsTmaSmem<TZ, NRAW, HALL ? 14 : 11, !V0>;
     const int smem = (int)sizeof(SM);
     static_assert(sizeof(SM) <= 232448, "shared memory of the TMA RHS kernel exceeds 227 KB");
     if (configure) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
     dim3 block(TR, TZ, 1);
     dim3 grid((a.L.nR - 4 + TR - 1) / TR, (a.L.nZ - 4 + TZ - 1) / TZ, a.phi_chunks);
-    kern<<<grid, block, smem, s>>>(a, tmU, tmJ);
+    kern<<<grid, block, smem, s>>>(a, tmU, tmJ, tmV);
     return cudaGetLastError();
 }
 
 template <bool HALL, bool SPEC>
-static cudaError_t launch_rhs_tma_hs(const RhsArgs &a, const CUtensorMap &tmU, const CUtensorMap &tmJ, int mode, bool v0,
-                                     cudaStream_t s, bool configure)
+static cudaError_t launch_rhs_tma_hs(const RhsArgs &a, const CUtensorMap &tmU, const CUtensorMap &tmJ, const CUtensorMap &tmV, int mode,
+                                     bool v0, cudaStream_t s, bool configure)
 {
 #define CLT_CASE(M)                                                                                 \
     case M:                                                                                         \
-        return v0 ? launch_rhs_tma_t<M, true, HALL, SPEC>(a, tmU, tmJ, s, configure)                \
-                  : launch_rhs_tma_t<M, false, HALL, SPEC>(a, tmU, tmJ, s, configure);
+        return v0 ? launch_rhs_tma_t<M, true, HALL, SPEC>(a, tmU, tmJ, tmV, s, configure)           \
+                  : launch_rhs_tma_t<M, false, HALL, SPEC>(a, tmU, tmJ, tmV, s, configure);
     switch (mode) {
         CLT_CASE(RHS_MODE_K)
         CLT_CASE(RHS_MODE_S1)
@@ -919,15 +943,16 @@ static cudaError_t launch_rhs_tma_hs(const RhsArgs &a, const CUtensorMap &tmU, c
 #undef CLT_CASE
 }
 
-cudaError_t launch_rhs_tma(const RhsArgs &a, const void *tmU, const void *tmJ, int mode, bool has_v0, bool hall, bool spec,
-                           cudaStream_t s, bool configure)
+cudaError_t launch_rhs_tma(const RhsArgs &a, const void *tmU, const void *tmJ, const void *tmV, int mode, bool has_v0, bool hall,
+                           bool spec, cudaStream_t s, bool configure)
 {
     const CUtensorMap &mU = *reinterpret_cast<const CUtensorMap *>(tmU);
     const CUtensorMap &mJ = *reinterpret_cast<const CUtensorMap *>(tmJ);
-    if (hall && spec) return launch_rhs_tma_hs<true, true>(a, mU, mJ, mode, has_v0, s, configure);
-    if (hall) return launch_rhs_tma_hs<true, false>(a, mU, mJ, mode, has_v0, s, configure);
-    if (spec) return launch_rhs_tma_hs<false, true>(a, mU, mJ, mode, has_v0, s, configure);
-    return launch_rhs_tma_hs<false, false>(a, mU, mJ, mode, has_v0, s, configure);
+    const CUtensorMap &mV = *reinterpret_cast<const CUtensorMap *>(tmV);
+    if (hall && spec) return launch_rhs_tma_hs<true, true>(a, mU, mJ, mV, mode, has_v0, s, configure);
+    if (hall) return launch_rhs_tma_hs<true, false>(a, mU, mJ, mV, mode, has_v0, s, configure);
+    if (spec) return launch_rhs_tma_hs<false, true>(a, mU, mJ, mV, mode, has_v0, s, configure);
+    return launch_rhs_tma_hs<false, false>(a, mU, mJ, mV, mode, has_v0, s, configure);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -1885,7 +1910,7 @@ cudaError_t configure_kernels()
             cudaError_t e = launch_rhs(ra, mode, v0 != 0, nullptr, true);
             if (e != cudaSuccess) return e;
             for (int hs = 0; hs < 4; ++hs) {
-                e = launch_rhs_tma(ra, &tm, &tm, mode, v0 != 0, (hs & 1) != 0, (hs & 2) != 0, nullptr, true);
+                e = launch_rhs_tma(ra, &tm, &tm, &tm, mode, v0 != 0, (hs & 1) != 0, (hs & 2) != 0, nullptr, true);
                 if (e != cudaSuccess) return e;
             }
         }
