@@ -156,6 +156,22 @@ int clt_get_rows(clt_ctx *ctx, int buffer, int k0, int nrows, double *dst);
 int clt_set_rows(clt_ctx *ctx, int buffer, int k0, int nrows, const double *src);
 int clt_set_owned_rows(clt_ctx *ctx, int k_first, int k_last, int deep_first, int deep_last);
 
+/* Adaptive time step [L139, Fig. 3-4] for a GROUP of contexts that share one dt (the slabs of one grid), with dt kept on
+ * the device as in clt_step_cfl -- no host round trip per step:
+ *   clt_cfl_open(ctx, cfl)        enters adaptive mode: SETDT of the current state over the context's owned rows
+ *                                 (cfl <= 0: params.cfl).  CLT_ESTATE inside a step or if already open.
+ *   clt_cfl_commit(ctxs, n, init) one single-thread kernel: the minimum over the n contexts (init = 1: of the SETDT values
+ *                                 clt_cfl_open computed; init = 0: of the minima stage 4 collected over the owned rows
+ *                                 of the new state, after advancing every clock by the dt just used) becomes every
+ *                                 context's dt.  All contexts on one device; n <= 64; stream-ordered (events).
+ *   clt_step_stage(ctx, 1..4)     runs with the committed dt; the caller exchanges ghost rows in between.
+ *   clt_cfl_close(ctx, ..)        leaves adaptive mode; returns the dt the next step would use and the time advanced
+ *                                 since clt_cfl_open (synchronises).  CLT_ENONFINITE like clt_step_cfl.
+ * One context alone: open, commit(init = 1), { four stages, commit(init = 0) } x steps, close == clt_step_cfl, bit for bit. */
+int clt_cfl_open(clt_ctx *ctx, double cfl);
+int clt_cfl_commit(clt_ctx *const *ctxs, int n, int init);
+int clt_cfl_close(clt_ctx *ctx, double *dt_next, double *time_advanced);
+
 /* A slab of a larger grid carries the GLOBAL spacing: dZ replaces (Zmax - Zmin)/(nZ - 1) of this context's own grid in
  * every stencil weight, table and diagnostic weight, so that a decomposed run reproduces the undivided run bit for bit
  * (the method has no other use for Z than its spacing).  Call it right after clt_create: it invalidates the

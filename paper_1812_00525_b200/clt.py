@@ -44,7 +44,7 @@ class clt_profile(ctypes.Structure):
 # every symbol include/clt.h declares
 EXPORTS = ["clt_workspace_bytes", "clt_create", "clt_destroy", "clt_set_equilibrium", "clt_set_state", "clt_get_state",
            "clt_rhs", "clt_curl_J1", "clt_hall_G", "clt_step", "clt_step_cfl", "clt_step_stage", "clt_get_rows", "clt_set_rows",
-           "clt_set_owned_rows", "clt_set_z_spacing", "clt_push_rows", "clt_set_dt", "clt_diagnostics", "clt_suggest_dt", "clt_set_tuning",
+           "clt_set_owned_rows", "clt_set_z_spacing", "clt_push_rows", "clt_cfl_open", "clt_cfl_commit", "clt_cfl_close", "clt_set_dt", "clt_diagnostics", "clt_suggest_dt", "clt_set_tuning",
            "clt_set_kernel_variant", "clt_spectral_workspace_bytes", "clt_set_phi_scheme", "clt_set_profiling", "clt_get_profile", "clt_launch_count", "clt_stream", "clt_strerror", "clt_last_cuda_error", "clt_version"]
 
 LIB_TEXTBOOK_PATH = os.path.join(_HERE, "libclt_textbook.so")
@@ -106,6 +106,12 @@ def load(path=None):
         getattr(L, name).argtypes = [vp, i, i, i, vp]
     L.clt_set_owned_rows.restype = i
     L.clt_set_owned_rows.argtypes = [vp, i, i, i, i]
+    L.clt_cfl_open.restype = i
+    L.clt_cfl_open.argtypes = [vp, d]
+    L.clt_cfl_commit.restype = i
+    L.clt_cfl_commit.argtypes = [ctypes.POINTER(vp), i, i]
+    L.clt_cfl_close.restype = i
+    L.clt_cfl_close.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
     L.clt_set_z_spacing.restype = i
     L.clt_set_z_spacing.argtypes = [vp, d]
     L.clt_push_rows.restype = i
@@ -242,6 +248,15 @@ class Clt:
     def set_owned_rows(self, k_first, k_last, deep_first, deep_last):
         self._ck(self.L.clt_set_owned_rows(self.h, int(k_first), int(k_last), int(deep_first), int(deep_last)))
 
+    def cfl_open(self, cfl=0.0):
+        self._ck(self.L.clt_cfl_open(self.h, float(cfl)))
+
+    def cfl_close(self):
+        """Returns (dt of the next step, time advanced since cfl_open)."""
+        a, b = ctypes.c_double(), ctypes.c_double()
+        self._ck(self.L.clt_cfl_close(self.h, ctypes.byref(a), ctypes.byref(b)))
+        return a.value, b.value
+
     def set_z_spacing(self, dZ):
         """A slab of a larger grid: the global dZ, bit for bit (call before set_equilibrium / set_state)."""
         self._ck(self.L.clt_set_z_spacing(self.h, float(dZ)))
@@ -307,6 +322,12 @@ class Clt:
     @property
     def launch_count(self):
         return int(self.L.clt_launch_count(self.h))
+
+
+def cfl_commit(ctxs, init):
+    """clt_cfl_commit over the contexts `ctxs` (Clt objects of one library build and one device)."""
+    arr = (ctypes.c_void_p * len(ctxs))(*[c.h for c in ctxs])
+    ctxs[0]._ck(ctxs[0].L.clt_cfl_commit(arr, len(ctxs), int(bool(init))))
 
 
 def version():

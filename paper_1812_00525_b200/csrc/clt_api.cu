@@ -345,6 +345,7 @@ int run_rhs(clt_ctx *ctx, int mode, const double *in, double *out)
     a.coef = ctx->adaptive ? ctx->result + 8 : ctx->result + 24;
     a.dtmin_bits = ctx->adaptive ? (unsigned long long *)(ctx->result + 16) : nullptr;
     a.cfl = ctx->adaptive_cfl;
+    a.own_k0 = ctx->k_first; a.own_k1 = ctx->k_last;
     const bool tma = ctx->variant == 0;
     if ((ctx->hall || ctx->spectral) && !tma) {
         snprintf(ctx->cuda_err, sizeof(ctx->cuda_err),
@@ -839,7 +840,87 @@ int clt_step_stage(clt_ctx *ctx, int stage)
     int r = enqueue_stage(ctx, stage);
     if (r) return r;
     ctx->next_stage = stage == 4 ? 1 : stage + 1;
-    if (stage == 4) { ctx->step += 1; ctx->time += ctx->dt; }
+    if (stage == 4) { ctx->step += 1; if (!ctx->adaptive) ctx->time += ctx->dt; }     // adaptive: clt_cfl_close adds the time
+    return CLT_OK;
+}
+
+// ---- adaptive stepping of a GROUP of contexts that share one time step (slabs of one grid; NEXT-1 + NEXT-4) ----------
+int clt_cfl_open(clt_ctx *ctx, double cfl)
+{
+    DeviceGuard device_guard(ctx);
+    if (!ctx) return CLT_EINVAL;
+    if (!ctx->has_state || ctx->next_stage != 1 || ctx->adaptive) return CLT_ESTATE;
+    if (!(cfl > 0.0)) cfl = ctx->par.cfl;
+    if (!(cfl > 0.0) || !isfinite(cfl)) return CLT_EINVAL;
+    int r;
+    if ((r = resolve_v0(ctx))) return r;
+    DiagArgs a;
+    a.L = ctx->L; a.ph = ctx->ph;
+    a.U = ctx->Un; a.tab = ctx->tab;
+    a.R = ctx->Rtab + LP; a.invR = ctx->invRtab + LP;
+    a.cs = ctx->cs; a.partial = ctx->partial; a.cfl = cfl; a.ihZ = 1.0 / ctx->ph.dZ;
+    a.spec_c1 = ctx->spectral ? ctx->spec_ctab : nullptr;
+    a.k_first = ctx->k_first; a.k_last = ctx->k_last; a.kd_first = ctx->kd_first; a.kd_last = ctx->kd_last;
+    CK(launch_diag(a, ctx->nblocks_diag, ctx->result, ctx->stream));       // result[5] = SETDT of the owned rows
+    ctx->launches += 2;
+    ctx->adaptive = true;
+    ctx->adaptive_cfl = cfl;
+    return CLT_OK;
+}
+
+int clt_cfl_commit(clt_ctx *const *ctxs, int n, int init)
+{
+    if (!ctxs || n < 1 || n > DT_GROUP_MAX) return CLT_EINVAL;
+    DtGroup g;
+    g.n = n;
+    for (int c = 0; c < n; ++c) {
+        if (!ctxs[c] || !ctxs[c]->adaptive || ctxs[c]->next_stage != 1) return ctxs[c] ? CLT_ESTATE : CLT_EINVAL;
+        if (ctxs[c]->device != ctxs[0]->device) return CLT_EINVAL;       // one kernel reads every clock: one device
+        g.clock[c] = ctxs[c]->result + 8;
+        g.dtmin_bits[c] = (unsigned long long *)(ctxs[c]->result + 16);
+        g.diag6[c] = ctxs[c]->result;
+    }
+    clt_ctx *ctx = ctxs[0];
+    DeviceGuard device_guard(ctx);
+    // the kernel runs on the first context's stream, after everything the others have enqueued; they wait for it
+    cudaEvent_t ev = nullptr;
+    bool others = false;
+    for (int c = 1; c < n; ++c) others = others || ctxs[c]->stream != ctx->stream;
+    if (others) {
+        CK(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+        for (int c = 1; c < n; ++c)
+            if (ctxs[c]->stream != ctx->stream) {
+                cudaError_t e = cudaEventRecord(ev, ctxs[c]->stream);
+                if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->stream, ev, 0);
+                if (e != cudaSuccess) { cudaEventDestroy(ev); return cuda_fail(ctx, e, "clt_cfl_commit: stream order"); }
+            }
+    }
+    cudaError_t e = launch_dt_commit_group(g, init, ctx->stream);
+    if (e == cudaSuccess && others) {
+        e = cudaEventRecord(ev, ctx->stream);
+        for (int c = 1; c < n && e == cudaSuccess; ++c)
+            if (ctxs[c]->stream != ctx->stream) e = cudaStreamWaitEvent(ctxs[c]->stream, ev, 0);
+    }
+    if (ev) cudaEventDestroy(ev);
+    for (int c = 0; c < n; ++c) ctxs[c]->prof_chain = false;
+    ctx->launches++;
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "dt_commit_group_kernel");
+    return CLT_OK;
+}
+
+int clt_cfl_close(clt_ctx *ctx, double *dt_next, double *time_advanced)
+{
+    DeviceGuard device_guard(ctx);
+    if (!ctx) return CLT_EINVAL;
+    if (!ctx->adaptive || ctx->next_stage != 1) return CLT_ESTATE;
+    double h[6] = { 0, 0, 0, 0, 0, 0 };
+    ctx->adaptive = false;
+    CK(cudaMemcpyAsync(h, ctx->result + 8, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    ctx->time += h[4];
+    if (dt_next) *dt_next = h[0];
+    if (time_advanced) *time_advanced = h[4];
+    if (h[5] != 0.0) return CLT_ENONFINITE;
     return CLT_OK;
 }
 

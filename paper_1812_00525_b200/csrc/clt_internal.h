@@ -66,6 +66,16 @@ struct RhsArgs {
     // adaptive stepping (clt_step_cfl): non-null = stage 4 folds the SETDT minimum of the new state into *dtmin_bits
     unsigned long long *dtmin_bits;
     double cfl;
+    int own_k0, own_k1;   // rows whose new state enters that minimum (a slab's owned rows; default 2 .. nZ-3)
+};
+
+// clocks of a group of contexts that share one adaptive time step (clt_cfl_commit)
+constexpr int DT_GROUP_MAX = 64;
+struct DtGroup {
+    int n;
+    double *clock[DT_GROUP_MAX];
+    unsigned long long *dtmin_bits[DT_GROUP_MAX];
+    const double *diag6[DT_GROUP_MAX];
 };
 
 struct CurlArgs {
@@ -148,6 +158,7 @@ cudaError_t launch_curl_tma(const CurlArgs &a, const void *tmU, bool hall, bool 
 cudaError_t launch_phi_spectral(const SpecArgs &a, cudaStream_t s, bool configure = false);
 int curl_tma_tile_z();
 int rhs_tile_z();
+cudaError_t launch_dt_commit_group(const DtGroup &g, int init, cudaStream_t s);
 cudaError_t launch_dt_commit(double *clock, unsigned long long *dtmin_bits, const double *diag6, int init, cudaStream_t s);
 cudaError_t launch_diag(const DiagArgs &a, int nblocks, double *result6, cudaStream_t s);
 int diag_blocks(const Layout &L);

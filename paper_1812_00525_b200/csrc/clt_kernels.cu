@@ -262,7 +262,7 @@ __device__ __forceinline__ StageCoef load_stage_coef(const RhsArgs &a)
 }
 template <int MODE>
 __device__ __forceinline__ void epilogue_store(const RhsArgs &a, long long g, long long field, const EpiOperands &e,
-                                               const double (&K)[8], double iR, double &rate, const StageCoef &sc)
+                                               const double (&K)[8], double iR, double &rate, const StageCoef &sc, bool collect)
 {
     constexpr double third = 1.0 / 3.0;
     const double an = sc.an, bn = sc.bn;
@@ -293,7 +293,7 @@ __device__ __forceinline__ void epilogue_store(const RhsArgs &a, long long g, lo
             st_out(a.out + gm, out[m]);
         }
     }
-    if (MODE == RHS_MODE_S4 && a.dtmin_bits) {
+    if (MODE == RHS_MODE_S4 && a.dtmin_bits && collect) {
         // SETDT of Fig. 4 regrouped (rounding order only): dt = cfl / max_d (|v_d| + c) / h_d with the uniform spacings
         // 1/dR = 12 cR1, 1/dZ = 12 cZ1, 1/(R dphi) = 12 cP1 / R; one division and one square root per node here, the
         // division by the largest rate once per thread in dtmin_commit
@@ -341,6 +341,34 @@ __global__ void dt_commit_kernel(double *clock, unsigned long long *dtmin_bits, 
     }
     clock[0] = dt; clock[1] = 0.5 * dt; clock[2] = dt / 3.0; clock[3] = dt / 6.0;
     *dtmin_bits = (unsigned long long)__double_as_longlong(100.0);      // Fig. 4: DT1 starts at 100
+}
+
+// The same for a group of contexts that share one time step (slabs of one grid): the minimum over all of them goes to
+// every clock.
+__global__ void dt_commit_group_kernel(DtGroup g, int init)
+{
+    double dt = 100.0;
+    bool marked = false;
+    for (int c = 0; c < g.n; ++c) {
+        const double mine = init ? g.diag6[c][5] : __longlong_as_double((long long)*g.dtmin_bits[c]);
+        if (!(mine > 0.0)) marked = true;
+        dt = fmin(dt, mine);
+        if (!init && g.clock[c][5] != 0.0) marked = true;
+    }
+    if (marked) dt = 0.0;
+    for (int c = 0; c < g.n; ++c) {
+        double *clock = g.clock[c];
+        if (init) clock[4] = 0.0; else clock[4] += clock[0];
+        clock[5] = marked ? 1.0 : 0.0;
+        clock[0] = dt; clock[1] = 0.5 * dt; clock[2] = dt / 3.0; clock[3] = dt / 6.0;
+        *g.dtmin_bits[c] = (unsigned long long)__double_as_longlong(100.0);
+    }
+}
+
+cudaError_t launch_dt_commit_group(const DtGroup &g, int init, cudaStream_t s)
+{
+    dt_commit_group_kernel<<<1, 1, 0, s>>>(g, init);
+    return cudaGetLastError();
 }
 
 cudaError_t launch_dt_commit(double *clock, unsigned long long *dtmin_bits, const double *diag6, int init, cudaStream_t s)
@@ -535,7 +563,7 @@ __global__ void __launch_bounds__(TR *TZ, 1) rhs_kernel(const __grid_constant__ 
             EpiOperands eo;
             // plain coherent loads: stage 4 updates U^n in place through a.out, so the non-coherent path is not allowed here
             epilogue_load<MODE, 0>(a, g, L.field, eo, [](const double *p) { return *p; });
-            epilogue_store<MODE>(a, g, L.field, eo, K, iR, rate, coef);
+            epilogue_store<MODE>(a, g, L.field, eo, K, iR, rate, coef, k >= a.own_k0 && k <= a.own_k1);
         }
         advance();
     }
@@ -901,7 +929,7 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
                             }, pd1, pd2);
 
         // ---- a6: RK4 stage combine in the epilogue (L125, L139) --------------------------------
-        if (valid) epilogue_store<MODE>(a, g, L.field, eo, K, iR, rate, coef);
+        if (valid) epilogue_store<MODE>(a, g, L.field, eo, K, iR, rate, coef, k >= a.own_k0 && k <= a.own_k1);
         advance();
     }
     if (MODE == RHS_MODE_S4) dtmin_commit(a, rate);

@@ -184,8 +184,20 @@ class SlabGroup:
 
     def step_cfl(self, n=1, cfl=0.0):
         """n adaptive RK4 steps (Fig. 3-4): every step runs with the global SETDT minimum of the state at
-        its start -- the minimum of the slabs' reductions (one MIN all-reduce and one host round trip per step; the
-        device-resident clock of clt_step_cfl needs a single context).  Returns the time advanced."""
+        its start.  Slabs of one process on one device keep dt on the device; across processes it is the minimum of the
+        slabs' reductions (one MIN all-reduce and one host round trip per step).  Returns the time advanced."""
+        if self.dist is None and n > 0 and len({str(s.device) for s in self.slabs}) == 1:
+            # all slabs on one device: dt stays on the device (clt_cfl_open / clt_cfl_commit / clt_cfl_close) -- stage 4
+            # collects each slab's minimum over its owned rows, one single-thread kernel takes the minimum over the slabs
+            from . import clt
+            ctxs = [s.g for s in self.slabs]
+            for g in ctxs:
+                g.cfl_open(cfl)
+            clt.cfl_commit(ctxs, init=True)
+            for _ in range(n):
+                self.step(1)
+                clt.cfl_commit(ctxs, init=False)
+            return [g.cfl_close() for g in ctxs][0][1]
         t = 0.0
         for _ in range(n):
             dt = self.suggest_dt(cfl)
