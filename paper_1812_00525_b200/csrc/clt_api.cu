@@ -728,7 +728,8 @@ int clt_step(clt_ctx *ctx, int n)
     return CLT_OK;
 }
 
-static int run_diag(clt_ctx *ctx, double cfl, double out6[6])
+// a7 + SETDT: the reduction kernels over the current state -> ctx->result[0..5] (device)
+static int enqueue_diag(clt_ctx *ctx, double cfl)
 {
     DiagArgs a;
     a.L = ctx->L; a.ph = ctx->ph;
@@ -737,8 +738,17 @@ static int run_diag(clt_ctx *ctx, double cfl, double out6[6])
     a.cs = ctx->cs; a.partial = ctx->partial; a.cfl = cfl; a.ihZ = 1.0 / ctx->ph.dZ;
     a.spec_c1 = ctx->spectral ? ctx->spec_ctab : nullptr;
     a.k_first = ctx->k_first; a.k_last = ctx->k_last; a.kd_first = ctx->kd_first; a.kd_last = ctx->kd_last;
-    CK(launch_diag(a, ctx->nblocks_diag, ctx->result, ctx->stream));
+    alignas(64) CUtensorMap tmU;
+    const bool tma = ctx->variant == 0 && !ctx->spectral && make_map(ctx, ctx->Un, 8, diag_tma_tile_z(), &tmU, 8);
+    CK(launch_diag(a, ctx->nblocks_diag, ctx->result, ctx->stream, tma ? &tmU : nullptr));
     ctx->launches += 2;
+    return CLT_OK;
+}
+
+static int run_diag(clt_ctx *ctx, double cfl, double out6[6])
+{
+    int r = enqueue_diag(ctx, cfl);
+    if (r) return r;
     CK(cudaMemcpyAsync(out6, ctx->result, 6 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
     return CLT_OK;
@@ -854,15 +864,7 @@ int clt_cfl_open(clt_ctx *ctx, double cfl)
     if (!(cfl > 0.0) || !isfinite(cfl)) return CLT_EINVAL;
     int r;
     if ((r = resolve_v0(ctx))) return r;
-    DiagArgs a;
-    a.L = ctx->L; a.ph = ctx->ph;
-    a.U = ctx->Un; a.tab = ctx->tab;
-    a.R = ctx->Rtab + LP; a.invR = ctx->invRtab + LP;
-    a.cs = ctx->cs; a.partial = ctx->partial; a.cfl = cfl; a.ihZ = 1.0 / ctx->ph.dZ;
-    a.spec_c1 = ctx->spectral ? ctx->spec_ctab : nullptr;
-    a.k_first = ctx->k_first; a.k_last = ctx->k_last; a.kd_first = ctx->kd_first; a.kd_last = ctx->kd_last;
-    CK(launch_diag(a, ctx->nblocks_diag, ctx->result, ctx->stream));       // result[5] = SETDT of the owned rows
-    ctx->launches += 2;
+    if ((r = enqueue_diag(ctx, cfl))) return r;       // result[5] = SETDT of the owned rows
     ctx->adaptive = true;
     ctx->adaptive_cfl = cfl;
     return CLT_OK;
@@ -1031,16 +1033,10 @@ int clt_step_cfl(clt_ctx *ctx, int n, double cfl, double *dt_last, double *time_
     double h[6] = { 0, 0, 0, 0, 0, 0 };
     if (n > 0) {
         // dt of the first step: SETDT of the current state (the reduction kernel of clt_suggest_dt, no host round trip)
-        DiagArgs a;
-        a.L = ctx->L; a.ph = ctx->ph;
-        a.U = ctx->Un; a.tab = ctx->tab;
-        a.R = ctx->Rtab + LP; a.invR = ctx->invRtab + LP;
-        a.cs = ctx->cs; a.partial = ctx->partial; a.cfl = cfl; a.ihZ = 1.0 / ctx->ph.dZ;
-        a.spec_c1 = ctx->spectral ? ctx->spec_ctab : nullptr;
-        a.k_first = ctx->k_first; a.k_last = ctx->k_last; a.kd_first = ctx->kd_first; a.kd_last = ctx->kd_last;
-        CK(launch_diag(a, ctx->nblocks_diag, ctx->result, ctx->stream));
+        int rd = enqueue_diag(ctx, cfl);
+        if (rd) return rd;
         CK(launch_dt_commit(clock, bits, ctx->result, 1, ctx->stream));
-        ctx->launches += 3;
+        ctx->launches += 1;
         ctx->adaptive = true;
         ctx->adaptive_cfl = cfl;
         int r = CLT_OK;

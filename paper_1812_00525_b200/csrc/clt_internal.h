@@ -160,7 +160,8 @@ int curl_tma_tile_z();
 int rhs_tile_z();
 cudaError_t launch_dt_commit_group(const DtGroup &g, int init, cudaStream_t s);
 cudaError_t launch_dt_commit(double *clock, unsigned long long *dtmin_bits, const double *diag6, int init, cudaStream_t s);
-cudaError_t launch_diag(const DiagArgs &a, int nblocks, double *result6, cudaStream_t s);
+cudaError_t launch_diag(const DiagArgs &a, int nblocks, double *result6, cudaStream_t s, const void *tmU = nullptr, bool configure = false);
+int diag_tma_tile_z();
 int diag_blocks(const Layout &L);
 cudaError_t configure_kernels();
 

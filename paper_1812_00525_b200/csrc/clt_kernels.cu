@@ -1879,6 +1879,133 @@ __global__ void __launch_bounds__(DG_BX *DG_G, 2) diag_kernel(const __grid_const
     }
 }
 
+// TMA-fed variant of the reduction (finite-difference phi scheme; the default): the curl kernel's sweep.  A CTA owns a
+// 32 x DGT_TZ tile and marches over all planes; one bulk copy per plane brings the 8 fields of the tile with its halo into a
+// DGT_NS-slot ring three planes ahead, so nothing waits for HBM in front of the square root and the division of SETDT;
+// B_phi's phi neighbours sit in a register pipeline, the R / Z neighbours of div_c B come from the tile, and a thread sees
+// all planes of its node: the Fourier sums of the n = 1 harmonic are complete in its registers.
+constexpr int DGT_TZ = 8, DGT_NS = 4;
+struct DiagTmaSmem {
+    static constexpr int HT = (DGT_TZ + 4) * SW;
+    alignas(128) double raw[DGT_NS][8][HT];
+    alignas(8) unsigned long long full[DGT_NS];
+    double red[DGT_TZ][DG_N];
+};
+
+__global__ void __launch_bounds__(TR *DGT_TZ, 2) diag_tma_kernel(const __grid_constant__ DiagArgs a, const __grid_constant__ CUtensorMap tmU)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    DiagTmaSmem &S = *reinterpret_cast<DiagTmaSmem *>(smem_raw);
+    constexpr int HT = DiagTmaSmem::HT, NS = DGT_NS, TZ = DGT_TZ;
+    static_assert(HT % 16 == 0, "a box that spans the field axis fills a ring slot densely");
+    const Layout &L = a.L;
+    const Phys &ph = a.ph;
+    const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * TR + tx, n = L.nphi;
+    const int i0 = 2 + TR * blockIdx.x, k0 = 2 + TZ * blockIdx.y;
+    const int i = i0 + tx, k = k0 + ty;
+    const bool valid = i <= L.nR - 3 && k <= L.nZ - 3 && k >= a.k_first && k <= a.k_last;
+    const bool deep = valid && i >= 4 && i <= L.nR - 5 && k >= a.kd_first && k <= a.kd_last;
+    const int ic = min(i, L.nR - 3), kc = min(k, L.nZ - 3);
+    const long long o = (long long)kc * L.pR + (LP + ic);
+    const int cs = (ty + 2) * SW + (tx + 2);
+    const int total = n + 4;                                  // planes -2 .. n+1
+
+    if (tid == 0) {
+        for (int q = 0; q < NS; ++q) mbar_init(&S.full[q], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmU) : "memory");
+    }
+    __syncthreads();
+    auto issue = [&](int q) {                                 // plane number q counts from plane -2
+        const int st = q % NS;
+        mbar_expect_tx(&S.full[st], (unsigned)(8 * HT * sizeof(double)));
+        tma_load_4d(&S.raw[st][0][0], &tmU, LP + i0 - 2, k0 - 2, wrap_phi(q - 2, n), 0, &S.full[st]);
+    };
+    if (tid == 0)
+        for (int q = 0; q < NS && q < total; ++q) issue(q);
+
+    const double inf = __longlong_as_double(0x7ff0000000000000LL);
+    const double Ri = a.R[ic], iR = a.invR[ic];
+    const double b0R = a.tab[T_B0R * L.plane + o], b0P = a.tab[T_B0P * L.plane + o], b0Z = a.tab[T_B0Z * L.plane + o];
+    const double ihR = 1.0 / fabs(Ri - a.R[ic - 1]), ihP = 1.0 / fabs(Ri * ph.dphi);
+    const double rr[4] = { a.R[ic - 2], a.R[ic - 1], a.R[ic + 1], a.R[ic + 2] };
+    double ke = 0.0, me = 0.0, mep = 0.0, mdiv = 0.0, rate = 0.0;
+    double fa[3] = { 0, 0, 0 }, fb[3] = { 0, 0, 0 };
+    double bp[5] = { 0, 0, 0, 0, 0 };                         // B_phi of planes j-2 .. j+2 at the own node
+#pragma unroll 1
+    for (int q = 0; q < 4; ++q) {
+        mbar_wait(&S.full[q % NS], (unsigned)((q / NS) & 1));
+        bp[q + 1] = S.raw[q % NS][6][cs];
+    }
+    __syncthreads();                                          // planes 0 and 1 are never centre planes: recycle their slots
+    if (tid == 0) {
+        if (NS < total) issue(NS);
+        if (NS + 1 < total) issue(NS + 1);
+    }
+#pragma unroll 1
+    for (int j = 0; j < n; ++j) {
+        const int nc = j + 2;                                 // plane number of the centre plane
+        mbar_wait(&S.full[(nc + 2) % NS], (unsigned)(((nc + 2) / NS) & 1));
+#pragma unroll
+        for (int d = 0; d < 4; ++d) bp[d] = bp[d + 1];
+        bp[4] = S.raw[(nc + 2) % NS][6][cs];
+        const double (*f)[HT] = S.raw[nc % NS];
+        const double rho = f[0][cs], p = f[1][cs], vR = f[2][cs], vP = f[3][cs], vZ = f[4][cs], BR = f[5][cs], BZ = f[7][cs];
+        const double BP = bp[2];
+        if (valid) {
+            const double b2 = BR * BR + BP * BP + BZ * BZ;
+            ke += 0.5 * rho * (vR * vR + vP * vP + vZ * vZ);
+            me += 0.5 * b2;
+            const double b1[3] = { BR - b0R, BP - b0P, BZ - b0Z };
+            mep += 0.5 * (b1[0] * b1[0] + b1[1] * b1[1] + b1[2] * b1[2]);
+            const double c = a.cs[j], s = a.cs[n + j];
+#pragma unroll
+            for (int d = 0; d < 3; ++d) { fa[d] += b1[d] * c; fb[d] += b1[d] * s; }
+            // SETDT, Fig. 4: signal speed and the three rates
+            const double cf = sqrt(fabs((ph.gamma * p + b2) / rho));
+            const double rR = (fabs(vR) + cf) * ihR, rZ = (fabs(vZ) + cf) * a.ihZ, rP = (fabs(vP) + cf) * ihP;
+            rate = fmax(rate, fmax(rP, fmax(rR, rZ)));
+            if (!(rR + rP + rZ <= 1.79769313486231570815e308)) rate = inf;     // fmax drops NaN: mark a non-finite state
+            if (deep) {
+                // div_c B = d_R(R B_R)/R + d_phi B_phi / R + d_Z B_Z
+                const double *br = &f[5][cs], *bz = &f[7][cs];
+                const double dRR = fd1(rr[0] * br[-2], rr[1] * br[-1], rr[2] * br[1], rr[3] * br[2]);
+                const double dPs = fd1(bp[0], bp[1], bp[3], bp[4]) * ph.cP1;
+                const double dZ = fd1(bz[-2 * SW], bz[-SW], bz[SW], bz[2 * SW]);
+                mdiv = fmax(mdiv, fabs(dRR * ph.cR1 * iR + dPs * iR + dZ * ph.cZ1));
+            }
+        }
+        __syncthreads();                                      // the centre plane's slot is free again
+        if (tid == 0 && nc + NS < total) issue(nc + NS);
+    }
+    double out[DG_N] = { 0, 0, 0, 0, 0, 0 };
+    if (valid) {
+        const double w = Ri * ph.dR * ph.dphi * ph.dZ;
+        out[0] = ke * w; out[1] = me * w; out[2] = mep * w;
+        const double sc = 2.0 / (double)n;
+        double e1 = 0.0;
+#pragma unroll
+        for (int d = 0; d < 3; ++d) { const double A = fa[d] * sc, B = fb[d] * sc; e1 += A * A + B * B; }
+        out[3] = 0.25 * e1 * (Ri * ph.dR * ph.dZ * ph.Lphi);
+        out[4] = mdiv; out[5] = rate;
+    }
+#pragma unroll
+    for (int q = 0; q < 4; ++q) out[q] = warp_sum(out[q]);
+    out[4] = warp_max(out[4]); out[5] = warp_max(out[5]);
+    if (tx == 0)
+        for (int q = 0; q < DG_N; ++q) S.red[ty][q] = out[q];
+    __syncthreads();
+    if (tid == 0) {                                           // warps in a fixed order (deterministic)
+        double r[DG_N] = { 0, 0, 0, 0, 0, 0 };
+        for (int w = 0; w < TZ; ++w) {
+            for (int q = 0; q < 4; ++q) r[q] += S.red[w][q];
+            r[4] = fmax(r[4], S.red[w][4]); r[5] = fmax(r[5], S.red[w][5]);
+        }
+        double *dst = a.partial + (long long)(blockIdx.y * gridDim.x + blockIdx.x) * DG_N;
+        for (int q = 0; q < DG_N; ++q) dst[q] = r[q];
+    }
+}
+
 // result = { kinetic, magnetic, magnetic_pert, magnetic_n1, max |div_c B|, dt = min(100, cfl / max rate) }; an infinite
 // rate (non-finite state) gives dt = 0
 __global__ void __launch_bounds__(256) diag_final_kernel(const double *partial, int nblocks, double cfl, double *result)
@@ -1915,11 +2042,25 @@ int diag_blocks(const Layout &L)
     return ((L.nR - 4 + DG_BX - 1) / DG_BX) * (L.nZ - 4);
 }
 
-cudaError_t launch_diag(const DiagArgs &a, int nblocks, double *result6, cudaStream_t s)
+int diag_tma_tile_z() { return DGT_TZ; }
+
+// tmU != nullptr (and the finite-difference phi scheme): the TMA-fed kernel; tmU maps the 8 fields of the state with box
+// (TR+4, diag_tma_tile_z()+4, 1, 8).  configure = true: only the shared-memory opt-in.
+cudaError_t launch_diag(const DiagArgs &a, int nblocks, double *result6, cudaStream_t s, const void *tmU, bool configure)
 {
-    dim3 block(DG_BX, DG_G), grid((a.L.nR - 4 + DG_BX - 1) / DG_BX, a.L.nZ - 4);
-    diag_kernel<<<grid, block, 0, s>>>(a);
-    cudaError_t e = cudaGetLastError();
+    if (configure)
+        return cudaFuncSetAttribute(diag_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(DiagTmaSmem));
+    cudaError_t e;
+    if (tmU && !a.spec_c1) {
+        dim3 block(TR, DGT_TZ), grid((a.L.nR - 4 + TR - 1) / TR, (a.L.nZ - 4 + DGT_TZ - 1) / DGT_TZ);
+        nblocks = (int)(grid.x * grid.y);
+        diag_tma_kernel<<<grid, block, sizeof(DiagTmaSmem), s>>>(a, *reinterpret_cast<const CUtensorMap *>(tmU));
+        e = cudaGetLastError();
+    } else {
+        dim3 block(DG_BX, DG_G), grid((a.L.nR - 4 + DG_BX - 1) / DG_BX, a.L.nZ - 4);
+        diag_kernel<<<grid, block, 0, s>>>(a);
+        e = cudaGetLastError();
+    }
     if (e != cudaSuccess) return e;
     diag_final_kernel<<<1, 256, 0, s>>>(a.partial, nblocks, a.cfl, result6);
     return cudaGetLastError();
@@ -1946,7 +2087,9 @@ cudaError_t configure_kernels()
         cudaError_t e = launch_curl_tma(ca, &tm, (hs & 1) != 0, (hs & 2) != 0, nullptr, true);
         if (e != cudaSuccess) return e;
     }
-    return launch_phi_spectral(sa, nullptr, true);
+    cudaError_t e = launch_phi_spectral(sa, nullptr, true);
+    if (e != cudaSuccess) return e;
+    return launch_diag(DiagArgs{}, 0, nullptr, nullptr, nullptr, true);
 }
 
 }  // namespace clt
