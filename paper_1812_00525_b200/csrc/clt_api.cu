@@ -359,7 +359,7 @@ int run_rhs(clt_ctx *ctx, int mode, const double *in, double *out)
     alignas(64) CUtensorMap tmU, tmJ, tmV;
     const int nJ = ctx->hall ? 6 : 3;
     // static reference state: rho, p and B land in the raw buffer, v in a ring of its own (three boxes over the stage state)
-    const int nU = ctx->has_v0 ? 8 : 2;
+    const int nU = (ctx->has_v0 || ctx->spectral) ? 8 : 2;      // must match rhs_velocity_ring() of the kernels
     if (tma && (!make_map(ctx, in, 8, rhs_tile_z(), &tmU, nU) || !make_map(ctx, in, 8, rhs_tile_z(), &tmV, 3)
                 || !make_map(ctx, ctx->J1, nJ, rhs_tile_z(), &tmJ, nJ))) {
         snprintf(ctx->cuda_err, sizeof(ctx->cuda_err), "cuTensorMapEncodeTiled failed");

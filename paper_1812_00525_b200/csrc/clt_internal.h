@@ -147,8 +147,8 @@ cudaError_t launch_zero_boundary(const Layout &L, int nfields, double *dst, int 
 cudaError_t launch_curl(const CurlArgs &a, cudaStream_t s);
 cudaError_t launch_rhs(const RhsArgs &a, int mode, bool has_v0, cudaStream_t s, bool configure = false);
 // TMA variant: tmU / tmJ / tmV point to CUtensorMap objects (4-D: pR, nZ, nphi, field) with boxes (TR+4, rhs_tile_z()+4, 1, nf)
-// that span the field axis.  Moving reference state (has_v0): tmU over the stage state with nf = 8, tmV unused.  Static
-// reference state: tmU with nf = 2 (rho, p), tmV with nf = 3 (v at field 2, B at field 5).  tmJ over J1 with nf = 3
+// that span the field axis.  Moving reference state (has_v0) or pseudo-spectral scheme: tmU over the stage state with nf = 8,
+// tmV unused.  Static reference state with finite differences: tmU with nf = 2 (rho, p), tmV with nf = 3 (v at field 2, B at field 5).  tmJ over J1 with nf = 3
 // (hall: 6 fields, J1 then G; the kernel adds d_i * G to E1).
 cudaError_t launch_rhs_tma(const RhsArgs &a, const void *tmU, const void *tmJ, const void *tmV, int mode, bool has_v0, bool hall,
                            bool spec, cudaStream_t s, bool configure = false);

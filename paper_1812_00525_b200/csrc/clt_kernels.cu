@@ -687,6 +687,10 @@ struct RhsTmaSmem {
     alignas(8) unsigned long long ready;       // split CTA barrier: "this plane is staged" (one arrival per warp)
 };
 
+// the velocity ring is used with a static reference state and the finite-difference phi scheme (with the pre-pass
+// derivatives of the pseudo-spectral scheme it measured 4-6 % slower than converting v like the other fields)
+__host__ __device__ constexpr bool rhs_velocity_ring(bool v0, bool spec) { return !v0 && !spec; }
+
 template <int TZ, int NRAW, int MODE, bool V0, bool HALL, bool SPEC>
 __global__ void __launch_bounds__(TR *TZ, 1)
 rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmJ,
@@ -696,7 +700,7 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
     // tmV: box of 3 fields (VR: v at field 2, B at field 5); tmJ: J1 [and G]
     extern __shared__ __align__(128) unsigned char smem_raw[];
     constexpr int NF = HALL ? 14 : 11;
-    constexpr bool VR = !V0;
+    constexpr bool VR = rhs_velocity_ring(V0, SPEC);
     using SM = RhsTmaSmem<TZ, NRAW, NF, VR>;
     SM &S = *reinterpret_cast<SM *>(smem_raw);
     constexpr int HT = SM::HT, NH = SM::NH;
@@ -941,7 +945,7 @@ static cudaError_t launch_rhs_tma_t(const RhsArgs &a, const CUtensorMap &tmU, co
 {
     constexpr int TZ = RHS_TZ, NRAW = 2;
     auto kern = rhs_tma_kernel<TZ, NRAW, MODE, V0, HALL, SPEC>;
-    using SM = RhsTmaSmem<TZ, NRAW, HALL ? 14 : 11, !V0>;
+    using SM = RhsTmaSmem<TZ, NRAW, HALL ? 14 : 11, rhs_velocity_ring(V0, SPEC)>;
     const int smem = (int)sizeof(SM);
     static_assert(sizeof(SM) <= 232448, "shared memory of the TMA RHS kernel exceeds 227 KB");
     if (configure) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
@@ -1467,8 +1471,8 @@ __device__ __forceinline__ void fft64(cpx (&x)[8], const cpx (&tw)[8], cpx *ex, 
 
 constexpr int FFT_N = 64, FFT_PITCH = 33, FFT_LINES = 32;     // lines per CTA; staging rows padded against bank conflicts
 // Grid: (R tile, Z row, job).  Measured alternatives, both slower: the job index fastest (so that the quantities of the
-// same lines run together and share their reads in L2: 9.15 ms per step against 8.87) and one CTA working through all
-// quantities of its lines (9.69 ms).
+// same lines run together and share their reads in L2: +0.3 ms per step) and one CTA working through all quantities of
+// its lines (+0.8 ms).
 template <bool WANT2>
 __global__ void __launch_bounds__(128) phi_fft64_kernel(const __grid_constant__ SpecArgs a, int job_base)
 {
