@@ -1775,9 +1775,8 @@ __global__ void __launch_bounds__(DG_BX *DG_G, 2) diag_kernel(const __grid_const
             for (int d = 0; d < 4; ++d) bp[d + 1] = Bp[(long long)wrap_phi(ja - 2 + d, n) * L.plane];
         }
         // Everything one node-plane needs is requested in ONE batch (own values, B_phi of plane j+2, the R and Z stencil
-        // neighbours of div_c B -- valid addresses for every interior node, used or not), and the batch of plane j+1 is
-        // requested before plane j is worked on: the kernel is a latency chain otherwise (ncu: 65 % of the warp time
-        // waiting for three dependent load batches per plane).
+        // neighbours of div_c B -- valid addresses for every interior node, used or not): the kernel is a latency chain
+        // otherwise (ncu: 65 % of the warp time waiting for three dependent load batches per plane).
         struct Batch {
             double rho, p, vR, vP, vZ, BR, BZ, bpn, br[4], bz[4];
         };
@@ -1794,11 +1793,9 @@ __global__ void __launch_bounds__(DG_BX *DG_G, 2) diag_kernel(const __grid_const
             q.bz[0] = bz[-2 * L.pR]; q.bz[1] = bz[-L.pR]; q.bz[2] = bz[L.pR]; q.bz[3] = bz[2 * L.pR];
             return q;
         };
-        Batch nx = request(ja);
 #pragma unroll 1
         for (int j = ja; j < jb; ++j) {
-            const Batch q = nx;
-            if (j + 1 < jb) nx = request(j + 1);
+            const Batch q = request(j);
             const double rho = q.rho, p = q.p, vR = q.vR, vP = q.vP, vZ = q.vZ, BR = q.BR, BZ = q.BZ;
             double BP;
             if (pipe) {
