@@ -148,9 +148,9 @@ int clt_step(clt_ctx *ctx, int n);
  *                    CLT_ESTATE if called out of order (clt_step is refused in the middle of a step).
  *   clt_get_rows / clt_set_rows : rows k0 .. k0+nrows-1 of buffer 0 = U^n, 1 = U_a, 2 = U_b as a dense array
  *                    double[8][nphi][nrows][nR] (host or device pointer; synchronous for host pointers).
- *   clt_set_owned_rows : the rows the diagnostics sums / SETDT minimum run over (default 2 .. nZ-3) and the rows of
- *                    max |div_c B| (default 4 .. nZ-5; first > last = none), so that slabs can be reduced without
- *                    counting ghost rows twice.                                                          */
+ *   clt_set_owned_rows : the rows this context is responsible for (default 2 .. nZ-3): the rows a stage writes, the
+ *                    diagnostics sums and the SETDT minimum run over them; and the rows of max |div_c B| (default
+ *                    4 .. nZ-5; first > last = none), so that slabs can be reduced without counting ghost rows twice. */
 int clt_step_stage(clt_ctx *ctx, int stage);
 int clt_get_rows(clt_ctx *ctx, int buffer, int k0, int nrows, double *dst);
 int clt_set_rows(clt_ctx *ctx, int buffer, int k0, int nrows, const double *src);
@@ -185,6 +185,17 @@ int clt_set_z_spacing(clt_ctx *ctx, double dZ);
  * enqueued on src's stream so far, and src's stream waits for it (events; nothing to do when both contexts share one
  * stream).  Contexts on different devices need peer access (CLT_ECUDA otherwise).                         */
 int clt_push_rows(clt_ctx *src, int buffer, int k0_src, int nrows, clt_ctx *dst, int k0_dst);
+
+/* Compute and exchange in ONE kernel [L250-256: the paper hands device pointers to MPI; here the neighbour's memory is
+ * written directly]: after clt_link_rows(ctx, side, peer, k0, nrows, k0_peer) every stage kernel of `ctx` stores rows
+ * k0 .. k0+nrows-1 (owned rows of ctx) of its output also into rows k0_peer .. of the same buffer of `peer` -- the
+ * peer's ghost rows -- straight from the RK4 epilogue, tile by tile, while the rest of the stage is still being computed.
+ * side = 0 (lower neighbour) or 1 (upper); peer = NULL removes the link.  A stage writes a context's owned rows only
+ * (clt_set_owned_rows, to be called first), so the peer's own kernels never touch its ghost rows.  Same nR and nphi;
+ * contexts on different devices need peer access (CLT_ECUDA otherwise).  clt_sync_peers(a, b) orders the two contexts'
+ * streams after each other's work so far (call it between stages; nothing happens when they share one stream).     */
+int clt_link_rows(clt_ctx *ctx, int side, clt_ctx *peer, int k0, int nrows, int k0_peer);
+int clt_sync_peers(clt_ctx *a, clt_ctx *b);
 
 /* NEXT-1 in the loop [L139 "the time step ... is calculated based on the latest rho, p, v, B"; Fig. 3: STEPON then
  * SETDT; Fig. 4]: n RK4 steps, each with dt = SETDT(cfl) of the state at its start.  The time step lives on the

@@ -44,7 +44,7 @@ class clt_profile(ctypes.Structure):
 # every symbol include/clt.h declares
 EXPORTS = ["clt_workspace_bytes", "clt_create", "clt_destroy", "clt_set_equilibrium", "clt_set_state", "clt_get_state",
            "clt_rhs", "clt_curl_J1", "clt_hall_G", "clt_step", "clt_step_cfl", "clt_step_stage", "clt_get_rows", "clt_set_rows",
-           "clt_set_owned_rows", "clt_set_z_spacing", "clt_push_rows", "clt_cfl_open", "clt_cfl_commit", "clt_cfl_close", "clt_set_dt", "clt_diagnostics", "clt_suggest_dt", "clt_set_tuning",
+           "clt_set_owned_rows", "clt_set_z_spacing", "clt_push_rows", "clt_link_rows", "clt_sync_peers", "clt_cfl_open", "clt_cfl_commit", "clt_cfl_close", "clt_set_dt", "clt_diagnostics", "clt_suggest_dt", "clt_set_tuning",
            "clt_set_kernel_variant", "clt_spectral_workspace_bytes", "clt_set_phi_scheme", "clt_set_profiling", "clt_get_profile", "clt_launch_count", "clt_stream", "clt_strerror", "clt_last_cuda_error", "clt_version"]
 
 LIB_TEXTBOOK_PATH = os.path.join(_HERE, "libclt_textbook.so")
@@ -106,6 +106,10 @@ def load(path=None):
         getattr(L, name).argtypes = [vp, i, i, i, vp]
     L.clt_set_owned_rows.restype = i
     L.clt_set_owned_rows.argtypes = [vp, i, i, i, i]
+    L.clt_link_rows.restype = i
+    L.clt_link_rows.argtypes = [vp, i, vp, i, i, i]
+    L.clt_sync_peers.restype = i
+    L.clt_sync_peers.argtypes = [vp, vp]
     L.clt_cfl_open.restype = i
     L.clt_cfl_open.argtypes = [vp, d]
     L.clt_cfl_commit.restype = i
@@ -266,6 +270,13 @@ class Clt:
         rc = self.L.clt_push_rows(self.h, int(buffer), int(k0), int(nrows), dst.h, int(k0_dst))
         if rc != 0:
             dst._ck(rc)
+
+    def link_rows(self, side, peer, k0=0, nrows=0, k0_peer=0):
+        """Every stage kernel also stores rows k0 .. k0+nrows-1 of its output into rows k0_peer .. of `peer` (None: unlink)."""
+        self._ck(self.L.clt_link_rows(self.h, int(side), peer.h if peer is not None else None, int(k0), int(nrows), int(k0_peer)))
+
+    def sync_peers(self, other):
+        self._ck(self.L.clt_sync_peers(self.h, other.h))
 
     def hall_G(self, out=None):
         if out is None:

@@ -32,7 +32,9 @@ struct clt_ctx {
     double *Un, *acc, *Ua, *Ub, *J1, *G, *tab, *Rtab, *invRtab, *cs, *partial, *result;
     int nblocks_diag;
     bool has_state, has_v0, hall;
-    int k_first, k_last, kd_first, kd_last;   // diagnostics row ranges (clt_set_owned_rows)
+    int k_first, k_last, kd_first, kd_last;   // owned rows / rows of max |div_c B| (clt_set_owned_rows)
+    // clt_link_rows: neighbouring slabs whose ghost rows the stage kernels of this context fill (0 = lower, 1 = upper)
+    struct { clt_ctx *peer; int k0, k1, dk; } link[2];
     bool adaptive;                 // inside clt_step_cfl: stage coefficients from the device clock
     double adaptive_cfl;
     int sm_count;                  // multiprocessors of that device (automatic phi chunking of small grids)
@@ -346,6 +348,15 @@ int run_rhs(clt_ctx *ctx, int mode, const double *in, double *out)
     a.dtmin_bits = ctx->adaptive ? (unsigned long long *)(ctx->result + 16) : nullptr;
     a.cfl = ctx->adaptive_cfl;
     a.own_k0 = ctx->k_first; a.own_k1 = ctx->k_last;
+    for (int side = 0; side < 2; ++side) {
+        clt_ctx *pc = ctx->link[side].peer;
+        double *pout = nullptr;
+        if (pc && mode != RHS_MODE_K) pout = out == ctx->Ua ? pc->Ua : (out == ctx->Ub ? pc->Ub : (out == ctx->Un ? pc->Un : nullptr));
+        a.peer[side].out = pout;
+        a.peer[side].plane = pc ? pc->L.plane : 0;
+        a.peer[side].field = pc ? pc->L.field : 0;
+        a.peer[side].k0 = ctx->link[side].k0; a.peer[side].k1 = ctx->link[side].k1; a.peer[side].dk = ctx->link[side].dk;
+    }
     const bool tma = ctx->variant == 0;
     if ((ctx->hall || ctx->spectral) && !tma) {
         snprintf(ctx->cuda_err, sizeof(ctx->cuda_err),
@@ -1018,6 +1029,58 @@ int clt_set_owned_rows(clt_ctx *ctx, int k_first, int k_last, int deep_first, in
     if (k_first < 2 || k_last > ctx->L.nZ - 3 || k_first > k_last) return CLT_EINVAL;
     if (deep_first < 2 || deep_last > ctx->L.nZ - 3) return CLT_EINVAL;      // an empty deep range is allowed
     ctx->k_first = k_first; ctx->k_last = k_last; ctx->kd_first = deep_first; ctx->kd_last = deep_last;
+    destroy_graph(ctx);          // the row range is a kernel argument of the captured step
+    return CLT_OK;
+}
+
+int clt_link_rows(clt_ctx *ctx, int side, clt_ctx *peer, int k0, int nrows, int k0_peer)
+{
+    if (!ctx || side < 0 || side > 1) return CLT_EINVAL;
+    destroy_graph(ctx);
+    if (!peer) { ctx->link[side].peer = nullptr; return CLT_OK; }
+    if (peer == ctx || nrows < 1 || k0 < ctx->k_first || k0 + nrows - 1 > ctx->k_last) return CLT_EINVAL;   // owned rows only
+    if (k0_peer < 0 || k0_peer + nrows > peer->L.nZ) return CLT_EINVAL;
+    if (peer->L.nR != ctx->L.nR || peer->L.nphi != ctx->L.nphi) return CLT_EINVAL;
+    if (peer->device != ctx->device) {
+        DeviceGuard device_guard(ctx);
+        int can = 0;
+        CK(cudaDeviceCanAccessPeer(&can, ctx->device, peer->device));
+        if (!can) { snprintf(ctx->cuda_err, sizeof(ctx->cuda_err), "clt_link_rows: no peer access between devices %d and %d", ctx->device, peer->device); return CLT_ECUDA; }
+        cudaError_t pe = cudaDeviceEnablePeerAccess(peer->device, 0);
+        if (pe != cudaSuccess && pe != cudaErrorPeerAccessAlreadyEnabled) return cuda_fail(ctx, pe, "cudaDeviceEnablePeerAccess");
+        cudaGetLastError();
+    }
+    ctx->link[side].peer = peer;
+    ctx->link[side].k0 = k0; ctx->link[side].k1 = k0 + nrows - 1; ctx->link[side].dk = k0_peer - k0;
+    return CLT_OK;
+}
+
+int clt_sync_peers(clt_ctx *a, clt_ctx *b)
+{
+    if (!a || !b) return CLT_EINVAL;
+    if (a->stream == b->stream && a->device == b->device) return CLT_OK;      // one stream: already ordered
+    clt_ctx *ctx = a;
+    cudaEvent_t ea = nullptr, eb = nullptr;
+    cudaError_t e;
+    {
+        DeviceGuard ga(a);
+        e = cudaEventCreateWithFlags(&ea, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventRecord(ea, a->stream);
+    }
+    if (e == cudaSuccess) {
+        DeviceGuard gb(b);
+        e = cudaEventCreateWithFlags(&eb, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventRecord(eb, b->stream);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(b->stream, ea, 0);
+    }
+    if (e == cudaSuccess) {
+        DeviceGuard ga(a);
+        e = cudaStreamWaitEvent(a->stream, eb, 0);
+    }
+    if (ea) cudaEventDestroy(ea);
+    if (eb) cudaEventDestroy(eb);
+    a->prof_chain = false; b->prof_chain = false;
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "clt_sync_peers");
     return CLT_OK;
 }
 

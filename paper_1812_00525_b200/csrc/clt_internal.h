@@ -66,7 +66,16 @@ struct RhsArgs {
     // adaptive stepping (clt_step_cfl): non-null = stage 4 folds the SETDT minimum of the new state into *dtmin_bits
     unsigned long long *dtmin_bits;
     double cfl;
-    int own_k0, own_k1;   // rows whose new state enters that minimum (a slab's owned rows; default 2 .. nZ-3)
+    // rows this context is responsible for (a slab's owned rows; default 2 .. nZ-3): the only rows a stage writes, and the
+    // rows whose new state enters the SETDT minimum
+    int own_k0, own_k1;
+    // NEXT-4: neighbouring slabs of the same process.  Rows k0 .. k1 of a stage's output are also stored into rows
+    // k + dk of the neighbour's buffer of the same stage (its ghost rows), straight from the epilogue.  out = nullptr: none.
+    struct Peer {
+        double *out;
+        long long plane, field;
+        int k0, k1, dk;
+    } peer[2];
 };
 
 // clocks of a group of contexts that share one adaptive time step (clt_cfl_commit)

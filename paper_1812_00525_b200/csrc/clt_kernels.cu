@@ -262,35 +262,44 @@ __device__ __forceinline__ StageCoef load_stage_coef(const RhsArgs &a)
 }
 template <int MODE>
 __device__ __forceinline__ void epilogue_store(const RhsArgs &a, long long g, long long field, const EpiOperands &e,
-                                               const double (&K)[8], double iR, double &rate, const StageCoef &sc, bool collect)
+                                               const double (&K)[8], double iR, double &rate, const StageCoef &sc, bool collect,
+                                               double *peer0 = nullptr, double *peer1 = nullptr)
 {
     constexpr double third = 1.0 / 3.0;
     const double an = sc.an, bn = sc.bn;
     double out[8];
+    // the stage's output at this node; peer0 / peer1: the same node in a neighbouring slab's buffer (its ghost row), or null
+    auto put = [&](int m, double v) {
+        st_out(a.out + m * field + g, v);
+        if (MODE != RHS_MODE_K) {
+            if (peer0) st_out(peer0 + m * a.peer[0].field, v);
+            if (peer1) st_out(peer1 + m * a.peer[1].field, v);
+        }
+    };
 #pragma unroll
     for (int m = 0; m < 8; ++m) {
         const long long gm = m * field + g;
         if (MODE == RHS_MODE_K) {
-            st_out(a.out + gm, K[m]);
+            put(m, K[m]);
         } else if (TEXTBOOK_RK4) {
             if (MODE == RHS_MODE_S1) {
-                st_out(a.out + gm, fma(an, K[m], e.un[m]));
+                put(m, fma(an, K[m], e.un[m]));
                 st_out(a.acc + gm, bn * K[m]);
             } else if (MODE == RHS_MODE_S2 || MODE == RHS_MODE_S3) {
-                st_out(a.out + gm, fma(an, K[m], e.un[m]));
+                put(m, fma(an, K[m], e.un[m]));
                 st_out(a.acc + gm, fma(bn, K[m], e.ac[m]));
             } else {
                 out[m] = e.un[m] + fma(bn, K[m], e.ac[m]);
-                st_out(a.out + gm, out[m]);
+                put(m, out[m]);
             }
         } else if (MODE == RHS_MODE_S1 || MODE == RHS_MODE_S3) {
-            st_out(a.out + gm, fma(an, K[m], e.un[m]));
+            put(m, fma(an, K[m], e.un[m]));
         } else if (MODE == RHS_MODE_S2) {
-            st_out(a.out + gm, fma(an, K[m], e.un[m]));
+            put(m, fma(an, K[m], e.un[m]));
             st_out(a.acc + gm, fma(bn, K[m], (e.us[m] - e.un[m]) * third));
         } else {
             out[m] = e.un[m] + fma(bn, K[m], fma(e.us[m] - e.un[m], third, e.ac[m]));
-            st_out(a.out + gm, out[m]);
+            put(m, out[m]);
         }
     }
     if (MODE == RHS_MODE_S4 && a.dtmin_bits && collect) {
@@ -306,6 +315,14 @@ __device__ __forceinline__ void epilogue_store(const RhsArgs &a, long long g, lo
         // dt = 0, which dt_commit_kernel turns into the clock's non-finite mark and clt_step_cfl into CLT_ENONFINITE.
         if (!(rR + rP + rZ <= 1.79769313486231570815e308)) rate = __longlong_as_double(0x7ff0000000000000LL);
     }
+}
+
+// the node (i, k, plane j) in the buffer of neighbouring slab `side`, if row k is one of the rows it takes from us
+__device__ __forceinline__ double *peer_node(const RhsArgs &a, int side, int i, int k, int j, int pR)
+{
+    const RhsArgs::Peer &p = a.peer[side];
+    if (!p.out || k < p.k0 || k > p.k1) return nullptr;
+    return p.out + (long long)j * p.plane + (long long)(k + p.dk) * pR + (LP + i);
 }
 
 // end of a stage-4 kernel: this thread's largest signal rate -> its SETDT value -> device-wide minimum (positive doubles
@@ -401,7 +418,8 @@ __global__ void __launch_bounds__(TR *TZ, 1) rhs_kernel(const __grid_constant__ 
     const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * TR + tx;
     const int i0 = 2 + TR * blockIdx.x, k0 = 2 + TZ * blockIdx.y;
     const int i = i0 + tx, k = k0 + ty;
-    const bool valid = (i <= L.nR - 3) && (k <= L.nZ - 3);
+    // a stage writes the context's owned rows only (clt_rhs: every interior row)
+    const bool valid = (i <= L.nR - 3) && (k <= L.nZ - 3) && (MODE == RHS_MODE_K || (k >= a.own_k0 && k <= a.own_k1));
     const int ic = min(i, L.nR - 1), kc = min(k, L.nZ - 1);
     const int ja = (int)(((long long)L.nphi * blockIdx.z) / a.phi_chunks);
     const int jb = (int)(((long long)L.nphi * (blockIdx.z + 1)) / a.phi_chunks);
@@ -563,7 +581,7 @@ __global__ void __launch_bounds__(TR *TZ, 1) rhs_kernel(const __grid_constant__ 
             EpiOperands eo;
             // plain coherent loads: stage 4 updates U^n in place through a.out, so the non-coherent path is not allowed here
             epilogue_load<MODE, 0>(a, g, L.field, eo, [](const double *p) { return *p; });
-            epilogue_store<MODE>(a, g, L.field, eo, K, iR, rate, coef, k >= a.own_k0 && k <= a.own_k1);
+            epilogue_store<MODE>(a, g, L.field, eo, K, iR, rate, coef, true, peer_node(a, 0, i, k, j, L.pR), peer_node(a, 1, i, k, j, L.pR));
         }
         advance();
     }
@@ -712,7 +730,8 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
     const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * TR + tx;
     const int i0 = 2 + TR * blockIdx.x, k0 = 2 + TZ * blockIdx.y;
     const int i = i0 + tx, k = k0 + ty;
-    const bool valid = (i <= L.nR - 3) && (k <= L.nZ - 3);
+    // a stage writes the context's owned rows only (clt_rhs: every interior row)
+    const bool valid = (i <= L.nR - 3) && (k <= L.nZ - 3) && (MODE == RHS_MODE_K || (k >= a.own_k0 && k <= a.own_k1));
     const int ic = min(i, L.nR - 1), kc = min(k, L.nZ - 1);
     const int ja = (int)(((long long)L.nphi * blockIdx.z) / a.phi_chunks);
     const int jb = (int)(((long long)L.nphi * (blockIdx.z + 1)) / a.phi_chunks);
@@ -933,7 +952,7 @@ rhs_tma_kernel(const __grid_constant__ RhsArgs a, const __grid_constant__ CUtens
                             }, pd1, pd2);
 
         // ---- a6: RK4 stage combine in the epilogue (L125, L139) --------------------------------
-        if (valid) epilogue_store<MODE>(a, g, L.field, eo, K, iR, rate, coef, k >= a.own_k0 && k <= a.own_k1);
+        if (valid) epilogue_store<MODE>(a, g, L.field, eo, K, iR, rate, coef, true, peer_node(a, 0, i, k, j, L.pR), peer_node(a, 1, i, k, j, L.pR));
         advance();
     }
     if (MODE == RHS_MODE_S4) dtmin_commit(a, rate);

@@ -6,8 +6,9 @@ along Z (R is the contiguous axis of the layout, so a ghost block is whole rows)
 [a_r, b_r) of the global grid and runs an ordinary libclt context on the rows [z0, z0 + nZ_local) = its owned rows
 plus GHOST = 4 rows per cut (or the two frozen boundary rows at the outer edges).  The kernels are unchanged: they
 never write the two outer rows of a context, they recompute rows 2-3 next to a cut from the ghost data (those values
-are discarded), and after every RK stage all 4 ghost rows of the stage's output buffer are overwritten with the
-neighbour's freshly computed owned rows.  Four exchanges of 4 rows x 8 fields per cut and step.
+are discarded), and after every RK stage all 4 ghost rows of the stage's output buffer hold the neighbour's freshly
+computed owned rows: slabs of one process get them written by the neighbour's stage kernel itself (clt_link_rows: peer
+stores from the RK4 epilogue), slabs of different processes by four exchanges of 4 rows x 8 fields per cut and step.
 
 Host logic only (argument marshalling, partition arithmetic, exchange order); every number is computed by the CUDA
 kernels behind ``clt.Clt``.  Two drivers over the same code:
@@ -167,20 +168,31 @@ class SlabGroup:
     """All slabs of a run that live in THIS process: every rank (in-process driver) or this rank's one slab
     (torch.distributed driver, `dist` = the initialised torch.distributed module)."""
 
-    def __init__(self, cfg, dt, U0, U, world, devices=("cuda:0",), dist=None, **kw):
+    def __init__(self, cfg, dt, U0, U, world, devices=("cuda:0",), dist=None, fused_exchange=True, **kw):
         self.cfg, self.world, self.dist = cfg, world, dist
         if dist is None:
             self.slabs = [Slab(cfg, dt, U0, U, r, world, device=devices[r % len(devices)], **kw) for r in range(world)]
         else:
             self.slabs = [Slab(cfg, dt, U0, U, dist.get_rank(), world, device=devices[0], **kw)]
         self.extents = [s.ext for s in self.slabs]
+        # slabs of one process: the stage kernels store the rows a neighbour needs straight into its ghost rows
+        # (clt_link_rows: compute and exchange in one kernel); fused_exchange=False keeps the separate clt_push_rows kernels
+        self.linked = dist is None and fused_exchange
+        if self.linked:
+            for lo, hi in zip(self.slabs[:-1], self.slabs[1:]):
+                lo.g.link_rows(1, hi.g, *lo.ext.send_up(), hi.ext.recv_from_lower()[0])
+                hi.g.link_rows(0, lo.g, *hi.ext.send_down(), lo.ext.recv_from_upper()[0])
 
     def step(self, n=1):
         for _ in range(n):
             for stage in (1, 2, 3, 4):
                 for s in self.slabs:
                     s.g.step_stage(stage)
-                exchange(self.slabs, self.extents, STAGE_BUFFER[stage], self.dist, _make_buffer)
+                if self.linked:
+                    for lo, hi in zip(self.slabs[:-1], self.slabs[1:]):
+                        lo.g.sync_peers(hi.g)          # stream order only (nothing to do on a shared stream)
+                else:
+                    exchange(self.slabs, self.extents, STAGE_BUFFER[stage], self.dist, _make_buffer)
 
     def step_cfl(self, n=1, cfl=0.0):
         """n adaptive RK4 steps (Fig. 3-4): every step runs with the global SETDT minimum of the state at
@@ -251,5 +263,9 @@ class SlabGroup:
         return U
 
     def close(self):
+        if self.linked:
+            for s in self.slabs:                  # no dangling peer pointers while contexts go away one by one
+                s.g.link_rows(0, None)
+                s.g.link_rows(1, None)
         for s in self.slabs:
             s.g.close()

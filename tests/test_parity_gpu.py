@@ -387,18 +387,21 @@ def _single(prob, **over):
 
 
 @pytest.mark.parametrize("world", [2, 3])
-@pytest.mark.parametrize("variant", ["fd", "hall", "spectral"])
+@pytest.mark.parametrize("variant", ["fd", "hall", "spectral", "fd-push-rows"])
 def test_slab_decomposition_matches_single_domain_and_oracle(world, variant):
     """Several sub-domain contexts in ONE process on one GPU (run one after the other, ghost rows pushed from buffer to
     buffer by clt_push_rows): the SAME BITS as the undivided run (a slab carries the global dZ, clt_set_z_spacing) and
     the oracle's state within the step tolerance."""
     from paper_1812_00525_b200 import slab
+    # default: ghost rows written by the neighbour's stage kernels (clt_link_rows); "fd-push-rows": by clt_push_rows kernels
+    fused = variant != "fd-push-rows"
+    variant = variant.split("-")[0]
     prob = inputs.make_custom_problem(45, 8, 41, index=21, rotation=0.05 if variant == "fd" else 0.0,
                                       poloidal=(0.03, -0.02) if variant != "spectral" else None)
     kw = {"fd": {}, "hall": dict(d_i=0.03), "spectral": dict(phi_scheme=1)}[variant]
     dt = prob.dt * (0.2 if variant == "hall" else 0.5)
     steps = 12
-    grp = slab.SlabGroup(prob.cfg, dt, prob.U0, prob.U, world, **kw)
+    grp = slab.SlabGroup(prob.cfg, dt, prob.U0, prob.U, world, fused_exchange=fused, **kw)
     g = _single(prob, dt=dt, **kw)
     o = make_oracle(prob, dt=dt, **kw)
     d0 = grp.diagnostics()
