@@ -358,6 +358,12 @@ int run_rhs(clt_ctx *ctx, int mode, const double *in, double *out)
         a.peer[side].k0 = ctx->link[side].k0; a.peer[side].k1 = ctx->link[side].k1; a.peer[side].dk = ctx->link[side].dk;
     }
     const bool tma = ctx->variant == 0;
+    const bool linked = ctx->link[0].peer || ctx->link[1].peer;
+    const bool slab = linked || ctx->k_first != 2 || ctx->k_last != ctx->L.nZ - 3;
+    if (linked && !tma) {
+        snprintf(ctx->cuda_err, sizeof(ctx->cuda_err), "linked slabs (clt_link_rows) need the default kernel variant");
+        return CLT_EINVAL;
+    }
     if ((ctx->hall || ctx->spectral) && !tma) {
         snprintf(ctx->cuda_err, sizeof(ctx->cuda_err),
                  "the Hall term and the pseudo-spectral phi scheme need the default kernel variant");
@@ -378,7 +384,7 @@ int run_rhs(clt_ctx *ctx, int mode, const double *in, double *out)
     }
     const long pe = prof_begin(ctx, mode);
     if (tma)
-        CK(launch_rhs_tma(a, &tmU, &tmJ, &tmV, mode, ctx->has_v0, ctx->hall, ctx->spectral, ctx->stream));
+        CK(launch_rhs_tma(a, &tmU, &tmJ, &tmV, mode, ctx->has_v0, ctx->hall, ctx->spectral, slab, ctx->stream));
     else
         CK(launch_rhs(a, mode, ctx->has_v0, ctx->stream));
     prof_end(ctx, pe);

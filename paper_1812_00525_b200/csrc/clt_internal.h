@@ -159,8 +159,9 @@ cudaError_t launch_rhs(const RhsArgs &a, int mode, bool has_v0, cudaStream_t s, 
 // that span the field axis.  Moving reference state (has_v0) or pseudo-spectral scheme: tmU over the stage state with nf = 8,
 // tmV unused.  Static reference state with finite differences: tmU with nf = 2 (rho, p), tmV with nf = 3 (v at field 2, B at field 5).  tmJ over J1 with nf = 3
 // (hall: 6 fields, J1 then G; the kernel adds d_i * G to E1).
+// slab: the context is a slab (owned rows set and / or neighbours linked, RhsArgs::own_k0 .. peer)
 cudaError_t launch_rhs_tma(const RhsArgs &a, const void *tmU, const void *tmJ, const void *tmV, int mode, bool has_v0, bool hall,
-                           bool spec, cudaStream_t s, bool configure = false);
+                           bool spec, bool slab, cudaStream_t s, bool configure = false);
 // TMA variant of the curl kernel: tmU is a CUtensorMap over the 8 fields of the stage state with box
 // (TR+4, curl_tma_tile_z()+4, 1, 1); hall = also write the Hall field G
 cudaError_t launch_curl_tma(const CurlArgs &a, const void *tmU, bool hall, bool spec, cudaStream_t s, bool configure = false);
