@@ -691,7 +691,7 @@ struct RhsTmaSmem {
     static constexpr int NH = 4 * TR + 4 * TZ;
     static constexpr int HTP = (HT + 15) / 16 * 16;   // every TMA destination 128-byte aligned
     static constexpr int NFR = VR ? NF - 3 : NF;      // fields per raw buffer
-    static constexpr int NV = VR ? 5 : 1;             // slots of the velocity ring
+    static constexpr int NV = VR ? NRAW + 3 : 1;      // slots of the velocity ring: planes j .. j+2 in use + NRAW in flight
     static constexpr int NS = VR ? 2 : 5;             // fields of sring
     // TMA destinations of one plane, tile with halo.  VR: rho, p, B (3), J1 (3) [, G (3)]; else U (8), J1 (3) [, G (3)]
     alignas(128) double raw[NRAW][NFR][HTP];
@@ -970,7 +970,10 @@ template <int MODE, bool V0, bool HALL, bool SPEC, bool SLAB>
 static cudaError_t launch_rhs_tma_t(const RhsArgs &a, const CUtensorMap &tmU, const CUtensorMap &tmJ, const CUtensorMap &tmV,
                                     cudaStream_t s, bool configure)
 {
-    constexpr int TZ = RHS_TZ, NRAW = 2;
+    // raw buffers (planes in flight): two; three in stage 1 where the shared memory is there (velocity ring, no Hall
+    // field).  Measured at 512x64x512: stage 1 (latency-bound, its prologue waits for every plane) 0.555 -> 0.540 ms with
+    // three, the HBM-bound stages 2 and 4 +2 % and +4 % slower, stage 3 unchanged.
+    constexpr int TZ = RHS_TZ, NRAW = (MODE == RHS_MODE_S1 && rhs_velocity_ring(V0, SPEC) && !HALL) ? 3 : 2;
     auto kern = rhs_tma_kernel<TZ, NRAW, MODE, V0, HALL, SPEC, SLAB>;
     using SM = RhsTmaSmem<TZ, NRAW, HALL ? 14 : 11, rhs_velocity_ring(V0, SPEC)>;
     const int smem = (int)sizeof(SM);
