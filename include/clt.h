@@ -193,7 +193,8 @@ int clt_push_rows(clt_ctx *src, int buffer, int k0_src, int nrows, clt_ctx *dst,
  * side = 0 (lower neighbour) or 1 (upper); peer = NULL removes the link.  A stage writes a context's owned rows only
  * (clt_set_owned_rows, to be called first), so the peer's own kernels never touch its ghost rows.  Same nR and nphi;
  * contexts on different devices need peer access (CLT_ECUDA otherwise).  clt_sync_peers(a, b) orders the two contexts'
- * streams after each other's work so far (call it between stages; nothing happens when they share one stream).     */
+ * streams after each other's work so far (call it between stages; nothing happens when they share one stream).  A
+ * link holds a pointer into the peer's workspace: remove it before the peer is destroyed.                          */
 int clt_link_rows(clt_ctx *ctx, int side, clt_ctx *peer, int k0, int nrows, int k0_peer);
 int clt_sync_peers(clt_ctx *a, clt_ctx *b);
 
