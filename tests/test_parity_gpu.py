@@ -424,6 +424,43 @@ def test_slab_decomposition_matches_single_domain_and_oracle(world, variant):
     grp.close()
 
 
+def test_thin_slabs_whose_rows_go_to_both_neighbours():
+    """Slabs of exactly 4 owned rows: every owned row is a ghost row of BOTH neighbours (two peer stores per node)."""
+    from paper_1812_00525_b200 import slab
+    prob = inputs.make_custom_problem(40, 6, 17, index=26, amplitude_scale=50.0)      # 13 interior rows -> 5 + 4 + 4
+    g = make_gpu(prob)
+    g.step(6)
+    for fused in (True, False):
+        grp = slab.SlabGroup(prob.cfg, prob.dt, prob.U0, prob.U, 3, fused_exchange=fused)
+        assert [e.b - e.a for e in grp.extents] == [5, 4, 4]
+        grp.step(6)
+        assert np.array_equal(grp.get_state(), g.get_state()), f"fused_exchange={fused}"
+        grp.close()
+
+
+def test_owned_rows_limit_what_a_stage_writes():
+    """clt_set_owned_rows: a stage writes the owned rows only (the slab instantiation of the fused kernel), on the
+    CUDA-graph path as well as stage by stage; the default range is every interior row."""
+    prob = inputs.make_custom_problem(40, 6, 30, index=27, amplitude_scale=50.0)
+    nZ = prob.cfg.nZ
+    a, b = make_gpu(prob), make_gpu(prob)
+    for g in (a, b):
+        g.set_owned_rows(6, nZ - 9, 6, nZ - 9)
+    a.step(2)                                   # CUDA graph
+    b.set_tuning(use_graph=2)
+    b.step(2)
+    Ua, Ub = a.get_state(), b.get_state()
+    assert np.array_equal(Ua, Ub)
+    assert np.array_equal(Ua[:, :, :6], prob.U[:, :, :6]) and np.array_equal(Ua[:, :, nZ - 8:], prob.U[:, :, nZ - 8:])
+    assert np.abs(Ua[:, :, 6:nZ - 8] - prob.U[:, :, 6:nZ - 8]).max() > 1e-7
+    a.set_owned_rows(2, nZ - 3, 4, nZ - 5)      # back to the default: the captured step is rebuilt
+    ref = make_gpu(prob)
+    a.set_state(np.ascontiguousarray(prob.U))
+    a.step(2)
+    ref.step(2)
+    assert np.array_equal(a.get_state(), ref.get_state())
+
+
 def test_push_rows_and_z_spacing():
     """clt_push_rows = clt_get_rows + clt_set_rows without the dense staging array; clt_set_z_spacing replaces the
     spacing in every weight (a context built with a wrong Z extent and the right dZ reproduces the reference bits)."""
