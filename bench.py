@@ -193,8 +193,8 @@ def run_reference(args):
 
 def run_slabs(args):
     """NEXT-4 measurement: the same workload cut into Z-slabs (paper_1812_00525_b200/slab.py).  --slabs K with one
-    process = K sub-domain contexts on ONE GPU run one after the other (measures the cost of the decomposition itself:
-    redundant ghost-row work + pack/unpack, no link); under torchrun (--gpus N > 1) = one slab per rank, strong scaling,
+    process = K sub-domain contexts on ONE GPU, a stream each (measures the cost of the decomposition itself:
+    redundant ghost-row work, no link); under torchrun (--gpus N > 1) = one slab per rank, strong scaling,
     ghost rows over NCCL.  Not the contract's default (north_star: replicas only)."""
     import torch
     import torch.distributed as dist
@@ -219,8 +219,10 @@ def run_slabs(args):
     replicas.barrier(f"cuda:{local}")
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     stream = grp.slabs[0].g.torch_stream
+    grp.join()
     e0.record(stream)
     grp.step(args.steps)
+    grp.join()               # in-process slabs run on a stream each: the first one's waits for the others
     e1.record(stream)
     replicas.barrier(f"cuda:{local}")
     ms = e0.elapsed_time(e1)

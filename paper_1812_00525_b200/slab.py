@@ -118,7 +118,7 @@ def exchange(backends, extents, buffer, dist=None, make_buffer=None):
 class Slab:
     """One sub-domain: a libclt context on the rows of `Extent`, built from the GLOBAL arrays."""
 
-    def __init__(self, cfg, dt, U0, U, rank, world, device="cuda:0", d_i=0.0, phi_scheme=0):
+    def __init__(self, cfg, dt, U0, U, rank, world, device="cuda:0", d_i=0.0, phi_scheme=0, stream=None):
         import torch
         from . import clt
         self.ext = ex = Extent(cfg.nZ, world, rank)
@@ -126,7 +126,7 @@ class Slab:
         Zmin = cfg.Zmin + ex.z0 * dZ
         Zmax = cfg.Zmin + (ex.z1 - 1) * dZ
         self.g = clt.Clt(cfg.nR, cfg.nphi, ex.nZ_local, cfg.Rmin, cfg.Rmax, Zmin, Zmax, cfg.phi_extent, cfg.gamma, cfg.eta,
-                         cfg.nu, cfg.D, cfg.kappa, dt, cfg.cfl, d_i=d_i, device=device)
+                         cfg.nu, cfg.D, cfg.kappa, dt, cfg.cfl, d_i=d_i, device=device, stream=stream)
         self.g.set_z_spacing(dZ)      # the global spacing itself, not (Zmax - Zmin)/(nZ_local - 1): slabs == undivided run, bit for bit
         if phi_scheme:
             self.g.set_phi_scheme(phi_scheme)
@@ -171,7 +171,12 @@ class SlabGroup:
     def __init__(self, cfg, dt, U0, U, world, devices=("cuda:0",), dist=None, fused_exchange=True, **kw):
         self.cfg, self.world, self.dist = cfg, world, dist
         if dist is None:
-            self.slabs = [Slab(cfg, dt, U0, U, r, world, device=devices[r % len(devices)], **kw) for r in range(world)]
+            # linked slabs get a stream each: the stage kernels of different slabs are independent of each other (the
+            # neighbours' streams are ordered between stages, clt_sync_peers), so on a shared GPU the last, partly filled
+            # wave of one slab's kernel is topped up by the next slab's
+            import torch
+            streams = [torch.cuda.Stream(devices[r % len(devices)]) if fused_exchange and world > 1 else None for r in range(world)]
+            self.slabs = [Slab(cfg, dt, U0, U, r, world, device=devices[r % len(devices)], stream=streams[r], **kw) for r in range(world)]
         else:
             self.slabs = [Slab(cfg, dt, U0, U, dist.get_rank(), world, device=devices[0], **kw)]
         self.extents = [s.ext for s in self.slabs]
@@ -182,6 +187,7 @@ class SlabGroup:
             for lo, hi in zip(self.slabs[:-1], self.slabs[1:]):
                 lo.g.link_rows(1, hi.g, *lo.ext.send_up(), hi.ext.recv_from_lower()[0])
                 hi.g.link_rows(0, lo.g, *hi.ext.send_down(), lo.ext.recv_from_upper()[0])
+                lo.g.sync_peers(hi.g)             # the neighbour's set-up is complete before anything is stored into its rows
 
     def step(self, n=1):
         for _ in range(n):
@@ -261,6 +267,11 @@ class SlabGroup:
         for lo, block in pieces:
             U[:, :, lo:lo + block.shape[2]] = block
         return U
+
+    def join(self):
+        """Orders the first slab's stream after everything enqueued on the others' (for timing events on that stream)."""
+        for s in self.slabs[1:]:
+            self.slabs[0].g.sync_peers(s.g)
 
     def close(self):
         if self.linked:
