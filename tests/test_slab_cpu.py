@@ -39,6 +39,13 @@ class FakeSlab:
         self.buf[buffer][:, :, k0:k0 + n] = src
 
 
+class FakePushSlab(FakeSlab):
+    """The same stand-in with the direct hand-over of clt_push_rows (rows of one buffer straight into another slab's)."""
+
+    def push_rows(self, buffer, k0, n, dst, k0_dst):
+        dst.buf[buffer][:, :, k0_dst:k0_dst + n] = self.buf[buffer][:, :, k0:k0 + n]
+
+
 def _truth(nZ):
     def f(b):
         g = torch.arange(nZ, dtype=torch.float64).view(1, 1, nZ, 1)
@@ -103,6 +110,37 @@ def test_exchange_in_process(world):
         for f in fakes:
             _check(f, truth, buffer)
     assert slab.STAGE_BUFFER == {1: 1, 2: 2, 3: 1, 4: 0}
+
+
+@pytest.mark.parametrize("world", [2, 3, 4])
+def test_exchange_in_process_by_direct_push(world):
+    """slab.exchange hands ghost rows over through push_rows when the backend has it (the CUDA context does): same
+    row arithmetic, no staging buffers (make_buffer must not be called)."""
+    nZ = 37
+    truth = _truth(nZ)
+    exts = [slab.Extent(nZ, world, r) for r in range(world)]
+    fakes = [FakePushSlab(e, truth) for e in exts]
+
+    def no_buffers(_slab, _n):
+        raise AssertionError("the push_rows path allocates no staging buffer")
+
+    for buffer in (1, 2, 0):
+        slab.exchange(fakes, exts, buffer, None, no_buffers)
+        for f in fakes:
+            _check(f, truth, buffer)
+
+
+def test_thin_slabs_send_all_their_rows_both_ways():
+    nZ, world = 4 + 12, 3                      # 12 interior rows -> three slabs of exactly GHOST rows
+    exts = [slab.Extent(nZ, world, r) for r in range(world)]
+    assert [e.b - e.a for e in exts] == [slab.GHOST] * 3
+    mid = exts[1]
+    assert mid.send_down() == mid.send_up() == (slab.GHOST, slab.GHOST)      # the same four rows go to both neighbours
+    truth = _truth(nZ)
+    fakes = [FakePushSlab(e, truth) for e in exts]
+    slab.exchange(fakes, exts, 1, None, _mk)
+    for f in fakes:
+        _check(f, truth, 1)
 
 
 def _free_port():
