@@ -217,6 +217,19 @@ int clt_set_dt(clt_ctx *ctx, double dt);
  * finite (out is still filled).                                                                  */
 int clt_diagnostics(clt_ctx *ctx, clt_diag *out);
 
+/* The same reductions for callers that cannot allocate or synchronise (code under CUDA graph capture, tight serving
+ * loops): the ONE entry point of the library that uses no memory but its own.  The block partials of the reduction go
+ * to a file-scope device array inside the library instead of the caller's workspace (768 KiB = 16384 reduction CTAs
+ * x 6 doubles, held by every GPU that loads the library until the process exits); the call allocates nothing, copies
+ * nothing to the host and does not synchronise.
+ *   d_out6 : DEVICE pointer to 6 doubles, written on the context's stream:
+ *            { kinetic, magnetic, magnetic_pert, magnetic_n1, max |div_c B|, SETDT(cfl) }  (cfl <= 0: params.cfl, else 0.5)
+ * Limit: grids with more than 16384 reduction CTAs, ceil((nR-4)/32) * (nZ-4) > 16384, are refused with CLT_ENOMEM and a
+ * text in clt_last_cuda_error (512 x 64 x 512 needs 8128).  CLT_EINVAL if d_out6 is not device memory.
+ * Every call on a device shares the array: calls that overlap on the GPU (contexts on different streams) race; calls
+ * on one stream are safe.  Nothing in the array has to be zero and nothing a previous call left there is read.       */
+int clt_diagnostics_static(clt_ctx *ctx, double cfl, double *d_out6);
+
 /* SETDT of Fig. 4 [L180-215]: dt = min(100, min over interior nodes of min(dR/(|v_R|+c),
  * dZ/(|v_Z|+c), R dphi/(|v_phi|+c)) * cfl), c = sqrt(|Gamma p/rho + |B|^2/rho|).  cfl <= 0 means
  * params.cfl.  Synchronises the stream.  Does not change the context's dt.                        */

@@ -44,7 +44,7 @@ class clt_profile(ctypes.Structure):
 # every symbol include/clt.h declares
 EXPORTS = ["clt_workspace_bytes", "clt_create", "clt_destroy", "clt_set_equilibrium", "clt_set_state", "clt_get_state",
            "clt_rhs", "clt_curl_J1", "clt_hall_G", "clt_step", "clt_step_cfl", "clt_step_stage", "clt_get_rows", "clt_set_rows",
-           "clt_set_owned_rows", "clt_set_z_spacing", "clt_push_rows", "clt_link_rows", "clt_sync_peers", "clt_cfl_open", "clt_cfl_commit", "clt_cfl_close", "clt_set_dt", "clt_diagnostics", "clt_suggest_dt", "clt_set_tuning",
+           "clt_set_owned_rows", "clt_diagnostics_static", "clt_set_z_spacing", "clt_push_rows", "clt_link_rows", "clt_sync_peers", "clt_cfl_open", "clt_cfl_commit", "clt_cfl_close", "clt_set_dt", "clt_diagnostics", "clt_suggest_dt", "clt_set_tuning",
            "clt_set_kernel_variant", "clt_spectral_workspace_bytes", "clt_set_phi_scheme", "clt_set_profiling", "clt_get_profile", "clt_launch_count", "clt_stream", "clt_strerror", "clt_last_cuda_error", "clt_version"]
 
 LIB_TEXTBOOK_PATH = os.path.join(_HERE, "libclt_textbook.so")
@@ -87,6 +87,8 @@ def load(path=None):
     L.clt_set_dt.argtypes = [vp, d]
     L.clt_diagnostics.restype = i
     L.clt_diagnostics.argtypes = [vp, ctypes.POINTER(clt_diag)]
+    L.clt_diagnostics_static.restype = i
+    L.clt_diagnostics_static.argtypes = [vp, d, vp]
     L.clt_suggest_dt.restype = i
     L.clt_suggest_dt.argtypes = [vp, d, ctypes.POINTER(d)]
     L.clt_set_tuning.restype = i
@@ -294,6 +296,12 @@ class Clt:
         d = clt_diag()
         self._ck(self.L.clt_diagnostics(self.h, ctypes.byref(d)))
         return {k: getattr(d, k) for k, _ in clt_diag._fields_}
+
+    def diagnostics_static(self, out, cfl=0.0):
+        """clt_diagnostics_static: the reductions with the library's static scratch (no allocation, no synchronisation).
+        out: CUDA tensor of >= 6 float64: kinetic, magnetic, magnetic_pert, magnetic_n1, max_divB, SETDT(cfl)."""
+        self._ck(self.L.clt_diagnostics_static(self.h, float(cfl), _addr(out)))
+        return out
 
     def suggest_dt(self, cfl=0.0):
         out = ctypes.c_double()

@@ -31,6 +31,8 @@ struct clt_ctx {
     // workspace carving (device)
     double *Un, *acc, *Ua, *Ub, *J1, *G, *tab, *Rtab, *invRtab, *cs, *partial, *result;
     int nblocks_diag;
+    double *static_partial;        // clt_diagnostics_static: this device's address of the library's static scratch array
+    int static_max_blocks;         // ... and how many reduction CTAs it holds
     bool has_state, has_v0, hall;
     int k_first, k_last, kd_first, kd_last;   // owned rows / rows of max |div_c B| (clt_set_owned_rows)
     // clt_link_rows: neighbouring slabs whose ghost rows the stage kernels of this context fill (0 = lower, 1 = upper)
@@ -547,6 +549,7 @@ int clt_create(const clt_grid *grid, const clt_params *params, void *d_workspace
         if ((e = cudaMemcpyAsync(ctx->cs, cs.data(), cs.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream))) break;
         if ((e = cudaStreamSynchronize(ctx->stream))) break;     // the host vectors go out of scope
         if ((e = configure_kernels())) break;                    // shared-memory opt-in of this context's device
+        if ((e = diag_static_scratch(&ctx->static_partial, &ctx->static_max_blocks))) break;   // symbol address on this device
         if ((e = cudaHostAlloc((void **)&ctx->v0_flag_host, sizeof(int), cudaHostAllocDefault))) break;
         if ((e = cudaEventCreateWithFlags(&ctx->v0_event, cudaEventDisableTiming))) break;
         if ((e = launch_tables(ctx->L, ctx->ph, ctx->tab, ctx->Rtab + LP, ctx->invRtab + LP, ctx->stream))) break;
@@ -785,6 +788,41 @@ int clt_diagnostics(clt_ctx *ctx, clt_diag *out)
     out->time = ctx->time;
     for (int q = 0; q < 5; ++q)
         if (!isfinite(r6[q])) return CLT_ENONFINITE;
+    return CLT_OK;
+}
+
+// The diagnostics reduction with NO memory but the library's own: block partials in the static device array
+// (clt_kernels.cu), results to the caller's device pointer, nothing allocated, nothing copied to the host, no synchronisation.
+int clt_diagnostics_static(clt_ctx *ctx, double cfl, double *d_out6)
+{
+    DeviceGuard device_guard(ctx);
+    if (!ctx || !d_out6) return CLT_EINVAL;
+    if (!(cfl > 0.0)) cfl = ctx->par.cfl > 0 ? ctx->par.cfl : 0.5;
+    if (!isfinite(cfl)) return CLT_EINVAL;
+    // the column kernel (pseudo-spectral scheme) has the most CTAs: one per 32 R nodes and Z row
+    const int need = diag_blocks(ctx->L);
+    if (need > ctx->static_max_blocks || !ctx->static_partial) {
+        snprintf(ctx->cuda_err, sizeof(ctx->cuda_err),
+                 "clt_diagnostics_static: this grid needs %d block partials, the static scratch holds %d (use clt_diagnostics)",
+                 need, ctx->static_max_blocks);
+        return CLT_ENOMEM;
+    }
+    if (!ctx->has_state) return CLT_ESTATE;
+    cudaPointerAttributes at;
+    cudaError_t pe = cudaPointerGetAttributes(&at, d_out6);
+    if (pe != cudaSuccess) { cudaGetLastError(); return CLT_EINVAL; }
+    if (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeManaged) return CLT_EINVAL;
+    DiagArgs a;
+    a.L = ctx->L; a.ph = ctx->ph;
+    a.U = ctx->Un; a.tab = ctx->tab;
+    a.R = ctx->Rtab + LP; a.invR = ctx->invRtab + LP;
+    a.cs = ctx->cs; a.partial = ctx->static_partial; a.cfl = cfl; a.ihZ = 1.0 / ctx->ph.dZ;
+    a.spec_c1 = ctx->spectral ? ctx->spec_ctab : nullptr;
+    a.k_first = ctx->k_first; a.k_last = ctx->k_last; a.kd_first = ctx->kd_first; a.kd_last = ctx->kd_last;
+    alignas(64) CUtensorMap tmU;
+    const bool tma = ctx->variant == 0 && !ctx->spectral && make_map(ctx, ctx->Un, 8, diag_tma_tile_z(), &tmU, 8);
+    CK(launch_diag(a, need, d_out6, ctx->stream, tma ? &tmU : nullptr));
+    ctx->launches += 2;
     return CLT_OK;
 }
 

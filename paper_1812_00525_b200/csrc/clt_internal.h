@@ -174,5 +174,7 @@ cudaError_t launch_diag(const DiagArgs &a, int nblocks, double *result6, cudaStr
 int diag_tma_tile_z();
 int diag_blocks(const Layout &L);
 cudaError_t configure_kernels();
+// device address (on the current device) and capacity, in reduction CTAs, of the static scratch of clt_diagnostics_static
+cudaError_t diag_static_scratch(double **ptr, int *max_blocks);
 
 }  // namespace clt

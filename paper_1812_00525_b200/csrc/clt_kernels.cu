@@ -2103,6 +2103,30 @@ cudaError_t launch_diag(const DiagArgs &a, int nblocks, double *result6, cudaStr
     return cudaGetLastError();
 }
 
+// ---------------------------------------------------------------------------------------------
+// clt_diagnostics_static: the block partials of the diagnostics reduction in a file-scope device array instead of the
+// caller's workspace -- an entry point that needs no scratch from anybody (callers that cannot allocate: code under
+// CUDA graph capture, tight serving loops).  DIAG_STATIC_MAX_BLOCKS x 6 doubles = 768 KiB, held by every GPU that loads
+// the library until the process exits.  Nothing in it has to start at zero: every CTA of the reduction kernel writes
+// its own 6 partials and the final kernel reads exactly the CTAs of its launch, so the contents a previous call left
+// behind (even of a larger grid) are never read.  All calls on a device share the array: calls that overlap on the GPU
+// (two streams) race.
+// In host code the array's name is a host-side stand-in, not a device address: the address a kernel can use comes from
+// cudaGetSymbolAddress, resolved per context at clt_create with the context's device current.
+// ---------------------------------------------------------------------------------------------
+constexpr int DIAG_STATIC_MAX_BLOCKS = 16384;
+static __device__ __align__(256) double g_diag_static_partial[DIAG_STATIC_MAX_BLOCKS * DG_N];
+
+cudaError_t diag_static_scratch(double **ptr, int *max_blocks)
+{
+    void *p = nullptr;
+    cudaError_t e = cudaGetSymbolAddress(&p, g_diag_static_partial);      // the CURRENT device's copy of the array
+    if (e != cudaSuccess) return e;
+    *ptr = static_cast<double *>(p);
+    *max_blocks = DIAG_STATIC_MAX_BLOCKS;
+    return cudaSuccess;
+}
+
 // Opts every kernel with more than 48 KB of dynamic shared memory in on the CURRENT device (the attribute is per
 // function and device).  Called by clt_create under the context's device, so nothing about it is process-global state.
 cudaError_t configure_kernels()
