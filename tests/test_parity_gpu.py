@@ -247,6 +247,24 @@ def test_config4_rhs_and_50_steps_match_oracle_in_the_bench_launch_configuration
     assert abs(d["max_divB"] - d0["max_divB"]) <= 1e-6 * d0["max_divB"] + 1e-12
 
 
+@pytest.mark.parametrize("variant", ["hall", "spectral", "hall+spectral"])
+def test_config4_rhs_of_the_hall_and_pseudo_spectral_variants_match_oracle_at_full_size(variant):
+    """The NEXT variants at BASELINE.json's full size, in the launch configuration their bench lines use (512x64x512:
+    nphi = 64 is the one size the FFT pre-pass serves): curl_J1, the Hall field and one RHS against the oracle."""
+    prob = inputs.make_problem(4)
+    over = {}
+    if "hall" in variant:
+        over.update(d_i=0.02, eta=1e-4)
+    if "spectral" in variant:
+        over.update(phi_scheme=1)
+    o, g = make_oracle(prob, **over), make_gpu(prob, **over)
+    record_margin(f"config4_curl_{variant}", assert_close(g.curl_J1(), o.curl_J1(prob.U), RHS_TOL, f"config 4 curl_J1, {variant}"))
+    if "hall" in variant:
+        record_margin(f"config4_hallG_{variant}", assert_close(g.hall_G(), o.hall_G(prob.U), RHS_TOL, f"config 4 Hall field, {variant}"))
+    record_margin(f"config4_rhs_{variant}", assert_close(g.rhs(), o.rhs(), RHS_TOL, f"config 4 rhs, {variant}"))
+    g.close()
+
+
 @pytest.mark.parametrize("index,steps", [(2, 100), (3, 100), (5, 100)])
 def test_textbook_rk4_schedule_build_against_the_reduced_schedule(index, steps):
     """A/B of the RK4 buffer schedule: libclt_textbook.so is the same source built with
