@@ -167,7 +167,8 @@ int clt_set_owned_rows(clt_ctx *ctx, int k_first, int k_last, int deep_first, in
  *   clt_step_stage(ctx, 1..4)     runs with the committed dt; the caller exchanges ghost rows in between.
  *   clt_cfl_close(ctx, ..)        leaves adaptive mode; returns the dt the next step would use and the time advanced
  *                                 since clt_cfl_open (synchronises).  CLT_ENONFINITE like clt_step_cfl.
- * One context alone: open, commit(init = 1), { four stages, commit(init = 0) } x steps, close == clt_step_cfl, bit for bit. */
+ * One context alone: open, commit(init = 1), { four stages, commit(init = 0) } x steps, close == clt_step_cfl, bit for bit.
+ * Between open and close clt_step and clt_step_cfl return CLT_ESTATE; clt_set_state ends the sequence.               */
 int clt_cfl_open(clt_ctx *ctx, double cfl);
 int clt_cfl_commit(clt_ctx *const *ctxs, int n, int init);
 int clt_cfl_close(clt_ctx *ctx, double *dt_next, double *time_advanced);

@@ -616,6 +616,7 @@ int clt_set_state(clt_ctx *ctx, const double *U)
 {
     DeviceGuard device_guard(ctx);
     if (!ctx || !U) return CLT_EINVAL;
+    ctx->adaptive = false;           // a new state ends an open clt_cfl_* sequence
     int r = copy_in(ctx, ctx->Un, U, (size_t)8 * ctx->L.nphi * ctx->L.nZ);
     if (r) return r;
     // a1: freeze the two boundary layers per R/Z side in every RK buffer
@@ -702,7 +703,7 @@ int clt_step(clt_ctx *ctx, int n)
 {
     DeviceGuard device_guard(ctx);
     if (!ctx || n < 0) return CLT_EINVAL;
-    if (!ctx->has_state || ctx->next_stage != 1) return CLT_ESTATE;
+    if (!ctx->has_state || ctx->next_stage != 1 || ctx->adaptive) return CLT_ESTATE;     // not between clt_cfl_open and clt_cfl_close
     if (!(ctx->dt > 0.0)) return CLT_EINVAL;
     // CUDA graph of the 8-launch step: 1 = always, 2 = never, 0 (default) = unless per-kernel profiling is on
     if (ctx->use_graph == 1 || (ctx->use_graph == 0 && !ctx->profiling)) {
@@ -1132,7 +1133,7 @@ int clt_step_cfl(clt_ctx *ctx, int n, double cfl, double *dt_last, double *time_
 {
     DeviceGuard device_guard(ctx);
     if (!ctx || n < 0) return CLT_EINVAL;
-    if (!ctx->has_state || ctx->next_stage != 1) return CLT_ESTATE;
+    if (!ctx->has_state || ctx->next_stage != 1 || ctx->adaptive) return CLT_ESTATE;     // not between clt_cfl_open and clt_cfl_close
     if (!(cfl > 0.0)) cfl = ctx->par.cfl;
     if (!(cfl > 0.0) || !isfinite(cfl)) return CLT_EINVAL;
     double *clock = ctx->result + 8;

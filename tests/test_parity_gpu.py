@@ -669,6 +669,10 @@ def test_group_adaptive_calls_equal_step_cfl_for_one_context():
     with pytest.raises(clt.CltError):
         b.cfl_open(0.4)                       # already open
     clt.cfl_commit([b], init=True)
+    with pytest.raises(clt.CltError):
+        b.step(1)                             # fixed-dt stepping is refused while the adaptive sequence is open
+    with pytest.raises(clt.CltError):
+        b.step_cfl(1, 0.4)
     for _ in range(4):
         for stage in (1, 2, 3, 4):
             b.step_stage(stage)
